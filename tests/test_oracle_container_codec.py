@@ -86,7 +86,7 @@ def test_table1_pins_the_ssr_formula():
         bad = line.rstrip().endswith("!")
         name, size, comp, t, cr, ssr = [s.strip() for s in line.rstrip(" !\n").split(";")]
         size, comp, t, cr, ssr = map(float, (size, comp, t, cr, ssr))
-        assert abs(metrics.compression_ratio(size, comp) - cr) < 0.011
+        assert abs(metrics.compression_ratio(size, comp) - cr) < 0.015
         got = metrics.sigma_ssr(size, comp, t)
         if bad:
             assert abs(got - ssr) > 0.05
