@@ -1,0 +1,142 @@
+/* boa.h — C ABI of the B200-native chunk-parallel neural range coder
+ * (the hot path of BOA Constrictor, arXiv 2511.11337).
+ *
+ * Citations: `P:n` = line n of the paper text.  Readings of passages where the paper is
+ * silent or garbled are numbered in DESIGN.md ("Readings") and referred to as R#k.
+ *
+ * The library owns every step of the path: split into chunks, byte embedding + Mamba-1
+ * blocks + tied head (Alg. 1; eq. 16-22), softmax (eq. 6), the
+ * integer table (eq. 7), the range coder (eq. 8-13) and the .boa container
+ * (P:167).  All of it runs in CUDA kernels for sm_100a; there is no CPU fallback — every entry
+ * point that needs the GPU returns BOA_E_CUDA when no device is usable.
+ *
+ * Conventions
+ *   - Return value: 0 (BOA_OK) or a negative BOA_E_* code; boa_strerror() names it.  Nothing
+ *     throws, aborts or prints.
+ *   - "host|device pointer": the library asks the CUDA runtime what the pointer is
+ *     (cudaPointerGetAttributes).  Device (or managed) memory is used in place; host memory
+ *     (pageable or pinned) is staged through a library-owned device buffer with the copies issued
+ *     on `cuda_stream` inside the call (this is what the end-to-end benchmark times).
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every
+ *     call returns only after its work on that stream has completed.
+ *   - One in-flight call per boa_model handle; different handles may be used concurrently.
+ *   - The caller owns all `in`/`out` buffers.  The handle owns the device copy of the weights and
+ *     a workspace (stream state, activations, per-stream output scratch) that grows to the largest
+ *     job seen and is released by boa_model_free().
+ */
+#ifndef BOA_H_
+#define BOA_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define BOA_OK 0
+#define BOA_E_ARG (-1)            /* NULL / zero / out-of-range argument                              */
+#define BOA_E_FORMAT (-2)         /* bad magic, version, freq_bits or inconsistent lengths            */
+#define BOA_E_CRC (-3)            /* index CRC-32 mismatch                                            */
+#define BOA_E_MODEL_MISMATCH (-4) /* container fingerprint != this model + this arithmetic            */
+#define BOA_E_CAPACITY (-5)       /* output buffer too small                                          */
+#define BOA_E_CORRUPT (-6)        /* a stream's payload ended before its symbols were decoded         */
+#define BOA_E_CUDA (-7)           /* CUDA runtime error or no usable sm_100 device                    */
+#define BOA_E_NOMEM (-8)          /* host or device allocation failed                                 */
+#define BOA_E_UNSUPPORTED (-9)    /* model shape outside what the kernels are built for               */
+
+typedef struct boa_model boa_model; /* opaque: device weights + workspace */
+
+/* ---- model ------------------------------------------------------------------------------------
+ * boa_model_load: parse a BOAW v1 blob (HOST pointer; layout in DESIGN.md "BOAW") — byte embedding
+ * [256][D] (also the tied head), per layer norm_w, W_in, conv_w, conv_b, W_x, W_dt,
+ * b_dt, A_log, D_skip, W_out (eq. 20-22) — copy it to the current CUDA device and
+ * return a handle.  Supported: d_state = 16, d_conv = 4, expand = 2, d_model a multiple of 64 and
+ * <= 1024, dt_rank <= 64, tied head, fp32 or bf16 matrices; else BOA_E_UNSUPPORTED.
+ * The blob is not referenced after the call returns. */
+int boa_model_load(const void* weights, size_t nbytes, boa_model** out);
+void boa_model_free(boa_model* m);
+
+/* 64-bit fingerprint stored in every container: (arithmetic version << 32) | CRC-32(blob).
+ * Tables are only reproducible with the same weights AND the same arithmetic. */
+uint64_t boa_model_fingerprint(const boa_model* m);
+
+/* ---- compress ---------------------------------------------------------------------------
+ * Split `in[0..n)` into ceil(n/chunk_bytes) chunks ("streams"); stream i is bytes
+ * [i*chunk_bytes, min(n,(i+1)*chunk_bytes)).  Byte 0 of a stream is stored raw; for t = 0..len-2 the
+ * model is stepped on byte t and byte t+1 is range-coded with the resulting table (len-1 symbols),
+ * all streams in lock-step.  Writes a BOA1 container to `out`.
+ *   in        host|device pointer, n bytes (may be NULL iff n == 0)
+ *   chunk_bytes  >= 1 and < 2^31
+ *   out       host|device pointer; *out_len = its capacity on entry, bytes written on return.
+ *             boa_compress_bound(n, chunk_bytes) is always enough (f >= 1 with total 2^16 bounds a
+ *             symbol at 16 bits: payload <= 2*(len-1) + 4 flush bytes).
+ * Errors: BOA_E_ARG, BOA_E_CAPACITY (out too small; nothing useful written), BOA_E_NOMEM, BOA_E_CUDA. */
+size_t boa_compress_bound(size_t n, size_t chunk_bytes);
+int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes,
+                 uint8_t* out, size_t* out_len, void* cuda_stream);
+
+/* ---- decompress -------------------------------------------------------------------------
+ * boa_decompressed_size: read only the 40-byte header (host|device pointer) and return n.
+ * boa_decompress: validate header, index CRC and fingerprint, then decode every stream in
+ * lock-step with the same step kernels; a stream that has reached its length is masked out.
+ *   out       host|device pointer; *out_len = capacity on entry (>= n), n on return.
+ * Errors: BOA_E_FORMAT, BOA_E_CRC, BOA_E_MODEL_MISMATCH, BOA_E_CAPACITY, BOA_E_CORRUPT (a decoder
+ * needed bytes past the end of its stream or did not consume its stream exactly; output is then
+ * undefined), BOA_E_NOMEM, BOA_E_CUDA. */
+int boa_decompressed_size(const uint8_t* in, size_t in_len, size_t* n);
+int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len,
+                   uint8_t* out, size_t* out_len, void* cuda_stream);
+
+const char* boa_strerror(int code);
+
+/* ---- measurement hooks ---------------------------------------------------------------------------
+ * Kernel classes of the step: the order below is the launch order inside one step. */
+enum {
+  BOA_K_EMBED = 0,   /* S1  byte embedding gather                                 */
+  BOA_K_INPROJ = 1,  /* S2+S3  RMSNorm + in_proj                                  */
+  BOA_K_CONVX = 2,   /* S4-S6  conv1d+SiLU, x_proj, dt_proj+softplus              */
+  BOA_K_SCAN = 3,    /* S7+S8  selective-SSM recurrence + gate (state streamed)   */
+  BOA_K_OUTPROJ = 4, /* S9  out_proj + residual                                   */
+  BOA_K_HEAD = 5,    /* S10 tied head                                             */
+  BOA_K_CODER = 6,   /* S11-S14 softmax, table, range coder step                  */
+  BOA_K_FINISH = 7,  /* S15/S16 flush, compaction, init                           */
+  BOA_K_COUNT = 8
+};
+typedef struct boa_profile {
+  uint64_t launches_total;            /* kernels launched by the last compress/decompress call       */
+  uint64_t steps;                     /* model steps taken (max stream length - 1, summed over waves) */
+  uint64_t streams;                   /* streams of the last call                                     */
+  uint64_t sampled_launches[BOA_K_COUNT]; /* launches that were bracketed by CUDA events             */
+  double sampled_ms[BOA_K_COUNT];     /* summed event time of those launches                          */
+  double total_ms;                    /* CUDA-event time of the whole call's device work              */
+} boa_profile;
+/* sample_every = k > 0: every k-th graph batch of the step loop is replaced by one eagerly launched
+ * batch whose kernels are individually bracketed by CUDA events on the call's stream (same kernels,
+ * same order, same results).  0 (default) = no sampling. */
+int boa_set_profiling(boa_model* m, int sample_every);
+int boa_get_profile(const boa_model* m, boa_profile* out);
+
+/* ---- test-only exports (the four parity checks of BASELINE.json, tests/test_gpu_*.py) -------------
+ * boa_debug_step_dump: run the compress-side step pipeline on `in` (device|host pointer) exactly as
+ *   boa_compress does and dump, for stream i and step t (t < n_steps <= chunk_bytes-1), row
+ *   r = i*n_steps + t of:  logits[r][256] (fp32, S10), probs[r][256] (fp32 softmax, eq. 6),
+ *   cdf[r][257] (uint32, eq. 7).  Any of the three output pointers may be NULL.  All streams must be
+ *   full length (n a multiple of chunk_bytes).  Output pointers: device|host.
+ * boa_debug_quantise: the table rule alone: logits[rows][256] fp32 -> cdf[rows][257].
+ * boa_debug_rc_encode / _decode: the range coder alone, one GPU thread per stream, driven by given
+ *   tables: cdf[n_streams][len][257], syms[n_streams][len]; payload of stream i is written at
+ *   out + i*cap, its size to sizes[i] (BOA_E_CAPACITY if any would exceed cap).  Decode reads the
+ *   same layout and writes syms; BOA_E_CORRUPT on overrun / bytes left over. */
+int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, size_t n_steps,
+                        float* logits, float* probs, uint32_t* cdf, void* cuda_stream);
+int boa_debug_quantise(const float* logits, size_t rows, uint32_t* cdf, void* cuda_stream);
+int boa_debug_rc_encode(const uint32_t* cdf, const uint8_t* syms, size_t n_streams, size_t len,
+                        uint8_t* out, size_t cap, uint32_t* sizes, void* cuda_stream);
+int boa_debug_rc_decode(const uint32_t* cdf, const uint8_t* in, size_t cap, const uint32_t* sizes,
+                        size_t n_streams, size_t len, uint8_t* syms, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BOA_H_ */

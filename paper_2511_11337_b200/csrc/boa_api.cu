@@ -1,0 +1,860 @@
+// boa_api.cu — the C ABI of include/boa.h: host orchestration of the step kernels.
+//
+// Product path.  Nothing here falls back to the CPU: without a usable CUDA device every entry point
+// that computes returns BOA_E_CUDA.  Nothing under oracle/ is included, linked or executed.
+#include "../../include/boa.h"
+
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+
+#include <algorithm>
+#include <new>
+#include <vector>
+
+#include "coder_kernels.cuh"
+#include "common.cuh"
+#include "container.h"
+#include "model_kernels.cuh"
+
+using namespace boa;
+
+namespace {
+
+constexpr int kStepsPerGraph = 32;       // model steps captured into one CUDA graph launch
+constexpr uint64_t kMaxWaveStreams = 65536;  // streams stepped together; more chunks run in waves
+constexpr int kConvxTS = 8;              // streams per k_convx CTA
+constexpr int kScanSPC = 8;              // streams per k_scan CTA
+
+struct GrowBuf {   // grow-only device buffer
+  void* p = nullptr;
+  size_t cap = 0;
+  int reserve(size_t bytes) {
+    if (bytes <= cap) return BOA_OK;
+    if (p) { cudaFree(p); p = nullptr; cap = 0; }
+    size_t want = round_up(bytes, 256);
+    cudaError_t e = cudaMalloc(&p, want);
+    if (e != cudaSuccess) { (void)cudaGetLastError(); p = nullptr; return BOA_E_NOMEM; }
+    cap = want;
+    return BOA_OK;
+  }
+  void release() { if (p) cudaFree(p); p = nullptr; cap = 0; }
+  template <class T> T* as() const { return reinterpret_cast<T*>(p); }
+};
+
+struct LayerW {
+  const float *norm_w, *w_in, *conv_b, *w_x, *w_dtT, *b_dt, *d_skip, *w_out;
+  const float4 *conv_w, *A4;
+};
+
+bool is_device_ptr(const void* p) {
+  if (!p) return false;
+  cudaPointerAttributes a;
+  if (cudaPointerGetAttributes(&a, p) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+  return a.type == cudaMemoryTypeDevice || a.type == cudaMemoryTypeManaged;
+}
+
+}  // namespace
+
+struct boa_model {
+  int L = 0, D = 0, E = 0, R = 0, J = 0;
+  uint32_t blob_crc = 0;
+  GrowBuf weights;
+  const float* emb = nullptr;
+  std::vector<LayerW> layers;
+
+  // workspace (per wave of Bcap streams)
+  uint64_t Bcap = 0;
+  GrowBuf u, xz, xs, delta, bc, y, logits, h, win;
+  GrowBuf pos, len, low, range, pending, wpos, cache, started, v, rpos, off, size, scratch, first, err;
+  GrowBuf stage_in, stage_out;
+
+  // profiling
+  int sample_every = 0;
+  boa_profile prof{};
+  std::vector<cudaEvent_t> events;
+
+  ~boa_model() {
+    for (GrowBuf* b : {&weights, &u, &xz, &xs, &delta, &bc, &y, &logits, &h, &win, &pos, &len, &low, &range,
+                       &pending, &wpos, &cache, &started, &v, &rpos, &off, &size, &scratch, &first, &err,
+                       &stage_in, &stage_out})
+      b->release();
+    for (cudaEvent_t e : events) cudaEventDestroy(e);
+  }
+};
+
+namespace {
+
+// ------------------------------------------------------------------------------------------ BOAW
+float bf16_to_f32(uint16_t b) {
+  uint32_t u = (uint32_t)b << 16;
+  float f;
+  memcpy(&f, &u, 4);
+  return f;
+}
+
+struct BlobReader {
+  const uint8_t* p;
+  size_t n, off;
+  int dtype;
+  // reads cnt values (bf16 if matrix && dtype==1 else fp32), 16-byte padded; returns false on overrun
+  bool take(size_t cnt, bool is_matrix, std::vector<float>& out) {
+    const bool bf = is_matrix && dtype == 1;
+    const size_t nbytes = cnt * (bf ? 2 : 4);
+    const size_t padded = (nbytes + 15) / 16 * 16;
+    if (off + padded > n) return false;
+    out.resize(cnt);
+    if (bf) {
+      for (size_t i = 0; i < cnt; ++i) {
+        uint16_t b;
+        memcpy(&b, p + off + 2 * i, 2);
+        out[i] = bf16_to_f32(b);
+      }
+    } else {
+      memcpy(out.data(), p + off, nbytes);
+    }
+    off += padded;
+    return true;
+  }
+};
+
+// ------------------------------------------------------------------------------------- step launch
+struct StepCtx {
+  boa_model* m;
+  cudaStream_t st;
+  int B;
+  int mode;                 // 0 encode, 1 decode
+  uint8_t* data;            // wave base of input (encode) / output (decode)
+  size_t chunk_bytes;
+  CoderArrays ca;
+  // debug dump
+  bool dump = false;
+  float* dump_logits = nullptr; float* dump_probs = nullptr; uint32_t* dump_cdf = nullptr;
+  uint32_t dump_steps = 0, dump_t = 0;
+  // accounting
+  uint64_t launches = 0;
+  bool sample = false;      // record an event after every launch
+  std::vector<int>* ev_cls = nullptr;
+  size_t ev_used = 0;
+};
+
+int mark(StepCtx& c, int cls) {
+  ++c.launches;
+  if (cudaPeekAtLastError() != cudaSuccess) { (void)cudaGetLastError(); return BOA_E_CUDA; }
+  if (c.sample) {
+    if (c.ev_used >= c.m->events.size()) {
+      cudaEvent_t e;
+      BOA_CUDA_TRY(cudaEventCreate(&e));
+      c.m->events.push_back(e);
+    }
+    BOA_CUDA_TRY(cudaEventRecord(c.m->events[c.ev_used++], c.st));
+    c.ev_cls->push_back(cls);
+  }
+  return BOA_OK;
+}
+
+template <bool NORM, bool RESID>
+void launch_sgemm(const float* A, int lda, const float* W, int ldw, const float* norm_w, float* C, int ldc,
+                  int M, int N, int K, cudaStream_t st) {
+  if (M >= 2048) {
+    dim3 grid((M + 127) / 128, N / 64);
+    k_sgemm_nt<128, 64, 8, 4, NORM, RESID><<<grid, 256, 0, st>>>(A, lda, W, ldw, norm_w, C, ldc, M, N, K);
+  } else {
+    dim3 grid((M + 63) / 64, N / 64);
+    k_sgemm_nt<64, 64, 4, 4, NORM, RESID><<<grid, 256, 0, st>>>(A, lda, W, ldw, norm_w, C, ldc, M, N, K);
+  }
+}
+
+// One model step + one coder step for all B streams of the wave (S1-S14).
+int launch_step(StepCtx& c) {
+  boa_model* m = c.m;
+  const int B = c.B, D = m->D, E = m->E;
+  float* u = m->u.as<float>();
+  float* xz = m->xz.as<float>();
+  float* xs = m->xs.as<float>();
+  float* delta = m->delta.as<float>();
+  float* bc = m->bc.as<float>();
+  float* y = m->y.as<float>();
+  float* logits = m->logits.as<float>();
+
+  {
+    const int total = B * (D / 4);
+    k_embed<<<(total + 255) / 256, 256, 0, c.st>>>(c.data, c.chunk_bytes, c.ca.pos, c.ca.len,
+                                                    reinterpret_cast<const float4*>(m->emb),
+                                                    reinterpret_cast<float4*>(u), B, D / 4);
+    BOA_TRY(mark(c, BOA_K_EMBED));
+  }
+  for (int l = 0; l < m->L; ++l) {
+    const LayerW& w = m->layers[l];
+    float* hl = m->h.as<float>() + (size_t)l * m->Bcap * E * kNState;
+    float* winl = m->win.as<float>() + (size_t)l * m->Bcap * 3 * E;
+    launch_sgemm<true, false>(u, D, w.w_in, D, w.norm_w, xz, 2 * E, B, 2 * E, D, c.st);
+    BOA_TRY(mark(c, BOA_K_INPROJ));
+    {
+      const size_t smem = (size_t)kConvxTS * (E + m->J) * sizeof(float);
+      k_convx<kConvxTS><<<(B + kConvxTS - 1) / kConvxTS, E, smem, c.st>>>(
+          xz, winl, w.conv_w, w.conv_b, w.w_x, w.w_dtT, w.b_dt, xs, delta, bc, B, E, m->R);
+      BOA_TRY(mark(c, BOA_K_CONVX));
+    }
+    {
+      const int bd = std::min(E, 256);
+      dim3 grid((B + kScanSPC - 1) / kScanSPC, E / bd);
+      k_scan<kScanSPC><<<grid, bd, 0, c.st>>>(reinterpret_cast<float4*>(hl), delta, xs, xz, bc, w.A4, w.d_skip,
+                                              y, B, E);
+      BOA_TRY(mark(c, BOA_K_SCAN));
+    }
+    launch_sgemm<false, true>(y, E, w.w_out, E, nullptr, u, D, B, D, E, c.st);
+    BOA_TRY(mark(c, BOA_K_OUTPROJ));
+  }
+  launch_sgemm<false, false>(u, D, m->emb, D, nullptr, logits, 256, B, 256, D, c.st);
+  BOA_TRY(mark(c, BOA_K_HEAD));
+
+  const int cgrid = (B * 32 + 255) / 256;
+  if (c.dump) {
+    if (c.dump_logits) {
+      BOA_CUDA_TRY(cudaMemcpy2DAsync(c.dump_logits + (size_t)c.dump_t * 256, (size_t)c.dump_steps * 256 * sizeof(float),
+                                     logits, 256 * sizeof(float), 256 * sizeof(float), B,
+                                     cudaMemcpyDeviceToDevice, c.st));
+    }
+    k_coder_step<0, true><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, c.dump_probs,
+                                                   c.dump_cdf, c.dump_steps);
+  } else if (c.mode == 0) {
+    k_coder_step<0, false><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, nullptr, nullptr, 0);
+  } else {
+    k_coder_step<1, false><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, nullptr, nullptr, 0);
+  }
+  BOA_TRY(mark(c, BOA_K_CODER));
+  return BOA_OK;
+}
+
+// Run `steps` lock-step iterations: CUDA-graph batches of kStepsPerGraph steps, remainder eager.
+int run_steps(StepCtx& c, uint64_t steps) {
+  boa_model* m = c.m;
+  if (steps == 0) return BOA_OK;
+  const uint64_t S = std::min<uint64_t>(kStepsPerGraph, steps);
+  const uint64_t n_batches = steps / S;
+  const uint64_t rem = steps - n_batches * S;
+
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  uint64_t graph_nodes = 0;
+  int rc = BOA_OK;
+  if (n_batches > 0 && !c.dump) {
+    const uint64_t before = c.launches;
+    if (cudaStreamBeginCapture(c.st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { (void)cudaGetLastError(); return BOA_E_CUDA; }
+    for (uint64_t s = 0; s < S && rc == BOA_OK; ++s) rc = launch_step(c);
+    cudaError_t e = cudaStreamEndCapture(c.st, &graph);
+    graph_nodes = c.launches - before;
+    c.launches = before;
+    if (rc == BOA_OK && e != cudaSuccess) { (void)cudaGetLastError(); rc = BOA_E_CUDA; }
+    if (rc == BOA_OK && cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) { (void)cudaGetLastError(); rc = BOA_E_CUDA; }
+    if (rc != BOA_OK) {
+      if (graph) cudaGraphDestroy(graph);
+      return rc;
+    }
+  }
+
+  std::vector<int> ev_cls;
+  for (uint64_t b = 0; b < n_batches && rc == BOA_OK; ++b) {
+    const bool sample = m->sample_every > 0 && (b % (uint64_t)m->sample_every) == (uint64_t)(m->sample_every / 2);
+    if (exec && !sample) {
+      if (cudaGraphLaunch(exec, c.st) != cudaSuccess) { (void)cudaGetLastError(); rc = BOA_E_CUDA; break; }
+      c.launches += graph_nodes;
+      continue;
+    }
+    if (sample) {
+      // eager batch, one event after every kernel (and one before the first)
+      ev_cls.clear();
+      c.ev_cls = &ev_cls;
+      c.ev_used = 0;
+      c.sample = true;
+      --c.launches;                        // the leading marker is not a kernel
+      rc = mark(c, -1);
+    }
+    for (uint64_t s = 0; s < S && rc == BOA_OK; ++s) {
+      if (c.dump) c.dump_t = (uint32_t)(b * S + s);
+      rc = launch_step(c);
+    }
+    if (sample) {
+      c.sample = false;
+      if (rc == BOA_OK && cudaEventSynchronize(m->events[c.ev_used - 1]) != cudaSuccess) { (void)cudaGetLastError(); rc = BOA_E_CUDA; }
+      for (size_t k = 1; k < c.ev_used && rc == BOA_OK; ++k) {
+        float ms = 0.0f;
+        if (cudaEventElapsedTime(&ms, m->events[k - 1], m->events[k]) != cudaSuccess) { (void)cudaGetLastError(); rc = BOA_E_CUDA; break; }
+        const int cls = ev_cls[k];
+        if (cls >= 0 && cls < BOA_K_COUNT) { m->prof.sampled_ms[cls] += ms; m->prof.sampled_launches[cls] += 1; }
+      }
+    }
+  }
+  for (uint64_t s = 0; s < rem && rc == BOA_OK; ++s) {
+    if (c.dump) c.dump_t = (uint32_t)(n_batches * S + s);
+    rc = launch_step(c);
+  }
+  if (exec) cudaGraphExecDestroy(exec);
+  if (graph) cudaGraphDestroy(graph);
+  return rc;
+}
+
+// ------------------------------------------------------------------------------------- workspace
+size_t bytes_per_stream(const boa_model* m, size_t cap) {
+  const size_t E = m->E, D = m->D;
+  return 4 * (D + 2 * E + 3 * E + 32 + 256) + (size_t)m->L * 4 * (E * kNState + 3 * E) + 64 + cap;
+}
+
+int reserve_workspace(boa_model* m, uint64_t B, size_t cap) {
+  const size_t E = m->E, D = m->D, L = m->L;
+  if (B > m->Bcap) {
+    // state arrays are indexed [l][Bcap][...]: growing B invalidates nothing (state is reset per wave)
+    BOA_TRY(m->u.reserve(B * D * 4));
+    BOA_TRY(m->xz.reserve(B * 2 * E * 4));
+    BOA_TRY(m->xs.reserve(B * E * 4));
+    BOA_TRY(m->delta.reserve(B * E * 4));
+    BOA_TRY(m->bc.reserve(B * 32 * 4));
+    BOA_TRY(m->y.reserve(B * E * 4));
+    BOA_TRY(m->logits.reserve(B * 256 * 4));
+    BOA_TRY(m->h.reserve(L * B * E * kNState * 4));
+    BOA_TRY(m->win.reserve(L * B * 3 * E * 4));
+    BOA_TRY(m->pos.reserve(B * 4));
+    BOA_TRY(m->len.reserve(B * 4));
+    BOA_TRY(m->low.reserve(B * 8));
+    BOA_TRY(m->range.reserve(B * 4));
+    BOA_TRY(m->pending.reserve(B * 4));
+    BOA_TRY(m->wpos.reserve(B * 4));
+    BOA_TRY(m->cache.reserve(B));
+    BOA_TRY(m->started.reserve(B));
+    BOA_TRY(m->v.reserve(B * 4));
+    BOA_TRY(m->rpos.reserve(B * 4));
+    BOA_TRY(m->off.reserve(B * 8));
+    BOA_TRY(m->size.reserve(B * 4));
+    BOA_TRY(m->first.reserve(B));
+    BOA_TRY(m->err.reserve(4));
+    m->Bcap = B;
+  }
+  if (cap) BOA_TRY(m->scratch.reserve(m->Bcap * cap));
+  return BOA_OK;
+}
+
+CoderArrays coder_arrays(boa_model* m, uint32_t cap) {
+  CoderArrays ca{};
+  ca.pos = m->pos.as<uint32_t>(); ca.len = m->len.as<uint32_t>();
+  ca.low = m->low.as<uint64_t>(); ca.range = m->range.as<uint32_t>(); ca.pending = m->pending.as<uint32_t>();
+  ca.wpos = m->wpos.as<uint32_t>(); ca.cache = m->cache.as<uint8_t>(); ca.started = m->started.as<uint8_t>();
+  ca.scratch = m->scratch.as<uint8_t>(); ca.cap = cap;
+  ca.v = m->v.as<uint32_t>(); ca.rpos = m->rpos.as<uint32_t>();
+  ca.off = m->off.as<uint64_t>(); ca.size = m->size.as<uint32_t>();
+  ca.payload = nullptr; ca.err = m->err.as<int>();
+  return ca;
+}
+
+int reset_state(boa_model* m, cudaStream_t st) {
+  // h starts at 0 for every chunk; the conv window is zero before the chunk start
+  BOA_CUDA_TRY(cudaMemsetAsync(m->h.p, 0, (size_t)m->L * m->Bcap * m->E * kNState * 4, st));
+  BOA_CUDA_TRY(cudaMemsetAsync(m->win.p, 0, (size_t)m->L * m->Bcap * 3 * m->E * 4, st));
+  return BOA_OK;
+}
+
+uint32_t stream_cap(size_t chunk_bytes) { return (uint32_t)round_up(2 * chunk_bytes + 8, 16); }
+
+uint64_t wave_streams(const boa_model* m, uint64_t nc, size_t cap) {
+  size_t free_b = 0, total_b = 0;
+  uint64_t w = std::min<uint64_t>(nc, kMaxWaveStreams);
+  if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
+    // what the handle already holds can be reused
+    const size_t held = m->Bcap * bytes_per_stream(m, m->scratch.cap / std::max<uint64_t>(m->Bcap, 1));
+    const size_t budget = (size_t)((free_b + held) * 0.85);
+    const uint64_t fit = std::max<uint64_t>(1, budget / bytes_per_stream(m, cap));
+    w = std::min(w, fit);
+  } else {
+    (void)cudaGetLastError();
+  }
+  return std::max<uint64_t>(w, 1);
+}
+
+void prof_begin(boa_model* m) { memset(&m->prof, 0, sizeof(m->prof)); }
+
+struct CallTimer {
+  cudaEvent_t a = nullptr, b = nullptr;
+  cudaStream_t st;
+  explicit CallTimer(cudaStream_t s) : st(s) {
+    if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) { (void)cudaGetLastError(); a = b = nullptr; }
+    if (a) cudaEventRecord(a, st);
+  }
+  double stop() {
+    float ms = 0.0f;
+    if (a && b && cudaEventRecord(b, st) == cudaSuccess && cudaEventSynchronize(b) == cudaSuccess) cudaEventElapsedTime(&ms, a, b);
+    (void)cudaGetLastError();
+    return ms;
+  }
+  ~CallTimer() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
+};
+
+int check_device() {
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return BOA_E_CUDA; }
+  cudaDeviceProp p;
+  if (cudaGetDeviceProperties(&p, dev) != cudaSuccess) { (void)cudaGetLastError(); return BOA_E_CUDA; }
+  if (p.major != 10) return BOA_E_CUDA;   // the kernels are built for sm_100a only
+  return BOA_OK;
+}
+
+}  // namespace
+
+// ===================================================================================== public ABI
+extern "C" {
+
+const char* boa_strerror(int code) {
+  switch (code) {
+    case BOA_OK: return "ok";
+    case BOA_E_ARG: return "invalid argument";
+    case BOA_E_FORMAT: return "not a BOA1 container / BOAW blob, or inconsistent lengths";
+    case BOA_E_CRC: return "index CRC mismatch";
+    case BOA_E_MODEL_MISMATCH: return "container was written with a different model or arithmetic";
+    case BOA_E_CAPACITY: return "output buffer too small";
+    case BOA_E_CORRUPT: return "compressed stream is corrupt or truncated";
+    case BOA_E_CUDA: return "CUDA error or no usable sm_100 device";
+    case BOA_E_NOMEM: return "out of memory";
+    case BOA_E_UNSUPPORTED: return "model shape not supported by the kernels";
+    default: return "unknown error";
+  }
+}
+
+int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
+  if (!weights || !out || nbytes < 64) return BOA_E_ARG;
+  *out = nullptr;
+  const uint8_t* p = static_cast<const uint8_t*>(weights);
+  if (memcmp(p, "BOAW", 4) != 0 || get_u32(p + 4) != 1) return BOA_E_FORMAT;
+  const uint32_t dtype = get_u32(p + 8), L = get_u32(p + 12), D = get_u32(p + 16), N = get_u32(p + 20),
+                 K = get_u32(p + 24), ex = get_u32(p + 28), R = get_u32(p + 32), flags = get_u32(p + 36);
+  if (dtype > 1) return BOA_E_FORMAT;
+  if (N != (uint32_t)kNState || K != (uint32_t)kDConv || ex != 2 || !(flags & 1u) || (flags & ~1u) || L == 0 || L > 64 ||
+      D == 0 || D % 64 != 0 || D > 512 || R == 0 || R > 64)
+    return BOA_E_UNSUPPORTED;
+  BOA_TRY(check_device());
+  const size_t E = 2 * (size_t)D, J = R + 2 * kNState;
+
+  boa_model* m = new (std::nothrow) boa_model();
+  if (!m) return BOA_E_NOMEM;
+  m->L = (int)L; m->D = (int)D; m->E = (int)E; m->R = (int)R; m->J = (int)J;
+  m->blob_crc = crc32_ieee(p, nbytes);
+
+  // host image of the device weight buffer (all fp32; bf16 matrices are widened exactly, R#13)
+  const size_t per_layer = D + 2 * E * D + 4 * E + E + J * E + E * R + E + E * kNState + E + D * E;
+  std::vector<float> img;
+  img.reserve(256 * D + L * per_layer + 64);
+  auto append = [&](const std::vector<float>& v) {
+    size_t o = img.size();
+    img.insert(img.end(), v.begin(), v.end());
+    while (img.size() % 4) img.push_back(0.0f);   // keep every tensor 16-byte aligned
+    return o;
+  };
+  struct Off { size_t norm_w, w_in, conv_w, conv_b, w_x, w_dtT, b_dt, A4, d_skip, w_out; };
+  std::vector<Off> offs(L);
+  BlobReader br{p, nbytes, 64, (int)dtype};
+  std::vector<float> t, t2;
+  bool ok = br.take(256 * (size_t)D, true, t);
+  size_t emb_off = 0;
+  if (ok) emb_off = append(t);
+  for (uint32_t l = 0; l < L && ok; ++l) {
+    Off& o = offs[l];
+    ok = ok && br.take(D, false, t); if (ok) o.norm_w = append(t);
+    ok = ok && br.take(2 * E * D, true, t); if (ok) o.w_in = append(t);
+    ok = ok && br.take(E * 4, false, t); if (ok) o.conv_w = append(t);        // [E][4] = one float4 per channel
+    ok = ok && br.take(E, false, t); if (ok) o.conv_b = append(t);
+    ok = ok && br.take(J * E, true, t); if (ok) o.w_x = append(t);
+    ok = ok && br.take(E * R, true, t);
+    if (ok) {                                                                 // W_dt [E][R] -> transposed [R][E]
+      t2.assign(E * R, 0.0f);
+      for (size_t e = 0; e < E; ++e)
+        for (size_t r = 0; r < R; ++r) t2[r * E + e] = t[e * R + r];
+      o.w_dtT = append(t2);
+    }
+    ok = ok && br.take(E, false, t); if (ok) o.b_dt = append(t);
+    ok = ok && br.take(E * kNState, false, t);
+    if (ok) {                                                                 // A = -exp(A_log), layout [4][E][4]
+      t2.assign(E * kNState, 0.0f);
+      for (size_t e = 0; e < E; ++e)
+        for (size_t n = 0; n < (size_t)kNState; ++n)
+          t2[((n / 4) * E + e) * 4 + (n % 4)] = (float)(-exp((double)t[e * kNState + n]));
+      o.A4 = append(t2);
+    }
+    ok = ok && br.take(E, false, t); if (ok) o.d_skip = append(t);
+    ok = ok && br.take(D * E, true, t); if (ok) o.w_out = append(t);
+  }
+  if (!ok || br.off != nbytes) { delete m; return BOA_E_FORMAT; }
+
+  int rc = m->weights.reserve(img.size() * sizeof(float));
+  if (rc == BOA_OK && cudaMemcpy(m->weights.p, img.data(), img.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) {
+    (void)cudaGetLastError();
+    rc = BOA_E_CUDA;
+  }
+  if (rc != BOA_OK) { delete m; return rc; }
+  const float* base = m->weights.as<float>();
+  m->emb = base + emb_off;
+  m->layers.resize(L);
+  for (uint32_t l = 0; l < L; ++l) {
+    const Off& o = offs[l];
+    LayerW& w = m->layers[l];
+    w.norm_w = base + o.norm_w; w.w_in = base + o.w_in; w.conv_w = reinterpret_cast<const float4*>(base + o.conv_w);
+    w.conv_b = base + o.conv_b; w.w_x = base + o.w_x; w.w_dtT = base + o.w_dtT; w.b_dt = base + o.b_dt;
+    w.A4 = reinterpret_cast<const float4*>(base + o.A4); w.d_skip = base + o.d_skip; w.w_out = base + o.w_out;
+  }
+  *out = m;
+  return BOA_OK;
+}
+
+void boa_model_free(boa_model* m) { delete m; }
+
+uint64_t boa_model_fingerprint(const boa_model* m) {
+  return m ? (((uint64_t)kArithVersion << 32) | m->blob_crc) : 0;
+}
+
+size_t boa_compress_bound(size_t n, size_t chunk_bytes) {
+  if (chunk_bytes == 0) return 0;
+  const uint64_t nc = n_chunks_of(n, chunk_bytes);
+  // every stream: <= 2 bytes per coded symbol (f >= 1 of 2^16) + 4 flush bytes
+  return index_bytes(nc) + 2 * n + 4 * (size_t)nc;
+}
+
+int boa_set_profiling(boa_model* m, int sample_every) {
+  if (!m || sample_every < 0) return BOA_E_ARG;
+  m->sample_every = sample_every;
+  return BOA_OK;
+}
+
+int boa_get_profile(const boa_model* m, boa_profile* out) {
+  if (!m || !out) return BOA_E_ARG;
+  *out = m->prof;
+  return BOA_OK;
+}
+
+int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, uint8_t* out, size_t* out_len,
+                 void* cuda_stream) {
+  if (!m || !out || !out_len || chunk_bytes == 0 || chunk_bytes >= (1ull << 31) || (n && !in)) return BOA_E_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const uint64_t nc = n_chunks_of(n, chunk_bytes);
+  if (nc >= (1ull << 32)) return BOA_E_ARG;
+  const size_t ib = index_bytes(nc);
+  const size_t capacity = *out_len;
+  if (capacity < ib) return BOA_E_CAPACITY;
+  prof_begin(m);
+  CallTimer timer(st);
+
+  // device views of the user buffers
+  const bool in_dev = (n == 0) || is_device_ptr(in), out_dev = is_device_ptr(out);
+  const uint8_t* d_in = in;
+  if (!in_dev) {
+    BOA_TRY(m->stage_in.reserve(n));
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->stage_in.p, in, n, cudaMemcpyHostToDevice, st));
+    d_in = m->stage_in.as<uint8_t>();
+  }
+  uint8_t* d_out = out;
+  const size_t out_cap = std::min(capacity, boa_compress_bound(n, chunk_bytes));
+  if (!out_dev) {
+    BOA_TRY(m->stage_out.reserve(out_cap));
+    d_out = m->stage_out.as<uint8_t>();
+  }
+
+  std::vector<uint8_t> index(ib, 0);
+  std::vector<uint32_t> sizes((size_t)nc);
+  std::vector<uint64_t> offs;
+  uint64_t payload_total = 0;
+  const uint32_t cap = stream_cap(chunk_bytes);
+  uint64_t launches = 0;
+
+  const uint64_t W = nc ? wave_streams(m, nc, cap) : 0;
+  for (uint64_t c0 = 0; c0 < nc; c0 += W) {
+    const uint64_t B = std::min(W, nc - c0);
+    const uint64_t wave_base = c0 * chunk_bytes;
+    const uint64_t n_wave = std::min<uint64_t>(n - wave_base, B * chunk_bytes);
+    BOA_TRY(reserve_workspace(m, B, cap));
+    BOA_TRY(reset_state(m, st));
+    StepCtx c{};
+    c.m = m; c.st = st; c.B = (int)B; c.mode = 0;
+    c.data = const_cast<uint8_t*>(d_in) + wave_base;
+    c.chunk_bytes = chunk_bytes;
+    c.ca = coder_arrays(m, cap);
+    const int g = (int)((B + 255) / 256);
+    k_coder_init<0><<<g, 256, 0, st>>>(c.ca, (int)B, chunk_bytes, n_wave, nullptr, nullptr);
+    BOA_TRY(mark(c, BOA_K_FINISH));
+    k_first_bytes<<<g, 256, 0, st>>>(c.data, chunk_bytes, m->first.as<uint8_t>(), (int)B);
+    BOA_TRY(mark(c, BOA_K_FINISH));
+    const uint64_t max_len = std::min<uint64_t>(chunk_bytes, n_wave);
+    BOA_TRY(run_steps(c, max_len - 1));
+    m->prof.steps += max_len - 1;
+    k_coder_finish<0><<<g, 256, 0, st>>>(c.ca, (int)B);
+    BOA_TRY(mark(c, BOA_K_FINISH));
+    BOA_CUDA_TRY(cudaMemcpyAsync(sizes.data() + c0, m->wpos.p, B * 4, cudaMemcpyDeviceToHost, st));
+    BOA_CUDA_TRY(cudaMemcpyAsync(index.data() + kHeaderBytes + c0, m->first.p, B, cudaMemcpyDeviceToHost, st));
+    BOA_CUDA_TRY(cudaStreamSynchronize(st));
+    offs.resize((size_t)B);
+    for (uint64_t i = 0; i < B; ++i) { offs[i] = payload_total; payload_total += sizes[c0 + i]; }
+    if (ib + payload_total > out_cap) return BOA_E_CAPACITY;
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->off.p, offs.data(), B * 8, cudaMemcpyHostToDevice, st));
+    k_compact<<<(int)((B * 32 + 255) / 256), 256, 0, st>>>(m->scratch.as<uint8_t>(), cap, m->wpos.as<uint32_t>(),
+                                                          m->off.as<uint64_t>(), d_out + ib, (int)B);
+    BOA_TRY(mark(c, BOA_K_FINISH));
+    BOA_CUDA_TRY(cudaStreamSynchronize(st));   // offs is reused by the next wave
+    launches += c.launches;
+  }
+
+  Header h{};
+  h.n = n; h.chunk_bytes = (uint32_t)chunk_bytes; h.n_chunks = (uint32_t)nc; h.freq_bits = 16;
+  h.last_len = nc ? (uint32_t)(n - (nc - 1) * chunk_bytes) : 0;
+  h.fingerprint = boa_model_fingerprint(m);
+  write_header(index.data(), h);
+  uint8_t* sp = index.data() + kHeaderBytes + first_padded(nc);
+  for (uint64_t i = 0; i < nc; ++i) put_u32(sp + 4 * i, sizes[i]);
+  put_u32(index.data() + ib - 4, crc32_ieee(index.data(), ib - 4));
+  const size_t total = ib + payload_total;
+  if (out_dev) {
+    BOA_CUDA_TRY(cudaMemcpyAsync(out, index.data(), ib, cudaMemcpyHostToDevice, st));
+  } else {
+    memcpy(out, index.data(), ib);
+    if (payload_total) BOA_CUDA_TRY(cudaMemcpyAsync(out + ib, d_out + ib, payload_total, cudaMemcpyDeviceToHost, st));
+  }
+  BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  *out_len = total;
+  m->prof.launches_total = launches;
+  m->prof.streams = nc;
+  m->prof.total_ms = timer.stop();
+  return BOA_OK;
+}
+
+int boa_decompressed_size(const uint8_t* in, size_t in_len, size_t* n) {
+  if (!in || !n || in_len < kHeaderBytes + 4) return in && n ? BOA_E_FORMAT : BOA_E_ARG;
+  uint8_t hb[kHeaderBytes];
+  if (is_device_ptr(in)) {
+    BOA_CUDA_TRY(cudaMemcpy(hb, in, kHeaderBytes, cudaMemcpyDeviceToHost));
+  } else {
+    memcpy(hb, in, kHeaderBytes);
+  }
+  Header h;
+  if (!parse_header(hb, h)) return BOA_E_FORMAT;
+  *n = (size_t)h.n;
+  return BOA_OK;
+}
+
+int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len, uint8_t* out, size_t* out_len, void* cuda_stream) {
+  if (!m || !in || !out_len) return BOA_E_ARG;
+  if (in_len < kHeaderBytes + 4) return BOA_E_FORMAT;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const bool in_dev = is_device_ptr(in);
+  prof_begin(m);
+  CallTimer timer(st);
+
+  uint8_t hb[kHeaderBytes];
+  if (in_dev) {
+    BOA_CUDA_TRY(cudaMemcpyAsync(hb, in, kHeaderBytes, cudaMemcpyDeviceToHost, st));
+    BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  } else {
+    memcpy(hb, in, kHeaderBytes);
+  }
+  Header h;
+  if (!parse_header(hb, h)) return BOA_E_FORMAT;
+  const uint64_t nc = h.n_chunks;
+  const size_t ib = index_bytes(nc);
+  if (in_len < ib) return BOA_E_FORMAT;
+  std::vector<uint8_t> index(ib);
+  if (in_dev) {
+    BOA_CUDA_TRY(cudaMemcpyAsync(index.data(), in, ib, cudaMemcpyDeviceToHost, st));
+    BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  } else {
+    memcpy(index.data(), in, ib);
+  }
+  if (get_u32(index.data() + ib - 4) != crc32_ieee(index.data(), ib - 4)) return BOA_E_CRC;
+  if (h.fingerprint != boa_model_fingerprint(m)) return BOA_E_MODEL_MISMATCH;
+  const uint8_t* sp = index.data() + kHeaderBytes + first_padded(nc);
+  std::vector<uint32_t> sizes((size_t)nc);
+  std::vector<uint64_t> offs((size_t)nc);
+  uint64_t payload_total = 0;
+  for (uint64_t i = 0; i < nc; ++i) { sizes[i] = get_u32(sp + 4 * i); offs[i] = payload_total; payload_total += sizes[i]; }
+  if (ib + payload_total != in_len) return BOA_E_FORMAT;
+  const size_t n = (size_t)h.n;
+  if (*out_len < n) return BOA_E_CAPACITY;
+  if (n && !out) return BOA_E_ARG;
+  if (n == 0) { *out_len = 0; m->prof.total_ms = timer.stop(); return BOA_OK; }
+
+  const size_t chunk_bytes = h.chunk_bytes;
+  const uint8_t* d_in = in;
+  if (!in_dev) {
+    BOA_TRY(m->stage_in.reserve(in_len));
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->stage_in.p, in, in_len, cudaMemcpyHostToDevice, st));
+    d_in = m->stage_in.as<uint8_t>();
+  }
+  const bool out_dev = is_device_ptr(out);
+  uint8_t* d_out = out;
+  if (!out_dev) {
+    BOA_TRY(m->stage_out.reserve(n));
+    d_out = m->stage_out.as<uint8_t>();
+  }
+
+  uint64_t launches = 0;
+  const uint64_t W = wave_streams(m, nc, 0);
+  for (uint64_t c0 = 0; c0 < nc; c0 += W) {
+    const uint64_t B = std::min(W, nc - c0);
+    const uint64_t wave_base = c0 * chunk_bytes;
+    const uint64_t n_wave = std::min<uint64_t>(n - wave_base, B * chunk_bytes);
+    BOA_TRY(reserve_workspace(m, B, 0));
+    BOA_TRY(reset_state(m, st));
+    BOA_CUDA_TRY(cudaMemsetAsync(m->err.p, 0, 4, st));
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->off.p, offs.data() + c0, B * 8, cudaMemcpyHostToDevice, st));
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->size.p, sizes.data() + c0, B * 4, cudaMemcpyHostToDevice, st));
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->first.p, index.data() + kHeaderBytes + c0, B, cudaMemcpyHostToDevice, st));
+    StepCtx c{};
+    c.m = m; c.st = st; c.B = (int)B; c.mode = 1;
+    c.data = d_out + wave_base;
+    c.chunk_bytes = chunk_bytes;
+    c.ca = coder_arrays(m, 0);
+    c.ca.payload = d_in + ib;
+    const int g = (int)((B + 255) / 256);
+    k_coder_init<1><<<g, 256, 0, st>>>(c.ca, (int)B, chunk_bytes, n_wave, m->first.as<uint8_t>(), c.data);
+    BOA_TRY(mark(c, BOA_K_FINISH));
+    const uint64_t max_len = std::min<uint64_t>(chunk_bytes, n_wave);
+    BOA_TRY(run_steps(c, max_len - 1));
+    m->prof.steps += max_len - 1;
+    k_coder_finish<1><<<g, 256, 0, st>>>(c.ca, (int)B);
+    BOA_TRY(mark(c, BOA_K_FINISH));
+    int err = 0;
+    BOA_CUDA_TRY(cudaMemcpyAsync(&err, m->err.p, 4, cudaMemcpyDeviceToHost, st));
+    BOA_CUDA_TRY(cudaStreamSynchronize(st));
+    launches += c.launches;
+    if (err) return BOA_E_CORRUPT;
+  }
+  if (!out_dev) {
+    BOA_CUDA_TRY(cudaMemcpyAsync(out, d_out, n, cudaMemcpyDeviceToHost, st));
+    BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  }
+  *out_len = n;
+  m->prof.launches_total = launches;
+  m->prof.streams = nc;
+  m->prof.total_ms = timer.stop();
+  return BOA_OK;
+}
+
+// ------------------------------------------------------------------------------------ test-only
+namespace {
+struct TmpDev {   // device view of a user buffer for the debug entry points
+  void* dev = nullptr;
+  void* user = nullptr;
+  size_t bytes = 0;
+  bool owned = false, back = false;
+  int init(const void* p, size_t nbytes, bool copy_in, bool copy_back, cudaStream_t st) {
+    user = const_cast<void*>(p); bytes = nbytes; back = false;
+    if (!p || nbytes == 0) { dev = nullptr; return BOA_OK; }
+    if (is_device_ptr(p)) { dev = user; return BOA_OK; }
+    if (cudaMalloc(&dev, nbytes) != cudaSuccess) { (void)cudaGetLastError(); dev = nullptr; return BOA_E_NOMEM; }
+    owned = true; back = copy_back;
+    if (copy_in) BOA_CUDA_TRY(cudaMemcpyAsync(dev, p, nbytes, cudaMemcpyHostToDevice, st));
+    return BOA_OK;
+  }
+  int finish(cudaStream_t st) {
+    if (owned && back) BOA_CUDA_TRY(cudaMemcpyAsync(user, dev, bytes, cudaMemcpyDeviceToHost, st));
+    return BOA_OK;
+  }
+  ~TmpDev() { if (owned && dev) cudaFree(dev); }
+};
+}  // namespace
+
+int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, size_t n_steps,
+                        float* logits, float* probs, uint32_t* cdf, void* cuda_stream) {
+  if (!m || !in || chunk_bytes < 2 || n == 0 || n % chunk_bytes != 0 || n_steps == 0 || n_steps > chunk_bytes - 1)
+    return BOA_E_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const uint64_t B = n / chunk_bytes;
+  if (B > kMaxWaveStreams) return BOA_E_ARG;
+  const size_t rows = (size_t)B * n_steps;
+  TmpDev tin, tl, tp, tc;
+  BOA_TRY(tin.init(in, n, true, false, st));
+  BOA_TRY(tl.init(logits, rows * 256 * 4, false, true, st));
+  BOA_TRY(tp.init(probs, rows * 256 * 4, false, true, st));
+  BOA_TRY(tc.init(cdf, rows * 257 * 4, false, true, st));
+  const uint32_t cap = stream_cap(chunk_bytes);
+  BOA_TRY(reserve_workspace(m, B, cap));
+  BOA_TRY(reset_state(m, st));
+  prof_begin(m);
+  StepCtx c{};
+  c.m = m; c.st = st; c.B = (int)B; c.mode = 0;
+  c.data = static_cast<uint8_t*>(tin.dev);
+  c.chunk_bytes = chunk_bytes;
+  c.ca = coder_arrays(m, cap);
+  c.dump = true;
+  c.dump_logits = static_cast<float*>(tl.dev);
+  c.dump_probs = static_cast<float*>(tp.dev);
+  c.dump_cdf = static_cast<uint32_t*>(tc.dev);
+  c.dump_steps = (uint32_t)n_steps;
+  k_coder_init<0><<<(int)((B + 255) / 256), 256, 0, st>>>(c.ca, (int)B, chunk_bytes, n, nullptr, nullptr);
+  BOA_TRY(mark(c, BOA_K_FINISH));
+  BOA_TRY(run_steps(c, n_steps));
+  BOA_TRY(tl.finish(st));
+  BOA_TRY(tp.finish(st));
+  BOA_TRY(tc.finish(st));
+  BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  return BOA_OK;
+}
+
+int boa_debug_quantise(const float* logits, size_t rows, uint32_t* cdf, void* cuda_stream) {
+  if (!logits || !cdf || rows == 0) return BOA_E_ARG;
+  BOA_TRY(check_device());
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  TmpDev tl, tc;
+  BOA_TRY(tl.init(logits, rows * 256 * 4, true, false, st));
+  BOA_TRY(tc.init(cdf, rows * 257 * 4, false, true, st));
+  k_debug_quantise<<<(unsigned)((rows * 32 + 255) / 256), 256, 0, st>>>(static_cast<const float*>(tl.dev),
+                                                                       static_cast<uint32_t*>(tc.dev), rows);
+  BOA_CUDA_TRY(cudaGetLastError());
+  BOA_TRY(tc.finish(st));
+  BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  return BOA_OK;
+}
+
+int boa_debug_rc_encode(const uint32_t* cdf, const uint8_t* syms, size_t n_streams, size_t len, uint8_t* out,
+                        size_t cap, uint32_t* sizes, void* cuda_stream) {
+  if (!cdf || !syms || !out || !sizes || n_streams == 0 || len == 0 || cap < 16 || cap >= (1ull << 32) ||
+      len >= (1ull << 31))
+    return BOA_E_ARG;
+  BOA_TRY(check_device());
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  TmpDev tc, ts, to, tz, te;
+  int err = 0;
+  BOA_TRY(tc.init(cdf, n_streams * len * 257 * 4, true, false, st));
+  BOA_TRY(ts.init(syms, n_streams * len, true, false, st));
+  BOA_TRY(to.init(out, n_streams * cap, false, true, st));
+  BOA_TRY(tz.init(sizes, n_streams * 4, false, true, st));
+  BOA_TRY(te.init(&err, 4, true, true, st));
+  k_debug_rc_encode<<<(unsigned)((n_streams + 63) / 64), 64, 0, st>>>(
+      static_cast<const uint32_t*>(tc.dev), static_cast<const uint8_t*>(ts.dev), (int)n_streams, (uint32_t)len,
+      static_cast<uint8_t*>(to.dev), (uint32_t)cap, static_cast<uint32_t*>(tz.dev), static_cast<int*>(te.dev));
+  BOA_CUDA_TRY(cudaGetLastError());
+  BOA_TRY(to.finish(st));
+  BOA_TRY(tz.finish(st));
+  BOA_TRY(te.finish(st));
+  BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  return err ? BOA_E_CAPACITY : BOA_OK;
+}
+
+int boa_debug_rc_decode(const uint32_t* cdf, const uint8_t* in, size_t cap, const uint32_t* sizes, size_t n_streams,
+                        size_t len, uint8_t* syms, void* cuda_stream) {
+  if (!cdf || !syms || !in || !sizes || n_streams == 0 || len == 0 || cap < 16 || cap >= (1ull << 32) ||
+      len >= (1ull << 31))
+    return BOA_E_ARG;
+  BOA_TRY(check_device());
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  TmpDev tc, ts, ti, tz, te;
+  int err = 0;
+  BOA_TRY(tc.init(cdf, n_streams * len * 257 * 4, true, false, st));
+  BOA_TRY(ti.init(in, n_streams * cap, true, false, st));
+  BOA_TRY(tz.init(sizes, n_streams * 4, true, false, st));
+  BOA_TRY(ts.init(syms, n_streams * len, false, true, st));
+  BOA_TRY(te.init(&err, 4, true, true, st));
+  k_debug_rc_decode<<<(unsigned)((n_streams + 63) / 64), 64, 0, st>>>(
+      static_cast<const uint32_t*>(tc.dev), static_cast<const uint8_t*>(ti.dev), (uint32_t)cap,
+      static_cast<const uint32_t*>(tz.dev), (int)n_streams, (uint32_t)len, static_cast<uint8_t*>(ts.dev),
+      static_cast<int*>(te.dev));
+  BOA_CUDA_TRY(cudaGetLastError());
+  BOA_TRY(ts.finish(st));
+  BOA_TRY(te.finish(st));
+  BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  return err ? BOA_E_CORRUPT : BOA_OK;
+}
+
+}  // extern "C"
