@@ -17,8 +17,10 @@
  *     (cudaPointerGetAttributes).  Device (or managed) memory is used in place; host memory
  *     (pageable or pinned) is staged through a library-owned device buffer with the copies issued
  *     on `cuda_stream` inside the call (this is what the end-to-end benchmark times).
- *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  Every
- *     call returns only after its work on that stream has completed.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  The
+ *     library orders its work after everything already enqueued on that stream (it records an event
+ *     there and runs on a stream of its own, because the step loop is replayed from CUDA graphs and
+ *     the legacy stream cannot be captured) and returns only after all of its work has completed.
  *   - One in-flight call per boa_model handle; different handles may be used concurrently.
  *   - The caller owns all `in`/`out` buffers.  The handle owns the device copy of the weights and
  *     a workspace (stream state, activations, per-stream output scratch) that grows to the largest
@@ -52,7 +54,7 @@ typedef struct boa_model boa_model; /* opaque: device weights + workspace */
  * [256][D] (also the tied head), per layer norm_w, W_in, conv_w, conv_b, W_x, W_dt,
  * b_dt, A_log, D_skip, W_out (eq. 20-22) — copy it to the current CUDA device and
  * return a handle.  Supported: d_state = 16, d_conv = 4, expand = 2, d_model a multiple of 64 and
- * <= 1024, dt_rank <= 64, tied head, fp32 or bf16 matrices; else BOA_E_UNSUPPORTED.
+ * <= 512, dt_rank <= 64, tied head, fp32 or bf16 matrices; else BOA_E_UNSUPPORTED.
  * The blob is not referenced after the call returns. */
 int boa_model_load(const void* weights, size_t nbytes, boa_model** out);
 void boa_model_free(boa_model* m);
@@ -89,6 +91,8 @@ int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len,
                    uint8_t* out, size_t* out_len, void* cuda_stream);
 
 const char* boa_strerror(int code);
+/* "file:line: cudaErrorName" of the last CUDA failure seen by the calling thread ("" if none).  Diagnostic only. */
+const char* boa_last_cuda_error(void);
 
 /* ---- measurement hooks ---------------------------------------------------------------------------
  * Kernel classes of the step: the order below is the launch order inside one step. */

@@ -1,0 +1,231 @@
+"""Thin binding over the C ABI of include/boa.h (libboa.so).  Argument marshalling only: every step
+of the path runs inside the library's CUDA kernels.  Buffers are torch tensors (uint8; CUDA tensors
+are used in place, CPU tensors are passed as host pointers and staged by the library).
+
+There is no CPU fallback: importing works anywhere (the symbol table is checked), but every call
+that computes raises BoaError(BOA_E_CUDA) without a usable sm_100 device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import torch
+
+from . import build as _build
+
+OK = 0
+E_ARG, E_FORMAT, E_CRC, E_MODEL_MISMATCH, E_CAPACITY, E_CORRUPT, E_CUDA, E_NOMEM, E_UNSUPPORTED = range(-1, -10, -1)
+K_NAMES = ("embed", "inproj", "convx", "scan", "outproj", "head", "coder", "finish")
+K_COUNT = 8
+
+EXPORTS = ("boa_model_load", "boa_model_free", "boa_model_fingerprint", "boa_compress_bound", "boa_compress",
+           "boa_decompressed_size", "boa_decompress", "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",
+           "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
+
+
+class Profile(C.Structure):
+    _fields_ = [("launches_total", C.c_uint64), ("steps", C.c_uint64), ("streams", C.c_uint64),
+                ("sampled_launches", C.c_uint64 * K_COUNT), ("sampled_ms", C.c_double * K_COUNT),
+                ("total_ms", C.c_double)]
+
+
+class BoaError(RuntimeError):
+    def __init__(self, code: int, what: str):
+        detail = lib().boa_last_cuda_error().decode() if code == E_CUDA else ""
+        super().__init__(f"{what}: {strerror(code)} ({code})" + (f" [{detail}]" if detail else ""))
+        self.code = code
+
+
+_lib = None
+
+
+def lib() -> C.CDLL:
+    """Load libboa.so (building it with nvcc if missing or stale).  Fails loudly if it cannot."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.is_stale():
+        have_nvcc = os.path.exists(os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc"))
+        if have_nvcc or not os.path.exists(path):
+            path = _build.build_library()   # raises if nvcc is missing or fails: no silent fallback
+    l = C.CDLL(path)
+    vp, sz, u8p = C.c_void_p, C.c_size_t, C.c_void_p
+    l.boa_model_load.argtypes = [vp, sz, C.POINTER(vp)]
+    l.boa_model_load.restype = C.c_int
+    l.boa_model_free.argtypes = [vp]
+    l.boa_model_free.restype = None
+    l.boa_model_fingerprint.argtypes = [vp]
+    l.boa_model_fingerprint.restype = C.c_uint64
+    l.boa_compress_bound.argtypes = [sz, sz]
+    l.boa_compress_bound.restype = sz
+    l.boa_compress.argtypes = [vp, u8p, sz, sz, u8p, C.POINTER(sz), vp]
+    l.boa_compress.restype = C.c_int
+    l.boa_decompressed_size.argtypes = [u8p, sz, C.POINTER(sz)]
+    l.boa_decompressed_size.restype = C.c_int
+    l.boa_decompress.argtypes = [vp, u8p, sz, u8p, C.POINTER(sz), vp]
+    l.boa_decompress.restype = C.c_int
+    l.boa_strerror.argtypes = [C.c_int]
+    l.boa_strerror.restype = C.c_char_p
+    l.boa_last_cuda_error.argtypes = []
+    l.boa_last_cuda_error.restype = C.c_char_p
+    l.boa_set_profiling.argtypes = [vp, C.c_int]
+    l.boa_set_profiling.restype = C.c_int
+    l.boa_get_profile.argtypes = [vp, C.POINTER(Profile)]
+    l.boa_get_profile.restype = C.c_int
+    l.boa_debug_step_dump.argtypes = [vp, u8p, sz, sz, sz, vp, vp, vp, vp]
+    l.boa_debug_step_dump.restype = C.c_int
+    l.boa_debug_quantise.argtypes = [vp, sz, vp, vp]
+    l.boa_debug_quantise.restype = C.c_int
+    l.boa_debug_rc_encode.argtypes = [vp, u8p, sz, sz, u8p, sz, vp, vp]
+    l.boa_debug_rc_encode.restype = C.c_int
+    l.boa_debug_rc_decode.argtypes = [vp, u8p, sz, vp, sz, sz, u8p, vp]
+    l.boa_debug_rc_decode.restype = C.c_int
+    _lib = l
+    return l
+
+
+def strerror(code: int) -> str:
+    return lib().boa_strerror(code).decode()
+
+
+def _check(code: int, what: str):
+    if code != OK:
+        raise BoaError(code, what)
+
+
+def _ptr(t: torch.Tensor | None) -> int | None:
+    if t is None:
+        return None
+    assert t.is_contiguous()
+    return t.data_ptr() if t.numel() else None
+
+
+def _stream(device=None) -> int:
+    return torch.cuda.current_stream(device).cuda_stream if torch.cuda.is_available() else 0
+
+
+def as_u8(data, device=None, pin: bool = False) -> torch.Tensor:
+    """bytes / numpy / tensor -> contiguous uint8 tensor (on `device` if given)."""
+    if isinstance(data, torch.Tensor):
+        t = data
+    else:
+        t = torch.frombuffer(bytearray(data), dtype=torch.uint8) if len(data) else torch.empty(0, dtype=torch.uint8)
+    t = t.contiguous().view(torch.uint8) if t.dtype != torch.uint8 else t.contiguous()
+    if device is not None:
+        t = t.to(device)
+    elif pin and torch.cuda.is_available():
+        t = t.pin_memory()
+    return t
+
+
+class Model:
+    """boa_model handle.  `weights` is a BOAW blob (bytes)."""
+
+    def __init__(self, weights: bytes):
+        self._h = C.c_void_p()
+        buf = (C.c_char * len(weights)).from_buffer_copy(weights)
+        _check(lib().boa_model_load(C.cast(buf, C.c_void_p), len(weights), C.byref(self._h)), "boa_model_load")
+
+    def close(self):
+        if self._h:
+            lib().boa_model_free(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def fingerprint(self) -> int:
+        return lib().boa_model_fingerprint(self._h)
+
+    def set_profiling(self, sample_every: int):
+        _check(lib().boa_set_profiling(self._h, sample_every), "boa_set_profiling")
+
+    def profile(self) -> dict:
+        p = Profile()
+        _check(lib().boa_get_profile(self._h, C.byref(p)), "boa_get_profile")
+        return {"launches_total": p.launches_total, "steps": p.steps, "streams": p.streams, "total_ms": p.total_ms,
+                "sampled_launches": {K_NAMES[k]: p.sampled_launches[k] for k in range(K_COUNT)},
+                "sampled_ms": {K_NAMES[k]: p.sampled_ms[k] for k in range(K_COUNT)}}
+
+    # -- the product calls ---------------------------------------------------------------------------
+    def compress_into(self, src: torch.Tensor, chunk_bytes: int, dst: torch.Tensor) -> int:
+        """boa_compress: src, dst uint8 tensors (each CUDA or CPU).  Returns bytes written."""
+        n = C.c_size_t(dst.numel())
+        _check(lib().boa_compress(self._h, _ptr(src), src.numel(), chunk_bytes, _ptr(dst), C.byref(n), _stream()),
+               "boa_compress")
+        return n.value
+
+    def decompress_into(self, src: torch.Tensor, dst: torch.Tensor) -> int:
+        n = C.c_size_t(dst.numel())
+        _check(lib().boa_decompress(self._h, _ptr(src), src.numel(), _ptr(dst) or 0, C.byref(n), _stream()),
+               "boa_decompress")
+        return n.value
+
+    def compress(self, data, chunk_bytes: int, device="cuda") -> torch.Tensor:
+        src = as_u8(data, device)
+        dst = torch.empty(compress_bound(src.numel(), chunk_bytes), dtype=torch.uint8, device=src.device)
+        return dst[: self.compress_into(src, chunk_bytes, dst)]
+
+    def decompress(self, blob, device="cuda") -> torch.Tensor:
+        src = as_u8(blob, device)
+        dst = torch.empty(decompressed_size(src), dtype=torch.uint8, device=src.device)
+        self.decompress_into(src, dst)
+        return dst
+
+    # -- test-only -----------------------------------------------------------------------------------
+    def debug_step_dump(self, data, chunk_bytes: int, n_steps: int, want=("logits", "probs", "cdf"), device="cuda"):
+        src = as_u8(data, device)
+        rows = (src.numel() // chunk_bytes) * n_steps
+        out = {}
+        if "logits" in want:
+            out["logits"] = torch.empty((rows, 256), dtype=torch.float32, device=device)
+        if "probs" in want:
+            out["probs"] = torch.empty((rows, 256), dtype=torch.float32, device=device)
+        if "cdf" in want:
+            out["cdf"] = torch.empty((rows, 257), dtype=torch.int32, device=device)
+        _check(lib().boa_debug_step_dump(self._h, _ptr(src), src.numel(), chunk_bytes, n_steps, _ptr(out.get("logits")),
+                                         _ptr(out.get("probs")), _ptr(out.get("cdf")), _stream()), "boa_debug_step_dump")
+        b = src.numel() // chunk_bytes
+        return {k: v.view(b, n_steps, -1) for k, v in out.items()}
+
+
+def compress_bound(n: int, chunk_bytes: int) -> int:
+    return lib().boa_compress_bound(n, chunk_bytes)
+
+
+def decompressed_size(blob: torch.Tensor) -> int:
+    n = C.c_size_t(0)
+    _check(lib().boa_decompressed_size(_ptr(blob) or 0, blob.numel(), C.byref(n)), "boa_decompressed_size")
+    return n.value
+
+
+def debug_quantise(logits: torch.Tensor) -> torch.Tensor:
+    """logits [rows,256] fp32 (CUDA or CPU) -> cdf [rows,257] int32 on the same device."""
+    logits = logits.contiguous()
+    cdf = torch.empty((logits.shape[0], 257), dtype=torch.int32, device=logits.device)
+    _check(lib().boa_debug_quantise(_ptr(logits), logits.shape[0], _ptr(cdf), _stream()), "boa_debug_quantise")
+    return cdf
+
+
+def debug_rc_encode(cdf: torch.Tensor, syms: torch.Tensor, cap: int):
+    """cdf [S,len,257] int32, syms [S,len] uint8 -> (out [S,cap] uint8, sizes [S] int32)."""
+    s, ln = syms.shape
+    out = torch.zeros((s, cap), dtype=torch.uint8, device=syms.device)
+    sizes = torch.zeros(s, dtype=torch.int32, device=syms.device)
+    _check(lib().boa_debug_rc_encode(_ptr(cdf.contiguous()), _ptr(syms.contiguous()), s, ln, _ptr(out), cap, _ptr(sizes),
+                                     _stream()), "boa_debug_rc_encode")
+    return out, sizes
+
+
+def debug_rc_decode(cdf: torch.Tensor, payload: torch.Tensor, sizes: torch.Tensor, length: int) -> torch.Tensor:
+    s, cap = payload.shape
+    syms = torch.zeros((s, length), dtype=torch.uint8, device=payload.device)
+    _check(lib().boa_debug_rc_decode(_ptr(cdf.contiguous()), _ptr(payload.contiguous()), cap, _ptr(sizes.contiguous()),
+                                     s, length, _ptr(syms), _stream()), "boa_debug_rc_decode")
+    return syms

@@ -69,6 +69,11 @@ struct boa_model {
   GrowBuf pos, len, low, range, pending, wpos, cache, started, v, rpos, off, size, scratch, first, err;
   GrowBuf stage_in, stage_out;
 
+  // the library's own stream (capturable, unlike the legacy default stream) and the event that orders it
+  // after the caller's stream
+  cudaStream_t own = nullptr;
+  cudaEvent_t user_ev = nullptr;
+
   // profiling
   int sample_every = 0;
   boa_profile prof{};
@@ -80,6 +85,8 @@ struct boa_model {
                        &stage_in, &stage_out})
       b->release();
     for (cudaEvent_t e : events) cudaEventDestroy(e);
+    if (user_ev) cudaEventDestroy(user_ev);
+    if (own) cudaStreamDestroy(own);
   }
 };
 
@@ -140,7 +147,7 @@ struct StepCtx {
 
 int mark(StepCtx& c, int cls) {
   ++c.launches;
-  if (cudaPeekAtLastError() != cudaSuccess) { (void)cudaGetLastError(); return BOA_E_CUDA; }
+  BOA_CUDA_TRY(cudaPeekAtLastError());
   if (c.sample) {
     if (c.ev_used >= c.m->events.size()) {
       cudaEvent_t e;
@@ -241,13 +248,13 @@ int run_steps(StepCtx& c, uint64_t steps) {
   int rc = BOA_OK;
   if (n_batches > 0 && !c.dump) {
     const uint64_t before = c.launches;
-    if (cudaStreamBeginCapture(c.st, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { (void)cudaGetLastError(); return BOA_E_CUDA; }
+    BOA_CUDA_TRY(cudaStreamBeginCapture(c.st, cudaStreamCaptureModeThreadLocal));
     for (uint64_t s = 0; s < S && rc == BOA_OK; ++s) rc = launch_step(c);
     cudaError_t e = cudaStreamEndCapture(c.st, &graph);
     graph_nodes = c.launches - before;
     c.launches = before;
-    if (rc == BOA_OK && e != cudaSuccess) { (void)cudaGetLastError(); rc = BOA_E_CUDA; }
-    if (rc == BOA_OK && cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) { (void)cudaGetLastError(); rc = BOA_E_CUDA; }
+    if (rc == BOA_OK && e != cudaSuccess) rc = note_cuda_error(e, __FILE__, __LINE__);
+    if (rc == BOA_OK && (e = cudaGraphInstantiate(&exec, graph, 0)) != cudaSuccess) rc = note_cuda_error(e, __FILE__, __LINE__);
     if (rc != BOA_OK) {
       if (graph) cudaGraphDestroy(graph);
       return rc;
@@ -258,7 +265,8 @@ int run_steps(StepCtx& c, uint64_t steps) {
   for (uint64_t b = 0; b < n_batches && rc == BOA_OK; ++b) {
     const bool sample = m->sample_every > 0 && (b % (uint64_t)m->sample_every) == (uint64_t)(m->sample_every / 2);
     if (exec && !sample) {
-      if (cudaGraphLaunch(exec, c.st) != cudaSuccess) { (void)cudaGetLastError(); rc = BOA_E_CUDA; break; }
+      cudaError_t ge = cudaGraphLaunch(exec, c.st);
+      if (ge != cudaSuccess) { rc = note_cuda_error(ge, __FILE__, __LINE__); break; }
       c.launches += graph_nodes;
       continue;
     }
@@ -388,6 +396,14 @@ struct CallTimer {
   ~CallTimer() { if (a) cudaEventDestroy(a); if (b) cudaEventDestroy(b); }
 };
 
+// Order the library's stream after everything already enqueued on the caller's stream.
+int enter(boa_model* m, void* user_stream, cudaStream_t* st) {
+  BOA_CUDA_TRY(cudaEventRecord(m->user_ev, static_cast<cudaStream_t>(user_stream)));
+  BOA_CUDA_TRY(cudaStreamWaitEvent(m->own, m->user_ev, 0));
+  *st = m->own;
+  return BOA_OK;
+}
+
 int check_device() {
   int dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return BOA_E_CUDA; }
@@ -401,6 +417,8 @@ int check_device() {
 
 // ===================================================================================== public ABI
 extern "C" {
+
+const char* boa_last_cuda_error(void) { return last_cuda_error_buf(); }
 
 const char* boa_strerror(int code) {
   switch (code) {
@@ -483,6 +501,11 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
   if (!ok || br.off != nbytes) { delete m; return BOA_E_FORMAT; }
 
   int rc = m->weights.reserve(img.size() * sizeof(float));
+  if (rc == BOA_OK && (cudaStreamCreateWithFlags(&m->own, cudaStreamNonBlocking) != cudaSuccess ||
+                       cudaEventCreateWithFlags(&m->user_ev, cudaEventDisableTiming) != cudaSuccess)) {
+    (void)cudaGetLastError();
+    rc = BOA_E_CUDA;
+  }
   if (rc == BOA_OK && cudaMemcpy(m->weights.p, img.data(), img.size() * sizeof(float), cudaMemcpyHostToDevice) != cudaSuccess) {
     (void)cudaGetLastError();
     rc = BOA_E_CUDA;
@@ -530,7 +553,8 @@ int boa_get_profile(const boa_model* m, boa_profile* out) {
 int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, uint8_t* out, size_t* out_len,
                  void* cuda_stream) {
   if (!m || !out || !out_len || chunk_bytes == 0 || chunk_bytes >= (1ull << 31) || (n && !in)) return BOA_E_ARG;
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  cudaStream_t st;
+  BOA_TRY(enter(m, cuda_stream, &st));
   const uint64_t nc = n_chunks_of(n, chunk_bytes);
   if (nc >= (1ull << 32)) return BOA_E_ARG;
   const size_t ib = index_bytes(nc);
@@ -637,7 +661,8 @@ int boa_decompressed_size(const uint8_t* in, size_t in_len, size_t* n) {
 int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len, uint8_t* out, size_t* out_len, void* cuda_stream) {
   if (!m || !in || !out_len) return BOA_E_ARG;
   if (in_len < kHeaderBytes + 4) return BOA_E_FORMAT;
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  cudaStream_t st;
+  BOA_TRY(enter(m, cuda_stream, &st));
   const bool in_dev = is_device_ptr(in);
   prof_begin(m);
   CallTimer timer(st);
@@ -759,7 +784,8 @@ int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_
                         float* logits, float* probs, uint32_t* cdf, void* cuda_stream) {
   if (!m || !in || chunk_bytes < 2 || n == 0 || n % chunk_bytes != 0 || n_steps == 0 || n_steps > chunk_bytes - 1)
     return BOA_E_ARG;
-  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  cudaStream_t st;
+  BOA_TRY(enter(m, cuda_stream, &st));
   const uint64_t B = n / chunk_bytes;
   if (B > kMaxWaveStreams) return BOA_E_ARG;
   const size_t rows = (size_t)B * n_steps;

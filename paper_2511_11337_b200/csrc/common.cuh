@@ -20,13 +20,17 @@ constexpr float kEps = 1e-5f;        // RMSNorm epsilon (R#10)
 // arithmetic (operation order, fusion, precision).
 constexpr uint32_t kArithVersion = 0x42320001u;
 
+// Last CUDA failure seen by this thread ("file:line: cudaErrorName"), for boa_last_cuda_error().
+inline char* last_cuda_error_buf() {
+  static thread_local char buf[256] = "";
+  return buf;
+}
+inline int note_cuda_error(cudaError_t e, const char* file, int line);
+
 #define BOA_CUDA_TRY(expr)                      \
   do {                                          \
     cudaError_t _e = (expr);                    \
-    if (_e != cudaSuccess) {                    \
-      (void)cudaGetLastError();                 \
-      return (_e == cudaErrorMemoryAllocation) ? BOA_E_NOMEM : BOA_E_CUDA; \
-    }                                           \
+    if (_e != cudaSuccess) return boa::note_cuda_error(_e, __FILE__, __LINE__); \
   } while (0)
 
 #define BOA_TRY(expr)            \
@@ -34,6 +38,18 @@ constexpr uint32_t kArithVersion = 0x42320001u;
     int _r = (expr);             \
     if (_r != BOA_OK) return _r; \
   } while (0)
+
+}  // namespace boa
+#include <stdio.h>
+#include "../../include/boa.h"
+namespace boa {
+inline int note_cuda_error(cudaError_t e, const char* file, int line) {
+  const char* slash = file;
+  for (const char* c = file; *c; ++c) if (*c == '/') slash = c + 1;
+  snprintf(last_cuda_error_buf(), 256, "%s:%d: %s", slash, line, cudaGetErrorName(e));
+  (void)cudaGetLastError();
+  return (e == cudaErrorMemoryAllocation) ? BOA_E_NOMEM : BOA_E_CUDA;
+}
 
 __host__ __device__ inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 

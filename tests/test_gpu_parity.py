@@ -1,0 +1,225 @@
+"""GPU parity tests (run on the B200 box with -m gpu): the CUDA path, called through the C ABI, against the
+CPU oracle on the same seeded inputs.  The four checks of BASELINE.json's north_star plus the table rule:
+
+  1. range coder bit-exact with the oracle's, given the oracle's frequency tables
+  2. probabilities within max-abs 1e-5 of the oracle's (fp64)
+  3. compressed size within 0.5 % of the oracle's
+  4. GPU compress -> GPU decompress byte-exact on every input
+  5. integer tables bit-exact with the oracle's rule applied to the same fp32 logits (a float decides an
+     integer there, so both sides take the decision in fp32 by the same specified EXP, R#5)
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import codec, container, model, quantise, rangecoder
+from paper_2511_11337_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+PROB_TOL = 1e-5      # north_star: "probabilities must be within max-abs 1e-5 of the oracle's"
+SIZE_TOL = 0.005     # north_star: "compressed size must be within 0.5% of the oracle's"
+
+
+def _np(t):
+    return t.detach().cpu().numpy()
+
+
+def _cases():
+    s1 = synth.CONFIGS[1]
+    s2 = synth.CONFIGS[2]
+    small2 = synth.ModelShape(2, 128, dt_rank=8)
+    return {
+        "cfg1": (s1.weights(), s1),
+        "cfg1_sharp": (s1.weights(emb_std=0.25), s1),
+        "d128_l2_bf16_sharp": (synth.make_weights(small2, 7, synth.DTYPE_BF16, emb_std=0.25), s1),
+        "cfg2_shape_sharp": (synth.make_weights(s2.shape, 1, emb_std=0.25), s2),
+    }
+
+
+@pytest.fixture(scope="module", params=list(_cases()))
+def case(request, boa):
+    blob, cfg = _cases()[request.param]
+    return request.param, blob, cfg, boa.Model(blob), model.load_weights(blob)
+
+
+# ---------------------------------------------------------------------------------------------- check 5
+def test_quantiser_bit_exact_on_given_logits(boa):
+    g = np.random.Generator(np.random.PCG64(11))
+    rows = []
+    rows.append(g.normal(0, 0.02, (300, 256)))                    # near-uniform regime of the configured weights
+    rows.append(g.normal(0, 3.0, (300, 256)))                     # sharp
+    rows.append(g.normal(0, 30.0, (300, 256)))                    # f = 1 floor everywhere but a few symbols
+    rows.append(np.zeros((1, 256)))                               # uniform -> f = 256
+    one = np.full((1, 256), -100.0); one[0, 17] = 5.0             # one-hot -> 65281 + 255 ones
+    tie = np.full((1, 256), -100.0); tie[0, [3, 200]] = 1.0       # two-way tie -> 32641 each
+    bad = np.zeros((3, 256)); bad[0, 5] = np.nan; bad[1, 9] = np.inf; bad[2, :] = -np.inf
+    neg = np.zeros((1, 256)); neg[0, 100] = -np.inf               # -inf below a finite max is legal
+    logits = np.concatenate(rows + [one, tie, bad, neg]).astype(np.float32)
+    want = quantise.quantise(logits)
+    got = _np(boa.debug_quantise(torch.from_numpy(logits).cuda())).astype(np.int64)
+    assert np.array_equal(got, want)
+    f = np.diff(got, axis=1)
+    assert f.min() >= 1 and np.all(got[:, 0] == 0) and np.all(got[:, 256] == 65536)
+    assert np.all(f[900] == 256) and f[901, 17] == 65281 and f[902, 3] == f[902, 200] == 32641
+    assert np.all(f[903:906] == 256)
+
+
+# ---------------------------------------------------------------------------------------------- check 1
+@pytest.mark.parametrize("kind", ["uniform", "peaked", "random"])
+def test_range_coder_bit_exact_given_oracle_tables(boa, kind):
+    g = np.random.Generator(np.random.PCG64(5))
+    S, T = 37, 700                                                 # > one block of 64 coder threads, ragged
+    if kind == "uniform":
+        logits = np.zeros((S, T, 256), np.float32)
+    elif kind == "peaked":                                         # long runs of f=65281 symbols, then rare ones:
+        logits = np.full((S, T, 256), -50.0, np.float32)           # exercises pending-0xFF runs and carries
+        logits[:, :, 255] = 0.0
+    else:
+        logits = g.normal(0, 4.0, (S, T, 256)).astype(np.float32)
+    C = quantise.quantise(logits)                                  # the ORACLE's tables
+    syms = g.integers(0, 256, (S, T)).astype(np.uint8)
+    if kind == "peaked":
+        syms = np.where(g.random((S, T)) < 0.97, 255, syms).astype(np.uint8)
+    want = [rangecoder.encode_stream(C[i], syms[i].astype(np.int64)) for i in range(S)]
+    cap = 2 * T + 16
+    out, sizes = boa.debug_rc_encode(torch.from_numpy(C.astype(np.int32)).cuda(), torch.from_numpy(syms).cuda(), cap)
+    out, sizes = _np(out), _np(sizes)
+    for i in range(S):
+        assert sizes[i] == len(want[i]) and out[i, : sizes[i]].tobytes() == want[i], (kind, i)
+    # and the GPU decoder inverts the ORACLE's encoder
+    pay = np.zeros((S, cap), np.uint8)
+    for i in range(S):
+        pay[i, : len(want[i])] = np.frombuffer(want[i], np.uint8)
+    dec = boa.debug_rc_decode(torch.from_numpy(C.astype(np.int32)).cuda(), torch.from_numpy(pay).cuda(),
+                              torch.from_numpy(np.array([len(w) for w in want], np.int32)).cuda(), T)
+    assert np.array_equal(_np(dec), syms)
+    if kind == "uniform":
+        assert all(len(w) == T + 4 for w in want)                 # uniform table: exactly n + 4 bytes
+
+
+def test_range_coder_golden_vectors(boa):
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "rc_vectors.txt")
+    tables = {"uniform": np.arange(257) * 256,
+              "peak0": np.concatenate([[0], 65281 + np.arange(256)]),
+              "peak255": np.concatenate([np.arange(256), [65536]])}
+    for line in open(path):
+        if line.startswith("#") or not line.strip():
+            continue
+        tname, s, pay = [x.strip() for x in line.split(";")]
+        if "x" in s:
+            b, cnt = s.split("x")
+            syms = [int(b, 16)] * int(cnt)
+        else:
+            syms = [int(x, 16) for x in s.split()]
+        C = np.tile(tables[tname].astype(np.int32), (1, len(syms), 1))
+        out, sizes = boa.debug_rc_encode(torch.from_numpy(C).cuda(), torch.tensor([syms], dtype=torch.uint8).cuda(),
+                                         2 * len(syms) + 16)
+        assert _np(out)[0, : int(sizes[0])].tobytes() == bytes(int(x, 16) for x in pay.split()), line
+
+
+# ---------------------------------------------------------------------------------------- checks 2 and 5
+def test_probabilities_and_tables_against_oracle(case, boa):
+    name, blob, cfg, gm, w = case
+    S, T = 5, 96                                                   # 5 streams: ragged vs the 8-stream tiles
+    data = np.frombuffer(cfg.data(S * T), np.uint8).reshape(S, T)
+    d = gm.debug_step_dump(data.tobytes(), T, T - 1)
+    logits64 = model.logits_for_chunks(w, data)
+    p_ref = quantise.softmax(logits64)
+    p_gpu = _np(d["probs"]).astype(np.float64)
+    assert np.abs(p_gpu - p_ref).max() <= PROB_TOL, name
+    assert np.abs(_np(d["logits"]) - logits64).max() <= 2e-4 * max(1.0, np.abs(logits64).max())
+    # tables: the oracle's rule on the GPU's own fp32 logits must give the GPU's tables, bit for bit
+    assert np.array_equal(_np(d["cdf"]).astype(np.int64), quantise.quantise(_np(d["logits"])))
+    if "sharp" in name:
+        assert p_ref.max() > 0.05                                   # the sharp sets are actually sharp
+
+
+# ---------------------------------------------------------------------------------------- checks 3 and 4
+def test_round_trip_and_size_against_oracle(case, boa):
+    name, blob, cfg, gm, w = case
+    chunk = 160
+    data = cfg.data(7 * chunk + 33)                                # ragged last chunk
+    comp = gm.compress(data, chunk)
+    assert _np(gm.decompress(comp)).tobytes() == data
+    ref = codec.compress(w, data, chunk)
+    assert abs(len(comp) - len(ref)) <= SIZE_TOL * len(ref), (name, len(comp), len(ref))
+    # container structure: parse with the oracle's reader, GPU fingerprint
+    n, cb, last, first, payloads = container.unpack(_np(comp).tobytes(), gm.fingerprint)
+    assert (n, cb, last) == (len(data), chunk, 33) and first == bytes(data[i * chunk] for i in range(8))
+    # eq. 1: each GPU payload is within (0,5) bytes of the ideal code length under the GPU's own tables
+    full = np.frombuffer(data[: 7 * chunk], np.uint8).reshape(7, chunk)
+    C = _np(gm.debug_step_dump(full.tobytes(), chunk, chunk - 1, want=("cdf",))["cdf"]).astype(np.int64)
+    for i in range(7):
+        assert 0 < len(payloads[i]) - codec.ideal_bytes(C[i], full[i, 1:]) < 5
+
+
+def test_host_pointers_and_device_pointers_agree(case, boa):
+    name, blob, cfg, gm, w = case
+    data = cfg.data(3000)
+    a = gm.compress(data, 500, device="cuda")
+    b = gm.compress(data, 500, device="cpu")                       # host buffers, staged by the library
+    assert b.device.type == "cpu" and _np(a).tobytes() == _np(b).tobytes()
+    assert _np(gm.decompress(b, device="cpu")).tobytes() == data
+
+
+# ---------------------------------------------------------------------------------------------- edges
+def test_edge_cases(boa):
+    cfg = synth.CONFIGS[1]
+    gm = boa.Model(cfg.weights())
+    empty = gm.compress(b"", 4096)
+    assert empty.numel() == 44 and gm.decompress(empty).numel() == 0
+    for n, chunk in [(1, 4096), (5, 1), (4096, 4096), (4097, 4096), (1000, 7), (300, 2)]:
+        data = cfg.data(n)
+        comp = gm.compress(data, chunk)
+        assert comp.numel() <= boa.compress_bound(n, chunk)
+        assert _np(gm.decompress(comp)).tobytes() == data, (n, chunk)
+    # 1-byte chunks code zero symbols: payload = 4 flush bytes each
+    comp = _np(gm.compress(cfg.data(5), 1)).tobytes()
+    assert len(comp) == container.index_bytes(5) + 5 * 4
+
+
+def test_errors(boa):
+    cfg = synth.CONFIGS[1]
+    gm = boa.Model(cfg.weights())
+    other = boa.Model(cfg.weights(emb_std=0.25))
+    data = cfg.data(2000)
+    comp = gm.compress(data, 250)
+    dst = torch.empty(2000, dtype=torch.uint8, device="cuda")
+
+    def code(fn):
+        with pytest.raises(boa.BoaError) as e:
+            fn()
+        return e.value.code
+
+    assert code(lambda: other.decompress(comp)) == boa.E_MODEL_MISMATCH
+    bad = comp.clone(); bad[45] ^= 1                               # index byte -> CRC
+    assert code(lambda: gm.decompress_into(bad, dst)) == boa.E_CRC
+    bad = comp.clone(); bad[0] = 0
+    assert code(lambda: gm.decompress_into(bad, dst)) == boa.E_FORMAT
+    assert code(lambda: gm.decompress_into(comp[:-3], dst)) == boa.E_FORMAT
+    assert code(lambda: gm.decompress_into(comp, dst[:100])) == boa.E_CAPACITY
+    small = torch.empty(60, dtype=torch.uint8, device="cuda")
+    assert code(lambda: gm.compress_into(torch.zeros(2000, dtype=torch.uint8, device="cuda"), 250, small)) == boa.E_CAPACITY
+    # payload corruption: either detected (BOA_E_CORRUPT) or decodes to different bytes, never a crash
+    bad = comp.clone(); bad[-40:] = 0xFF
+    try:
+        out = gm.decompress(bad)
+        assert _np(out).tobytes() != data
+    except boa.BoaError as e:
+        assert e.code == boa.E_CORRUPT
+
+
+def test_result_independent_of_batch_and_position(boa):
+    """P:116 lock-step determinism, strengthened: a chunk's payload does not depend on which other chunks are
+    stepped with it, so any B reproduces the same tables."""
+    cfg = synth.CONFIGS[1]
+    gm = boa.Model(cfg.weights(emb_std=0.25))
+    chunk = 200
+    data = cfg.data(70 * chunk)                                    # 70 streams: two 64-row GEMM tiles
+    _, _, _, _, pa = container.unpack(_np(gm.compress(data, chunk)).tobytes())
+    for i in (0, 9, 63, 64, 69):
+        solo = gm.compress(data[i * chunk:(i + 1) * chunk], chunk)
+        _, _, _, _, ps = container.unpack(_np(solo).tobytes())
+        assert ps[0] == pa[i], i
