@@ -132,6 +132,12 @@ int boa_get_profile(const boa_model* m, boa_profile* out);
  *   tables: cdf[n_streams][len][257], syms[n_streams][len]; payload of stream i is written at
  *   out + i*cap, its size to sizes[i] (BOA_E_CAPACITY if any would exceed cap).  Decode reads the
  *   same layout and writes syms; BOA_E_CORRUPT on overrun / bytes left over. */
+/* boa_debug_gemm: the tensor-core contraction kernel alone (S3/S5/S9/S10; tc_gemm.cuh):
+ *   C[M][N] = A[M][K] W[N][K]^T, A and C host|device fp32 row-major, W a HOST fp32 matrix that is cut into
+ *   `weight_pieces` (1 or 3) bf16 pieces exactly as boa_model_load does; tile_n = 64 or 128 selects the
+ *   instantiation.  K % 64 == 0. */
+int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N, int weight_pieces, int tile_n,
+                   float* C, void* cuda_stream);
 int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, size_t n_steps,
                         float* logits, float* probs, uint32_t* cdf, void* cuda_stream);
 int boa_debug_quantise(const float* logits, size_t rows, uint32_t* cdf, void* cuda_stream);

@@ -21,7 +21,7 @@ K_COUNT = 8
 
 EXPORTS = ("boa_model_load", "boa_model_free", "boa_model_fingerprint", "boa_compress_bound", "boa_compress",
            "boa_decompressed_size", "boa_decompress", "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",
-           "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
+           "boa_debug_gemm", "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
 
 
 class Profile(C.Structure):
@@ -74,6 +74,8 @@ def lib() -> C.CDLL:
     l.boa_set_profiling.restype = C.c_int
     l.boa_get_profile.argtypes = [vp, C.POINTER(Profile)]
     l.boa_get_profile.restype = C.c_int
+    l.boa_debug_gemm.argtypes = [vp, sz, sz, vp, sz, C.c_int, C.c_int, vp, vp]
+    l.boa_debug_gemm.restype = C.c_int
     l.boa_debug_step_dump.argtypes = [vp, u8p, sz, sz, sz, vp, vp, vp, vp]
     l.boa_debug_step_dump.restype = C.c_int
     l.boa_debug_quantise.argtypes = [vp, sz, vp, vp]
@@ -203,6 +205,16 @@ def decompressed_size(blob: torch.Tensor) -> int:
     n = C.c_size_t(0)
     _check(lib().boa_decompressed_size(_ptr(blob) or 0, blob.numel(), C.byref(n)), "boa_decompressed_size")
     return n.value
+
+
+def debug_gemm(a: torch.Tensor, w: torch.Tensor, weight_pieces: int, tile_n: int) -> torch.Tensor:
+    """a [M,K] fp32 (CUDA or CPU), w [N,K] fp32 CPU -> a @ w.T [M,N] fp32 on a's device, by the tensor-core kernel."""
+    a = a.contiguous()
+    w = w.contiguous().cpu()
+    c = torch.empty((a.shape[0], w.shape[0]), dtype=torch.float32, device=a.device)
+    _check(lib().boa_debug_gemm(_ptr(a), a.shape[0], a.shape[1], _ptr(w), w.shape[0], weight_pieces, tile_n, _ptr(c),
+                                _stream()), "boa_debug_gemm")
+    return c
 
 
 def debug_quantise(logits: torch.Tensor) -> torch.Tensor:

@@ -16,6 +16,7 @@
 #include "common.cuh"
 #include "container.h"
 #include "model_kernels.cuh"
+#include "tc_gemm.cuh"
 
 using namespace boa;
 
@@ -23,7 +24,6 @@ namespace {
 
 constexpr int kStepsPerGraph = 32;       // model steps captured into one CUDA graph launch
 constexpr uint64_t kMaxWaveStreams = 65536;  // streams stepped together; more chunks run in waves
-constexpr int kConvxTS = 8;              // streams per k_convx CTA
 constexpr int kScanSPC = 8;              // streams per k_scan CTA
 
 struct GrowBuf {   // grow-only device buffer
@@ -43,8 +43,9 @@ struct GrowBuf {   // grow-only device buffer
 };
 
 struct LayerW {
-  const float *norm_w, *w_in, *conv_b, *w_x, *w_dtT, *b_dt, *d_skip, *w_out;
+  const float *norm_w, *conv_b, *w_dtT, *b_dt, *d_skip;
   const float4 *conv_w, *A4;
+  const uint16_t *img_in, *img_x, *img_out;   // tensor-core weight images (tc_gemm.cuh)
 };
 
 bool is_device_ptr(const void* p) {
@@ -58,14 +59,17 @@ bool is_device_ptr(const void* p) {
 
 struct boa_model {
   int L = 0, D = 0, E = 0, R = 0, J = 0;
+  int npw = 3;                 // bf16 pieces per weight: 3 for fp32 blobs, 1 for bf16 blobs (exact)
+  int ldj = 64;                // row stride of the x_proj output = its tile width (64 or 128)
   uint32_t blob_crc = 0;
-  GrowBuf weights;
+  GrowBuf weights, wimg;
   const float* emb = nullptr;
+  const uint16_t* img_head = nullptr;
   std::vector<LayerW> layers;
 
   // workspace (per wave of Bcap streams)
   uint64_t Bcap = 0;
-  GrowBuf u, xz, xs, delta, bc, y, logits, h, win;
+  GrowBuf u, xz, dbc, y, logits, h, win;
   GrowBuf pos, len, low, range, pending, wpos, cache, started, v, rpos, off, size, scratch, first, err;
   GrowBuf stage_in, stage_out;
 
@@ -80,7 +84,7 @@ struct boa_model {
   std::vector<cudaEvent_t> events;
 
   ~boa_model() {
-    for (GrowBuf* b : {&weights, &u, &xz, &xs, &delta, &bc, &y, &logits, &h, &win, &pos, &len, &low, &range,
+    for (GrowBuf* b : {&weights, &wimg, &u, &xz, &dbc, &y, &logits, &h, &win, &pos, &len, &low, &range,
                        &pending, &wpos, &cache, &started, &v, &rpos, &off, &size, &scratch, &first, &err,
                        &stage_in, &stage_out})
       b->release();
@@ -98,6 +102,40 @@ float bf16_to_f32(uint16_t b) {
   float f;
   memcpy(&f, &u, 4);
   return f;
+}
+
+uint16_t f32_to_bf16_rne(float f) {
+  uint32_t u;
+  memcpy(&u, &f, 4);
+  if ((u & 0x7FFFFFFFu) > 0x7F800000u) return 0x7FC0;     // NaN
+  u += 0x7FFFu + ((u >> 16) & 1u);
+  return (uint16_t)(u >> 16);
+}
+
+// Tensor-core weight image of W[N][K] (tc_gemm.cuh): [ceil(N/BN)][K/64][npw] tiles of BN x 64 bf16 in the
+// K-major 128-byte-swizzled shared-memory layout; piece p of w is bf16(w - sum of the earlier pieces).
+// Rows >= N are zero.  Returns the offset (in uint16) of the image inside `img`.
+size_t append_w_image(const float* W, size_t N, size_t K, int BN, int npw, std::vector<uint16_t>& img) {
+  const size_t NT = (N + BN - 1) / BN, KB = K / 64, tile = (size_t)BN * 64;
+  const size_t off = img.size();
+  img.resize(off + NT * KB * npw * tile, 0);
+  uint16_t* base = img.data() + off;
+  for (size_t nt = 0; nt < NT; ++nt)
+    for (size_t kb = 0; kb < KB; ++kb)
+      for (size_t n = 0; n < (size_t)BN; ++n) {
+        const size_t row = nt * BN + n;
+        if (row >= N) continue;
+        for (size_t k = 0; k < 64; ++k) {
+          float r = W[row * K + kb * 64 + k];
+          const size_t o = (n / 8) * 512 + (n % 8) * 64 + (((k / 8) ^ (n % 8)) * 8) + (k % 8);
+          for (int p = 0; p < npw; ++p) {
+            const uint16_t b = f32_to_bf16_rne(r);
+            base[((nt * KB + kb) * npw + p) * tile + o] = b;
+            r -= bf16_to_f32(b);
+          }
+        }
+      }
+  return off;
 }
 
 struct BlobReader {
@@ -160,16 +198,38 @@ int mark(StepCtx& c, int cls) {
   return BOA_OK;
 }
 
-template <bool NORM, bool RESID>
-void launch_sgemm(const float* A, int lda, const float* W, int ldw, const float* norm_w, float* C, int ldc,
-                  int M, int N, int K, cudaStream_t st) {
-  if (M >= 2048) {
-    dim3 grid((M + 127) / 128, N / 64);
-    k_sgemm_nt<128, 64, 8, 4, NORM, RESID><<<grid, 256, 0, st>>>(A, lda, W, ldw, norm_w, C, ldc, M, N, K);
-  } else {
-    dim3 grid((M + 63) / 64, N / 64);
-    k_sgemm_nt<64, 64, 4, 4, NORM, RESID><<<grid, 256, 0, st>>>(A, lda, W, ldw, norm_w, C, ldc, M, N, K);
-  }
+// ---- tensor-core GEMM launch (tc_gemm.cuh).  The dynamic shared-memory opt-in is set once per instantiation.
+template <int BN, int NPW, int EPI>
+int launch_tc(const tc::GemmArgs& g, int N, cudaStream_t st) {
+  using C = tc::Cfg<BN, NPW>;
+  dim3 grid((g.M + tc::BM - 1) / tc::BM, (N + BN - 1) / BN);
+  tc::k_tc_gemm<BN, NPW, EPI><<<grid, 160, C::SMEM, st>>>(g);
+  return BOA_OK;
+}
+template <int BN, int NPW, int EPI>
+int optin_tc() {
+  BOA_CUDA_TRY(cudaFuncSetAttribute(tc::k_tc_gemm<BN, NPW, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                    tc::Cfg<BN, NPW>::SMEM));
+  return BOA_OK;
+}
+// Shared-memory opt-ins of every kernel instantiation the step can launch (called by boa_model_load, outside
+// any stream capture).
+int init_kernels() {
+  BOA_TRY((optin_tc<128, 1, tc::EPI_INPROJ>()));
+  BOA_TRY((optin_tc<128, 3, tc::EPI_INPROJ>()));
+  BOA_TRY((optin_tc<128, 1, tc::EPI_STORE>()));
+  BOA_TRY((optin_tc<128, 3, tc::EPI_STORE>()));
+  BOA_TRY((optin_tc<64, 1, tc::EPI_STORE>()));
+  BOA_TRY((optin_tc<64, 3, tc::EPI_STORE>()));
+  BOA_TRY((optin_tc<64, 1, tc::EPI_RESID>()));
+  BOA_TRY((optin_tc<64, 3, tc::EPI_RESID>()));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<kScanSPC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 256 * 4));
+  return BOA_OK;
+}
+
+template <int BN, int EPI>
+int launch_tc_npw(int npw, const tc::GemmArgs& g, int N, cudaStream_t st) {
+  return npw == 1 ? launch_tc<BN, 1, EPI>(g, N, st) : launch_tc<BN, 3, EPI>(g, N, st);
 }
 
 // One model step + one coder step for all B streams of the wave (S1-S14).
@@ -178,9 +238,7 @@ int launch_step(StepCtx& c) {
   const int B = c.B, D = m->D, E = m->E;
   float* u = m->u.as<float>();
   float* xz = m->xz.as<float>();
-  float* xs = m->xs.as<float>();
-  float* delta = m->delta.as<float>();
-  float* bc = m->bc.as<float>();
+  float* dbc = m->dbc.as<float>();
   float* y = m->y.as<float>();
   float* logits = m->logits.as<float>();
 
@@ -195,26 +253,44 @@ int launch_step(StepCtx& c) {
     const LayerW& w = m->layers[l];
     float* hl = m->h.as<float>() + (size_t)l * m->Bcap * E * kNState;
     float* winl = m->win.as<float>() + (size_t)l * m->Bcap * 3 * E;
-    launch_sgemm<true, false>(u, D, w.w_in, D, w.norm_w, xz, 2 * E, B, 2 * E, D, c.st);
-    BOA_TRY(mark(c, BOA_K_INPROJ));
-    {
-      const size_t smem = (size_t)kConvxTS * (E + m->J) * sizeof(float);
-      k_convx<kConvxTS><<<(B + kConvxTS - 1) / kConvxTS, E, smem, c.st>>>(
-          xz, winl, w.conv_w, w.conv_b, w.w_x, w.w_dtT, w.b_dt, xs, delta, bc, B, E, m->R);
+    {  // S2-S4: xz = [SiLU(conv(W_in_x r)) ; W_in_z r],  r = RMSNorm(u)
+      tc::GemmArgs g{};
+      g.A = u; g.lda = D; g.M = B; g.K = D; g.colscale = w.norm_w; g.W = w.img_in;
+      g.C = xz; g.ldc = 2 * E; g.n_valid = 2 * E;
+      g.win = winl; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
+      BOA_TRY((launch_tc_npw<128, tc::EPI_INPROJ>(m->npw, g, 2 * E, c.st)));
+      BOA_TRY(mark(c, BOA_K_INPROJ));
+    }
+    {  // S5: [dlt;Bv;Cv] = W_x xs
+      tc::GemmArgs g{};
+      g.A = xz; g.lda = 2 * E; g.M = B; g.K = E; g.W = w.img_x;
+      g.C = dbc; g.ldc = m->ldj; g.n_valid = m->J;
+      if (m->ldj == 64) BOA_TRY((launch_tc_npw<64, tc::EPI_STORE>(m->npw, g, 64, c.st)));
+      else BOA_TRY((launch_tc_npw<128, tc::EPI_STORE>(m->npw, g, 128, c.st)));
       BOA_TRY(mark(c, BOA_K_CONVX));
     }
-    {
+    {  // S6-S8
       const int bd = std::min(E, 256);
       dim3 grid((B + kScanSPC - 1) / kScanSPC, E / bd);
-      k_scan<kScanSPC><<<grid, bd, 0, c.st>>>(reinterpret_cast<float4*>(hl), delta, xs, xz, bc, w.A4, w.d_skip,
-                                              y, B, E);
+      k_scan<kScanSPC><<<grid, bd, (size_t)m->R * bd * sizeof(float), c.st>>>(
+          reinterpret_cast<float4*>(hl), xz, dbc, m->ldj, w.w_dtT, w.b_dt, w.A4, w.d_skip, y, B, E, m->R);
       BOA_TRY(mark(c, BOA_K_SCAN));
     }
-    launch_sgemm<false, true>(y, E, w.w_out, E, nullptr, u, D, B, D, E, c.st);
-    BOA_TRY(mark(c, BOA_K_OUTPROJ));
+    {  // S9: u += W_out y
+      tc::GemmArgs g{};
+      g.A = y; g.lda = E; g.M = B; g.K = E; g.W = w.img_out;
+      g.C = u; g.ldc = D; g.n_valid = D;
+      BOA_TRY((launch_tc_npw<64, tc::EPI_RESID>(m->npw, g, D, c.st)));
+      BOA_TRY(mark(c, BOA_K_OUTPROJ));
+    }
   }
-  launch_sgemm<false, false>(u, D, m->emb, D, nullptr, logits, 256, B, 256, D, c.st);
-  BOA_TRY(mark(c, BOA_K_HEAD));
+  {  // S10: logits = Emb u
+    tc::GemmArgs g{};
+    g.A = u; g.lda = D; g.M = B; g.K = D; g.W = m->img_head;
+    g.C = logits; g.ldc = 256; g.n_valid = 256;
+    BOA_TRY((launch_tc_npw<64, tc::EPI_STORE>(m->npw, g, 256, c.st)));
+    BOA_TRY(mark(c, BOA_K_HEAD));
+  }
 
   const int cgrid = (B * 32 + 255) / 256;
   if (c.dump) {
@@ -306,7 +382,7 @@ int run_steps(StepCtx& c, uint64_t steps) {
 // ------------------------------------------------------------------------------------- workspace
 size_t bytes_per_stream(const boa_model* m, size_t cap) {
   const size_t E = m->E, D = m->D;
-  return 4 * (D + 2 * E + 3 * E + 32 + 256) + (size_t)m->L * 4 * (E * kNState + 3 * E) + 64 + cap;
+  return 4 * (D + 2 * E + E + 128 + 256) + (size_t)m->L * 4 * (E * kNState + 3 * E) + 64 + cap;
 }
 
 int reserve_workspace(boa_model* m, uint64_t B, size_t cap) {
@@ -315,9 +391,7 @@ int reserve_workspace(boa_model* m, uint64_t B, size_t cap) {
     // state arrays are indexed [l][Bcap][...]: growing B invalidates nothing (state is reset per wave)
     BOA_TRY(m->u.reserve(B * D * 4));
     BOA_TRY(m->xz.reserve(B * 2 * E * 4));
-    BOA_TRY(m->xs.reserve(B * E * 4));
-    BOA_TRY(m->delta.reserve(B * E * 4));
-    BOA_TRY(m->bc.reserve(B * 32 * 4));
+    BOA_TRY(m->dbc.reserve(B * (size_t)m->ldj * 4));
     BOA_TRY(m->y.reserve(B * E * 4));
     BOA_TRY(m->logits.reserve(B * 256 * 4));
     BOA_TRY(m->h.reserve(L * B * E * kNState * 4));
@@ -454,31 +528,36 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
   if (!m) return BOA_E_NOMEM;
   m->L = (int)L; m->D = (int)D; m->E = (int)E; m->R = (int)R; m->J = (int)J;
   m->blob_crc = crc32_ieee(p, nbytes);
+  m->npw = dtype == 1 ? 1 : 3;         // a bf16 weight is one exact piece; an fp32 weight is cut into three
+  m->ldj = J <= 64 ? 64 : 128;
 
-  // host image of the device weight buffer (all fp32; bf16 matrices are widened exactly, R#13)
-  const size_t per_layer = D + 2 * E * D + 4 * E + E + J * E + E * R + E + E * kNState + E + D * E;
+  // host image of the device buffers: small fp32 tensors (img) and the tensor-core images of the matrices (wimg);
+  // bf16 matrices are widened exactly (R#13)
+  const size_t per_layer = D + 4 * E + E + E * R + E + E * kNState + E;
   std::vector<float> img;
+  std::vector<uint16_t> wimg;
   img.reserve(256 * D + L * per_layer + 64);
+  wimg.reserve(((size_t)256 * D + L * (2 * E * D + (size_t)m->ldj * E + D * E)) * m->npw + 64);
   auto append = [&](const std::vector<float>& v) {
     size_t o = img.size();
     img.insert(img.end(), v.begin(), v.end());
     while (img.size() % 4) img.push_back(0.0f);   // keep every tensor 16-byte aligned
     return o;
   };
-  struct Off { size_t norm_w, w_in, conv_w, conv_b, w_x, w_dtT, b_dt, A4, d_skip, w_out; };
+  struct Off { size_t norm_w, conv_w, conv_b, w_dtT, b_dt, A4, d_skip, img_in, img_x, img_out; };
   std::vector<Off> offs(L);
   BlobReader br{p, nbytes, 64, (int)dtype};
   std::vector<float> t, t2;
   bool ok = br.take(256 * (size_t)D, true, t);
-  size_t emb_off = 0;
-  if (ok) emb_off = append(t);
+  size_t emb_off = 0, head_off = 0;
+  if (ok) { emb_off = append(t); head_off = append_w_image(t.data(), 256, D, 64, m->npw, wimg); }
   for (uint32_t l = 0; l < L && ok; ++l) {
     Off& o = offs[l];
     ok = ok && br.take(D, false, t); if (ok) o.norm_w = append(t);
-    ok = ok && br.take(2 * E * D, true, t); if (ok) o.w_in = append(t);
+    ok = ok && br.take(2 * E * D, true, t); if (ok) o.img_in = append_w_image(t.data(), 2 * E, D, 128, m->npw, wimg);
     ok = ok && br.take(E * 4, false, t); if (ok) o.conv_w = append(t);        // [E][4] = one float4 per channel
     ok = ok && br.take(E, false, t); if (ok) o.conv_b = append(t);
-    ok = ok && br.take(J * E, true, t); if (ok) o.w_x = append(t);
+    ok = ok && br.take(J * E, true, t); if (ok) o.img_x = append_w_image(t.data(), J, E, m->ldj, m->npw, wimg);
     ok = ok && br.take(E * R, true, t);
     if (ok) {                                                                 // W_dt [E][R] -> transposed [R][E]
       t2.assign(E * R, 0.0f);
@@ -496,11 +575,13 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
       o.A4 = append(t2);
     }
     ok = ok && br.take(E, false, t); if (ok) o.d_skip = append(t);
-    ok = ok && br.take(D * E, true, t); if (ok) o.w_out = append(t);
+    ok = ok && br.take(D * E, true, t); if (ok) o.img_out = append_w_image(t.data(), D, E, 64, m->npw, wimg);
   }
   if (!ok || br.off != nbytes) { delete m; return BOA_E_FORMAT; }
 
   int rc = m->weights.reserve(img.size() * sizeof(float));
+  if (rc == BOA_OK) rc = m->wimg.reserve(wimg.size() * sizeof(uint16_t));
+  if (rc == BOA_OK) rc = init_kernels();
   if (rc == BOA_OK && (cudaStreamCreateWithFlags(&m->own, cudaStreamNonBlocking) != cudaSuccess ||
                        cudaEventCreateWithFlags(&m->user_ev, cudaEventDisableTiming) != cudaSuccess)) {
     (void)cudaGetLastError();
@@ -510,16 +591,23 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
     (void)cudaGetLastError();
     rc = BOA_E_CUDA;
   }
+  if (rc == BOA_OK && cudaMemcpy(m->wimg.p, wimg.data(), wimg.size() * sizeof(uint16_t), cudaMemcpyHostToDevice) != cudaSuccess) {
+    (void)cudaGetLastError();
+    rc = BOA_E_CUDA;
+  }
   if (rc != BOA_OK) { delete m; return rc; }
   const float* base = m->weights.as<float>();
+  const uint16_t* wbase = m->wimg.as<uint16_t>();
   m->emb = base + emb_off;
+  m->img_head = wbase + head_off;
   m->layers.resize(L);
   for (uint32_t l = 0; l < L; ++l) {
     const Off& o = offs[l];
     LayerW& w = m->layers[l];
-    w.norm_w = base + o.norm_w; w.w_in = base + o.w_in; w.conv_w = reinterpret_cast<const float4*>(base + o.conv_w);
-    w.conv_b = base + o.conv_b; w.w_x = base + o.w_x; w.w_dtT = base + o.w_dtT; w.b_dt = base + o.b_dt;
-    w.A4 = reinterpret_cast<const float4*>(base + o.A4); w.d_skip = base + o.d_skip; w.w_out = base + o.w_out;
+    w.norm_w = base + o.norm_w; w.conv_w = reinterpret_cast<const float4*>(base + o.conv_w);
+    w.conv_b = base + o.conv_b; w.w_dtT = base + o.w_dtT; w.b_dt = base + o.b_dt;
+    w.A4 = reinterpret_cast<const float4*>(base + o.A4); w.d_skip = base + o.d_skip;
+    w.img_in = wbase + o.img_in; w.img_x = wbase + o.img_x; w.img_out = wbase + o.img_out;
   }
   *out = m;
   return BOA_OK;
@@ -816,6 +904,40 @@ int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_
   BOA_TRY(tc.finish(st));
   BOA_CUDA_TRY(cudaStreamSynchronize(st));
   return BOA_OK;
+}
+
+int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N, int weight_pieces, int tile_n,
+                   float* C, void* cuda_stream) {
+  if (!A || !W || !C || M == 0 || N == 0 || K == 0 || K % 64 != 0 || (weight_pieces != 1 && weight_pieces != 3) ||
+      (tile_n != 64 && tile_n != 128) || M >= (1u << 30) || N >= (1u << 20) || K >= (1u << 20))
+    return BOA_E_ARG;
+  BOA_TRY(check_device());
+  BOA_TRY(init_kernels());
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const size_t Np = round_up(N, (size_t)tile_n);
+  std::vector<uint16_t> img;
+  append_w_image(W, N, K, tile_n, weight_pieces, img);
+  TmpDev ta, tw, tc_;
+  BOA_TRY(ta.init(A, M * K * 4, true, false, st));
+  BOA_TRY(tw.init(img.data(), img.size() * 2, true, false, st));
+  // the kernel stores whole 4-column groups of a row: give it a padded C and copy the valid columns out
+  void* cpad = nullptr;
+  if (cudaMalloc(&cpad, M * Np * 4) != cudaSuccess) { (void)cudaGetLastError(); return BOA_E_NOMEM; }
+  tc::GemmArgs g{};
+  g.A = static_cast<const float*>(ta.dev); g.lda = (int)K; g.M = (int)M; g.K = (int)K;
+  g.W = static_cast<const uint16_t*>(tw.dev);
+  g.C = static_cast<float*>(cpad); g.ldc = (int)Np; g.n_valid = (int)Np;
+  int rc = tile_n == 64 ? launch_tc_npw<64, tc::EPI_STORE>(weight_pieces, g, (int)Np, st)
+                        : launch_tc_npw<128, tc::EPI_STORE>(weight_pieces, g, (int)Np, st);
+  cudaError_t e = cudaGetLastError();
+  if (rc == BOA_OK && e != cudaSuccess) rc = note_cuda_error(e, __FILE__, __LINE__);
+  if (rc == BOA_OK) {
+    e = cudaMemcpy2DAsync(C, N * 4, cpad, Np * 4, N * 4, M, cudaMemcpyDefault, st);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) rc = note_cuda_error(e, __FILE__, __LINE__);
+  }
+  cudaFree(cpad);
+  return rc;
 }
 
 int boa_debug_quantise(const float* logits, size_t rows, uint32_t* cdf, void* cuda_stream) {

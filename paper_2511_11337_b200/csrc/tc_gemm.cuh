@@ -1,0 +1,359 @@
+// tc_gemm.cuh — the stream-batch contractions of the step on the 5th-generation tensor cores.
+//
+//   in_proj   xz = W_in RMSNorm(u)          S2+S3 (+ S4 conv1d+SiLU in the epilogue)   P:142; R#1, R#10, R#11
+//   x_proj    [dlt;Bv;Cv] = W_x xs          S5                                         eq. 21-22
+//   out_proj  u += W_out y                  S9                                         Alg. 1 l.3
+//   head      logits = Emb u                S10                                        Alg. 1 l.5
+//
+// One CTA computes a 128-stream x BN tile:  C[m][n] = sum_k A[m][k] * W[n][k].
+//
+// Precision.  The activations are fp32 and the four parity checks need
+// fp32-level products, so each operand is cut into bf16 pieces that sum to it exactly (a = a1+a2+a3, 8 significant
+// bits each) and the tensor cores multiply the pieces: tcgen05.mma kind::f16 (bf16 x bf16 -> fp32 in TMEM).
+//   bf16 weights (one exact piece w):   a1 w | a2 w + a3 w                               3 MMAs per k-step
+//   fp32 weights (w = w1+w2+w3):        a1 w1 | a1 w3 + a3 w1 + a2 w2 + a1 w2 + a2 w1    6 MMAs per k-step
+// The leading product has its own TMEM accumulator; all correction products (2^-8 and smaller) go to a second one and
+// the two are added once, in fp32, in the epilogue.  Dropped products are below 2^-24 of |a||w|.
+//
+// Data movement.  The weight pieces are cut and laid out once, at boa_model_load, as the exact shared-memory image of
+// a tile (K-major, 128-byte swizzle): a stage's weight tile is ONE contiguous block that the bulk-copy engine (TMA,
+// cp.async.bulk -> SASS UBLKCP) drops into shared memory, signalling an mbarrier.  The activation tile is loaded by
+// four producer warps (coalesced 128-bit loads from L2), cut into pieces in registers and stored in the same swizzled
+// layout.  One elected thread issues the MMAs; tcgen05.commit releases the stage.  The producer warps then become the
+// epilogue: tcgen05.ld (one TMEM lane = one stream per thread), fused epilogue, 128-byte row segments to global.
+//
+// Determinism: row m of the result depends only on row m of A, on W and on a fixed issue order; it does not
+// depend on M, on the tile the stream falls in, or on encode vs decode.
+#pragma once
+#include "common.cuh"
+
+namespace boa {
+namespace tc {
+
+constexpr int BM = 128;          // streams per tile = TMEM lanes
+constexpr int BK = 64;           // k per stage: 64 bf16 = one 128-byte swizzle row
+constexpr int NPA = 3;           // bf16 pieces of an activation
+constexpr int A_PLANE = BM * 128;  // bytes of one activation piece tile
+
+enum { EPI_STORE = 0, EPI_RESID = 1, EPI_INPROJ = 2 };
+
+struct GemmArgs {
+  const float* A;          // [M][lda] fp32 activations (row = stream)
+  int lda, M, K;           // K % 64 == 0
+  const float* colscale;   // [K] or nullptr: A[m][k] is multiplied by colscale[k] before it is cut (RMSNorm weight)
+  const uint16_t* W;       // weight image [N/BN][K/64][NPW][BN x 64 bf16, swizzled]
+  float* C;                // [M][ldc]
+  int ldc, n_valid;        // columns >= n_valid are not stored (zero-padded weight rows)
+  // EPI_INPROJ only
+  float* win;              // [M][3][E] conv window of this layer
+  const float4* conv_w;    // [E] taps (x = t-3 ... w = t)
+  const float* conv_b;     // [E]
+  int E;
+};
+
+// ------------------------------------------------------------------------------------------ PTX wrappers
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_barrier_init() { asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory"); }
+__device__ __forceinline__ void mbar_arrive(uint32_t bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}" ::"r"(bar), "r"(parity) : "memory");
+}
+// global -> shared bulk copy by the TMA engine; completes `bytes` on the mbarrier
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+// generic-proxy shared stores -> visible to the async proxy (tensor core operand reads)
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
+__device__ __forceinline__ void tc_fence_after() { asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory"); }
+
+__device__ __forceinline__ void tmem_alloc(uint32_t dst_smem, uint32_t ncols) {   // whole warp
+  asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(dst_smem), "r"(ncols) : "memory");
+  asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_dealloc(uint32_t taddr, uint32_t ncols) {    // whole warp
+  asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(taddr), "r"(ncols) : "memory");
+}
+
+// D[tmem] (+)= A[smem] * B[smem]^T, bf16 inputs, fp32 accumulate; one thread issues for the CTA
+__device__ __forceinline__ void umma(uint32_t d_tmem, uint64_t adesc, uint64_t bdesc, uint32_t idesc, uint32_t accumulate) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "setp.ne.b32 p, %4, 0;\n"
+      "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n"
+      "}" ::"r"(d_tmem), "l"(adesc), "l"(bdesc), "r"(idesc), "r"(accumulate) : "memory");
+}
+// arrive on the mbarrier when every MMA issued so far by this thread has completed
+__device__ __forceinline__ void umma_commit(uint32_t bar) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+
+// 32 consecutive fp32 columns of this thread's TMEM lane
+__device__ __forceinline__ void tmem_ld32(uint32_t taddr, float (&v)[32]) {
+  uint32_t r[32];
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x32.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15, "
+      "%16, %17, %18, %19, %20, %21, %22, %23, %24, %25, %26, %27, %28, %29, %30, %31}, [%32];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]),
+        "=r"(r[8]), "=r"(r[9]), "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]),
+        "=r"(r[16]), "=r"(r[17]), "=r"(r[18]), "=r"(r[19]), "=r"(r[20]), "=r"(r[21]), "=r"(r[22]), "=r"(r[23]),
+        "=r"(r[24]), "=r"(r[25]), "=r"(r[26]), "=r"(r[27]), "=r"(r[28]), "=r"(r[29]), "=r"(r[30]), "=r"(r[31])
+      : "r"(taddr) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]);
+}
+
+// Shared-memory matrix descriptor: K-major operand, 128-byte swizzle, rows of 128 bytes, 8-row groups 1024 bytes
+// apart (SBO), descriptor version 1 (sm_100).  `addr` is a shared-window byte address.
+__device__ __forceinline__ uint64_t smem_desc_sw128(uint32_t addr) {
+  const uint32_t lo = ((addr & 0x3FFFFu) >> 4) | (1u << 16);             // start address | LBO (unused for swizzled K-major)
+  const uint32_t hi = (1024u >> 4) | (1u << 14) | (2u << 29);            // SBO | version | SWIZZLE_128B
+  return ((uint64_t)hi << 32) | lo;
+}
+// Instruction descriptor: D fp32, A and B bf16, both K-major, M = 128, N = n
+__host__ __device__ constexpr uint32_t idesc_bf16(int n) {
+  return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
+}
+
+// two floats -> packed bf16x2 (lo = first), round to nearest even; and the exact remainders
+__device__ __forceinline__ uint32_t cut2(float& a, float& b) {
+  uint32_t p;
+  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(p) : "f"(b), "f"(a));
+  a = __fsub_rn(a, __uint_as_float(p << 16));
+  b = __fsub_rn(b, __uint_as_float(p & 0xFFFF0000u));
+  return p;
+}
+
+template <int BN, int NPW>
+struct Cfg {
+  static constexpr int W_PLANE = BN * 128;
+  static constexpr int STAGE = NPA * A_PLANE + NPW * W_PLANE;
+  static constexpr int NST = (3 * STAGE <= 216 * 1024) ? 3 : 2;
+  static constexpr int SMEM = NST * STAGE + 1024;             // + alignment slack
+  static constexpr int TMEM_COLS = (2 * BN <= 32) ? 32 : (2 * BN <= 64) ? 64 : (2 * BN <= 128) ? 128 : (2 * BN <= 256) ? 256 : 512;
+};
+
+__device__ __forceinline__ float sigmoid_tc(float x) { return 1.0f / (1.0f + expf(-x)); }
+
+// ------------------------------------------------------------------------------------------ the kernel
+// grid = (ceil(M/128), N/BN), block = 160: warps 0-3 produce the activation pieces and then run the epilogue,
+// warp 4 owns TMEM and its lane 0 issues the MMAs.  Thread 0 also starts the weight bulk copies.
+template <int BN, int NPW, int EPI>
+__global__ void __launch_bounds__(160, 1) k_tc_gemm(const GemmArgs g) {
+  using C = Cfg<BN, NPW>;
+  static_assert(BN % 32 == 0 && BN >= 32 && BN <= 128, "tile N");
+  static_assert(NPW == 1 || NPW == 3, "weight pieces");
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t full_bar[C::NST], empty_bar[C::NST], acc_bar;
+  __shared__ uint32_t tmem_base_s;
+  __shared__ float rstd_s[BM];
+
+  const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+  const int m0 = blockIdx.x * BM;
+  const int n0 = blockIdx.y * BN;
+  const int KB = g.K / BK;
+  const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+
+  if (warp == 4) {
+    if (lane == 0) {
+      for (int s = 0; s < C::NST; ++s) {
+        mbar_init(smem_u32(&full_bar[s]), 129);   // 128 producer threads + the expect_tx arrival of thread 0
+        mbar_init(smem_u32(&empty_bar[s]), 1);    // one tcgen05.commit
+      }
+      mbar_init(smem_u32(&acc_bar), 1);
+      fence_barrier_init();
+    }
+    __syncwarp();
+    tmem_alloc(smem_u32(&tmem_base_s), C::TMEM_COLS);
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem = tmem_base_s;
+
+  if (warp < 4) {
+    // ===================================================================== producers
+    const int c = tid & 7;                       // 16-byte chunk (8 k) of the 128-byte row
+    const int r7 = (tid >> 3) & 7;               // row within the 8-row swizzle group
+    const uint32_t soff = (uint32_t)((tid >> 6) * 1024 + r7 * 128 + ((c ^ r7) << 4));
+    float ss[8];
+#pragma unroll
+    for (int it = 0; it < 8; ++it) ss[it] = 0.0f;
+    const uint16_t* wsrc = g.W + (size_t)blockIdx.y * KB * (NPW * BN * 64);
+
+    for (int kb = 0; kb < KB; ++kb) {
+      const int s = kb % C::NST, round = kb / C::NST;
+      if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
+      const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
+      if (tid == 0) {
+        const uint32_t fb = smem_u32(&full_bar[s]);
+        mbar_arrive_expect_tx(fb, (uint32_t)(NPW * C::W_PLANE));
+#pragma unroll
+        for (int q = 0; q < NPW; ++q)
+          bulk_g2s(sA + NPA * A_PLANE + q * C::W_PLANE, wsrc + ((size_t)kb * NPW + q) * (BN * 64), (uint32_t)C::W_PLANE, fb);
+      }
+      float4 va[8], vb[8];
+#pragma unroll
+      for (int it = 0; it < 8; ++it) {
+        const int row = it * 16 + (tid >> 3);
+        const float4* src = reinterpret_cast<const float4*>(g.A + (size_t)min(m0 + row, g.M - 1) * g.lda + kb * BK + c * 8);
+        va[it] = src[0];
+        vb[it] = src[1];
+      }
+      float4 sc0 = make_float4(1.f, 1.f, 1.f, 1.f), sc1 = sc0;
+      if (g.colscale) {
+        const float4* sp = reinterpret_cast<const float4*>(g.colscale + kb * BK + c * 8);
+        sc0 = sp[0];
+        sc1 = sp[1];
+      }
+#pragma unroll
+      for (int it = 0; it < 8; ++it) {
+        float v[8] = {va[it].x, va[it].y, va[it].z, va[it].w, vb[it].x, vb[it].y, vb[it].z, vb[it].w};
+        if (EPI == EPI_INPROJ) {
+#pragma unroll
+          for (int j = 0; j < 8; ++j) ss[it] = fmaf(v[j], v[j], ss[it]);
+        }
+        if (g.colscale) {
+          v[0] *= sc0.x; v[1] *= sc0.y; v[2] *= sc0.z; v[3] *= sc0.w;
+          v[4] *= sc1.x; v[5] *= sc1.y; v[6] *= sc1.z; v[7] *= sc1.w;
+        }
+        const uint32_t dst = sA + (uint32_t)it * 2048u + soff;
+#pragma unroll
+        for (int p = 0; p < NPA; ++p) {
+          uint4 w;
+          w.x = cut2(v[0], v[1]); w.y = cut2(v[2], v[3]); w.z = cut2(v[4], v[5]); w.w = cut2(v[6], v[7]);
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst + p * A_PLANE), "r"(w.x), "r"(w.y), "r"(w.z), "r"(w.w) : "memory");
+        }
+      }
+      fence_proxy_async();
+      mbar_arrive(smem_u32(&full_bar[s]));
+    }
+
+    // ===================================================================== epilogue
+    if (EPI == EPI_INPROJ) {
+#pragma unroll
+      for (int it = 0; it < 8; ++it) {
+        float v = ss[it];
+        v += __shfl_xor_sync(0xffffffffu, v, 1);
+        v += __shfl_xor_sync(0xffffffffu, v, 2);
+        v += __shfl_xor_sync(0xffffffffu, v, 4);
+        if (c == 0) rstd_s[it * 16 + (tid >> 3)] = 1.0f / sqrtf(v / (float)g.K + kEps);
+      }
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+    }
+    mbar_wait(smem_u32(&acc_bar), 0u);
+    tc_fence_after();
+    const int row = m0 + tid;
+    const bool live = row < g.M;
+    const uint32_t tlane = tmem + ((uint32_t)(warp * 32) << 16);
+    const float rs = (EPI == EPI_INPROJ) ? rstd_s[tid] : 1.0f;
+#pragma unroll 1
+    for (int ch = 0; ch < BN / 32; ++ch) {
+      float v[32], w[32];
+      tmem_ld32(tlane + (uint32_t)(ch * 32), v);
+      tmem_ld32(tlane + (uint32_t)(BN + ch * 32), w);
+#pragma unroll
+      for (int j = 0; j < 32; ++j) v[j] = (v[j] + w[j]) * rs;
+      const int nb = n0 + ch * 32;
+      if (!live) continue;
+      float* cp = g.C + (size_t)row * g.ldc + nb;
+      if (EPI == EPI_INPROJ && nb < g.E) {
+        // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU; the window moves one step (R#11)
+        float* wp = g.win + (size_t)row * 3 * g.E + nb;
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) {
+          const float4 w0 = *reinterpret_cast<const float4*>(wp + j);
+          const float4 w1 = *reinterpret_cast<const float4*>(wp + g.E + j);
+          const float4 w2 = *reinterpret_cast<const float4*>(wp + 2 * g.E + j);
+          const float a0[4] = {w0.x, w0.y, w0.z, w0.w}, a1[4] = {w1.x, w1.y, w1.z, w1.w}, a2[4] = {w2.x, w2.y, w2.z, w2.w};
+          float o[4];
+#pragma unroll
+          for (int q = 0; q < 4; ++q) {
+            const float4 cw = __ldg(g.conv_w + nb + j + q);
+            float xc = fmaf(cw.w, v[j + q], __ldg(g.conv_b + nb + j + q));
+            xc = fmaf(cw.x, a0[q], xc);
+            xc = fmaf(cw.y, a1[q], xc);
+            xc = fmaf(cw.z, a2[q], xc);
+            o[q] = xc * sigmoid_tc(xc);
+          }
+          *reinterpret_cast<float4*>(wp + j) = w1;
+          *reinterpret_cast<float4*>(wp + g.E + j) = w2;
+          *reinterpret_cast<float4*>(wp + 2 * g.E + j) = make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+          *reinterpret_cast<float4*>(cp + j) = make_float4(o[0], o[1], o[2], o[3]);
+        }
+      } else {
+#pragma unroll
+        for (int j = 0; j < 32; j += 4) {
+          if (nb + j >= g.n_valid) break;
+          float4 o = make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]);
+          if (EPI == EPI_RESID) {
+            const float4 r = *reinterpret_cast<const float4*>(cp + j);
+            o.x += r.x; o.y += r.y; o.z += r.z; o.w += r.w;
+          }
+          *reinterpret_cast<float4*>(cp + j) = o;
+        }
+      }
+    }
+  } else if (lane == 0) {
+    // ===================================================================== MMA issuer
+    constexpr uint32_t idesc = idesc_bf16(BN);
+    for (int kb = 0; kb < KB; ++kb) {
+      const int s = kb % C::NST, round = kb / C::NST;
+      mbar_wait(smem_u32(&full_bar[s]), (uint32_t)(round & 1));
+      tc_fence_after();
+      const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
+      const uint32_t sW = sA + NPA * A_PLANE;
+#pragma unroll
+      for (int k4 = 0; k4 < BK / 16; ++k4) {
+        const uint32_t first = (kb | k4) ? 1u : 0u;
+        const uint32_t ko = (uint32_t)k4 * 32u;
+        auto A_ = [&](int p) { return smem_desc_sw128(sA + p * A_PLANE + ko); };
+        auto W_ = [&](int q) { return smem_desc_sw128(sW + q * C::W_PLANE + ko); };
+        umma(tmem, A_(0), W_(0), idesc, first);                 // leading product -> accumulator 0
+        if (NPW == 3) {                                         // corrections, smallest first -> accumulator 1
+          umma(tmem + BN, A_(0), W_(2), idesc, first);
+          umma(tmem + BN, A_(2), W_(0), idesc, 1u);
+          umma(tmem + BN, A_(1), W_(1), idesc, 1u);
+          umma(tmem + BN, A_(0), W_(1), idesc, 1u);
+          umma(tmem + BN, A_(1), W_(0), idesc, 1u);
+        } else {
+          umma(tmem + BN, A_(2), W_(0), idesc, first);
+          umma(tmem + BN, A_(1), W_(0), idesc, 1u);
+        }
+      }
+      umma_commit(smem_u32(&empty_bar[s]));                     // stage free when these MMAs have read it
+    }
+    umma_commit(smem_u32(&acc_bar));                            // accumulators complete
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 4) {
+    __syncwarp();
+    tmem_dealloc(tmem, C::TMEM_COLS);
+  }
+}
+
+}  // namespace tc
+}  // namespace boa

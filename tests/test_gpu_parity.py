@@ -65,6 +65,33 @@ def test_quantiser_bit_exact_on_given_logits(boa):
     assert np.all(f[903:906] == 256)
 
 
+# ------------------------------------------------------------------- the tensor-core contraction kernel alone
+def _to_bf16(x):
+    u = np.ascontiguousarray(x, np.float32).view(np.uint32).astype(np.uint64)
+    u = (u + 0x7FFF + ((u >> 16) & 1)) & 0xFFFF0000
+    return u.astype(np.uint32).view(np.float32)
+
+
+@pytest.mark.parametrize("pieces,tile_n", [(3, 64), (3, 128), (1, 64), (1, 128)])
+@pytest.mark.parametrize("M,N,K", [(300, 48, 512), (128, 256, 64), (1, 64, 256), (517, 320, 1024)])
+def test_tensor_core_gemm_against_fp64(boa, pieces, tile_n, M, N, K):
+    """C = A W^T by tcgen05 on bf16 pieces (tc_gemm.cuh) against numpy fp64 matmul: every product is kept to
+    ~2^-24, so the error is bounded by a few ulp of sum_k |a||w| (several tiles, ragged M, padded N)."""
+    g = np.random.Generator(np.random.PCG64(M * 7 + N * 3 + K + pieces))
+    a = (g.normal(0, 1.0, (M, K)) * np.exp(g.normal(0, 2.0, (M, 1)))).astype(np.float32)   # rows of very different scale
+    w = g.normal(0, 0.05, (N, K)).astype(np.float32)
+    if pieces == 1:
+        w = _to_bf16(w)                                             # a bf16 blob: one exact piece
+    want = a.astype(np.float64) @ w.astype(np.float64).T
+    scale = np.abs(a).astype(np.float64) @ np.abs(w).astype(np.float64).T
+    got = _np(boa.debug_gemm(torch.from_numpy(a).cuda(), torch.from_numpy(w), pieces, tile_n)).astype(np.float64)
+    err = np.abs(got - want) / scale
+    assert err.max() <= 2.0 ** -20, (err.max(), np.unravel_index(err.argmax(), err.shape))
+    # and from host pointers
+    got_h = _np(boa.debug_gemm(torch.from_numpy(a), torch.from_numpy(w), pieces, tile_n))
+    assert np.array_equal(got_h.astype(np.float64), got)
+
+
 # ---------------------------------------------------------------------------------------------- check 1
 @pytest.mark.parametrize("kind", ["uniform", "peaked", "random"])
 def test_range_coder_bit_exact_given_oracle_tables(boa, kind):
@@ -122,7 +149,7 @@ def test_range_coder_golden_vectors(boa):
 # ---------------------------------------------------------------------------------------- checks 2 and 5
 def test_probabilities_and_tables_against_oracle(case, boa):
     name, blob, cfg, gm, w = case
-    S, T = 5, 96                                                   # 5 streams: ragged vs the 8-stream tiles
+    S, T = 5, 96                                                   # 5 streams: a ragged 128-row tile
     data = np.frombuffer(cfg.data(S * T), np.uint8).reshape(S, T)
     d = gm.debug_step_dump(data.tobytes(), T, T - 1)
     logits64 = model.logits_for_chunks(w, data)
@@ -217,9 +244,9 @@ def test_result_independent_of_batch_and_position(boa):
     cfg = synth.CONFIGS[1]
     gm = boa.Model(cfg.weights(emb_std=0.25))
     chunk = 200
-    data = cfg.data(70 * chunk)                                    # 70 streams: two 64-row GEMM tiles
+    data = cfg.data(140 * chunk)                                   # 140 streams: two 128-row tensor-core tiles
     _, _, _, _, pa = container.unpack(_np(gm.compress(data, chunk)).tobytes())
-    for i in (0, 9, 63, 64, 69):
+    for i in (0, 9, 127, 128, 139):
         solo = gm.compress(data[i * chunk:(i + 1) * chunk], chunk)
         _, _, _, _, ps = container.unpack(_np(solo).tobytes())
         assert ps[0] == pa[i], i
