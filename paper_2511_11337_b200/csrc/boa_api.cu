@@ -24,7 +24,6 @@ namespace {
 
 constexpr int kStepsPerGraph = 32;       // model steps captured into one CUDA graph launch
 constexpr uint64_t kMaxWaveStreams = 65536;  // streams stepped together; more chunks run in waves
-constexpr int kScanSPC = 8;              // streams per k_scan CTA
 
 struct GrowBuf {   // grow-only device buffer
   void* p = nullptr;
@@ -61,6 +60,7 @@ struct boa_model {
   int L = 0, D = 0, E = 0, R = 0, J = 0;
   int npw = 3;                 // bf16 pieces per weight: 3 for fp32 blobs, 1 for bf16 blobs (exact)
   int ldj = 64;                // row stride of the x_proj output = its tile width (64 or 128)
+  int n_sm = 148;              // SM count of the device (persistent grids)
   uint32_t blob_crc = 0;
   GrowBuf weights, wimg;
   const float* emb = nullptr;
@@ -223,7 +223,7 @@ int init_kernels() {
   BOA_TRY((optin_tc<64, 3, tc::EPI_STORE>()));
   BOA_TRY((optin_tc<64, 1, tc::EPI_RESID>()));
   BOA_TRY((optin_tc<64, 3, tc::EPI_RESID>()));
-  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<kScanSPC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 256 * 4));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 64)));
   return BOA_OK;
 }
 
@@ -269,11 +269,13 @@ int launch_step(StepCtx& c) {
       else BOA_TRY((launch_tc_npw<128, tc::EPI_STORE>(m->npw, g, 128, c.st)));
       BOA_TRY(mark(c, BOA_K_CONVX));
     }
-    {  // S6-S8
-      const int bd = std::min(E, 256);
-      dim3 grid((B + kScanSPC - 1) / kScanSPC, E / bd);
-      k_scan<kScanSPC><<<grid, bd, (size_t)m->R * bd * sizeof(float), c.st>>>(
-          reinterpret_cast<float4*>(hl), xz, dbc, m->ldj, w.w_dtT, w.b_dt, w.A4, w.d_skip, y, B, E, m->R);
+    {  // S6-S8: persistent, two CTAs per SM, each walking over streams for one channel slice
+      ScanArgs sa{};
+      sa.h = hl; sa.xz = xz; sa.dbc = dbc; sa.W_dtT = w.w_dtT; sa.b_dt = w.b_dt; sa.A4 = w.A4; sa.Dskip = w.d_skip;
+      sa.y = y; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
+      const int ec = (E % 256 == 0) ? 256 : 128, slices = E / ec;
+      const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
+      k_scan<<<dim3(per_slice, slices), ec, scan::smem_bytes(ec, m->ldj, m->R), c.st>>>(sa);
       BOA_TRY(mark(c, BOA_K_SCAN));
     }
     {  // S9: u += W_out y
@@ -530,6 +532,12 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
   m->blob_crc = crc32_ieee(p, nbytes);
   m->npw = dtype == 1 ? 1 : 3;         // a bf16 weight is one exact piece; an fp32 weight is cut into three
   m->ldj = J <= 64 ? 64 : 128;
+  {
+    int dev = 0, n_sm = 0;
+    if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n_sm > 0)
+      m->n_sm = n_sm;
+    (void)cudaGetLastError();
+  }
 
   // host image of the device buffers: small fp32 tensors (img) and the tensor-core images of the matrices (wimg);
   // bf16 matrices are widened exactly (R#13)

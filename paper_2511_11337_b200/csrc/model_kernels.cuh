@@ -42,14 +42,31 @@ __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, con
 }
 
 // ---------------------------------------------------------------------------------------------------
-// S6-S8: one thread per (stream, channel) holds the 16 state values of that channel in registers.
+// S6-S8, the kernel that streams the SSM state (the only large object of the path) through the SM.
 //   delta = softplus(b_dt[e] + sum_r W_dt[e][r] dlt[r])                      (sequential fp32 FMA chain, r ascending)
 //   h[n] = exp(delta*A[n]) * h[n] + (delta*Bv[n]) * xs ;  y = sum_n Cv[n] h[n] + D xs ;  y *= SiLU(z)
-// State layout: h[i][j][e] is a float4 holding n = 4j..4j+3, so the 32
-// lanes of a warp read 512 contiguous bytes per load.  The state is the only large object on the
-// path and is touched once per step: it is loaded/stored with streaming (evict-first) hints so the
-// small activations stay in L2.  The next stream's state is prefetched while the current one is
-// being updated.  dbc[i][0..R) = dlt, [R..R+16) = Bv, [R+16..R+32) = Cv (x_proj output, row stride ldj).
+//
+// State layout: h[i][j][e] is a float4 holding n = 4j..4j+3, so the state of one
+// stream and a slice of EC channels is four contiguous runs of EC*16 bytes.  HBM-bound: per stream and slice the
+// kernel moves 2*EC*64 bytes of state against ~160 instructions per channel, so the design goal is bytes in
+// flight, not arithmetic: a persistent CTA owns a channel slice and walks over streams with a ring of NSTG shared
+// memory stages.  Everything a stream-step needs (4 state runs, xs, z, the x_proj row) is brought in by the
+// bulk-copy engine (TMA, cp.async.bulk -> UBLKCP) against one mbarrier per stage; threads touch shared memory
+// only; the updated state and y go back with bulk stores.  State copies carry an L2 evict-first policy so the
+// small activations stay resident in L2.
+// One thread per channel of the slice holds A[e][0..15] in registers; W_dt^T of the slice lives in shared memory.
+struct ScanArgs {
+  float* h;                 // [B][4][E] float4 (this layer)
+  const float* xz;          // [B][2E]: xs | z
+  const float* dbc;         // [B][ldj]: dlt[R] | Bv[16] | Cv[16]
+  const float* W_dtT;       // [R][E]
+  const float* b_dt;        // [E]
+  const float4* A4;         // [4][E] float4: A = -exp(A_log)
+  const float* Dskip;       // [E]
+  float* y;                 // [B][E]
+  int ldj, B, E, R;
+};
+
 __device__ __forceinline__ void scan_update4(float4& h, const float4 a, const float4 bv, const float4 cv,
                                              float dl, float x, float& y) {
   h.x = fmaf(expf(dl * a.x), h.x, (dl * bv.x) * x); y = fmaf(cv.x, h.x, y);
@@ -58,58 +75,134 @@ __device__ __forceinline__ void scan_update4(float4& h, const float4 a, const fl
   h.w = fmaf(expf(dl * a.w), h.w, (dl * bv.w) * x); y = fmaf(cv.w, h.w, y);
 }
 
-template <int SPC>
-__global__ void __launch_bounds__(256)
-k_scan(float4* __restrict__ h, const float* __restrict__ xz, const float* __restrict__ dbc, int ldj,
-       const float* __restrict__ W_dtT, const float* __restrict__ b_dt, const float4* __restrict__ A4,
-       const float* __restrict__ Dskip, float* __restrict__ y, int B, int E, int R) {
-  extern __shared__ float wdt_s[];                 // [R][blockDim.x] slice of W_dt^T for this CTA's channels
-  const int e = blockIdx.y * blockDim.x + threadIdx.x;
-  for (int r = 0; r < R; ++r) wdt_s[r * blockDim.x + threadIdx.x] = W_dtT[(size_t)r * E + e];
-  const float4 a0 = A4[e], a1 = A4[E + e], a2 = A4[2 * E + e], a3 = A4[3 * E + e];
-  const float dsk = Dskip[e];
-  const float bdt = b_dt[e];
-  const int i0 = blockIdx.x * SPC;
-  const int iend = min(i0 + SPC, B);
-  if (i0 >= B) return;
+namespace scan {
+constexpr int NSTG = 4;
+__host__ __device__ inline int stage_bytes(int EC, int ldj) { return EC * 64 + 3 * EC * 4 + ldj * 4; }   // h | xs | z | y | dbc
+__host__ __device__ inline int smem_bytes(int EC, int ldj, int R) { return NSTG * stage_bytes(EC, ldj) + R * EC * 4 + NSTG * 8 + 128; }
 
-  float4 n0, n1, n2, n3;
-  {
-    const float4* hp = h + (size_t)i0 * 4 * E + e;
-    n0 = __ldcs(hp); n1 = __ldcs(hp + E); n2 = __ldcs(hp + 2 * E); n3 = __ldcs(hp + 3 * E);
+__device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void bar_init(uint32_t bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void bar_expect(uint32_t bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bar_wait(uint32_t bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred P1;\n"
+      "LAB_WAIT:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 P1, [%0], %1;\n"
+      "@P1 bra DONE;\n"
+      "bra LAB_WAIT;\n"
+      "DONE:\n"
+      "}" ::"r"(bar), "r"(parity) : "memory");
+}
+__device__ __forceinline__ void g2s(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void g2s_hint(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint64_t pol) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint [%0], [%1], %2, [%3], %4;"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void s2g(void* dst, uint32_t src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void s2g_hint(void* dst, uint32_t src, uint32_t bytes, uint64_t pol) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group.L2::cache_hint [%0], [%1], %2, %3;"
+               ::"l"(dst), "r"(src), "r"(bytes), "l"(pol) : "memory");
+}
+}  // namespace scan
+
+// grid = (CTAs per slice, E / EC), block = EC = min(E, 256) threads, 2 CTAs per SM.
+__global__ void __launch_bounds__(256, 2) k_scan(const ScanArgs a) {
+  using namespace scan;
+  extern __shared__ __align__(128) uint8_t scan_smem[];
+  const int EC = blockDim.x, tid = threadIdx.x;
+  const int e0 = blockIdx.y * EC, e = e0 + tid;
+  const int SB = stage_bytes(EC, a.ldj);
+  uint8_t* stages = scan_smem;
+  float* wdt = reinterpret_cast<float*>(scan_smem + NSTG * SB);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(scan_smem + NSTG * SB + a.R * EC * 4);
+  const int nk = (a.B - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // streams of this CTA
+  if (nk <= 0) return;
+
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+  const uint32_t tx = (uint32_t)(EC * 64 + 2 * EC * 4 + a.ldj * 4);
+  auto issue_load = [&](int k) {   // thread 0
+    const int s = k % NSTG;
+    const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+    const uint32_t st = s_u32(stages + s * SB), bar = s_u32(&bars[s]);
+    bar_expect(bar, tx);
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      g2s_hint(st + j * EC * 16, a.h + ((i * 4 + j) * a.E + e0) * 4, (uint32_t)(EC * 16), bar, pol);
+    g2s(st + EC * 64, a.xz + i * 2 * a.E + e0, (uint32_t)(EC * 4), bar);
+    g2s(st + EC * 64 + EC * 4, a.xz + i * 2 * a.E + a.E + e0, (uint32_t)(EC * 4), bar);
+    g2s(st + EC * 64 + 3 * EC * 4, a.dbc + i * a.ldj, (uint32_t)(a.ldj * 4), bar);
+  };
+
+  if (tid == 0) {
+    for (int s = 0; s < NSTG; ++s) bar_init(s_u32(&bars[s]), 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
-  for (int i = i0; i < iend; ++i) {
-    float4 h0 = n0, h1 = n1, h2 = n2, h3 = n3;
-    if (i + 1 < iend) {
-      const float4* hp = h + (size_t)(i + 1) * 4 * E + e;
-      n0 = __ldcs(hp); n1 = __ldcs(hp + E); n2 = __ldcs(hp + 2 * E); n3 = __ldcs(hp + 3 * E);
-    }
-    const float x = xz[(size_t)i * 2 * E + e];
-    const float z = xz[(size_t)i * 2 * E + E + e];
-    const float* row = dbc + (size_t)i * ldj;
+  __syncthreads();
+  if (tid == 0)
+    for (int k = 0; k < NSTG && k < nk; ++k) issue_load(k);
+
+  for (int r = 0; r < a.R; ++r) wdt[r * EC + tid] = a.W_dtT[(size_t)r * a.E + e];   // private column: no sync needed
+  const float4 a0 = a.A4[e], a1 = a.A4[a.E + e], a2 = a.A4[2 * a.E + e], a3 = a.A4[3 * a.E + e];
+  const float dsk = a.Dskip[e];
+  const float bdt = a.b_dt[e];
+
+  for (int k = 0; k < nk; ++k) {
+    const int s = k % NSTG;
+    uint8_t* st = stages + s * SB;
+    bar_wait(s_u32(&bars[s]), (uint32_t)((k / NSTG) & 1));
+    float4* hs = reinterpret_cast<float4*>(st);
+    const float* xs_s = reinterpret_cast<const float*>(st + EC * 64);
+    const float* row = reinterpret_cast<const float*>(st + EC * 64 + 3 * EC * 4);
+    const float x = xs_s[tid];
+    const float z = xs_s[EC + tid];
     float acc = bdt;
-    for (int r = 0; r < R; r += 4) {
-      const float4 d = __ldg(reinterpret_cast<const float4*>(row + r));
-      acc = fmaf(wdt_s[(r + 0) * blockDim.x + threadIdx.x], d.x, acc);
-      acc = fmaf(wdt_s[(r + 1) * blockDim.x + threadIdx.x], d.y, acc);
-      acc = fmaf(wdt_s[(r + 2) * blockDim.x + threadIdx.x], d.z, acc);
-      acc = fmaf(wdt_s[(r + 3) * blockDim.x + threadIdx.x], d.w, acc);
+    for (int r = 0; r < a.R; r += 4) {
+      const float4 d = *reinterpret_cast<const float4*>(row + r);
+      acc = fmaf(wdt[(r + 0) * EC + tid], d.x, acc);
+      acc = fmaf(wdt[(r + 1) * EC + tid], d.y, acc);
+      acc = fmaf(wdt[(r + 2) * EC + tid], d.z, acc);
+      acc = fmaf(wdt[(r + 3) * EC + tid], d.w, acc);
     }
     const float dl = softplusf_(acc);
-    const float4* bcp = reinterpret_cast<const float4*>(row + R);
-    const float4 b0 = __ldg(bcp), b1 = __ldg(bcp + 1), b2 = __ldg(bcp + 2), b3 = __ldg(bcp + 3);
-    const float4 c0 = __ldg(bcp + 4), c1 = __ldg(bcp + 5), c2 = __ldg(bcp + 6), c3 = __ldg(bcp + 7);
+    const float4* bcp = reinterpret_cast<const float4*>(row + a.R);
+    float4 h0 = hs[tid], h1 = hs[EC + tid], h2 = hs[2 * EC + tid], h3 = hs[3 * EC + tid];
     float yv = 0.0f;
-    scan_update4(h0, a0, b0, c0, dl, x, yv);
-    scan_update4(h1, a1, b1, c1, dl, x, yv);
-    scan_update4(h2, a2, b2, c2, dl, x, yv);
-    scan_update4(h3, a3, b3, c3, dl, x, yv);
+    scan_update4(h0, a0, bcp[0], bcp[4], dl, x, yv);
+    scan_update4(h1, a1, bcp[1], bcp[5], dl, x, yv);
+    scan_update4(h2, a2, bcp[2], bcp[6], dl, x, yv);
+    scan_update4(h3, a3, bcp[3], bcp[7], dl, x, yv);
     yv = fmaf(dsk, x, yv);
     yv *= siluf_(z);
-    float4* hq = h + (size_t)i * 4 * E + e;
-    __stcs(hq, h0); __stcs(hq + E, h1); __stcs(hq + 2 * E, h2); __stcs(hq + 3 * E, h3);
-    y[(size_t)i * E + e] = yv;
+    hs[tid] = h0; hs[EC + tid] = h1; hs[2 * EC + tid] = h2; hs[3 * EC + tid] = h3;
+    reinterpret_cast<float*>(st + EC * 64 + 2 * EC * 4)[tid] = yv;
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    __syncthreads();
+    if (tid == 0) {
+      const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+      const uint32_t sa = s_u32(st);
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+        s2g_hint(a.h + ((i * 4 + j) * a.E + e0) * 4, sa + j * EC * 16, (uint32_t)(EC * 16), pol);
+      s2g(a.y + i * a.E + e0, sa + EC * 64 + 2 * EC * 4, (uint32_t)(EC * 4));
+      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      if (k >= 1 && k - 1 + NSTG < nk) {
+        asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the stores of stream k-1 have left its stage
+        issue_load(k - 1 + NSTG);
+      }
+    }
   }
+  if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
 }  // namespace boa

@@ -264,55 +264,70 @@ __global__ void __launch_bounds__(160, 1) k_tc_gemm(const GemmArgs g) {
     }
     mbar_wait(smem_u32(&acc_bar), 0u);
     tc_fence_after();
-    const int row = m0 + tid;
-    const bool live = row < g.M;
-    const uint32_t tlane = tmem + ((uint32_t)(warp * 32) << 16);
-    const float rs = (EPI == EPI_INPROJ) ? rstd_s[tid] : 1.0f;
+    // Pass 1: TMEM -> registers (thread = stream row) -> shared staging tile, so that pass 2 can run with
+    // lane = column and every global access coalesced.  All MMAs have completed: the stage memory is free.
+    constexpr int LDS = BN + 4;                    // padded row: conflict-free 128-bit stores down a column
+    float* stile = reinterpret_cast<float*>(smem_raw + (sbase - smem_u32(smem_raw)));
+    {
+      const uint32_t tlane = tmem + ((uint32_t)(warp * 32) << 16);
+      const float rs = (EPI == EPI_INPROJ) ? rstd_s[tid] : 1.0f;
 #pragma unroll 1
-    for (int ch = 0; ch < BN / 32; ++ch) {
-      float v[32], w[32];
-      tmem_ld32(tlane + (uint32_t)(ch * 32), v);
-      tmem_ld32(tlane + (uint32_t)(BN + ch * 32), w);
+      for (int ch = 0; ch < BN / 32; ++ch) {
+        float v[32], w[32];
+        __syncwarp();
+        tmem_ld32(tlane + (uint32_t)(ch * 32), v);
+        tmem_ld32(tlane + (uint32_t)(BN + ch * 32), w);
+        float4* dst = reinterpret_cast<float4*>(stile + tid * LDS + ch * 32);
 #pragma unroll
-      for (int j = 0; j < 32; ++j) v[j] = (v[j] + w[j]) * rs;
-      const int nb = n0 + ch * 32;
-      if (!live) continue;
-      float* cp = g.C + (size_t)row * g.ldc + nb;
-      if (EPI == EPI_INPROJ && nb < g.E) {
-        // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU; the window moves one step (R#11)
+        for (int j = 0; j < 32; j += 4)
+          dst[j >> 2] = make_float4((v[j] + w[j]) * rs, (v[j + 1] + w[j + 1]) * rs, (v[j + 2] + w[j + 2]) * rs,
+                                    (v[j + 3] + w[j + 3]) * rs);
+      }
+    }
+    asm volatile("bar.sync 1, 128;" ::: "memory");
+    // Pass 2: a group of BN/4 lanes owns one row segment; 4 consecutive columns per lane.
+    constexpr int LPR = BN / 4;                    // lanes per row
+    constexpr int RPI = 32 / LPR;                  // rows per warp instruction
+    const int col = (lane % LPR) * 4;
+    const int nb = n0 + col;
+    if (EPI == EPI_INPROJ && n0 < g.E) {
+      // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU; the window moves one step (R#11).
+      // The lane's four channels are fixed, so their taps and biases live in registers.
+      const float4 cw0 = g.conv_w[nb], cw1 = g.conv_w[nb + 1], cw2 = g.conv_w[nb + 2], cw3 = g.conv_w[nb + 3];
+      const float4 cb = *reinterpret_cast<const float4*>(g.conv_b + nb);
+#pragma unroll 4
+      for (int i = 0; i < BM / (4 * RPI); ++i) {
+        const int r = (warp + 4 * i) * RPI + lane / LPR;
+        const int row = m0 + r;
+        if (row >= g.M) continue;
+        const float4 x = *reinterpret_cast<const float4*>(stile + r * LDS + col);
         float* wp = g.win + (size_t)row * 3 * g.E + nb;
-#pragma unroll
-        for (int j = 0; j < 32; j += 4) {
-          const float4 w0 = *reinterpret_cast<const float4*>(wp + j);
-          const float4 w1 = *reinterpret_cast<const float4*>(wp + g.E + j);
-          const float4 w2 = *reinterpret_cast<const float4*>(wp + 2 * g.E + j);
-          const float a0[4] = {w0.x, w0.y, w0.z, w0.w}, a1[4] = {w1.x, w1.y, w1.z, w1.w}, a2[4] = {w2.x, w2.y, w2.z, w2.w};
-          float o[4];
-#pragma unroll
-          for (int q = 0; q < 4; ++q) {
-            const float4 cw = __ldg(g.conv_w + nb + j + q);
-            float xc = fmaf(cw.w, v[j + q], __ldg(g.conv_b + nb + j + q));
-            xc = fmaf(cw.x, a0[q], xc);
-            xc = fmaf(cw.y, a1[q], xc);
-            xc = fmaf(cw.z, a2[q], xc);
-            o[q] = xc * sigmoid_tc(xc);
-          }
-          *reinterpret_cast<float4*>(wp + j) = w1;
-          *reinterpret_cast<float4*>(wp + g.E + j) = w2;
-          *reinterpret_cast<float4*>(wp + 2 * g.E + j) = make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]);
-          *reinterpret_cast<float4*>(cp + j) = make_float4(o[0], o[1], o[2], o[3]);
+        const float4 w0 = *reinterpret_cast<const float4*>(wp);
+        const float4 w1 = *reinterpret_cast<const float4*>(wp + g.E);
+        const float4 w2 = *reinterpret_cast<const float4*>(wp + 2 * g.E);
+        float4 o;
+        { float xc = fmaf(cw0.w, x.x, cb.x); xc = fmaf(cw0.x, w0.x, xc); xc = fmaf(cw0.y, w1.x, xc); xc = fmaf(cw0.z, w2.x, xc); o.x = xc * sigmoid_tc(xc); }
+        { float xc = fmaf(cw1.w, x.y, cb.y); xc = fmaf(cw1.x, w0.y, xc); xc = fmaf(cw1.y, w1.y, xc); xc = fmaf(cw1.z, w2.y, xc); o.y = xc * sigmoid_tc(xc); }
+        { float xc = fmaf(cw2.w, x.z, cb.z); xc = fmaf(cw2.x, w0.z, xc); xc = fmaf(cw2.y, w1.z, xc); xc = fmaf(cw2.z, w2.z, xc); o.z = xc * sigmoid_tc(xc); }
+        { float xc = fmaf(cw3.w, x.w, cb.w); xc = fmaf(cw3.x, w0.w, xc); xc = fmaf(cw3.y, w1.w, xc); xc = fmaf(cw3.z, w2.w, xc); o.w = xc * sigmoid_tc(xc); }
+        *reinterpret_cast<float4*>(wp) = w1;
+        *reinterpret_cast<float4*>(wp + g.E) = w2;
+        *reinterpret_cast<float4*>(wp + 2 * g.E) = x;
+        *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + nb) = o;
+      }
+    } else if (nb < g.n_valid) {
+#pragma unroll 4
+      for (int i = 0; i < BM / (4 * RPI); ++i) {
+        const int r = (warp + 4 * i) * RPI + lane / LPR;
+        const int row = m0 + r;
+        if (row >= g.M) continue;
+        float4 o = *reinterpret_cast<const float4*>(stile + r * LDS + col);
+        float4* cp = reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + nb);
+        if (EPI == EPI_RESID) {
+          const float4 q = *cp;
+          o.x += q.x; o.y += q.y; o.z += q.z; o.w += q.w;
         }
-      } else {
-#pragma unroll
-        for (int j = 0; j < 32; j += 4) {
-          if (nb + j >= g.n_valid) break;
-          float4 o = make_float4(v[j], v[j + 1], v[j + 2], v[j + 3]);
-          if (EPI == EPI_RESID) {
-            const float4 r = *reinterpret_cast<const float4*>(cp + j);
-            o.x += r.x; o.y += r.y; o.z += r.z; o.w += r.w;
-          }
-          *reinterpret_cast<float4*>(cp + j) = o;
-        }
+        *cp = o;
       }
     }
   } else if (lane == 0) {
