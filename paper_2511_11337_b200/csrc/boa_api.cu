@@ -203,7 +203,7 @@ template <int BN, int NPW, int EPI>
 int launch_tc(const tc::GemmArgs& g, int N, cudaStream_t st) {
   using C = tc::Cfg<BN, NPW>;
   dim3 grid((g.M + tc::BM - 1) / tc::BM, (N + BN - 1) / BN);
-  tc::k_tc_gemm<BN, NPW, EPI><<<grid, 160, C::SMEM, st>>>(g);
+  tc::k_tc_gemm<BN, NPW, EPI><<<grid, tc::NTHREADS, C::SMEM, st>>>(g);
   return BOA_OK;
 }
 template <int BN, int NPW, int EPI>

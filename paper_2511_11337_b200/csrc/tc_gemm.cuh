@@ -49,7 +49,16 @@ struct GemmArgs {
   const float4* conv_w;    // [E] taps (x = t-3 ... w = t)
   const float* conv_b;     // [E]
   int E;
+#ifdef BOA_TC_TRACE
+  long long* trace;        // [gridDim.x*gridDim.y][64] SM-clock timestamps (development builds only)
+#endif
 };
+
+#ifdef BOA_TC_TRACE
+#define TC_TRACE(slot) do { g.trace[(size_t)(blockIdx.y * gridDim.x + blockIdx.x) * 64 + (slot)] = clock64(); } while (0)
+#else
+#define TC_TRACE(slot) do { } while (0)
+#endif
 
 // ------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -156,13 +165,16 @@ struct Cfg {
 
 __device__ __forceinline__ float sigmoid_tc(float x) { return 1.0f / (1.0f + expf(-x)); }
 
+constexpr int NPROD = 256;       // producer / epilogue threads (warps 0-7); warp 8 owns TMEM and issues the MMAs
+constexpr int NTHREADS = NPROD + 32;
+
 // ------------------------------------------------------------------------------------------ the kernel
-// grid = (ceil(M/128), N/BN), block = 160: warps 0-3 produce the activation pieces and then run the epilogue,
-// warp 4 owns TMEM and its lane 0 issues the MMAs.  Thread 0 also starts the weight bulk copies.
+// grid = (ceil(M/128), N/BN), block = 288.  Warps 0-7 load the activation tile (software-prefetched one k-block
+// ahead), cut it into pieces, and then run the epilogue; thread 0 also starts the weight bulk copies.
 template <int BN, int NPW, int EPI>
-__global__ void __launch_bounds__(160, 1) k_tc_gemm(const GemmArgs g) {
+__global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   using C = Cfg<BN, NPW>;
-  static_assert(BN % 32 == 0 && BN >= 32 && BN <= 128, "tile N");
+  static_assert(BN == 64 || BN == 128, "tile N");
   static_assert(NPW == 1 || NPW == 3, "weight pieces");
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t full_bar[C::NST], empty_bar[C::NST], acc_bar;
@@ -174,12 +186,13 @@ __global__ void __launch_bounds__(160, 1) k_tc_gemm(const GemmArgs g) {
   const int n0 = blockIdx.y * BN;
   const int KB = g.K / BK;
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
+  if (tid == 0) TC_TRACE(0);
 
-  if (warp == 4) {
+  if (warp == 8) {
     if (lane == 0) {
       for (int s = 0; s < C::NST; ++s) {
-        mbar_init(smem_u32(&full_bar[s]), 129);   // 128 producer threads + the expect_tx arrival of thread 0
-        mbar_init(smem_u32(&empty_bar[s]), 1);    // one tcgen05.commit
+        mbar_init(smem_u32(&full_bar[s]), NPROD + 1);   // producer threads + the expect_tx arrival of thread 0
+        mbar_init(smem_u32(&empty_bar[s]), 1);          // one tcgen05.commit
       }
       mbar_init(smem_u32(&acc_bar), 1);
       fence_barrier_init();
@@ -191,35 +204,35 @@ __global__ void __launch_bounds__(160, 1) k_tc_gemm(const GemmArgs g) {
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
+  if (tid == 0) TC_TRACE(1);
 
-  if (warp < 4) {
+  if (warp < 8) {
     // ===================================================================== producers
-    const int c = tid & 7;                       // 16-byte chunk (8 k) of the 128-byte row
-    const int r7 = (tid >> 3) & 7;               // row within the 8-row swizzle group
+    // item (it, tid): row = it*32 + tid/8, 16-byte chunk c = tid%8 (8 consecutive k) of the 128-byte swizzled row
+    const int c = tid & 7;
+    const int r7 = (tid >> 3) & 7;
     const uint32_t soff = (uint32_t)((tid >> 6) * 1024 + r7 * 128 + ((c ^ r7) << 4));
-    float ss[8];
-#pragma unroll
-    for (int it = 0; it < 8; ++it) ss[it] = 0.0f;
+    float ss[4] = {0.f, 0.f, 0.f, 0.f};
     const uint16_t* wsrc = g.W + (size_t)blockIdx.y * KB * (NPW * BN * 64);
+    const float* arow[4];
+#pragma unroll
+    for (int it = 0; it < 4; ++it) arow[it] = g.A + (size_t)min(m0 + it * 32 + (tid >> 3), g.M - 1) * g.lda + c * 8;
 
+    float4 va[4], vb[4];
+#pragma unroll
+    for (int it = 0; it < 4; ++it) {
+      va[it] = *reinterpret_cast<const float4*>(arow[it]);
+      vb[it] = *reinterpret_cast<const float4*>(arow[it] + 4);
+    }
     for (int kb = 0; kb < KB; ++kb) {
       const int s = kb % C::NST, round = kb / C::NST;
-      if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
-      const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
-      if (tid == 0) {
-        const uint32_t fb = smem_u32(&full_bar[s]);
-        mbar_arrive_expect_tx(fb, (uint32_t)(NPW * C::W_PLANE));
+      float4 na[4], nb[4];
+      if (kb + 1 < KB) {                                   // next k-block's loads fly while this one is cut
 #pragma unroll
-        for (int q = 0; q < NPW; ++q)
-          bulk_g2s(sA + NPA * A_PLANE + q * C::W_PLANE, wsrc + ((size_t)kb * NPW + q) * (BN * 64), (uint32_t)C::W_PLANE, fb);
-      }
-      float4 va[8], vb[8];
-#pragma unroll
-      for (int it = 0; it < 8; ++it) {
-        const int row = it * 16 + (tid >> 3);
-        const float4* src = reinterpret_cast<const float4*>(g.A + (size_t)min(m0 + row, g.M - 1) * g.lda + kb * BK + c * 8);
-        va[it] = src[0];
-        vb[it] = src[1];
+        for (int it = 0; it < 4; ++it) {
+          na[it] = *reinterpret_cast<const float4*>(arow[it] + (kb + 1) * BK);
+          nb[it] = *reinterpret_cast<const float4*>(arow[it] + (kb + 1) * BK + 4);
+        }
       }
       float4 sc0 = make_float4(1.f, 1.f, 1.f, 1.f), sc1 = sc0;
       if (g.colscale) {
@@ -227,8 +240,18 @@ __global__ void __launch_bounds__(160, 1) k_tc_gemm(const GemmArgs g) {
         sc0 = sp[0];
         sc1 = sp[1];
       }
+      if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
+      const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
+      if (tid == 0 && kb < 16) TC_TRACE(8 + kb);
+      if (tid == 0) {
+        const uint32_t fb = smem_u32(&full_bar[s]);
+        mbar_arrive_expect_tx(fb, (uint32_t)(NPW * C::W_PLANE));
 #pragma unroll
-      for (int it = 0; it < 8; ++it) {
+        for (int q = 0; q < NPW; ++q)
+          bulk_g2s(sA + NPA * A_PLANE + q * C::W_PLANE, wsrc + ((size_t)kb * NPW + q) * (BN * 64), (uint32_t)C::W_PLANE, fb);
+      }
+#pragma unroll
+      for (int it = 0; it < 4; ++it) {
         float v[8] = {va[it].x, va[it].y, va[it].z, va[it].w, vb[it].x, vb[it].y, vb[it].z, vb[it].w};
         if (EPI == EPI_INPROJ) {
 #pragma unroll
@@ -238,56 +261,68 @@ __global__ void __launch_bounds__(160, 1) k_tc_gemm(const GemmArgs g) {
           v[0] *= sc0.x; v[1] *= sc0.y; v[2] *= sc0.z; v[3] *= sc0.w;
           v[4] *= sc1.x; v[5] *= sc1.y; v[6] *= sc1.z; v[7] *= sc1.w;
         }
-        const uint32_t dst = sA + (uint32_t)it * 2048u + soff;
+        const uint32_t dst = sA + (uint32_t)it * 4096u + soff;
 #pragma unroll
         for (int p = 0; p < NPA; ++p) {
           uint4 w;
           w.x = cut2(v[0], v[1]); w.y = cut2(v[2], v[3]); w.z = cut2(v[4], v[5]); w.w = cut2(v[6], v[7]);
-          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst + p * A_PLANE), "r"(w.x), "r"(w.y), "r"(w.z), "r"(w.w) : "memory");
+          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst + p * A_PLANE), "r"(w.x), "r"(w.y), "r"(w.z), "r"(w.w));
         }
       }
       fence_proxy_async();
       mbar_arrive(smem_u32(&full_bar[s]));
+      if (tid == 0 && kb < 16) TC_TRACE(24 + kb);
+      if (kb + 1 < KB) {
+#pragma unroll
+        for (int it = 0; it < 4; ++it) { va[it] = na[it]; vb[it] = nb[it]; }
+      }
     }
 
     // ===================================================================== epilogue
     if (EPI == EPI_INPROJ) {
 #pragma unroll
-      for (int it = 0; it < 8; ++it) {
+      for (int it = 0; it < 4; ++it) {
         float v = ss[it];
         v += __shfl_xor_sync(0xffffffffu, v, 1);
         v += __shfl_xor_sync(0xffffffffu, v, 2);
         v += __shfl_xor_sync(0xffffffffu, v, 4);
-        if (c == 0) rstd_s[it * 16 + (tid >> 3)] = 1.0f / sqrtf(v / (float)g.K + kEps);
+        if (c == 0) rstd_s[it * 32 + (tid >> 3)] = 1.0f / sqrtf(v / (float)g.K + kEps);
       }
-      asm volatile("bar.sync 1, 128;" ::: "memory");
+      asm volatile("bar.sync 1, 256;" ::: "memory");
     }
     mbar_wait(smem_u32(&acc_bar), 0u);
     tc_fence_after();
-    // Pass 1: TMEM -> registers (thread = stream row) -> shared staging tile, so that pass 2 can run with
-    // lane = column and every global access coalesced.  All MMAs have completed: the stage memory is free.
+    if (tid == 0) TC_TRACE(2);
+    // Pass 1: TMEM -> registers (thread = stream row; warps w and w+4 share the 32 TMEM lanes of rows
+    // 32*(w%4).. and split the columns) -> shared staging tile, so that pass 2 can run with lane = column and
+    // every global access coalesced.  All MMAs have completed: the stage memory is free.
     constexpr int LDS = BN + 4;                    // padded row: conflict-free 128-bit stores down a column
     float* stile = reinterpret_cast<float*>(smem_raw + (sbase - smem_u32(smem_raw)));
     {
-      const uint32_t tlane = tmem + ((uint32_t)(warp * 32) << 16);
-      const float rs = (EPI == EPI_INPROJ) ? rstd_s[tid] : 1.0f;
+      const int r = (warp & 3) * 32 + lane;
+      const uint32_t tlane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
+      const float rs = (EPI == EPI_INPROJ) ? rstd_s[r] : 1.0f;
+      constexpr int CPW = BN / 64;                 // 32-column chunks per warp
 #pragma unroll 1
-      for (int ch = 0; ch < BN / 32; ++ch) {
+      for (int q = 0; q < CPW; ++q) {
+        const int ch = (warp >> 2) * CPW + q;
         float v[32], w[32];
         __syncwarp();
         tmem_ld32(tlane + (uint32_t)(ch * 32), v);
         tmem_ld32(tlane + (uint32_t)(BN + ch * 32), w);
-        float4* dst = reinterpret_cast<float4*>(stile + tid * LDS + ch * 32);
+        float4* dst = reinterpret_cast<float4*>(stile + r * LDS + ch * 32);
 #pragma unroll
         for (int j = 0; j < 32; j += 4)
           dst[j >> 2] = make_float4((v[j] + w[j]) * rs, (v[j + 1] + w[j + 1]) * rs, (v[j + 2] + w[j + 2]) * rs,
                                     (v[j + 3] + w[j + 3]) * rs);
       }
     }
-    asm volatile("bar.sync 1, 128;" ::: "memory");
+    asm volatile("bar.sync 1, 256;" ::: "memory");
+    if (tid == 0) TC_TRACE(3);
     // Pass 2: a group of BN/4 lanes owns one row segment; 4 consecutive columns per lane.
     constexpr int LPR = BN / 4;                    // lanes per row
     constexpr int RPI = 32 / LPR;                  // rows per warp instruction
+    constexpr int NIT = BM / (8 * RPI);            // row groups per warp
     const int col = (lane % LPR) * 4;
     const int nb = n0 + col;
     if (EPI == EPI_INPROJ && n0 < g.E) {
@@ -296,38 +331,40 @@ __global__ void __launch_bounds__(160, 1) k_tc_gemm(const GemmArgs g) {
       const float4 cw0 = g.conv_w[nb], cw1 = g.conv_w[nb + 1], cw2 = g.conv_w[nb + 2], cw3 = g.conv_w[nb + 3];
       const float4 cb = *reinterpret_cast<const float4*>(g.conv_b + nb);
 #pragma unroll 4
-      for (int i = 0; i < BM / (4 * RPI); ++i) {
-        const int r = (warp + 4 * i) * RPI + lane / LPR;
+      for (int i = 0; i < NIT; ++i) {
+        const int r = (warp + 8 * i) * RPI + lane / LPR;
         const int row = m0 + r;
-        if (row >= g.M) continue;
-        const float4 x = *reinterpret_cast<const float4*>(stile + r * LDS + col);
-        float* wp = g.win + (size_t)row * 3 * g.E + nb;
-        const float4 w0 = *reinterpret_cast<const float4*>(wp);
-        const float4 w1 = *reinterpret_cast<const float4*>(wp + g.E);
-        const float4 w2 = *reinterpret_cast<const float4*>(wp + 2 * g.E);
-        float4 o;
-        { float xc = fmaf(cw0.w, x.x, cb.x); xc = fmaf(cw0.x, w0.x, xc); xc = fmaf(cw0.y, w1.x, xc); xc = fmaf(cw0.z, w2.x, xc); o.x = xc * sigmoid_tc(xc); }
-        { float xc = fmaf(cw1.w, x.y, cb.y); xc = fmaf(cw1.x, w0.y, xc); xc = fmaf(cw1.y, w1.y, xc); xc = fmaf(cw1.z, w2.y, xc); o.y = xc * sigmoid_tc(xc); }
-        { float xc = fmaf(cw2.w, x.z, cb.z); xc = fmaf(cw2.x, w0.z, xc); xc = fmaf(cw2.y, w1.z, xc); xc = fmaf(cw2.z, w2.z, xc); o.z = xc * sigmoid_tc(xc); }
-        { float xc = fmaf(cw3.w, x.w, cb.w); xc = fmaf(cw3.x, w0.w, xc); xc = fmaf(cw3.y, w1.w, xc); xc = fmaf(cw3.z, w2.w, xc); o.w = xc * sigmoid_tc(xc); }
-        *reinterpret_cast<float4*>(wp) = w1;
-        *reinterpret_cast<float4*>(wp + g.E) = w2;
-        *reinterpret_cast<float4*>(wp + 2 * g.E) = x;
-        *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + nb) = o;
+        if (row < g.M) {
+          const float4 x = *reinterpret_cast<const float4*>(stile + r * LDS + col);
+          float* wp = g.win + (size_t)row * 3 * g.E + nb;
+          const float4 w0 = *reinterpret_cast<const float4*>(wp);
+          const float4 w1 = *reinterpret_cast<const float4*>(wp + g.E);
+          const float4 w2 = *reinterpret_cast<const float4*>(wp + 2 * g.E);
+          float4 o;
+          { float xc = fmaf(cw0.w, x.x, cb.x); xc = fmaf(cw0.x, w0.x, xc); xc = fmaf(cw0.y, w1.x, xc); xc = fmaf(cw0.z, w2.x, xc); o.x = xc * sigmoid_tc(xc); }
+          { float xc = fmaf(cw1.w, x.y, cb.y); xc = fmaf(cw1.x, w0.y, xc); xc = fmaf(cw1.y, w1.y, xc); xc = fmaf(cw1.z, w2.y, xc); o.y = xc * sigmoid_tc(xc); }
+          { float xc = fmaf(cw2.w, x.z, cb.z); xc = fmaf(cw2.x, w0.z, xc); xc = fmaf(cw2.y, w1.z, xc); xc = fmaf(cw2.z, w2.z, xc); o.z = xc * sigmoid_tc(xc); }
+          { float xc = fmaf(cw3.w, x.w, cb.w); xc = fmaf(cw3.x, w0.w, xc); xc = fmaf(cw3.y, w1.w, xc); xc = fmaf(cw3.z, w2.w, xc); o.w = xc * sigmoid_tc(xc); }
+          *reinterpret_cast<float4*>(wp) = w1;
+          *reinterpret_cast<float4*>(wp + g.E) = w2;
+          *reinterpret_cast<float4*>(wp + 2 * g.E) = x;
+          *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + nb) = o;
+        }
       }
     } else if (nb < g.n_valid) {
 #pragma unroll 4
-      for (int i = 0; i < BM / (4 * RPI); ++i) {
-        const int r = (warp + 4 * i) * RPI + lane / LPR;
+      for (int i = 0; i < NIT; ++i) {
+        const int r = (warp + 8 * i) * RPI + lane / LPR;
         const int row = m0 + r;
-        if (row >= g.M) continue;
-        float4 o = *reinterpret_cast<const float4*>(stile + r * LDS + col);
-        float4* cp = reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + nb);
-        if (EPI == EPI_RESID) {
-          const float4 q = *cp;
-          o.x += q.x; o.y += q.y; o.z += q.z; o.w += q.w;
+        if (row < g.M) {
+          float4 o = *reinterpret_cast<const float4*>(stile + r * LDS + col);
+          float4* cp = reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + nb);
+          if (EPI == EPI_RESID) {
+            const float4 q = *cp;
+            o.x += q.x; o.y += q.y; o.z += q.z; o.w += q.w;
+          }
+          *cp = o;
         }
-        *cp = o;
       }
     }
   } else if (lane == 0) {
@@ -337,6 +374,7 @@ __global__ void __launch_bounds__(160, 1) k_tc_gemm(const GemmArgs g) {
       const int s = kb % C::NST, round = kb / C::NST;
       mbar_wait(smem_u32(&full_bar[s]), (uint32_t)(round & 1));
       tc_fence_after();
+      if (kb < 16) TC_TRACE(40 + kb);
       const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
       const uint32_t sW = sA + NPA * A_PLANE;
 #pragma unroll
@@ -362,9 +400,11 @@ __global__ void __launch_bounds__(160, 1) k_tc_gemm(const GemmArgs g) {
     umma_commit(smem_u32(&acc_bar));                            // accumulators complete
   }
 
+  if (tid == 0) TC_TRACE(4);
   tc_fence_before();
   __syncthreads();
-  if (warp == 4) {
+  if (tid == 0) TC_TRACE(5);
+  if (warp == 8) {
     __syncwarp();
     tmem_dealloc(tmem, C::TMEM_COLS);
   }
