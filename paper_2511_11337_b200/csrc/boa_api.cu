@@ -69,7 +69,8 @@ struct boa_model {
 
   // workspace (per wave of Bcap streams)
   uint64_t Bcap = 0;
-  GrowBuf u, xz, dbc, y, logits, h, win;
+  GrowBuf u, xz, dbc, logits, h, win;
+  GrowBuf u_img, xs_img, y_img;   // activation images: operands of the tensor-core contractions (tc_gemm.cuh)
   GrowBuf pos, len, low, range, pending, wpos, cache, started, v, rpos, off, size, scratch, first, err;
   GrowBuf stage_in, stage_out;
 
@@ -84,7 +85,7 @@ struct boa_model {
   std::vector<cudaEvent_t> events;
 
   ~boa_model() {
-    for (GrowBuf* b : {&weights, &wimg, &u, &xz, &dbc, &y, &logits, &h, &win, &pos, &len, &low, &range,
+    for (GrowBuf* b : {&weights, &wimg, &u, &xz, &dbc, &u_img, &xs_img, &y_img, &logits, &h, &win, &pos, &len, &low, &range,
                        &pending, &wpos, &cache, &started, &v, &rpos, &off, &size, &scratch, &first, &err,
                        &stage_in, &stage_out})
       b->release();
@@ -239,31 +240,34 @@ int launch_step(StepCtx& c) {
   float* u = m->u.as<float>();
   float* xz = m->xz.as<float>();
   float* dbc = m->dbc.as<float>();
-  float* y = m->y.as<float>();
   float* logits = m->logits.as<float>();
+  uint8_t* u_img = m->u_img.as<uint8_t>();
+  uint8_t* xs_img = m->xs_img.as<uint8_t>();
+  uint8_t* y_img = m->y_img.as<uint8_t>();
 
   {
     const int total = B * (D / 4);
     k_embed<<<(total + 255) / 256, 256, 0, c.st>>>(c.data, c.chunk_bytes, c.ca.pos, c.ca.len,
-                                                    reinterpret_cast<const float4*>(m->emb),
-                                                    reinterpret_cast<float4*>(u), B, D / 4);
+                                                    reinterpret_cast<const float4*>(m->emb), reinterpret_cast<float4*>(u),
+                                                    reinterpret_cast<const float4*>(m->layers[0].norm_w), u_img, B, D / 4);
     BOA_TRY(mark(c, BOA_K_EMBED));
   }
   for (int l = 0; l < m->L; ++l) {
     const LayerW& w = m->layers[l];
     float* hl = m->h.as<float>() + (size_t)l * m->Bcap * E * kNState;
     float* winl = m->win.as<float>() + (size_t)l * m->Bcap * 3 * E;
-    {  // S2-S4: xz = [SiLU(conv(W_in_x r)) ; W_in_z r],  r = RMSNorm(u)
+    {  // S2-S4: xz = [SiLU(conv(W_in_x r)) ; W_in_z r],  r = RMSNorm(u);  xs also as the image for x_proj
       tc::GemmArgs g{};
-      g.A = u; g.lda = D; g.M = B; g.K = D; g.colscale = w.norm_w; g.W = w.img_in;
+      g.A = u_img; g.M = B; g.KB = D / 64; g.W = w.img_in;
       g.C = xz; g.ldc = 2 * E; g.n_valid = 2 * E;
-      g.win = winl; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
+      g.U = u; g.win = winl; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
+      g.out_img = xs_img; g.out_KB = E / 64;
       BOA_TRY((launch_tc_npw<128, tc::EPI_INPROJ>(m->npw, g, 2 * E, c.st)));
       BOA_TRY(mark(c, BOA_K_INPROJ));
     }
     {  // S5: [dlt;Bv;Cv] = W_x xs
       tc::GemmArgs g{};
-      g.A = xz; g.lda = 2 * E; g.M = B; g.K = E; g.W = w.img_x;
+      g.A = xs_img; g.M = B; g.KB = E / 64; g.W = w.img_x;
       g.C = dbc; g.ldc = m->ldj; g.n_valid = m->J;
       if (m->ldj == 64) BOA_TRY((launch_tc_npw<64, tc::EPI_STORE>(m->npw, g, 64, c.st)));
       else BOA_TRY((launch_tc_npw<128, tc::EPI_STORE>(m->npw, g, 128, c.st)));
@@ -272,23 +276,25 @@ int launch_step(StepCtx& c) {
     {  // S6-S8: persistent, two CTAs per SM, each walking over streams for one channel slice
       ScanArgs sa{};
       sa.h = hl; sa.xz = xz; sa.dbc = dbc; sa.W_dtT = w.w_dtT; sa.b_dt = w.b_dt; sa.A4 = w.A4; sa.Dskip = w.d_skip;
-      sa.y = y; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
+      sa.y_img = y_img; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
       const int ec = (E % 256 == 0) ? 256 : 128, slices = E / ec;
       const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
       k_scan<<<dim3(per_slice, slices), ec, scan::smem_bytes(ec, m->ldj, m->R), c.st>>>(sa);
       BOA_TRY(mark(c, BOA_K_SCAN));
     }
-    {  // S9: u += W_out y
+    {  // S9: u += W_out y;  the new u also as the image for the next in_proj (times its RMSNorm weight) or the head
       tc::GemmArgs g{};
-      g.A = y; g.lda = E; g.M = B; g.K = E; g.W = w.img_out;
+      g.A = y_img; g.M = B; g.KB = E / 64; g.W = w.img_out;
       g.C = u; g.ldc = D; g.n_valid = D;
+      g.out_img = u_img; g.out_KB = D / 64;
+      g.out_scale = (l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
       BOA_TRY((launch_tc_npw<64, tc::EPI_RESID>(m->npw, g, D, c.st)));
       BOA_TRY(mark(c, BOA_K_OUTPROJ));
     }
   }
   {  // S10: logits = Emb u
     tc::GemmArgs g{};
-    g.A = u; g.lda = D; g.M = B; g.K = D; g.W = m->img_head;
+    g.A = u_img; g.M = B; g.KB = D / 64; g.W = m->img_head;
     g.C = logits; g.ldc = 256; g.n_valid = 256;
     BOA_TRY((launch_tc_npw<64, tc::EPI_STORE>(m->npw, g, 256, c.st)));
     BOA_TRY(mark(c, BOA_K_HEAD));
@@ -384,7 +390,7 @@ int run_steps(StepCtx& c, uint64_t steps) {
 // ------------------------------------------------------------------------------------- workspace
 size_t bytes_per_stream(const boa_model* m, size_t cap) {
   const size_t E = m->E, D = m->D;
-  return 4 * (D + 2 * E + E + 128 + 256) + (size_t)m->L * 4 * (E * kNState + 3 * E) + 64 + cap;
+  return 4 * (D + 2 * E + 128 + 256) + 6 * (D + 2 * E) + (size_t)m->L * 4 * (E * kNState + 3 * E) + 64 + cap;
 }
 
 int reserve_workspace(boa_model* m, uint64_t B, size_t cap) {
@@ -394,7 +400,9 @@ int reserve_workspace(boa_model* m, uint64_t B, size_t cap) {
     BOA_TRY(m->u.reserve(B * D * 4));
     BOA_TRY(m->xz.reserve(B * 2 * E * 4));
     BOA_TRY(m->dbc.reserve(B * (size_t)m->ldj * 4));
-    BOA_TRY(m->y.reserve(B * E * 4));
+    BOA_TRY(m->u_img.reserve(tc::img_bytes(B, D)));
+    BOA_TRY(m->xs_img.reserve(tc::img_bytes(B, E)));
+    BOA_TRY(m->y_img.reserve(tc::img_bytes(B, E)));
     BOA_TRY(m->logits.reserve(B * 256 * 4));
     BOA_TRY(m->h.reserve(L * B * E * kNState * 4));
     BOA_TRY(m->win.reserve(L * B * 3 * E * 4));
@@ -931,8 +939,15 @@ int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N,
   // the kernel stores whole 4-column groups of a row: give it a padded C and copy the valid columns out
   void* cpad = nullptr;
   if (cudaMalloc(&cpad, M * Np * 4) != cudaSuccess) { (void)cudaGetLastError(); return BOA_E_NOMEM; }
+  void* aimg = nullptr;
+  if (cudaMalloc(&aimg, tc::img_bytes(M, K)) != cudaSuccess) { (void)cudaGetLastError(); cudaFree(cpad); return BOA_E_NOMEM; }
+  {
+    const size_t total = M * (K / 4);
+    tc::k_cut_rows<<<(unsigned)((total + 255) / 256), 256, 0, st>>>(static_cast<const float*>(ta.dev), (int)K, (int)M, (int)K,
+                                                                    nullptr, static_cast<uint8_t*>(aimg));
+  }
   tc::GemmArgs g{};
-  g.A = static_cast<const float*>(ta.dev); g.lda = (int)K; g.M = (int)M; g.K = (int)K;
+  g.A = static_cast<const uint8_t*>(aimg); g.M = (int)M; g.KB = (int)(K / 64);
   g.W = static_cast<const uint16_t*>(tw.dev);
   g.C = static_cast<float*>(cpad); g.ldc = (int)Np; g.n_valid = (int)Np;
   int rc = tile_n == 64 ? launch_tc_npw<64, tc::EPI_STORE>(weight_pieces, g, (int)Np, st)
@@ -945,6 +960,7 @@ int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N,
     if (e != cudaSuccess) rc = note_cuda_error(e, __FILE__, __LINE__);
   }
   cudaFree(cpad);
+  cudaFree(aimg);
   return rc;
 }
 

@@ -13,6 +13,7 @@
 // no atomics.
 #pragma once
 #include "common.cuh"
+#include "tc_gemm.cuh"
 
 namespace boa {
 
@@ -30,15 +31,19 @@ __device__ __forceinline__ float softplusf_(float v) { return fmaxf(v, 0.0f) + l
 // ---------------------------------------------------------------------------------------------------
 // S1: u[i][:] = Emb[src[i*chunk + min(pos_i, len_i-1)]].  In compress mode `src` is the input; in
 // decompress mode it is the output buffer, whose byte pos_i was written by the previous coder step.
+// Also writes the image of u * norm_w(layer 0), the operand of the first in_proj (tc_gemm.cuh).
 __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, const uint32_t* __restrict__ pos,
                         const uint32_t* __restrict__ len, const float4* __restrict__ emb, float4* __restrict__ u,
-                        int B, int D4) {
+                        const float4* __restrict__ norm_w, uint8_t* __restrict__ u_img, int B, int D4) {
   int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= B * D4) return;
   int i = idx / D4, q = idx - i * D4;
   uint32_t p = min(pos[i], len[i] - 1u);
   uint32_t s = src[(size_t)i * chunk_bytes + p];
-  u[idx] = emb[s * D4 + q];
+  const float4 v = emb[s * D4 + q];
+  u[idx] = v;
+  const float4 w = norm_w[q];
+  tc::cut4_store(u_img, D4 >> 4, i, q * 4, make_float4(v.x * w.x, v.y * w.y, v.z * w.z, v.w * w.w));
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -52,8 +57,9 @@ __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, con
 // flight, not arithmetic: a persistent CTA owns a channel slice and walks over streams with a ring of NSTG shared
 // memory stages.  Everything a stream-step needs (4 state runs, xs, z, the x_proj row) is brought in by the
 // bulk-copy engine (TMA, cp.async.bulk -> UBLKCP) against one mbarrier per stage; threads touch shared memory
-// only; the updated state and y go back with bulk stores.  State copies carry an L2 evict-first policy so the
-// small activations stay resident in L2.
+// only; the updated state goes back with bulk stores.  State copies carry an L2 evict-first policy so the
+// small activations stay resident in L2.  y leaves cut into bf16 pieces, written into the image of out_proj's
+// operand tile (tc_gemm.cuh).
 // One thread per channel of the slice holds A[e][0..15] in registers; W_dt^T of the slice lives in shared memory.
 struct ScanArgs {
   float* h;                 // [B][4][E] float4 (this layer)
@@ -63,7 +69,7 @@ struct ScanArgs {
   const float* b_dt;        // [E]
   const float4* A4;         // [4][E] float4: A = -exp(A_log)
   const float* Dskip;       // [E]
-  float* y;                 // [B][E]
+  uint8_t* y_img;           // image of y[B][E] for out_proj (tc_gemm.cuh)
   int ldj, B, E, R;
 };
 
@@ -77,7 +83,7 @@ __device__ __forceinline__ void scan_update4(float4& h, const float4 a, const fl
 
 namespace scan {
 constexpr int NSTG = 4;
-__host__ __device__ inline int stage_bytes(int EC, int ldj) { return EC * 64 + 3 * EC * 4 + ldj * 4; }   // h | xs | z | y | dbc
+__host__ __device__ inline int stage_bytes(int EC, int ldj) { return EC * 64 + 2 * EC * 4 + EC * 6 + ldj * 4; }   // h | xs | z | y pieces | dbc
 __host__ __device__ inline int smem_bytes(int EC, int ldj, int R) { return NSTG * stage_bytes(EC, ldj) + R * EC * 4 + NSTG * 8 + 128; }
 
 __device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -141,7 +147,7 @@ __global__ void __launch_bounds__(256, 2) k_scan(const ScanArgs a) {
       g2s_hint(st + j * EC * 16, a.h + ((i * 4 + j) * a.E + e0) * 4, (uint32_t)(EC * 16), bar, pol);
     g2s(st + EC * 64, a.xz + i * 2 * a.E + e0, (uint32_t)(EC * 4), bar);
     g2s(st + EC * 64 + EC * 4, a.xz + i * 2 * a.E + a.E + e0, (uint32_t)(EC * 4), bar);
-    g2s(st + EC * 64 + 3 * EC * 4, a.dbc + i * a.ldj, (uint32_t)(a.ldj * 4), bar);
+    g2s(st + EC * 64 + 2 * EC * 4 + EC * 6, a.dbc + i * a.ldj, (uint32_t)(a.ldj * 4), bar);
   };
 
   if (tid == 0) {
@@ -163,7 +169,7 @@ __global__ void __launch_bounds__(256, 2) k_scan(const ScanArgs a) {
     bar_wait(s_u32(&bars[s]), (uint32_t)((k / NSTG) & 1));
     float4* hs = reinterpret_cast<float4*>(st);
     const float* xs_s = reinterpret_cast<const float*>(st + EC * 64);
-    const float* row = reinterpret_cast<const float*>(st + EC * 64 + 3 * EC * 4);
+    const float* row = reinterpret_cast<const float*>(st + EC * 64 + 2 * EC * 4 + EC * 6);
     const float x = xs_s[tid];
     const float z = xs_s[EC + tid];
     float acc = bdt;
@@ -185,16 +191,31 @@ __global__ void __launch_bounds__(256, 2) k_scan(const ScanArgs a) {
     yv = fmaf(dsk, x, yv);
     yv *= siluf_(z);
     hs[tid] = h0; hs[EC + tid] = h1; hs[2 * EC + tid] = h2; hs[3 * EC + tid] = h3;
-    reinterpret_cast<float*>(st + EC * 64 + 2 * EC * 4)[tid] = yv;
+    const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+    {
+      // y -> three bf16 pieces (truncation split, exact), staged as [64-channel block][piece][128-byte swizzled row]
+      uint8_t* yp = st + EC * 64 + 2 * EC * 4 + ((tid >> 6) * 3) * 128 + (((((tid & 63) >> 3) ^ (int)i) & 7) << 4) + (tid & 7) * 2;
+#pragma unroll
+      for (int q = 0; q < 3; ++q) {
+        *reinterpret_cast<uint16_t*>(yp + q * 128) = (uint16_t)(__float_as_uint(yv) >> 16);
+        yv = __fsub_rn(yv, tc::trunc_bf16(yv));
+      }
+    }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
     __syncthreads();
+    if (tid < (EC >> 6) * 24) {
+      // one 16-byte chunk per thread: row (tid/8) = (64-channel block, piece), chunk tid%8 of its 128-byte row
+      const int rowid = tid >> 3, kt = rowid / 3, q = rowid - kt * 3;
+      const int r = (int)(i & 127);
+      uint8_t* dst = a.y_img + tc::img_block(i >> 7, (size_t)(e0 >> 6) + kt, (size_t)(a.E >> 6)) + (size_t)q * tc::A_PLANE +
+                     (r >> 3) * 1024 + (r & 7) * 128 + (tid & 7) * 16;
+      *reinterpret_cast<uint4*>(dst) = *reinterpret_cast<const uint4*>(st + EC * 64 + 2 * EC * 4 + rowid * 128 + (tid & 7) * 16);
+    }
     if (tid == 0) {
-      const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
       const uint32_t sa = s_u32(st);
 #pragma unroll
       for (int j = 0; j < 4; ++j)
         s2g_hint(a.h + ((i * 4 + j) * a.E + e0) * 4, sa + j * EC * 16, (uint32_t)(EC * 16), pol);
-      s2g(a.y + i * a.E + e0, sa + EC * 64 + 2 * EC * 4, (uint32_t)(EC * 4));
       asm volatile("cp.async.bulk.commit_group;" ::: "memory");
       if (k >= 1 && k - 1 + NSTG < nk) {
         asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the stores of stream k-1 have left its stage

@@ -15,12 +15,15 @@
 // The leading product has its own TMEM accumulator; all correction products (2^-8 and smaller) go to a second one and
 // the two are added once, in fp32, in the epilogue.  Dropped products are below 2^-24 of |a||w|.
 //
-// Data movement.  The weight pieces are cut and laid out once, at boa_model_load, as the exact shared-memory image of
-// a tile (K-major, 128-byte swizzle): a stage's weight tile is ONE contiguous block that the bulk-copy engine (TMA,
-// cp.async.bulk -> SASS UBLKCP) drops into shared memory, signalling an mbarrier.  The activation tile is loaded by
-// four producer warps (coalesced 128-bit loads from L2), cut into pieces in registers and stored in the same swizzled
-// layout.  One elected thread issues the MMAs; tcgen05.commit releases the stage.  The producer warps then become the
-// epilogue: tcgen05.ld (one TMEM lane = one stream per thread), fused epilogue, 128-byte row segments to global.
+// Data movement.  Both operands reach shared memory through the bulk-copy engine (TMA, cp.async.bulk -> SASS UBLKCP)
+// as ready-made images of a tile (K-major, 128-byte swizzle), so the main loop is TMA + MMA only:
+//   weights      cut and laid out once, at boa_model_load;
+//   activations  cut by the kernel that PRODUCES them (embedding, the conv epilogue of in_proj, the scan, the
+//                residual epilogue of out_proj), which writes the three pieces straight into the image of the
+//                consumer's tile - each activation is cut once per step, not once per consuming tile.
+// One warp drives the copies, one elected thread issues the MMAs, tcgen05.commit releases a stage.  Eight epilogue
+// warps read TMEM (one lane = one stream per thread), transpose through a shared staging tile and run the fused
+// epilogue with lane = column, so every global access is coalesced.
 //
 // Determinism: row m of the result depends only on row m of A, on W and on a fixed issue order; it does not
 // depend on M, on the tile the stream falls in, or on encode vs decode.
@@ -38,17 +41,21 @@ constexpr int A_PLANE = BM * 128;  // bytes of one activation piece tile
 enum { EPI_STORE = 0, EPI_RESID = 1, EPI_INPROJ = 2 };
 
 struct GemmArgs {
-  const float* A;          // [M][lda] fp32 activations (row = stream)
-  int lda, M, K;           // K % 64 == 0
-  const float* colscale;   // [K] or nullptr: A[m][k] is multiplied by colscale[k] before it is cut (RMSNorm weight)
+  const uint8_t* A;        // activation image of A[M][K]: [ceil(M/128)][K/64][3 pieces][128 x 64 bf16, swizzled]
+  int M, KB;               // KB = K/64
   const uint16_t* W;       // weight image [N/BN][K/64][NPW][BN x 64 bf16, swizzled]
-  float* C;                // [M][ldc]
+  float* C;                // [M][ldc] fp32 result (in_proj: xz = xs | z; out_proj: the residual stream u, updated)
   int ldc, n_valid;        // columns >= n_valid are not stored (zero-padded weight rows)
   // EPI_INPROJ only
+  const float* U;          // [M][K] fp32 residual stream: rstd = 1/sqrt(mean(u^2)+eps) is computed from it
   float* win;              // [M][3][E] conv window of this layer
   const float4* conv_w;    // [E] taps (x = t-3 ... w = t)
   const float* conv_b;     // [E]
   int E;
+  // image of the result for the next contraction (EPI_INPROJ: xs -> x_proj; EPI_RESID: u -> in_proj / head)
+  uint8_t* out_img;
+  int out_KB;              // k-blocks per row tile of that image
+  const float* out_scale;  // EPI_RESID: the consumer's RMSNorm weight (applied before cutting) or nullptr
 #ifdef BOA_TC_TRACE
   long long* trace;        // [gridDim.x*gridDim.y][64] SM-clock timestamps (development builds only)
 #endif
@@ -145,32 +152,65 @@ __host__ __device__ constexpr uint32_t idesc_bf16(int n) {
   return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)(n >> 3) << 17) | ((uint32_t)(BM >> 4) << 24);
 }
 
-// two floats -> packed bf16x2 (lo = first), round to nearest even; and the exact remainders
-__device__ __forceinline__ uint32_t cut2(float& a, float& b) {
-  uint32_t p;
-  asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(p) : "f"(b), "f"(a));
-  a = __fsub_rn(a, __uint_as_float(p << 16));
-  b = __fsub_rn(b, __uint_as_float(p & 0xFFFF0000u));
-  return p;
+// ------------------------------------------------------------------------------------------ activation images
+// Byte offset of element (r, k) of a 128 x 64 tile inside one 16 KB piece plane (K-major, 128-byte swizzle: the
+// 16-byte chunk index is XORed with the row index mod 8), and of k-block (mt, kb) inside an image.
+__host__ __device__ inline uint32_t plane_off(int r, int k) {
+  return (uint32_t)((r >> 3) * 1024 + (r & 7) * 128 + ((((k >> 3) ^ r) & 7) << 4) + (k & 7) * 2);
+}
+__host__ __device__ inline size_t img_block(size_t mt, size_t kb, size_t KB) { return (mt * KB + kb) * (size_t)(NPA * A_PLANE); }
+__host__ __device__ inline size_t img_bytes(size_t M, size_t K) { return ((M + BM - 1) / BM) * (K / BK) * (size_t)(NPA * A_PLANE); }
+
+// An fp32 value is cut into three bf16 pieces by truncation: piece = the top 16 bits, remainder = v - piece (exact);
+// 3 x 8 significant bits cover the 24-bit significand, so the pieces sum to v exactly.
+__device__ __forceinline__ float trunc_bf16(float v) { return __uint_as_float(__float_as_uint(v) & 0xFFFF0000u); }
+__device__ __forceinline__ uint32_t pack_hi(float lo, float hi) { return __byte_perm(__float_as_uint(lo), __float_as_uint(hi), 0x7632); }
+
+// Cut 4 consecutive values (row m, columns k..k+3, k % 4 == 0) and store the pieces into an image: 8 bytes per plane.
+__device__ __forceinline__ void cut4_store(uint8_t* img, int KB, int m, int k, float4 v) {
+  uint8_t* p = img + img_block((size_t)(m >> 7), (size_t)(k >> 6), (size_t)KB) + plane_off(m & 127, k & 63);
+#pragma unroll
+  for (int q = 0; q < NPA; ++q) {
+    *reinterpret_cast<uint2*>(p + q * A_PLANE) = make_uint2(pack_hi(v.x, v.y), pack_hi(v.z, v.w));
+    v.x = __fsub_rn(v.x, trunc_bf16(v.x)); v.y = __fsub_rn(v.y, trunc_bf16(v.y));
+    v.z = __fsub_rn(v.z, trunc_bf16(v.z)); v.w = __fsub_rn(v.w, trunc_bf16(v.w));
+  }
+}
+
+// X[M][ldx] fp32 (optionally times colscale[k]) -> image.  One thread per 4 columns.
+__global__ void k_cut_rows(const float* __restrict__ X, int ldx, int M, int K, const float* __restrict__ colscale,
+                           uint8_t* __restrict__ img) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int K4 = K >> 2;
+  if (idx >= M * K4) return;
+  const int m = idx / K4, k = (idx - m * K4) * 4;
+  float4 v = *reinterpret_cast<const float4*>(X + (size_t)m * ldx + k);
+  if (colscale) {
+    const float4 s = *reinterpret_cast<const float4*>(colscale + k);
+    v.x *= s.x; v.y *= s.y; v.z *= s.z; v.w *= s.w;
+  }
+  cut4_store(img, K >> 6, m, k, v);
 }
 
 template <int BN, int NPW>
 struct Cfg {
-  static constexpr int W_PLANE = BN * 128;
-  static constexpr int STAGE = NPA * A_PLANE + NPW * W_PLANE;
-  static constexpr int NST = (3 * STAGE <= 216 * 1024) ? 3 : 2;
+  static constexpr int W_BYTES = NPW * BN * 128;
+  static constexpr int A_BYTES = NPA * A_PLANE;
+  static constexpr int STAGE = A_BYTES + W_BYTES;
+  static constexpr int NST = (4 * STAGE <= 216 * 1024) ? 4 : (3 * STAGE <= 216 * 1024) ? 3 : 2;
   static constexpr int SMEM = NST * STAGE + 1024;             // + alignment slack
   static constexpr int TMEM_COLS = (2 * BN <= 32) ? 32 : (2 * BN <= 64) ? 64 : (2 * BN <= 128) ? 128 : (2 * BN <= 256) ? 256 : 512;
 };
 
 __device__ __forceinline__ float sigmoid_tc(float x) { return 1.0f / (1.0f + expf(-x)); }
 
-constexpr int NPROD = 256;       // producer / epilogue threads (warps 0-7); warp 8 owns TMEM and issues the MMAs
-constexpr int NTHREADS = NPROD + 32;
+constexpr int NEPI = 256;        // epilogue threads (warps 0-7); warp 8 owns TMEM and issues the MMAs; warp 9 drives the copies
+constexpr int NTHREADS = NEPI + 64;
 
 // ------------------------------------------------------------------------------------------ the kernel
-// grid = (ceil(M/128), N/BN), block = 288.  Warps 0-7 load the activation tile (software-prefetched one k-block
-// ahead), cut it into pieces, and then run the epilogue; thread 0 also starts the weight bulk copies.
+// grid = (ceil(M/128), N/BN), block = 320.  Warp 9 (one lane) streams the k-blocks of both operand images into
+// the stage ring; warp 8 (one lane) issues the MMAs; warps 0-7 compute the RMSNorm row scale meanwhile (in_proj)
+// and then run the epilogue.
 template <int BN, int NPW, int EPI>
 __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   using C = Cfg<BN, NPW>;
@@ -184,15 +224,15 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int m0 = blockIdx.x * BM;
   const int n0 = blockIdx.y * BN;
-  const int KB = g.K / BK;
+  const int KB = g.KB;
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   if (tid == 0) TC_TRACE(0);
 
   if (warp == 8) {
     if (lane == 0) {
       for (int s = 0; s < C::NST; ++s) {
-        mbar_init(smem_u32(&full_bar[s]), NPROD + 1);   // producer threads + the expect_tx arrival of thread 0
-        mbar_init(smem_u32(&empty_bar[s]), 1);          // one tcgen05.commit
+        mbar_init(smem_u32(&full_bar[s]), 1);     // the copy warp's arrive.expect_tx
+        mbar_init(smem_u32(&empty_bar[s]), 1);    // one tcgen05.commit
       }
       mbar_init(smem_u32(&acc_bar), 1);
       fence_barrier_init();
@@ -206,87 +246,82 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   const uint32_t tmem = tmem_base_s;
   if (tid == 0) TC_TRACE(1);
 
-  if (warp < 8) {
-    // ===================================================================== producers
-    // item (it, tid): row = it*32 + tid/8, 16-byte chunk c = tid%8 (8 consecutive k) of the 128-byte swizzled row
-    const int c = tid & 7;
-    const int r7 = (tid >> 3) & 7;
-    const uint32_t soff = (uint32_t)((tid >> 6) * 1024 + r7 * 128 + ((c ^ r7) << 4));
-    float ss[4] = {0.f, 0.f, 0.f, 0.f};
-    const uint16_t* wsrc = g.W + (size_t)blockIdx.y * KB * (NPW * BN * 64);
-    const float* arow[4];
-#pragma unroll
-    for (int it = 0; it < 4; ++it) arow[it] = g.A + (size_t)min(m0 + it * 32 + (tid >> 3), g.M - 1) * g.lda + c * 8;
-
-    float4 va[4], vb[4];
-#pragma unroll
-    for (int it = 0; it < 4; ++it) {
-      va[it] = *reinterpret_cast<const float4*>(arow[it]);
-      vb[it] = *reinterpret_cast<const float4*>(arow[it] + 4);
-    }
-    for (int kb = 0; kb < KB; ++kb) {
-      const int s = kb % C::NST, round = kb / C::NST;
-      float4 na[4], nb[4];
-      if (kb + 1 < KB) {                                   // next k-block's loads fly while this one is cut
-#pragma unroll
-        for (int it = 0; it < 4; ++it) {
-          na[it] = *reinterpret_cast<const float4*>(arow[it] + (kb + 1) * BK);
-          nb[it] = *reinterpret_cast<const float4*>(arow[it] + (kb + 1) * BK + 4);
-        }
-      }
-      float4 sc0 = make_float4(1.f, 1.f, 1.f, 1.f), sc1 = sc0;
-      if (g.colscale) {
-        const float4* sp = reinterpret_cast<const float4*>(g.colscale + kb * BK + c * 8);
-        sc0 = sp[0];
-        sc1 = sp[1];
-      }
-      if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
-      const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
-      if (tid == 0 && kb < 16) TC_TRACE(8 + kb);
-      if (tid == 0) {
-        const uint32_t fb = smem_u32(&full_bar[s]);
-        mbar_arrive_expect_tx(fb, (uint32_t)(NPW * C::W_PLANE));
-#pragma unroll
-        for (int q = 0; q < NPW; ++q)
-          bulk_g2s(sA + NPA * A_PLANE + q * C::W_PLANE, wsrc + ((size_t)kb * NPW + q) * (BN * 64), (uint32_t)C::W_PLANE, fb);
-      }
-#pragma unroll
-      for (int it = 0; it < 4; ++it) {
-        float v[8] = {va[it].x, va[it].y, va[it].z, va[it].w, vb[it].x, vb[it].y, vb[it].z, vb[it].w};
-        if (EPI == EPI_INPROJ) {
-#pragma unroll
-          for (int j = 0; j < 8; ++j) ss[it] = fmaf(v[j], v[j], ss[it]);
-        }
-        if (g.colscale) {
-          v[0] *= sc0.x; v[1] *= sc0.y; v[2] *= sc0.z; v[3] *= sc0.w;
-          v[4] *= sc1.x; v[5] *= sc1.y; v[6] *= sc1.z; v[7] *= sc1.w;
-        }
-        const uint32_t dst = sA + (uint32_t)it * 4096u + soff;
-#pragma unroll
-        for (int p = 0; p < NPA; ++p) {
-          uint4 w;
-          w.x = cut2(v[0], v[1]); w.y = cut2(v[2], v[3]); w.z = cut2(v[4], v[5]); w.w = cut2(v[6], v[7]);
-          asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(dst + p * A_PLANE), "r"(w.x), "r"(w.y), "r"(w.z), "r"(w.w));
-        }
-      }
-      fence_proxy_async();
-      mbar_arrive(smem_u32(&full_bar[s]));
-      if (tid == 0 && kb < 16) TC_TRACE(24 + kb);
-      if (kb + 1 < KB) {
-#pragma unroll
-        for (int it = 0; it < 4; ++it) { va[it] = na[it]; vb[it] = nb[it]; }
+  if (warp == 9) {
+    // ===================================================================== copy warp
+    if (lane == 0) {
+      const uint8_t* asrc = g.A + img_block((size_t)blockIdx.x, 0, (size_t)KB);
+      const uint16_t* wsrc = g.W + (size_t)blockIdx.y * KB * (NPW * BN * 64);
+      for (int kb = 0; kb < KB; ++kb) {
+        const int s = kb % C::NST, round = kb / C::NST;
+        if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
+        const uint32_t sA = sbase + (uint32_t)s * C::STAGE, fb = smem_u32(&full_bar[s]);
+        mbar_arrive_expect_tx(fb, (uint32_t)C::STAGE);
+        bulk_g2s(sA, asrc + (size_t)kb * C::A_BYTES, (uint32_t)C::A_BYTES, fb);
+        bulk_g2s(sA + C::A_BYTES, wsrc + (size_t)kb * (NPW * BN * 64), (uint32_t)C::W_BYTES, fb);
+        if (kb < 16) TC_TRACE(8 + kb);
       }
     }
-
-    // ===================================================================== epilogue
+  } else if (warp == 8) {
+    // ===================================================================== MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc = idesc_bf16(BN);
+      for (int kb = 0; kb < KB; ++kb) {
+        const int s = kb % C::NST, round = kb / C::NST;
+        mbar_wait(smem_u32(&full_bar[s]), (uint32_t)(round & 1));
+        tc_fence_after();
+        if (kb < 16) TC_TRACE(40 + kb);
+        const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
+        const uint32_t sW = sA + C::A_BYTES;
+#pragma unroll
+        for (int k4 = 0; k4 < BK / 16; ++k4) {
+          const uint32_t first = (kb | k4) ? 1u : 0u;
+          const uint32_t ko = (uint32_t)k4 * 32u;
+          auto A_ = [&](int p) { return smem_desc_sw128(sA + p * A_PLANE + ko); };
+          auto W_ = [&](int q) { return smem_desc_sw128(sW + q * (BN * 128) + ko); };
+          umma(tmem, A_(0), W_(0), idesc, first);                 // leading product -> accumulator 0
+          if (NPW == 3) {                                         // corrections, smallest first -> accumulator 1
+            umma(tmem + BN, A_(0), W_(2), idesc, first);
+            umma(tmem + BN, A_(2), W_(0), idesc, 1u);
+            umma(tmem + BN, A_(1), W_(1), idesc, 1u);
+            umma(tmem + BN, A_(0), W_(1), idesc, 1u);
+            umma(tmem + BN, A_(1), W_(0), idesc, 1u);
+          } else {
+            umma(tmem + BN, A_(2), W_(0), idesc, first);
+            umma(tmem + BN, A_(1), W_(0), idesc, 1u);
+          }
+        }
+        umma_commit(smem_u32(&empty_bar[s]));                     // stage free when these MMAs have read it
+        if (kb < 16) TC_TRACE(24 + kb);
+      }
+      umma_commit(smem_u32(&acc_bar));                            // accumulators complete
+    }
+  } else {
+    // ===================================================================== epilogue warps
     if (EPI == EPI_INPROJ) {
+      // S2: rstd of the tile's 128 rows from the fp32 residual stream, while the main loop runs.
+      // Fixed order: per lane ascending k, then the xor butterfly 16, 8, 4, 2, 1.
+      const int K = KB * BK;
+#pragma unroll 1
+      for (int j0 = 0; j0 < 16; j0 += 4) {
+        float ss[4] = {0.f, 0.f, 0.f, 0.f};
+        for (int q = lane; q < (K >> 2); q += 32) {
+          float4 v[4];
 #pragma unroll
-      for (int it = 0; it < 4; ++it) {
-        float v = ss[it];
-        v += __shfl_xor_sync(0xffffffffu, v, 1);
-        v += __shfl_xor_sync(0xffffffffu, v, 2);
-        v += __shfl_xor_sync(0xffffffffu, v, 4);
-        if (c == 0) rstd_s[it * 32 + (tid >> 3)] = 1.0f / sqrtf(v / (float)g.K + kEps);
+          for (int j = 0; j < 4; ++j)
+            v[j] = *reinterpret_cast<const float4*>(g.U + (size_t)min(m0 + warp * 16 + j0 + j, g.M - 1) * K + q * 4);
+#pragma unroll
+          for (int j = 0; j < 4; ++j) {
+            ss[j] = fmaf(v[j].x, v[j].x, ss[j]); ss[j] = fmaf(v[j].y, v[j].y, ss[j]);
+            ss[j] = fmaf(v[j].z, v[j].z, ss[j]); ss[j] = fmaf(v[j].w, v[j].w, ss[j]);
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+          float v = ss[j];
+#pragma unroll
+          for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+          if (lane == 0) rstd_s[warp * 16 + j0 + j] = 1.0f / sqrtf(v / (float)K + kEps);
+        }
       }
       asm volatile("bar.sync 1, 256;" ::: "memory");
     }
@@ -319,91 +354,82 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     }
     asm volatile("bar.sync 1, 256;" ::: "memory");
     if (tid == 0) TC_TRACE(3);
-    // Pass 2: a group of BN/4 lanes owns one row segment; 4 consecutive columns per lane.
+    // Pass 2: a group of BN/4 lanes owns one row segment; 4 consecutive columns per lane.  Rows are processed four
+    // at a time with all loads issued first.
     constexpr int LPR = BN / 4;                    // lanes per row
     constexpr int RPI = 32 / LPR;                  // rows per warp instruction
     constexpr int NIT = BM / (8 * RPI);            // row groups per warp
+    static_assert(NIT % 4 == 0, "row batching");
     const int col = (lane % LPR) * 4;
     const int nb = n0 + col;
     if (EPI == EPI_INPROJ && n0 < g.E) {
       // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU; the window moves one step (R#11).
-      // The lane's four channels are fixed, so their taps and biases live in registers.
+      // The lane's four channels are fixed, so their taps and biases live in registers.  xs goes out twice: fp32
+      // (the scan reads it) and cut into pieces in the image of x_proj's operand.
       const float4 cw0 = g.conv_w[nb], cw1 = g.conv_w[nb + 1], cw2 = g.conv_w[nb + 2], cw3 = g.conv_w[nb + 3];
       const float4 cb = *reinterpret_cast<const float4*>(g.conv_b + nb);
-#pragma unroll 4
-      for (int i = 0; i < NIT; ++i) {
-        const int r = (warp + 8 * i) * RPI + lane / LPR;
-        const int row = m0 + r;
-        if (row < g.M) {
-          const float4 x = *reinterpret_cast<const float4*>(stile + r * LDS + col);
-          float* wp = g.win + (size_t)row * 3 * g.E + nb;
-          const float4 w0 = *reinterpret_cast<const float4*>(wp);
-          const float4 w1 = *reinterpret_cast<const float4*>(wp + g.E);
-          const float4 w2 = *reinterpret_cast<const float4*>(wp + 2 * g.E);
+#pragma unroll 1
+      for (int i0 = 0; i0 < NIT; i0 += 4) {
+        float4 x[4], w0[4], w1[4], w2[4];
+        int rows[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int r = (warp + 8 * (i0 + u)) * RPI + lane / LPR;
+          rows[u] = m0 + r;
+          x[u] = *reinterpret_cast<const float4*>(stile + r * LDS + col);
+          const float* wp = g.win + (size_t)min(rows[u], g.M - 1) * 3 * g.E + nb;
+          w0[u] = *reinterpret_cast<const float4*>(wp);
+          w1[u] = *reinterpret_cast<const float4*>(wp + g.E);
+          w2[u] = *reinterpret_cast<const float4*>(wp + 2 * g.E);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          if (rows[u] >= g.M) continue;
           float4 o;
-          { float xc = fmaf(cw0.w, x.x, cb.x); xc = fmaf(cw0.x, w0.x, xc); xc = fmaf(cw0.y, w1.x, xc); xc = fmaf(cw0.z, w2.x, xc); o.x = xc * sigmoid_tc(xc); }
-          { float xc = fmaf(cw1.w, x.y, cb.y); xc = fmaf(cw1.x, w0.y, xc); xc = fmaf(cw1.y, w1.y, xc); xc = fmaf(cw1.z, w2.y, xc); o.y = xc * sigmoid_tc(xc); }
-          { float xc = fmaf(cw2.w, x.z, cb.z); xc = fmaf(cw2.x, w0.z, xc); xc = fmaf(cw2.y, w1.z, xc); xc = fmaf(cw2.z, w2.z, xc); o.z = xc * sigmoid_tc(xc); }
-          { float xc = fmaf(cw3.w, x.w, cb.w); xc = fmaf(cw3.x, w0.w, xc); xc = fmaf(cw3.y, w1.w, xc); xc = fmaf(cw3.z, w2.w, xc); o.w = xc * sigmoid_tc(xc); }
-          *reinterpret_cast<float4*>(wp) = w1;
-          *reinterpret_cast<float4*>(wp + g.E) = w2;
-          *reinterpret_cast<float4*>(wp + 2 * g.E) = x;
-          *reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + nb) = o;
+          { float xc = fmaf(cw0.w, x[u].x, cb.x); xc = fmaf(cw0.x, w0[u].x, xc); xc = fmaf(cw0.y, w1[u].x, xc); xc = fmaf(cw0.z, w2[u].x, xc); o.x = xc * sigmoid_tc(xc); }
+          { float xc = fmaf(cw1.w, x[u].y, cb.y); xc = fmaf(cw1.x, w0[u].y, xc); xc = fmaf(cw1.y, w1[u].y, xc); xc = fmaf(cw1.z, w2[u].y, xc); o.y = xc * sigmoid_tc(xc); }
+          { float xc = fmaf(cw2.w, x[u].z, cb.z); xc = fmaf(cw2.x, w0[u].z, xc); xc = fmaf(cw2.y, w1[u].z, xc); xc = fmaf(cw2.z, w2[u].z, xc); o.z = xc * sigmoid_tc(xc); }
+          { float xc = fmaf(cw3.w, x[u].w, cb.w); xc = fmaf(cw3.x, w0[u].w, xc); xc = fmaf(cw3.y, w1[u].w, xc); xc = fmaf(cw3.z, w2[u].w, xc); o.w = xc * sigmoid_tc(xc); }
+          float* wp = g.win + (size_t)rows[u] * 3 * g.E + nb;
+          *reinterpret_cast<float4*>(wp) = w1[u];
+          *reinterpret_cast<float4*>(wp + g.E) = w2[u];
+          *reinterpret_cast<float4*>(wp + 2 * g.E) = x[u];
+          *reinterpret_cast<float4*>(g.C + (size_t)rows[u] * g.ldc + nb) = o;
+          cut4_store(g.out_img, g.out_KB, rows[u], nb, o);
         }
       }
     } else if (nb < g.n_valid) {
-#pragma unroll 4
-      for (int i = 0; i < NIT; ++i) {
-        const int r = (warp + 8 * i) * RPI + lane / LPR;
-        const int row = m0 + r;
-        if (row < g.M) {
-          float4 o = *reinterpret_cast<const float4*>(stile + r * LDS + col);
-          float4* cp = reinterpret_cast<float4*>(g.C + (size_t)row * g.ldc + nb);
-          if (EPI == EPI_RESID) {
-            const float4 q = *cp;
-            o.x += q.x; o.y += q.y; o.z += q.z; o.w += q.w;
-          }
-          *cp = o;
-        }
-      }
-    }
-  } else if (lane == 0) {
-    // ===================================================================== MMA issuer
-    constexpr uint32_t idesc = idesc_bf16(BN);
-    for (int kb = 0; kb < KB; ++kb) {
-      const int s = kb % C::NST, round = kb / C::NST;
-      mbar_wait(smem_u32(&full_bar[s]), (uint32_t)(round & 1));
-      tc_fence_after();
-      if (kb < 16) TC_TRACE(40 + kb);
-      const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
-      const uint32_t sW = sA + NPA * A_PLANE;
+      float4 osc = make_float4(1.f, 1.f, 1.f, 1.f);
+      if (EPI == EPI_RESID && g.out_scale) osc = *reinterpret_cast<const float4*>(g.out_scale + nb);
+#pragma unroll 1
+      for (int i0 = 0; i0 < NIT; i0 += 4) {
+        float4 o[4], q[4];
+        int rows[4];
 #pragma unroll
-      for (int k4 = 0; k4 < BK / 16; ++k4) {
-        const uint32_t first = (kb | k4) ? 1u : 0u;
-        const uint32_t ko = (uint32_t)k4 * 32u;
-        auto A_ = [&](int p) { return smem_desc_sw128(sA + p * A_PLANE + ko); };
-        auto W_ = [&](int q) { return smem_desc_sw128(sW + q * C::W_PLANE + ko); };
-        umma(tmem, A_(0), W_(0), idesc, first);                 // leading product -> accumulator 0
-        if (NPW == 3) {                                         // corrections, smallest first -> accumulator 1
-          umma(tmem + BN, A_(0), W_(2), idesc, first);
-          umma(tmem + BN, A_(2), W_(0), idesc, 1u);
-          umma(tmem + BN, A_(1), W_(1), idesc, 1u);
-          umma(tmem + BN, A_(0), W_(1), idesc, 1u);
-          umma(tmem + BN, A_(1), W_(0), idesc, 1u);
-        } else {
-          umma(tmem + BN, A_(2), W_(0), idesc, first);
-          umma(tmem + BN, A_(1), W_(0), idesc, 1u);
+        for (int u = 0; u < 4; ++u) {
+          const int r = (warp + 8 * (i0 + u)) * RPI + lane / LPR;
+          rows[u] = m0 + r;
+          o[u] = *reinterpret_cast<const float4*>(stile + r * LDS + col);
+          if (EPI == EPI_RESID) q[u] = *reinterpret_cast<const float4*>(g.C + (size_t)min(rows[u], g.M - 1) * g.ldc + nb);
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          if (rows[u] >= g.M) continue;
+          if (EPI == EPI_RESID) {
+            // S9: the residual stream, and its image (times the consumer's RMSNorm weight) for the next contraction
+            o[u].x += q[u].x; o[u].y += q[u].y; o[u].z += q[u].z; o[u].w += q[u].w;
+            cut4_store(g.out_img, g.out_KB, rows[u], nb,
+                       make_float4(o[u].x * osc.x, o[u].y * osc.y, o[u].z * osc.z, o[u].w * osc.w));
+          }
+          *reinterpret_cast<float4*>(g.C + (size_t)rows[u] * g.ldc + nb) = o[u];
         }
       }
-      umma_commit(smem_u32(&empty_bar[s]));                     // stage free when these MMAs have read it
     }
-    umma_commit(smem_u32(&acc_bar));                            // accumulators complete
+    if (tid == 0) TC_TRACE(4);
   }
 
-  if (tid == 0) TC_TRACE(4);
   tc_fence_before();
   __syncthreads();
-  if (tid == 0) TC_TRACE(5);
   if (warp == 8) {
     __syncwarp();
     tmem_dealloc(tmem, C::TMEM_COLS);
