@@ -224,7 +224,10 @@ int init_kernels() {
   BOA_TRY((optin_tc<64, 3, tc::EPI_STORE>()));
   BOA_TRY((optin_tc<64, 1, tc::EPI_RESID>()));
   BOA_TRY((optin_tc<64, 3, tc::EPI_RESID>()));
-  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 64)));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 64)));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
   return BOA_OK;
 }
 
@@ -233,7 +236,18 @@ int launch_tc_npw(int npw, const tc::GemmArgs& g, int N, cudaStream_t st) {
   return npw == 1 ? launch_tc<BN, 1, EPI>(g, N, st) : launch_tc<BN, 3, EPI>(g, N, st);
 }
 
-// One model step + one coder step for all B streams of the wave (S1-S14).
+// S1 for the first step of a wave: u = Emb[byte 0] (later steps: fused into the coder step).
+int launch_embed(StepCtx& c) {
+  boa_model* m = c.m;
+  const int total = c.B * (m->D / 4);
+  k_embed<<<(total + 255) / 256, 256, 0, c.st>>>(c.data, c.chunk_bytes, c.ca.pos, c.ca.len,
+                                                  reinterpret_cast<const float4*>(m->emb), m->u.as<float4>(),
+                                                  reinterpret_cast<const float4*>(m->layers[0].norm_w),
+                                                  m->u_img.as<uint8_t>(), c.B, m->D / 4);
+  return mark(c, BOA_K_EMBED);
+}
+
+// One model step + one coder step for all B streams of the wave (S2-S14, and S1 of the next step).
 int launch_step(StepCtx& c) {
   boa_model* m = c.m;
   const int B = c.B, D = m->D, E = m->E;
@@ -245,13 +259,6 @@ int launch_step(StepCtx& c) {
   uint8_t* xs_img = m->xs_img.as<uint8_t>();
   uint8_t* y_img = m->y_img.as<uint8_t>();
 
-  {
-    const int total = B * (D / 4);
-    k_embed<<<(total + 255) / 256, 256, 0, c.st>>>(c.data, c.chunk_bytes, c.ca.pos, c.ca.len,
-                                                    reinterpret_cast<const float4*>(m->emb), reinterpret_cast<float4*>(u),
-                                                    reinterpret_cast<const float4*>(m->layers[0].norm_w), u_img, B, D / 4);
-    BOA_TRY(mark(c, BOA_K_EMBED));
-  }
   for (int l = 0; l < m->L; ++l) {
     const LayerW& w = m->layers[l];
     float* hl = m->h.as<float>() + (size_t)l * m->Bcap * E * kNState;
@@ -279,7 +286,13 @@ int launch_step(StepCtx& c) {
       sa.y_img = y_img; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
       const int ec = (E % 256 == 0) ? 256 : 128, slices = E / ec;
       const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
-      k_scan<<<dim3(per_slice, slices), ec, scan::smem_bytes(ec, m->ldj, m->R), c.st>>>(sa);
+      const dim3 grid(per_slice, slices);
+      switch (m->R) {   // W_dt's row in registers when it is short enough
+        case 4: k_scan<4><<<grid, ec + 32, scan::smem_bytes(ec, m->ldj, 0), c.st>>>(sa); break;
+        case 8: k_scan<8><<<grid, ec + 32, scan::smem_bytes(ec, m->ldj, 0), c.st>>>(sa); break;
+        case 16: k_scan<16><<<grid, ec + 32, scan::smem_bytes(ec, m->ldj, 0), c.st>>>(sa); break;
+        default: k_scan<0><<<grid, ec + 32, scan::smem_bytes(ec, m->ldj, m->R), c.st>>>(sa); break;
+      }
       BOA_TRY(mark(c, BOA_K_SCAN));
     }
     {  // S9: u += W_out y;  the new u also as the image for the next in_proj (times its RMSNorm weight) or the head
@@ -301,18 +314,21 @@ int launch_step(StepCtx& c) {
   }
 
   const int cgrid = (B * 32 + 255) / 256;
+  EmbedArgs ea{};
+  ea.emb = reinterpret_cast<const float4*>(m->emb); ea.norm_w = reinterpret_cast<const float4*>(m->layers[0].norm_w);
+  ea.u = m->u.as<float4>(); ea.u_img = u_img; ea.D4 = D / 4;
   if (c.dump) {
     if (c.dump_logits) {
       BOA_CUDA_TRY(cudaMemcpy2DAsync(c.dump_logits + (size_t)c.dump_t * 256, (size_t)c.dump_steps * 256 * sizeof(float),
                                      logits, 256 * sizeof(float), 256 * sizeof(float), B,
                                      cudaMemcpyDeviceToDevice, c.st));
     }
-    k_coder_step<0, true><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, c.dump_probs,
+    k_coder_step<0, true><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, ea, c.dump_probs,
                                                    c.dump_cdf, c.dump_steps);
   } else if (c.mode == 0) {
-    k_coder_step<0, false><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, nullptr, nullptr, 0);
+    k_coder_step<0, false><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, ea, nullptr, nullptr, 0);
   } else {
-    k_coder_step<1, false><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, nullptr, nullptr, 0);
+    k_coder_step<1, false><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, ea, nullptr, nullptr, 0);
   }
   BOA_TRY(mark(c, BOA_K_CODER));
   return BOA_OK;
@@ -583,11 +599,11 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
     }
     ok = ok && br.take(E, false, t); if (ok) o.b_dt = append(t);
     ok = ok && br.take(E * kNState, false, t);
-    if (ok) {                                                                 // A = -exp(A_log), layout [4][E][4]
-      t2.assign(E * kNState, 0.0f);
+    if (ok) {                                                // A * log2(e), A = -exp(A_log) (eq. 16), layout [4][E][4]:
+      t2.assign(E * kNState, 0.0f);                          // the scan computes exp(delta A) as 2^(delta * this)
       for (size_t e = 0; e < E; ++e)
         for (size_t n = 0; n < (size_t)kNState; ++n)
-          t2[((n / 4) * E + e) * 4 + (n % 4)] = (float)(-exp((double)t[e * kNState + n]));
+          t2[((n / 4) * E + e) * 4 + (n % 4)] = (float)(-exp((double)t[e * kNState + n]) * 1.4426950408889634);
       o.A4 = append(t2);
     }
     ok = ok && br.take(E, false, t); if (ok) o.d_skip = append(t);
@@ -707,6 +723,7 @@ int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, 
     k_first_bytes<<<g, 256, 0, st>>>(c.data, chunk_bytes, m->first.as<uint8_t>(), (int)B);
     BOA_TRY(mark(c, BOA_K_FINISH));
     const uint64_t max_len = std::min<uint64_t>(chunk_bytes, n_wave);
+    if (max_len > 1) BOA_TRY(launch_embed(c));
     BOA_TRY(run_steps(c, max_len - 1));
     m->prof.steps += max_len - 1;
     k_coder_finish<0><<<g, 256, 0, st>>>(c.ca, (int)B);
@@ -839,6 +856,7 @@ int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len, uint8_t* out,
     k_coder_init<1><<<g, 256, 0, st>>>(c.ca, (int)B, chunk_bytes, n_wave, m->first.as<uint8_t>(), c.data);
     BOA_TRY(mark(c, BOA_K_FINISH));
     const uint64_t max_len = std::min<uint64_t>(chunk_bytes, n_wave);
+    if (max_len > 1) BOA_TRY(launch_embed(c));
     BOA_TRY(run_steps(c, max_len - 1));
     m->prof.steps += max_len - 1;
     k_coder_finish<1><<<g, 256, 0, st>>>(c.ca, (int)B);
@@ -914,6 +932,7 @@ int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_
   c.dump_steps = (uint32_t)n_steps;
   k_coder_init<0><<<(int)((B + 255) / 256), 256, 0, st>>>(c.ca, (int)B, chunk_bytes, n, nullptr, nullptr);
   BOA_TRY(mark(c, BOA_K_FINISH));
+  BOA_TRY(launch_embed(c));
   BOA_TRY(run_steps(c, n_steps));
   BOA_TRY(tl.finish(st));
   BOA_TRY(tp.finish(st));

@@ -13,6 +13,7 @@
 // it carries the coder state of that stream ("one thread per chunk", R#19).
 #pragma once
 #include "common.cuh"
+#include "tc_gemm.cuh"
 
 namespace boa {
 
@@ -195,6 +196,24 @@ struct CoderArrays {
   int* err;             // device flag: != 0 -> BOA_E_CORRUPT
 };
 
+// S1 for the NEXT step, fused into the coder step: once the symbol is known the warp writes u = Emb[s] (fp32, the
+// residual stream) and the image of u * norm_w(layer 0), the operand of the first in_proj (tc_gemm.cuh).
+struct EmbedArgs {
+  const float4* emb;       // [256][D/4]
+  const float4* norm_w;    // [D/4] RMSNorm weight of layer 0
+  float4* u;               // [B][D/4]
+  uint8_t* u_img;
+  int D4;
+};
+__device__ __forceinline__ void embed_row(const EmbedArgs& ea, int i, uint32_t s, int lane) {
+  for (int q = lane; q < ea.D4; q += 32) {
+    const float4 v = ea.emb[s * ea.D4 + q];
+    ea.u[(size_t)i * ea.D4 + q] = v;
+    const float4 w = ea.norm_w[q];
+    tc::cut4_store(ea.u_img, ea.D4 >> 4, i, q * 4, make_float4(v.x * w.x, v.y * w.y, v.z * w.z, v.w * w.w));
+  }
+}
+
 // -------------------------------------------------------------------------------------- step kernel
 // MODE 0 = encode, 1 = decode.  One warp per stream.  `data` is the input (encode) or output (decode)
 // buffer of this wave: stream i, byte t at data[i*chunk + t].
@@ -202,7 +221,7 @@ struct CoderArrays {
 template <int MODE, bool DUMP>
 __global__ void __launch_bounds__(256)
 k_coder_step(const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes, CoderArrays ca, int B,
-             float* dump_probs, uint32_t* dump_cdf, uint32_t dump_steps) {
+             EmbedArgs ea, float* dump_probs, uint32_t* dump_cdf, uint32_t dump_steps) {
   const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   if (i >= B) return;
@@ -245,6 +264,7 @@ k_coder_step(const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes
   uint8_t* sdata = data + (size_t)i * chunk_bytes;
   if (MODE == 0) {
     const uint32_t s = sdata[pos + 1u];
+    embed_row(ea, i, s, lane);
     uint32_t c_lo, c_hi;
     table_interval(t, s, c_lo, c_hi);
     if (lane == 0) {
@@ -266,6 +286,7 @@ k_coder_step(const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes
     }
     x = __shfl_sync(0xffffffffu, x, 0);
     const uint32_t s = table_search(t, x);
+    embed_row(ea, i, s, lane);
     uint32_t c_lo, c_hi;
     table_interval(t, s, c_lo, c_hi);
     if (lane == 0) {

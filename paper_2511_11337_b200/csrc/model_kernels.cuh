@@ -51,8 +51,9 @@ __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, con
 //   delta = softplus(b_dt[e] + sum_r W_dt[e][r] dlt[r])                      (sequential fp32 FMA chain, r ascending)
 //   h[n] = exp(delta*A[n]) * h[n] + (delta*Bv[n]) * xs ;  y = sum_n Cv[n] h[n] + D xs ;  y *= SiLU(z)
 //
-// State layout: h[i][j][e] is a float4 holding n = 4j..4j+3, so the state of one
-// stream and a slice of EC channels is four contiguous runs of EC*16 bytes.  HBM-bound: per stream and slice the
+// State layout: h[i][slice][j][c] is a float4 holding n = 4j..4j+3 of channel slice*EC+c,
+// so the state of one stream and a slice of EC channels is ONE contiguous run of EC*64 bytes (one bulk copy in, one
+// out) and a warp reads 512 contiguous bytes of it per shared-memory load.  HBM-bound: per stream and slice the
 // kernel moves 2*EC*64 bytes of state against ~160 instructions per channel, so the design goal is bytes in
 // flight, not arithmetic: a persistent CTA owns a channel slice and walks over streams with a ring of NSTG shared
 // memory stages.  Everything a stream-step needs (4 state runs, xs, z, the x_proj row) is brought in by the
@@ -62,29 +63,21 @@ __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, con
 // operand tile (tc_gemm.cuh).
 // One thread per channel of the slice holds A[e][0..15] in registers; W_dt^T of the slice lives in shared memory.
 struct ScanArgs {
-  float* h;                 // [B][4][E] float4 (this layer)
+  float* h;                 // [B][E/EC][4][EC] float4 (this layer): the state of a stream and channel slice is one contiguous run
   const float* xz;          // [B][2E]: xs | z
   const float* dbc;         // [B][ldj]: dlt[R] | Bv[16] | Cv[16]
   const float* W_dtT;       // [R][E]
   const float* b_dt;        // [E]
-  const float4* A4;         // [4][E] float4: A = -exp(A_log)
+  const float4* A4;         // [4][E] float4: A * log2(e), A = -exp(A_log)
   const float* Dskip;       // [E]
   uint8_t* y_img;           // image of y[B][E] for out_proj (tc_gemm.cuh)
   int ldj, B, E, R;
 };
 
-__device__ __forceinline__ void scan_update4(float4& h, const float4 a, const float4 bv, const float4 cv,
-                                             float dl, float x, float& y) {
-  h.x = fmaf(expf(dl * a.x), h.x, (dl * bv.x) * x); y = fmaf(cv.x, h.x, y);
-  h.y = fmaf(expf(dl * a.y), h.y, (dl * bv.y) * x); y = fmaf(cv.y, h.y, y);
-  h.z = fmaf(expf(dl * a.z), h.z, (dl * bv.z) * x); y = fmaf(cv.z, h.z, y);
-  h.w = fmaf(expf(dl * a.w), h.w, (dl * bv.w) * x); y = fmaf(cv.w, h.w, y);
-}
-
 namespace scan {
 constexpr int NSTG = 4;
 __host__ __device__ inline int stage_bytes(int EC, int ldj) { return EC * 64 + 2 * EC * 4 + EC * 6 + ldj * 4; }   // h | xs | z | y pieces | dbc
-__host__ __device__ inline int smem_bytes(int EC, int ldj, int R) { return NSTG * stage_bytes(EC, ldj) + R * EC * 4 + NSTG * 8 + 128; }
+__host__ __device__ inline int smem_bytes(int EC, int ldj, int R) { return NSTG * stage_bytes(EC, ldj) + R * EC * 4 + 2 * NSTG * 8 + 128; }   // R = 0 when W_dt sits in registers
 
 __device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void bar_init(uint32_t bar, uint32_t count) {
@@ -121,44 +114,103 @@ __device__ __forceinline__ void s2g_hint(void* dst, uint32_t src, uint32_t bytes
 }
 }  // namespace scan
 
-// grid = (CTAs per slice, E / EC), block = EC = min(E, 256) threads, 2 CTAs per SM.
-__global__ void __launch_bounds__(256, 2) k_scan(const ScanArgs a) {
+// Fast forms for the stateless activations of the scan (relative error ~1e-6, far inside the 1e-5 probability bar;
+// encode and decode run the same code, so determinism is unaffected).
+__device__ __forceinline__ float silu_fast(float x) { return __fdividef(x, 1.0f + __expf(-x)); }
+__device__ __forceinline__ float softplus_fast(float v) { return fmaxf(v, 0.0f) + log1pf(__expf(-fabsf(v))); }
+__device__ __forceinline__ float ex2_approx(float x) {
+  float y;
+  asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+  return y;
+}
+// h <- 2^(dl*a2) h + (dl*Bv) x,  a2 = A*log2(e) (folded into the weights at load);  y += Cv h
+__device__ __forceinline__ void scan_update4(float4& h, const float4 a2, const float4 bv, const float4 cv,
+                                             float dl, float x, float& y) {
+  const float dx = dl * x;
+  h.x = fmaf(ex2_approx(dl * a2.x), h.x, dx * bv.x); y = fmaf(cv.x, h.x, y);
+  h.y = fmaf(ex2_approx(dl * a2.y), h.y, dx * bv.y); y = fmaf(cv.y, h.y, y);
+  h.z = fmaf(ex2_approx(dl * a2.z), h.z, dx * bv.z); y = fmaf(cv.z, h.z, y);
+  h.w = fmaf(ex2_approx(dl * a2.w), h.w, dx * bv.w); y = fmaf(cv.w, h.w, y);
+}
+
+// grid = (CTAs per slice, E / EC), block = EC + 32 threads (EC = 256 or 128), two CTAs per SM.
+// Warps 0..EC/32-1: one thread per channel of the slice.  The last warp drives the bulk copies and moves the y pieces.
+// RR = dt_rank when W_dt's row fits in registers (4, 8, 16), else 0 (row kept in shared memory).
+template <int RR>
+__global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   using namespace scan;
   extern __shared__ __align__(128) uint8_t scan_smem[];
-  const int EC = blockDim.x, tid = threadIdx.x;
-  const int e0 = blockIdx.y * EC, e = e0 + tid;
+  const int EC = blockDim.x - 32, tid = threadIdx.x;
+  const int slices = gridDim.y, sl = blockIdx.y;
+  const int e0 = sl * EC;
   const int SB = stage_bytes(EC, a.ldj);
   uint8_t* stages = scan_smem;
   float* wdt = reinterpret_cast<float*>(scan_smem + NSTG * SB);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(scan_smem + NSTG * SB + a.R * EC * 4);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(scan_smem + NSTG * SB + (RR ? 0 : a.R * EC * 4));   // full[NSTG], done[NSTG]
   const int nk = (a.B - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // streams of this CTA
   if (nk <= 0) return;
 
-  uint64_t pol;
-  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-  const uint32_t tx = (uint32_t)(EC * 64 + 2 * EC * 4 + a.ldj * 4);
-  auto issue_load = [&](int k) {   // thread 0
-    const int s = k % NSTG;
-    const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
-    const uint32_t st = s_u32(stages + s * SB), bar = s_u32(&bars[s]);
-    bar_expect(bar, tx);
-#pragma unroll
-    for (int j = 0; j < 4; ++j)
-      g2s_hint(st + j * EC * 16, a.h + ((i * 4 + j) * a.E + e0) * 4, (uint32_t)(EC * 16), bar, pol);
-    g2s(st + EC * 64, a.xz + i * 2 * a.E + e0, (uint32_t)(EC * 4), bar);
-    g2s(st + EC * 64 + EC * 4, a.xz + i * 2 * a.E + a.E + e0, (uint32_t)(EC * 4), bar);
-    g2s(st + EC * 64 + 2 * EC * 4 + EC * 6, a.dbc + i * a.ldj, (uint32_t)(a.ldj * 4), bar);
-  };
-
   if (tid == 0) {
-    for (int s = 0; s < NSTG; ++s) bar_init(s_u32(&bars[s]), 1);
+    for (int s = 0; s < NSTG; ++s) { bar_init(s_u32(&bars[s]), 1); bar_init(s_u32(&bars[NSTG + s]), (uint32_t)EC); }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
-  if (tid == 0)
-    for (int k = 0; k < NSTG && k < nk; ++k) issue_load(k);
 
-  for (int r = 0; r < a.R; ++r) wdt[r * EC + tid] = a.W_dtT[(size_t)r * a.E + e];   // private column: no sync needed
+  if (tid >= EC) {
+    // ===================================================================== copy warp
+    const int lane = tid - EC;
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    const uint32_t tx = (uint32_t)(EC * 64 + 2 * EC * 4 + a.ldj * 4);
+    auto issue_load = [&](int k) {   // lane 0
+      const int s = k % NSTG;
+      const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+      const uint32_t st = s_u32(stages + s * SB), bar = s_u32(&bars[s]);
+      bar_expect(bar, tx);
+      g2s_hint(st, a.h + ((i * slices + sl) * 4) * (size_t)EC * 4, (uint32_t)(EC * 64), bar, pol);
+      g2s(st + EC * 64, a.xz + i * 2 * a.E + e0, (uint32_t)(EC * 4), bar);
+      g2s(st + EC * 64 + EC * 4, a.xz + i * 2 * a.E + a.E + e0, (uint32_t)(EC * 4), bar);
+      g2s(st + EC * 64 + 2 * EC * 4 + EC * 6, a.dbc + i * a.ldj, (uint32_t)(a.ldj * 4), bar);
+    };
+    if (lane == 0)
+      for (int k = 0; k < NSTG && k < nk; ++k) issue_load(k);
+    const int nchunks = (EC >> 6) * 24;          // 16-byte chunks of the y pieces of one stream-slice
+    for (int k = 0; k < nk; ++k) {
+      const int s = k % NSTG;
+      uint8_t* st = stages + s * SB;
+      bar_wait(s_u32(&bars[NSTG + s]), (uint32_t)((k / NSTG) & 1));      // every channel of stream k is done
+      const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+      if (lane == 0) {
+        s2g_hint(a.h + ((i * slices + sl) * 4) * (size_t)EC * 4, s_u32(st), (uint32_t)(EC * 64), pol);
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+      }
+      // y pieces: row (c/8) = (64-channel block, piece), chunk c%8 of its 128-byte row in out_proj's operand image
+      const int r = (int)(i & 127);
+      for (int c = lane; c < nchunks; c += 32) {
+        const int rowid = c >> 3, kt = rowid / 3, q = rowid - kt * 3;
+        uint8_t* dst = a.y_img + tc::img_block(i >> 7, (size_t)(e0 >> 6) + kt, (size_t)(a.E >> 6)) + (size_t)q * tc::A_PLANE +
+                       (r >> 3) * 1024 + (r & 7) * 128 + (c & 7) * 16;
+        *reinterpret_cast<uint4*>(dst) = *reinterpret_cast<const uint4*>(st + EC * 64 + 2 * EC * 4 + rowid * 128 + (c & 7) * 16);
+      }
+      __syncwarp();
+      if (lane == 0 && k >= 1 && k - 1 + NSTG < nk) {
+        asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the store of stream k-1 has left its stage
+        issue_load(k - 1 + NSTG);
+      }
+    }
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    return;
+  }
+
+  // ======================================================================= channel threads
+  const int e = e0 + tid;
+  float wr[RR ? RR : 1];
+  if constexpr (RR > 0) {
+#pragma unroll
+    for (int r = 0; r < RR; ++r) wr[r] = a.W_dtT[(size_t)r * a.E + e];
+  } else {
+    for (int r = 0; r < a.R; ++r) wdt[r * EC + tid] = a.W_dtT[(size_t)r * a.E + e];   // private column: no sync needed
+  }
   const float4 a0 = a.A4[e], a1 = a.A4[a.E + e], a2 = a.A4[2 * a.E + e], a3 = a.A4[3 * a.E + e];
   const float dsk = a.Dskip[e];
   const float bdt = a.b_dt[e];
@@ -172,29 +224,40 @@ __global__ void __launch_bounds__(256, 2) k_scan(const ScanArgs a) {
     const float* row = reinterpret_cast<const float*>(st + EC * 64 + 2 * EC * 4 + EC * 6);
     const float x = xs_s[tid];
     const float z = xs_s[EC + tid];
-    float acc = bdt;
-    for (int r = 0; r < a.R; r += 4) {
-      const float4 d = *reinterpret_cast<const float4*>(row + r);
-      acc = fmaf(wdt[(r + 0) * EC + tid], d.x, acc);
-      acc = fmaf(wdt[(r + 1) * EC + tid], d.y, acc);
-      acc = fmaf(wdt[(r + 2) * EC + tid], d.z, acc);
-      acc = fmaf(wdt[(r + 3) * EC + tid], d.w, acc);
-    }
-    const float dl = softplusf_(acc);
-    const float4* bcp = reinterpret_cast<const float4*>(row + a.R);
     float4 h0 = hs[tid], h1 = hs[EC + tid], h2 = hs[2 * EC + tid], h3 = hs[3 * EC + tid];
+    float acc = bdt;
+    if constexpr (RR > 0) {
+#pragma unroll
+      for (int r = 0; r < RR; r += 4) {
+        const float4 d = *reinterpret_cast<const float4*>(row + r);
+        acc = fmaf(wr[r], d.x, acc);
+        acc = fmaf(wr[r + 1], d.y, acc);
+        acc = fmaf(wr[r + 2], d.z, acc);
+        acc = fmaf(wr[r + 3], d.w, acc);
+      }
+    } else {
+      for (int r = 0; r < a.R; r += 4) {
+        const float4 d = *reinterpret_cast<const float4*>(row + r);
+        acc = fmaf(wdt[(r + 0) * EC + tid], d.x, acc);
+        acc = fmaf(wdt[(r + 1) * EC + tid], d.y, acc);
+        acc = fmaf(wdt[(r + 2) * EC + tid], d.z, acc);
+        acc = fmaf(wdt[(r + 3) * EC + tid], d.w, acc);
+      }
+    }
+    const float dl = softplus_fast(acc);
+    const float4* bcp = reinterpret_cast<const float4*>(row + a.R);
     float yv = 0.0f;
     scan_update4(h0, a0, bcp[0], bcp[4], dl, x, yv);
     scan_update4(h1, a1, bcp[1], bcp[5], dl, x, yv);
     scan_update4(h2, a2, bcp[2], bcp[6], dl, x, yv);
     scan_update4(h3, a3, bcp[3], bcp[7], dl, x, yv);
     yv = fmaf(dsk, x, yv);
-    yv *= siluf_(z);
+    yv *= silu_fast(z);
     hs[tid] = h0; hs[EC + tid] = h1; hs[2 * EC + tid] = h2; hs[3 * EC + tid] = h3;
-    const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
     {
       // y -> three bf16 pieces (truncation split, exact), staged as [64-channel block][piece][128-byte swizzled row]
-      uint8_t* yp = st + EC * 64 + 2 * EC * 4 + ((tid >> 6) * 3) * 128 + (((((tid & 63) >> 3) ^ (int)i) & 7) << 4) + (tid & 7) * 2;
+      const int i7 = (int)((blockIdx.x + (size_t)k * gridDim.x) & 7);
+      uint8_t* yp = st + EC * 64 + 2 * EC * 4 + ((tid >> 6) * 3) * 128 + (((((tid & 63) >> 3) ^ i7) & 7) << 4) + (tid & 7) * 2;
 #pragma unroll
       for (int q = 0; q < 3; ++q) {
         *reinterpret_cast<uint16_t*>(yp + q * 128) = (uint16_t)(__float_as_uint(yv) >> 16);
@@ -202,28 +265,8 @@ __global__ void __launch_bounds__(256, 2) k_scan(const ScanArgs a) {
       }
     }
     asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-    __syncthreads();
-    if (tid < (EC >> 6) * 24) {
-      // one 16-byte chunk per thread: row (tid/8) = (64-channel block, piece), chunk tid%8 of its 128-byte row
-      const int rowid = tid >> 3, kt = rowid / 3, q = rowid - kt * 3;
-      const int r = (int)(i & 127);
-      uint8_t* dst = a.y_img + tc::img_block(i >> 7, (size_t)(e0 >> 6) + kt, (size_t)(a.E >> 6)) + (size_t)q * tc::A_PLANE +
-                     (r >> 3) * 1024 + (r & 7) * 128 + (tid & 7) * 16;
-      *reinterpret_cast<uint4*>(dst) = *reinterpret_cast<const uint4*>(st + EC * 64 + 2 * EC * 4 + rowid * 128 + (tid & 7) * 16);
-    }
-    if (tid == 0) {
-      const uint32_t sa = s_u32(st);
-#pragma unroll
-      for (int j = 0; j < 4; ++j)
-        s2g_hint(a.h + ((i * 4 + j) * a.E + e0) * 4, sa + j * EC * 16, (uint32_t)(EC * 16), pol);
-      asm volatile("cp.async.bulk.commit_group;" ::: "memory");
-      if (k >= 1 && k - 1 + NSTG < nk) {
-        asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the stores of stream k-1 have left its stage
-        issue_load(k - 1 + NSTG);
-      }
-    }
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(&bars[NSTG + s])) : "memory");
   }
-  if (tid == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
 }
 
 }  // namespace boa

@@ -10,10 +10,13 @@
 // Precision.  The activations are fp32 and the four parity checks need
 // fp32-level products, so each operand is cut into bf16 pieces that sum to it exactly (a = a1+a2+a3, 8 significant
 // bits each) and the tensor cores multiply the pieces: tcgen05.mma kind::f16 (bf16 x bf16 -> fp32 in TMEM).
-//   bf16 weights (one exact piece w):   a1 w | a2 w + a3 w                               3 MMAs per k-step
-//   fp32 weights (w = w1+w2+w3):        a1 w1 | a1 w3 + a3 w1 + a2 w2 + a1 w2 + a2 w1    6 MMAs per k-step
-// The leading product has its own TMEM accumulator; all correction products (2^-8 and smaller) go to a second one and
-// the two are added once, in fp32, in the epilogue.  Dropped products are below 2^-24 of |a||w|.
+//   bf16 weights (one exact piece w):   a1 w | a2 w + a3 w                               3 products per k-step
+//   fp32 weights (w = w1+w2+w3):        a1 w1 | a1 w2 + a2 w1 | a1 w3 + a2 w2 + a3 w1    6 products per k-step
+// Products of the same magnitude class (1, 2^-8, 2^-16) share a TMEM accumulator; the classes are added once, in
+// fp32, smallest first, in the epilogue.  Dropped products are below 2^-24 of |a||w|.
+// The weight pieces of a tile are stacked along N in shared memory ([w1; w2; w3]), so one MMA of a piece of A against
+// the stack yields several products at once and A is read from shared memory once for them:
+//   a1 x [w1;w2;w3] -> classes 0,1,2   a2 x [w1;w2] -> classes 1,2   a3 x [w1] -> class 2       (N = 3, 2, 1 x BN)
 //
 // Data movement.  Both operands reach shared memory through the bulk-copy engine (TMA, cp.async.bulk -> SASS UBLKCP)
 // as ready-made images of a tile (K-major, 128-byte swizzle), so the main loop is TMA + MMA only:
@@ -199,10 +202,12 @@ struct Cfg {
   static constexpr int STAGE = A_BYTES + W_BYTES;
   static constexpr int NST = (4 * STAGE <= 216 * 1024) ? 4 : (3 * STAGE <= 216 * 1024) ? 3 : 2;
   static constexpr int SMEM = NST * STAGE + 1024;             // + alignment slack
-  static constexpr int TMEM_COLS = (2 * BN <= 32) ? 32 : (2 * BN <= 64) ? 64 : (2 * BN <= 128) ? 128 : (2 * BN <= 256) ? 256 : 512;
+  static constexpr int NACC = NPW == 3 ? 3 : 2;               // accumulators (magnitude classes)
+  static constexpr int TMEM_COLS = (NACC * BN <= 128) ? 128 : (NACC * BN <= 256) ? 256 : 512;
 };
 
-__device__ __forceinline__ float sigmoid_tc(float x) { return 1.0f / (1.0f + expf(-x)); }
+// sigmoid for the SiLU of the conv epilogue: fast forms (relative error ~1e-6; same code on encode and decode)
+__device__ __forceinline__ float sigmoid_tc(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
 
 constexpr int NEPI = 256;        // epilogue threads (warps 0-7); warp 8 owns TMEM and issues the MMAs; warp 9 drives the copies
 constexpr int NTHREADS = NEPI + 64;
@@ -264,7 +269,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   } else if (warp == 8) {
     // ===================================================================== MMA issuer
     if (lane == 0) {
-      constexpr uint32_t idesc = idesc_bf16(BN);
       for (int kb = 0; kb < KB; ++kb) {
         const int s = kb % C::NST, round = kb / C::NST;
         mbar_wait(smem_u32(&full_bar[s]), (uint32_t)(round & 1));
@@ -278,16 +282,19 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
           const uint32_t ko = (uint32_t)k4 * 32u;
           auto A_ = [&](int p) { return smem_desc_sw128(sA + p * A_PLANE + ko); };
           auto W_ = [&](int q) { return smem_desc_sw128(sW + q * (BN * 128) + ko); };
-          umma(tmem, A_(0), W_(0), idesc, first);                 // leading product -> accumulator 0
-          if (NPW == 3) {                                         // corrections, smallest first -> accumulator 1
-            umma(tmem + BN, A_(0), W_(2), idesc, first);
-            umma(tmem + BN, A_(2), W_(0), idesc, 1u);
-            umma(tmem + BN, A_(1), W_(1), idesc, 1u);
-            umma(tmem + BN, A_(0), W_(1), idesc, 1u);
-            umma(tmem + BN, A_(1), W_(0), idesc, 1u);
+          if (NPW == 3 && BN == 64) {
+            umma(tmem, A_(0), W_(0), idesc_bf16(192), first);        // a1 x [w1;w2;w3] -> classes 0,1,2
+            umma(tmem + 64, A_(1), W_(0), idesc_bf16(128), 1u);      // a2 x [w1;w2]    -> classes 1,2
+            umma(tmem + 128, A_(2), W_(0), idesc_bf16(64), 1u);      // a3 x [w1]       -> class 2
+          } else if (NPW == 3) {                                     // BN = 128: the stack is split at N = 256
+            umma(tmem, A_(0), W_(0), idesc_bf16(256), first);        // a1 x [w1;w2]    -> classes 0,1
+            umma(tmem + 256, A_(0), W_(2), idesc_bf16(128), first);  // a1 x [w3]       -> class 2
+            umma(tmem + 128, A_(1), W_(0), idesc_bf16(256), 1u);     // a2 x [w1;w2]    -> classes 1,2
+            umma(tmem + 256, A_(2), W_(0), idesc_bf16(128), 1u);     // a3 x [w1]       -> class 2
           } else {
-            umma(tmem + BN, A_(2), W_(0), idesc, first);
-            umma(tmem + BN, A_(1), W_(0), idesc, 1u);
+            umma(tmem, A_(0), W_(0), idesc_bf16(BN), first);         // a1 w            -> class 0
+            umma(tmem + BN, A_(2), W_(0), idesc_bf16(BN), first);    // a3 w, a2 w      -> class 1
+            umma(tmem + BN, A_(1), W_(0), idesc_bf16(BN), 1u);
           }
         }
         umma_commit(smem_u32(&empty_bar[s]));                     // stage free when these MMAs have read it
@@ -343,8 +350,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
         const int ch = (warp >> 2) * CPW + q;
         float v[32], w[32];
         __syncwarp();
-        tmem_ld32(tlane + (uint32_t)(ch * 32), v);
-        tmem_ld32(tlane + (uint32_t)(BN + ch * 32), w);
+        tmem_ld32(tlane + (uint32_t)(BN + ch * 32), v);          // class 1
+        if (NPW == 3) {
+          tmem_ld32(tlane + (uint32_t)(2 * BN + ch * 32), w);    // class 2, added first
+#pragma unroll
+          for (int j = 0; j < 32; ++j) v[j] += w[j];
+        }
+        tmem_ld32(tlane + (uint32_t)(ch * 32), w);               // class 0
         float4* dst = reinterpret_cast<float4*>(stile + r * LDS + ch * 32);
 #pragma unroll
         for (int j = 0; j < 32; j += 4)

@@ -155,7 +155,10 @@ def test_probabilities_and_tables_against_oracle(case, boa):
     logits64 = model.logits_for_chunks(w, data)
     p_ref = quantise.softmax(logits64)
     p_gpu = _np(d["probs"]).astype(np.float64)
-    assert np.abs(p_gpu - p_ref).max() <= PROB_TOL, name
+    err = np.abs(p_gpu - p_ref).max()
+    print(f"[parity] {name}: max |p_gpu - p_oracle| = {err:.3e} (bar {PROB_TOL:g}), max p = {p_ref.max():.3f}, "
+          f"max |logit err| = {np.abs(_np(d['logits']) - logits64).max():.3e}")
+    assert err <= PROB_TOL, name
     assert np.abs(_np(d["logits"]) - logits64).max() <= 2e-4 * max(1.0, np.abs(logits64).max())
     # tables: the oracle's rule on the GPU's own fp32 logits must give the GPU's tables, bit for bit
     assert np.array_equal(_np(d["cdf"]).astype(np.int64), quantise.quantise(_np(d["logits"])))
