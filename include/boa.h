@@ -134,9 +134,10 @@ int boa_get_profile(const boa_model* m, boa_profile* out);
  *   same layout and writes syms; BOA_E_CORRUPT on overrun / bytes left over. */
 /* boa_debug_gemm: the tensor-core contraction kernel alone (S3/S5/S9/S10; tc_gemm.cuh):
  *   C[M][N] = A[M][K] W[N][K]^T, A and C host|device fp32 row-major, W a HOST fp32 matrix that is cut into
- *   `weight_pieces` (1 or 3) bf16 pieces exactly as boa_model_load does; tile_n = 64 or 128 selects the
- *   instantiation.  K % 64 == 0. */
-int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N, int weight_pieces, int tile_n,
+ *   `weight_pieces` (1 or 3) bf16 pieces exactly as boa_model_load does; A is cut into its three pieces by the same
+ *   device routine the step kernels use.  grid_ctas = 0 launches one persistent CTA per SM as the step does; a small
+ *   positive value forces several tiles per CTA (the accumulator double-buffering path).  K % 64 == 0. */
+int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N, int weight_pieces, int grid_ctas,
                    float* C, void* cuda_stream);
 int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, size_t n_steps,
                         float* logits, float* probs, uint32_t* cdf, void* cuda_stream);

@@ -207,12 +207,12 @@ def decompressed_size(blob: torch.Tensor) -> int:
     return n.value
 
 
-def debug_gemm(a: torch.Tensor, w: torch.Tensor, weight_pieces: int, tile_n: int) -> torch.Tensor:
+def debug_gemm(a: torch.Tensor, w: torch.Tensor, weight_pieces: int, grid_ctas: int = 0) -> torch.Tensor:
     """a [M,K] fp32 (CUDA or CPU), w [N,K] fp32 CPU -> a @ w.T [M,N] fp32 on a's device, by the tensor-core kernel."""
     a = a.contiguous()
     w = w.contiguous().cpu()
     c = torch.empty((a.shape[0], w.shape[0]), dtype=torch.float32, device=a.device)
-    _check(lib().boa_debug_gemm(_ptr(a), a.shape[0], a.shape[1], _ptr(w), w.shape[0], weight_pieces, tile_n, _ptr(c),
+    _check(lib().boa_debug_gemm(_ptr(a), a.shape[0], a.shape[1], _ptr(w), w.shape[0], weight_pieces, grid_ctas, _ptr(c),
                                 _stream()), "boa_debug_gemm")
     return c
 

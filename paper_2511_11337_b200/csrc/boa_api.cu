@@ -69,7 +69,7 @@ struct boa_model {
 
   // workspace (per wave of Bcap streams)
   uint64_t Bcap = 0;
-  GrowBuf u, xz, dbc, logits, h, win;
+  GrowBuf u, xz, dbc, logits, h, win, ssq;
   GrowBuf u_img, xs_img, y_img;   // activation images: operands of the tensor-core contractions (tc_gemm.cuh)
   GrowBuf pos, len, low, range, pending, wpos, cache, started, v, rpos, off, size, scratch, first, err;
   GrowBuf stage_in, stage_out;
@@ -85,7 +85,7 @@ struct boa_model {
   std::vector<cudaEvent_t> events;
 
   ~boa_model() {
-    for (GrowBuf* b : {&weights, &wimg, &u, &xz, &dbc, &u_img, &xs_img, &y_img, &logits, &h, &win, &pos, &len, &low, &range,
+    for (GrowBuf* b : {&weights, &wimg, &u, &xz, &dbc, &u_img, &xs_img, &y_img, &logits, &h, &win, &ssq, &pos, &len, &low, &range,
                        &pending, &wpos, &cache, &started, &v, &rpos, &off, &size, &scratch, &first, &err,
                        &stage_in, &stage_out})
       b->release();
@@ -200,30 +200,27 @@ int mark(StepCtx& c, int cls) {
 }
 
 // ---- tensor-core GEMM launch (tc_gemm.cuh).  The dynamic shared-memory opt-in is set once per instantiation.
-template <int BN, int NPW, int EPI>
-int launch_tc(const tc::GemmArgs& g, int N, cudaStream_t st) {
-  using C = tc::Cfg<BN, NPW>;
-  dim3 grid((g.M + tc::BM - 1) / tc::BM, (N + BN - 1) / BN);
-  tc::k_tc_gemm<BN, NPW, EPI><<<grid, tc::NTHREADS, C::SMEM, st>>>(g);
+template <int NPW, int EPI>
+int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
+  using C = tc::Cfg<NPW>;
+  const int tiles = ((g.M + tc::BM - 1) / tc::BM) * g.NT;
+  tc::k_tc_gemm<NPW, EPI><<<std::min(tiles, n_sm), tc::NTHREADS, C::SMEM, st>>>(g);   // persistent: one CTA per SM
   return BOA_OK;
 }
-template <int BN, int NPW, int EPI>
+template <int NPW, int EPI>
 int optin_tc() {
-  BOA_CUDA_TRY(cudaFuncSetAttribute(tc::k_tc_gemm<BN, NPW, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                    tc::Cfg<BN, NPW>::SMEM));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(tc::k_tc_gemm<NPW, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Cfg<NPW>::SMEM));
   return BOA_OK;
 }
 // Shared-memory opt-ins of every kernel instantiation the step can launch (called by boa_model_load, outside
 // any stream capture).
 int init_kernels() {
-  BOA_TRY((optin_tc<128, 1, tc::EPI_INPROJ>()));
-  BOA_TRY((optin_tc<128, 3, tc::EPI_INPROJ>()));
-  BOA_TRY((optin_tc<128, 1, tc::EPI_STORE>()));
-  BOA_TRY((optin_tc<128, 3, tc::EPI_STORE>()));
-  BOA_TRY((optin_tc<64, 1, tc::EPI_STORE>()));
-  BOA_TRY((optin_tc<64, 3, tc::EPI_STORE>()));
-  BOA_TRY((optin_tc<64, 1, tc::EPI_RESID>()));
-  BOA_TRY((optin_tc<64, 3, tc::EPI_RESID>()));
+  BOA_TRY((optin_tc<1, tc::EPI_INPROJ>()));
+  BOA_TRY((optin_tc<3, tc::EPI_INPROJ>()));
+  BOA_TRY((optin_tc<1, tc::EPI_STORE>()));
+  BOA_TRY((optin_tc<3, tc::EPI_STORE>()));
+  BOA_TRY((optin_tc<1, tc::EPI_RESID>()));
+  BOA_TRY((optin_tc<3, tc::EPI_RESID>()));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 64)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
@@ -231,9 +228,9 @@ int init_kernels() {
   return BOA_OK;
 }
 
-template <int BN, int EPI>
-int launch_tc_npw(int npw, const tc::GemmArgs& g, int N, cudaStream_t st) {
-  return npw == 1 ? launch_tc<BN, 1, EPI>(g, N, st) : launch_tc<BN, 3, EPI>(g, N, st);
+template <int EPI>
+int launch_tc_npw(int npw, const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
+  return npw == 1 ? launch_tc<1, EPI>(g, n_sm, st) : launch_tc<3, EPI>(g, n_sm, st);
 }
 
 // S1 for the first step of a wave: u = Emb[byte 0] (later steps: fused into the coder step).
@@ -243,7 +240,7 @@ int launch_embed(StepCtx& c) {
   k_embed<<<(total + 255) / 256, 256, 0, c.st>>>(c.data, c.chunk_bytes, c.ca.pos, c.ca.len,
                                                   reinterpret_cast<const float4*>(m->emb), m->u.as<float4>(),
                                                   reinterpret_cast<const float4*>(m->layers[0].norm_w),
-                                                  m->u_img.as<uint8_t>(), c.B, m->D / 4);
+                                                  m->u_img.as<uint8_t>(), m->ssq.as<float>(), c.B, m->D / 4);
   return mark(c, BOA_K_EMBED);
 }
 
@@ -265,19 +262,18 @@ int launch_step(StepCtx& c) {
     float* winl = m->win.as<float>() + (size_t)l * m->Bcap * 3 * E;
     {  // S2-S4: xz = [SiLU(conv(W_in_x r)) ; W_in_z r],  r = RMSNorm(u);  xs also as the image for x_proj
       tc::GemmArgs g{};
-      g.A = u_img; g.M = B; g.KB = D / 64; g.W = w.img_in;
+      g.A = u_img; g.M = B; g.KB = D / 64; g.W = w.img_in; g.NT = 2 * E / 64;
       g.C = xz; g.ldc = 2 * E; g.n_valid = 2 * E;
-      g.U = u; g.win = winl; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
+      g.ssq_in = m->ssq.as<float>(); g.win = winl; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
-      BOA_TRY((launch_tc_npw<128, tc::EPI_INPROJ>(m->npw, g, 2 * E, c.st)));
+      BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_INPROJ));
     }
     {  // S5: [dlt;Bv;Cv] = W_x xs
       tc::GemmArgs g{};
-      g.A = xs_img; g.M = B; g.KB = E / 64; g.W = w.img_x;
+      g.A = xs_img; g.M = B; g.KB = E / 64; g.W = w.img_x; g.NT = m->ldj / 64;
       g.C = dbc; g.ldc = m->ldj; g.n_valid = m->J;
-      if (m->ldj == 64) BOA_TRY((launch_tc_npw<64, tc::EPI_STORE>(m->npw, g, 64, c.st)));
-      else BOA_TRY((launch_tc_npw<128, tc::EPI_STORE>(m->npw, g, 128, c.st)));
+      BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_CONVX));
     }
     {  // S6-S8: persistent, two CTAs per SM, each walking over streams for one channel slice
@@ -297,26 +293,26 @@ int launch_step(StepCtx& c) {
     }
     {  // S9: u += W_out y;  the new u also as the image for the next in_proj (times its RMSNorm weight) or the head
       tc::GemmArgs g{};
-      g.A = y_img; g.M = B; g.KB = E / 64; g.W = w.img_out;
+      g.A = y_img; g.M = B; g.KB = E / 64; g.W = w.img_out; g.NT = D / 64;
       g.C = u; g.ldc = D; g.n_valid = D;
-      g.out_img = u_img; g.out_KB = D / 64;
+      g.out_img = u_img; g.out_KB = D / 64; g.ssq_out = m->ssq.as<float>();
       g.out_scale = (l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
-      BOA_TRY((launch_tc_npw<64, tc::EPI_RESID>(m->npw, g, D, c.st)));
+      BOA_TRY((launch_tc_npw<tc::EPI_RESID>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_OUTPROJ));
     }
   }
   {  // S10: logits = Emb u
     tc::GemmArgs g{};
-    g.A = u_img; g.M = B; g.KB = D / 64; g.W = m->img_head;
+    g.A = u_img; g.M = B; g.KB = D / 64; g.W = m->img_head; g.NT = 4;
     g.C = logits; g.ldc = 256; g.n_valid = 256;
-    BOA_TRY((launch_tc_npw<64, tc::EPI_STORE>(m->npw, g, 256, c.st)));
+    BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
     BOA_TRY(mark(c, BOA_K_HEAD));
   }
 
   const int cgrid = (B * 32 + 255) / 256;
   EmbedArgs ea{};
   ea.emb = reinterpret_cast<const float4*>(m->emb); ea.norm_w = reinterpret_cast<const float4*>(m->layers[0].norm_w);
-  ea.u = m->u.as<float4>(); ea.u_img = u_img; ea.D4 = D / 4;
+  ea.u = m->u.as<float4>(); ea.u_img = u_img; ea.ssq = m->ssq.as<float>(); ea.D4 = D / 4;
   if (c.dump) {
     if (c.dump_logits) {
       BOA_CUDA_TRY(cudaMemcpy2DAsync(c.dump_logits + (size_t)c.dump_t * 256, (size_t)c.dump_steps * 256 * sizeof(float),
@@ -416,6 +412,7 @@ int reserve_workspace(boa_model* m, uint64_t B, size_t cap) {
     BOA_TRY(m->u.reserve(B * D * 4));
     BOA_TRY(m->xz.reserve(B * 2 * E * 4));
     BOA_TRY(m->dbc.reserve(B * (size_t)m->ldj * 4));
+    BOA_TRY(m->ssq.reserve(B * (D / 64) * 4));
     BOA_TRY(m->u_img.reserve(tc::img_bytes(B, D)));
     BOA_TRY(m->xs_img.reserve(tc::img_bytes(B, E)));
     BOA_TRY(m->y_img.reserve(tc::img_bytes(B, E)));
@@ -586,10 +583,10 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
   for (uint32_t l = 0; l < L && ok; ++l) {
     Off& o = offs[l];
     ok = ok && br.take(D, false, t); if (ok) o.norm_w = append(t);
-    ok = ok && br.take(2 * E * D, true, t); if (ok) o.img_in = append_w_image(t.data(), 2 * E, D, 128, m->npw, wimg);
+    ok = ok && br.take(2 * E * D, true, t); if (ok) o.img_in = append_w_image(t.data(), 2 * E, D, 64, m->npw, wimg);
     ok = ok && br.take(E * 4, false, t); if (ok) o.conv_w = append(t);        // [E][4] = one float4 per channel
     ok = ok && br.take(E, false, t); if (ok) o.conv_b = append(t);
-    ok = ok && br.take(J * E, true, t); if (ok) o.img_x = append_w_image(t.data(), J, E, m->ldj, m->npw, wimg);
+    ok = ok && br.take(J * E, true, t); if (ok) o.img_x = append_w_image(t.data(), J, E, 64, m->npw, wimg);
     ok = ok && br.take(E * R, true, t);
     if (ok) {                                                                 // W_dt [E][R] -> transposed [R][E]
       t2.assign(E * R, 0.0f);
@@ -941,17 +938,17 @@ int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_
   return BOA_OK;
 }
 
-int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N, int weight_pieces, int tile_n,
+int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N, int weight_pieces, int grid_ctas,
                    float* C, void* cuda_stream) {
   if (!A || !W || !C || M == 0 || N == 0 || K == 0 || K % 64 != 0 || (weight_pieces != 1 && weight_pieces != 3) ||
-      (tile_n != 64 && tile_n != 128) || M >= (1u << 30) || N >= (1u << 20) || K >= (1u << 20))
+      grid_ctas < 0 || M >= (1u << 30) || N >= (1u << 20) || K >= (1u << 20))
     return BOA_E_ARG;
   BOA_TRY(check_device());
   BOA_TRY(init_kernels());
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  const size_t Np = round_up(N, (size_t)tile_n);
+  const size_t Np = round_up(N, (size_t)tc::BN);
   std::vector<uint16_t> img;
-  append_w_image(W, N, K, tile_n, weight_pieces, img);
+  append_w_image(W, N, K, tc::BN, weight_pieces, img);
   TmpDev ta, tw, tc_;
   BOA_TRY(ta.init(A, M * K * 4, true, false, st));
   BOA_TRY(tw.init(img.data(), img.size() * 2, true, false, st));
@@ -969,8 +966,14 @@ int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N,
   g.A = static_cast<const uint8_t*>(aimg); g.M = (int)M; g.KB = (int)(K / 64);
   g.W = static_cast<const uint16_t*>(tw.dev);
   g.C = static_cast<float*>(cpad); g.ldc = (int)Np; g.n_valid = (int)Np;
-  int rc = tile_n == 64 ? launch_tc_npw<64, tc::EPI_STORE>(weight_pieces, g, (int)Np, st)
-                        : launch_tc_npw<128, tc::EPI_STORE>(weight_pieces, g, (int)Np, st);
+  g.NT = (int)(Np / 64);
+  int n_sm = 148, dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+    (void)cudaGetLastError();
+    n_sm = 148;
+  }
+  if (grid_ctas > 0) n_sm = std::min(n_sm, grid_ctas);
+  int rc = launch_tc_npw<tc::EPI_STORE>(weight_pieces, g, n_sm, st);
   cudaError_t e = cudaGetLastError();
   if (rc == BOA_OK && e != cudaSuccess) rc = note_cuda_error(e, __FILE__, __LINE__);
   if (rc == BOA_OK) {

@@ -203,14 +203,25 @@ struct EmbedArgs {
   const float4* norm_w;    // [D/4] RMSNorm weight of layer 0
   float4* u;               // [B][D/4]
   uint8_t* u_img;
+  float* ssq;              // [B][D/64] sums of u^2 over 64-column blocks (same order as k_embed)
   int D4;
 };
+// all 32 lanes call (shuffles inside)
 __device__ __forceinline__ void embed_row(const EmbedArgs& ea, int i, uint32_t s, int lane) {
-  for (int q = lane; q < ea.D4; q += 32) {
-    const float4 v = ea.emb[s * ea.D4 + q];
-    ea.u[(size_t)i * ea.D4 + q] = v;
-    const float4 w = ea.norm_w[q];
-    tc::cut4_store(ea.u_img, ea.D4 >> 4, i, q * 4, make_float4(v.x * w.x, v.y * w.y, v.z * w.z, v.w * w.w));
+  for (int q0 = 0; q0 < ea.D4; q0 += 32) {
+    const int q = q0 + lane;
+    const bool live = q < ea.D4;                  // D4 is a multiple of 16: a 16-lane block is live as a whole
+    const float4 v = ea.emb[s * ea.D4 + (live ? q : 0)];
+    float ss = v.x * v.x;
+    ss = fmaf(v.y, v.y, ss); ss = fmaf(v.z, v.z, ss); ss = fmaf(v.w, v.w, ss);
+#pragma unroll
+    for (int d = 8; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
+    if (live) {
+      ea.u[(size_t)i * ea.D4 + q] = v;
+      if ((q & 15) == 0) ea.ssq[(size_t)i * (ea.D4 >> 4) + (q >> 4)] = ss;
+      const float4 w = ea.norm_w[q];
+      tc::cut4_store(ea.u_img, ea.D4 >> 4, i, q * 4, make_float4(v.x * w.x, v.y * w.y, v.z * w.z, v.w * w.w));
+    }
   }
 }
 

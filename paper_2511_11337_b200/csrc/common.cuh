@@ -18,7 +18,7 @@ constexpr float kEps = 1e-5f;        // RMSNorm epsilon (R#10)
 // are only reproducible with the same per-step floating-point arithmetic.
 // 'B2' + generation number.  Bump whenever any kernel upstream of the quantiser changes its
 // arithmetic (operation order, fusion, precision).
-constexpr uint32_t kArithVersion = 0x42320004u;
+constexpr uint32_t kArithVersion = 0x42320005u;
 
 // Last CUDA failure seen by this thread ("file:line: cudaErrorName"), for boa_last_cuda_error().
 inline char* last_cuda_error_buf() {

@@ -31,17 +31,26 @@ __device__ __forceinline__ float softplusf_(float v) { return fmaxf(v, 0.0f) + l
 // ---------------------------------------------------------------------------------------------------
 // S1: u[i][:] = Emb[src[i*chunk + min(pos_i, len_i-1)]].  In compress mode `src` is the input; in
 // decompress mode it is the output buffer, whose byte pos_i was written by the previous coder step.
-// Also writes the image of u * norm_w(layer 0), the operand of the first in_proj (tc_gemm.cuh).
+// Also writes the image of u * norm_w(layer 0), the operand of the first in_proj (tc_gemm.cuh), and the sums of
+// u^2 over each 64-column block (one thread per 4 columns: x, y, z, w, then the xor butterfly 8, 4, 2, 1 over the
+// 16 threads of the block) from which in_proj forms the RMSNorm row scale.
 __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, const uint32_t* __restrict__ pos,
                         const uint32_t* __restrict__ len, const float4* __restrict__ emb, float4* __restrict__ u,
-                        const float4* __restrict__ norm_w, uint8_t* __restrict__ u_img, int B, int D4) {
-  int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= B * D4) return;
-  int i = idx / D4, q = idx - i * D4;
-  uint32_t p = min(pos[i], len[i] - 1u);
-  uint32_t s = src[(size_t)i * chunk_bytes + p];
+                        const float4* __restrict__ norm_w, uint8_t* __restrict__ u_img, float* __restrict__ ssq,
+                        int B, int D4) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const bool live = idx < B * D4;                 // B*D4 is a multiple of 16: a 16-thread block is live as a whole
+  const int i = live ? idx / D4 : 0, q = live ? idx - i * D4 : 0;
+  const uint32_t p = min(pos[i], len[i] - 1u);
+  const uint32_t s = src[(size_t)i * chunk_bytes + p];
   const float4 v = emb[s * D4 + q];
+  float ss = v.x * v.x;
+  ss = fmaf(v.y, v.y, ss); ss = fmaf(v.z, v.z, ss); ss = fmaf(v.w, v.w, ss);
+#pragma unroll
+  for (int d = 8; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
+  if (!live) return;
   u[idx] = v;
+  if ((q & 15) == 0) ssq[(size_t)i * (D4 >> 4) + (q >> 4)] = ss;
   const float4 w = norm_w[q];
   tc::cut4_store(u_img, D4 >> 4, i, q * 4, make_float4(v.x * w.x, v.y * w.y, v.z * w.z, v.w * w.w));
 }

@@ -5,7 +5,9 @@
 //   out_proj  u += W_out y                  S9                                         Alg. 1 l.3
 //   head      logits = Emb u                S10                                        Alg. 1 l.5
 //
-// One CTA computes a 128-stream x BN tile:  C[m][n] = sum_k A[m][k] * W[n][k].
+// A tile is 128 streams x 64 columns:  C[m][n] = sum_k A[m][k] * W[n][k].  The kernel is persistent: one CTA per SM
+// walks over tiles; the TMEM accumulators are double-buffered so the epilogue of tile i overlaps the copies and MMAs
+// of tile i+1.
 //
 // Precision.  The activations are fp32 and the four parity checks need
 // fp32-level products, so each operand is cut into bf16 pieces that sum to it exactly (a = a1+a2+a3, 8 significant
@@ -16,7 +18,7 @@
 // fp32, smallest first, in the epilogue.  Dropped products are below 2^-24 of |a||w|.
 // The weight pieces of a tile are stacked along N in shared memory ([w1; w2; w3]), so one MMA of a piece of A against
 // the stack yields several products at once and A is read from shared memory once for them:
-//   a1 x [w1;w2;w3] -> classes 0,1,2   a2 x [w1;w2] -> classes 1,2   a3 x [w1] -> class 2       (N = 3, 2, 1 x BN)
+//   a1 x [w1;w2;w3] -> classes 0,1,2   a2 x [w1;w2] -> classes 1,2   a3 x [w1] -> class 2       (N = 192, 128, 64)
 //
 // Data movement.  Both operands reach shared memory through the bulk-copy engine (TMA, cp.async.bulk -> SASS UBLKCP)
 // as ready-made images of a tile (K-major, 128-byte swizzle), so the main loop is TMA + MMA only:
@@ -37,6 +39,7 @@ namespace boa {
 namespace tc {
 
 constexpr int BM = 128;          // streams per tile = TMEM lanes
+constexpr int BN = 64;           // output columns per tile
 constexpr int BK = 64;           // k per stage: 64 bf16 = one 128-byte swizzle row
 constexpr int NPA = 3;           // bf16 pieces of an activation
 constexpr int A_PLANE = BM * 128;  // bytes of one activation piece tile
@@ -46,11 +49,13 @@ enum { EPI_STORE = 0, EPI_RESID = 1, EPI_INPROJ = 2 };
 struct GemmArgs {
   const uint8_t* A;        // activation image of A[M][K]: [ceil(M/128)][K/64][3 pieces][128 x 64 bf16, swizzled]
   int M, KB;               // KB = K/64
-  const uint16_t* W;       // weight image [N/BN][K/64][NPW][BN x 64 bf16, swizzled]
+  const uint16_t* W;       // weight image [N/64][K/64][NPW][64 x 64 bf16, swizzled]
+  int NT;                  // column tiles (N/64, N padded with zero weight rows)
   float* C;                // [M][ldc] fp32 result (in_proj: xz = xs | z; out_proj: the residual stream u, updated)
   int ldc, n_valid;        // columns >= n_valid are not stored (zero-padded weight rows)
   // EPI_INPROJ only
-  const float* U;          // [M][K] fp32 residual stream: rstd = 1/sqrt(mean(u^2)+eps) is computed from it
+  const float* ssq_in;     // [M][KB]: sum of u^2 over each 64-column block of the residual stream (written by the
+                           // producer of u in a fixed order); rstd = 1/sqrt(sum/K + eps) (R#10)
   float* win;              // [M][3][E] conv window of this layer
   const float4* conv_w;    // [E] taps (x = t-3 ... w = t)
   const float* conv_b;     // [E]
@@ -59,6 +64,7 @@ struct GemmArgs {
   uint8_t* out_img;
   int out_KB;              // k-blocks per row tile of that image
   const float* out_scale;  // EPI_RESID: the consumer's RMSNorm weight (applied before cutting) or nullptr
+  float* ssq_out;          // EPI_RESID: [M][out_KB] sum of the new u^2 over this tile's 64 columns
 #ifdef BOA_TC_TRACE
   long long* trace;        // [gridDim.x*gridDim.y][64] SM-clock timestamps (development builds only)
 #endif
@@ -195,15 +201,18 @@ __global__ void k_cut_rows(const float* __restrict__ X, int ldx, int M, int K, c
   cut4_store(img, K >> 6, m, k, v);
 }
 
-template <int BN, int NPW>
+template <int NPW>
 struct Cfg {
   static constexpr int W_BYTES = NPW * BN * 128;
   static constexpr int A_BYTES = NPA * A_PLANE;
   static constexpr int STAGE = A_BYTES + W_BYTES;
-  static constexpr int NST = (4 * STAGE <= 216 * 1024) ? 4 : (3 * STAGE <= 216 * 1024) ? 3 : 2;
-  static constexpr int SMEM = NST * STAGE + 1024;             // + alignment slack
+  static constexpr int LDS = BN + 4;                          // staging row, padded: conflict-free column stores
+  static constexpr int STILE_BYTES = BM * LDS * 4;
+  static constexpr int NST = (3 * STAGE + STILE_BYTES <= 220 * 1024) ? 3 : 2;
+  static constexpr int SMEM = NST * STAGE + STILE_BYTES + 1024;   // + alignment slack
   static constexpr int NACC = NPW == 3 ? 3 : 2;               // accumulators (magnitude classes)
-  static constexpr int TMEM_COLS = (NACC * BN <= 128) ? 128 : (NACC * BN <= 256) ? 256 : 512;
+  static constexpr int ACC_COLS = NACC * BN;                  // TMEM columns of one accumulator buffer
+  static constexpr int TMEM_COLS = (2 * ACC_COLS <= 256) ? 256 : 512;   // two buffers
 };
 
 // sigmoid for the SiLU of the conv epilogue: fast forms (relative error ~1e-6; same code on encode and decode)
@@ -213,23 +222,20 @@ constexpr int NEPI = 256;        // epilogue threads (warps 0-7); warp 8 owns TM
 constexpr int NTHREADS = NEPI + 64;
 
 // ------------------------------------------------------------------------------------------ the kernel
-// grid = (ceil(M/128), N/BN), block = 320.  Warp 9 (one lane) streams the k-blocks of both operand images into
-// the stage ring; warp 8 (one lane) issues the MMAs; warps 0-7 compute the RMSNorm row scale meanwhile (in_proj)
-// and then run the epilogue.
-template <int BN, int NPW, int EPI>
+// grid = min(tiles, SMs), block = 320.  Tile t -> (row tile t / NT, column tile t % NT); CTA c takes tiles c,
+// c + grid, ...  Warp 9 (one lane) streams the k-blocks of both operand images into the stage ring; warp 8 (one lane)
+// issues the MMAs into accumulator buffer (tile iteration & 1); warps 0-7 drain the other buffer and run the epilogue.
+template <int NPW, int EPI>
 __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
-  using C = Cfg<BN, NPW>;
-  static_assert(BN == 64 || BN == 128, "tile N");
+  using C = Cfg<NPW>;
   static_assert(NPW == 1 || NPW == 3, "weight pieces");
   extern __shared__ uint8_t smem_raw[];
-  __shared__ __align__(8) uint64_t full_bar[C::NST], empty_bar[C::NST], acc_bar;
+  __shared__ __align__(8) uint64_t full_bar[C::NST], empty_bar[C::NST], acc_full[2], acc_empty[2];
   __shared__ uint32_t tmem_base_s;
-  __shared__ float rstd_s[BM];
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int m0 = blockIdx.x * BM;
-  const int n0 = blockIdx.y * BN;
-  const int KB = g.KB;
+  const int KB = g.KB, NT = g.NT;
+  const int ntiles = ((g.M + BM - 1) / BM) * NT;
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   if (tid == 0) TC_TRACE(0);
 
@@ -239,7 +245,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
         mbar_init(smem_u32(&full_bar[s]), 1);     // the copy warp's arrive.expect_tx
         mbar_init(smem_u32(&empty_bar[s]), 1);    // one tcgen05.commit
       }
-      mbar_init(smem_u32(&acc_bar), 1);
+      for (int b = 0; b < 2; ++b) {
+        mbar_init(smem_u32(&acc_full[b]), 1);     // one tcgen05.commit
+        mbar_init(smem_u32(&acc_empty[b]), NEPI); // every epilogue thread has drained its part
+      }
       fence_barrier_init();
     }
     __syncwarp();
@@ -254,188 +263,183 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   if (warp == 9) {
     // ===================================================================== copy warp
     if (lane == 0) {
-      const uint8_t* asrc = g.A + img_block((size_t)blockIdx.x, 0, (size_t)KB);
-      const uint16_t* wsrc = g.W + (size_t)blockIdx.y * KB * (NPW * BN * 64);
-      for (int kb = 0; kb < KB; ++kb) {
-        const int s = kb % C::NST, round = kb / C::NST;
-        if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
-        const uint32_t sA = sbase + (uint32_t)s * C::STAGE, fb = smem_u32(&full_bar[s]);
-        mbar_arrive_expect_tx(fb, (uint32_t)C::STAGE);
-        bulk_g2s(sA, asrc + (size_t)kb * C::A_BYTES, (uint32_t)C::A_BYTES, fb);
-        bulk_g2s(sA + C::A_BYTES, wsrc + (size_t)kb * (NPW * BN * 64), (uint32_t)C::W_BYTES, fb);
-        if (kb < 16) TC_TRACE(8 + kb);
+      int kbc = 0;                                 // k-blocks issued so far: position in the stage ring
+      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+        const int mt = tile / NT, nt = tile - mt * NT;
+        const uint8_t* asrc = g.A + img_block((size_t)mt, 0, (size_t)KB);
+        const uint16_t* wsrc = g.W + (size_t)nt * KB * (NPW * BN * 64);
+        for (int kb = 0; kb < KB; ++kb, ++kbc) {
+          const int s = kbc % C::NST, round = kbc / C::NST;
+          if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
+          const uint32_t sA = sbase + (uint32_t)s * C::STAGE, fb = smem_u32(&full_bar[s]);
+          mbar_arrive_expect_tx(fb, (uint32_t)C::STAGE);
+          bulk_g2s(sA, asrc + (size_t)kb * C::A_BYTES, (uint32_t)C::A_BYTES, fb);
+          bulk_g2s(sA + C::A_BYTES, wsrc + (size_t)kb * (NPW * BN * 64), (uint32_t)C::W_BYTES, fb);
+        }
       }
     }
   } else if (warp == 8) {
     // ===================================================================== MMA issuer
     if (lane == 0) {
-      for (int kb = 0; kb < KB; ++kb) {
-        const int s = kb % C::NST, round = kb / C::NST;
-        mbar_wait(smem_u32(&full_bar[s]), (uint32_t)(round & 1));
-        tc_fence_after();
-        if (kb < 16) TC_TRACE(40 + kb);
-        const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
-        const uint32_t sW = sA + C::A_BYTES;
-#pragma unroll
-        for (int k4 = 0; k4 < BK / 16; ++k4) {
-          const uint32_t first = (kb | k4) ? 1u : 0u;
-          const uint32_t ko = (uint32_t)k4 * 32u;
-          auto A_ = [&](int p) { return smem_desc_sw128(sA + p * A_PLANE + ko); };
-          auto W_ = [&](int q) { return smem_desc_sw128(sW + q * (BN * 128) + ko); };
-          if (NPW == 3 && BN == 64) {
-            umma(tmem, A_(0), W_(0), idesc_bf16(192), first);        // a1 x [w1;w2;w3] -> classes 0,1,2
-            umma(tmem + 64, A_(1), W_(0), idesc_bf16(128), 1u);      // a2 x [w1;w2]    -> classes 1,2
-            umma(tmem + 128, A_(2), W_(0), idesc_bf16(64), 1u);      // a3 x [w1]       -> class 2
-          } else if (NPW == 3) {                                     // BN = 128: the stack is split at N = 256
-            umma(tmem, A_(0), W_(0), idesc_bf16(256), first);        // a1 x [w1;w2]    -> classes 0,1
-            umma(tmem + 256, A_(0), W_(2), idesc_bf16(128), first);  // a1 x [w3]       -> class 2
-            umma(tmem + 128, A_(1), W_(0), idesc_bf16(256), 1u);     // a2 x [w1;w2]    -> classes 1,2
-            umma(tmem + 256, A_(2), W_(0), idesc_bf16(128), 1u);     // a3 x [w1]       -> class 2
-          } else {
-            umma(tmem, A_(0), W_(0), idesc_bf16(BN), first);         // a1 w            -> class 0
-            umma(tmem + BN, A_(2), W_(0), idesc_bf16(BN), first);    // a3 w, a2 w      -> class 1
-            umma(tmem + BN, A_(1), W_(0), idesc_bf16(BN), 1u);
-          }
+      int kbc = 0, it = 0;
+      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+        const int b = it & 1;
+        if (it >= 2) {                             // the epilogue has drained this buffer (tile it-2)
+          mbar_wait(smem_u32(&acc_empty[b]), (uint32_t)(((it >> 1) - 1) & 1));
+          tc_fence_after();
         }
-        umma_commit(smem_u32(&empty_bar[s]));                     // stage free when these MMAs have read it
-        if (kb < 16) TC_TRACE(24 + kb);
+        const uint32_t tacc = tmem + (uint32_t)(b * C::ACC_COLS);
+        for (int kb = 0; kb < KB; ++kb, ++kbc) {
+          const int s = kbc % C::NST, round = kbc / C::NST;
+          mbar_wait(smem_u32(&full_bar[s]), (uint32_t)(round & 1));
+          tc_fence_after();
+          const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
+          const uint32_t sW = sA + C::A_BYTES;
+#pragma unroll
+          for (int k4 = 0; k4 < BK / 16; ++k4) {
+            const uint32_t first = (kb | k4) ? 1u : 0u;
+            const uint32_t ko = (uint32_t)k4 * 32u;
+            auto A_ = [&](int p) { return smem_desc_sw128(sA + p * A_PLANE + ko); };
+            const uint64_t wd = smem_desc_sw128(sW + ko);
+            if (NPW == 3) {
+              umma(tacc, A_(0), wd, idesc_bf16(192), first);         // a1 x [w1;w2;w3] -> classes 0,1,2
+              umma(tacc + 64, A_(1), wd, idesc_bf16(128), 1u);       // a2 x [w1;w2]    -> classes 1,2
+              umma(tacc + 128, A_(2), wd, idesc_bf16(64), 1u);       // a3 x [w1]       -> class 2
+            } else {
+              umma(tacc, A_(0), wd, idesc_bf16(64), first);          // a1 w            -> class 0
+              umma(tacc + 64, A_(2), wd, idesc_bf16(64), first);     // a3 w, a2 w      -> class 1
+              umma(tacc + 64, A_(1), wd, idesc_bf16(64), 1u);
+            }
+          }
+          umma_commit(smem_u32(&empty_bar[s]));                      // stage free when these MMAs have read it
+        }
+        umma_commit(smem_u32(&acc_full[b]));                         // this tile's accumulators are complete
+        if (it < 8) TC_TRACE(8 + it);
       }
-      umma_commit(smem_u32(&acc_bar));                            // accumulators complete
     }
   } else {
     // ===================================================================== epilogue warps
-    if (EPI == EPI_INPROJ) {
-      // S2: rstd of the tile's 128 rows from the fp32 residual stream, while the main loop runs.
-      // Fixed order: per lane ascending k, then the xor butterfly 16, 8, 4, 2, 1.
-      const int K = KB * BK;
-#pragma unroll 1
-      for (int j0 = 0; j0 < 16; j0 += 4) {
-        float ss[4] = {0.f, 0.f, 0.f, 0.f};
-        for (int q = lane; q < (K >> 2); q += 32) {
-          float4 v[4];
-#pragma unroll
-          for (int j = 0; j < 4; ++j)
-            v[j] = *reinterpret_cast<const float4*>(g.U + (size_t)min(m0 + warp * 16 + j0 + j, g.M - 1) * K + q * 4);
-#pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            ss[j] = fmaf(v[j].x, v[j].x, ss[j]); ss[j] = fmaf(v[j].y, v[j].y, ss[j]);
-            ss[j] = fmaf(v[j].z, v[j].z, ss[j]); ss[j] = fmaf(v[j].w, v[j].w, ss[j]);
-          }
-        }
-#pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          float v = ss[j];
-#pragma unroll
-          for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-          if (lane == 0) rstd_s[warp * 16 + j0 + j] = 1.0f / sqrtf(v / (float)K + kEps);
-        }
+    constexpr int LDS = C::LDS;
+    float* stile = reinterpret_cast<float*>(smem_raw + (sbase - smem_u32(smem_raw)) + C::NST * C::STAGE);
+    constexpr int LPR = BN / 4;                    // lanes per row segment in pass 2 (4 columns per lane)
+    constexpr int RPI = 32 / LPR;                  // rows per warp instruction
+    constexpr int NIT = BM / (8 * RPI);            // row groups per warp
+    const int col = (lane % LPR) * 4;
+    int it = 0;
+    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+      const int b = it & 1;
+      const int mt = tile / NT, nt = tile - mt * NT;
+      const int m0 = mt * BM, n0 = nt * BN;
+      // Pass 1: TMEM -> registers (thread = stream row; warps w and w+4 share the 32 TMEM lanes of rows 32*(w%4)..
+      // and take one 32-column half each) -> shared staging tile, so that pass 2 can run with lane = column and
+      // every global access coalesced.
+      const int r1 = (warp & 3) * 32 + lane;
+      float rs = 1.0f;
+      if (EPI == EPI_INPROJ) {                     // S2: RMSNorm row scale from the block sums of u^2, ascending
+        const float* sp = g.ssq_in + (size_t)min(m0 + r1, g.M - 1) * KB;
+        float ss = 0.0f;
+        for (int q = 0; q < KB; ++q) ss += sp[q];
+        rs = 1.0f / sqrtf(ss / (float)(KB * BK) + kEps);
       }
-      asm volatile("bar.sync 1, 256;" ::: "memory");
-    }
-    mbar_wait(smem_u32(&acc_bar), 0u);
-    tc_fence_after();
-    if (tid == 0) TC_TRACE(2);
-    // Pass 1: TMEM -> registers (thread = stream row; warps w and w+4 share the 32 TMEM lanes of rows
-    // 32*(w%4).. and split the columns) -> shared staging tile, so that pass 2 can run with lane = column and
-    // every global access coalesced.  All MMAs have completed: the stage memory is free.
-    constexpr int LDS = BN + 4;                    // padded row: conflict-free 128-bit stores down a column
-    float* stile = reinterpret_cast<float*>(smem_raw + (sbase - smem_u32(smem_raw)));
-    {
-      const int r = (warp & 3) * 32 + lane;
-      const uint32_t tlane = tmem + ((uint32_t)((warp & 3) * 32) << 16);
-      const float rs = (EPI == EPI_INPROJ) ? rstd_s[r] : 1.0f;
-      constexpr int CPW = BN / 64;                 // 32-column chunks per warp
-#pragma unroll 1
-      for (int q = 0; q < CPW; ++q) {
-        const int ch = (warp >> 2) * CPW + q;
+      mbar_wait(smem_u32(&acc_full[b]), (uint32_t)((it >> 1) & 1));
+      tc_fence_after();
+      if (tid == 0 && it < 8) TC_TRACE(24 + it);
+      {
+        const uint32_t tl = tmem + (uint32_t)(b * C::ACC_COLS) + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * 32);
         float v[32], w[32];
         __syncwarp();
-        tmem_ld32(tlane + (uint32_t)(BN + ch * 32), v);          // class 1
+        tmem_ld32(tl + 64, v);                     // class 1
         if (NPW == 3) {
-          tmem_ld32(tlane + (uint32_t)(2 * BN + ch * 32), w);    // class 2, added first
+          tmem_ld32(tl + 128, w);                  // class 2, added first
 #pragma unroll
           for (int j = 0; j < 32; ++j) v[j] += w[j];
         }
-        tmem_ld32(tlane + (uint32_t)(ch * 32), w);               // class 0
-        float4* dst = reinterpret_cast<float4*>(stile + r * LDS + ch * 32);
+        tmem_ld32(tl, w);                          // class 0
+        tc_fence_before();
+        mbar_arrive(smem_u32(&acc_empty[b]));      // this thread's part of the buffer may be overwritten
+        float4* dst = reinterpret_cast<float4*>(stile + r1 * LDS + (warp >> 2) * 32);
 #pragma unroll
         for (int j = 0; j < 32; j += 4)
           dst[j >> 2] = make_float4((v[j] + w[j]) * rs, (v[j + 1] + w[j + 1]) * rs, (v[j + 2] + w[j + 2]) * rs,
                                     (v[j + 3] + w[j + 3]) * rs);
       }
-    }
-    asm volatile("bar.sync 1, 256;" ::: "memory");
-    if (tid == 0) TC_TRACE(3);
-    // Pass 2: a group of BN/4 lanes owns one row segment; 4 consecutive columns per lane.  Rows are processed four
-    // at a time with all loads issued first.
-    constexpr int LPR = BN / 4;                    // lanes per row
-    constexpr int RPI = 32 / LPR;                  // rows per warp instruction
-    constexpr int NIT = BM / (8 * RPI);            // row groups per warp
-    static_assert(NIT % 4 == 0, "row batching");
-    const int col = (lane % LPR) * 4;
-    const int nb = n0 + col;
-    if (EPI == EPI_INPROJ && n0 < g.E) {
-      // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU; the window moves one step (R#11).
-      // The lane's four channels are fixed, so their taps and biases live in registers.  xs goes out twice: fp32
-      // (the scan reads it) and cut into pieces in the image of x_proj's operand.
-      const float4 cw0 = g.conv_w[nb], cw1 = g.conv_w[nb + 1], cw2 = g.conv_w[nb + 2], cw3 = g.conv_w[nb + 3];
-      const float4 cb = *reinterpret_cast<const float4*>(g.conv_b + nb);
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+      // Pass 2: 16 lanes own one 64-column row segment (4 consecutive columns per lane), two rows per warp
+      // instruction; rows are processed four at a time with all loads issued first.
+      const int nb = n0 + col;
+      if (EPI == EPI_INPROJ && n0 < g.E) {
+        // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU; the window moves one step (R#11).
+        // The lane's four channels are fixed within a tile, so their taps and biases live in registers.  xs goes out
+        // twice: fp32 (the scan reads it) and cut into pieces in the image of x_proj's operand.
+        const float4 cw0 = g.conv_w[nb], cw1 = g.conv_w[nb + 1], cw2 = g.conv_w[nb + 2], cw3 = g.conv_w[nb + 3];
+        const float4 cb = *reinterpret_cast<const float4*>(g.conv_b + nb);
 #pragma unroll 1
-      for (int i0 = 0; i0 < NIT; i0 += 4) {
-        float4 x[4], w0[4], w1[4], w2[4];
-        int rows[4];
+        for (int i0 = 0; i0 < NIT; i0 += 4) {
+          float4 x[4], w0[4], w1[4], w2[4];
+          int rows[4];
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int r = (warp + 8 * (i0 + u)) * RPI + lane / LPR;
-          rows[u] = m0 + r;
-          x[u] = *reinterpret_cast<const float4*>(stile + r * LDS + col);
-          const float* wp = g.win + (size_t)min(rows[u], g.M - 1) * 3 * g.E + nb;
-          w0[u] = *reinterpret_cast<const float4*>(wp);
-          w1[u] = *reinterpret_cast<const float4*>(wp + g.E);
-          w2[u] = *reinterpret_cast<const float4*>(wp + 2 * g.E);
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          if (rows[u] >= g.M) continue;
-          float4 o;
-          { float xc = fmaf(cw0.w, x[u].x, cb.x); xc = fmaf(cw0.x, w0[u].x, xc); xc = fmaf(cw0.y, w1[u].x, xc); xc = fmaf(cw0.z, w2[u].x, xc); o.x = xc * sigmoid_tc(xc); }
-          { float xc = fmaf(cw1.w, x[u].y, cb.y); xc = fmaf(cw1.x, w0[u].y, xc); xc = fmaf(cw1.y, w1[u].y, xc); xc = fmaf(cw1.z, w2[u].y, xc); o.y = xc * sigmoid_tc(xc); }
-          { float xc = fmaf(cw2.w, x[u].z, cb.z); xc = fmaf(cw2.x, w0[u].z, xc); xc = fmaf(cw2.y, w1[u].z, xc); xc = fmaf(cw2.z, w2[u].z, xc); o.z = xc * sigmoid_tc(xc); }
-          { float xc = fmaf(cw3.w, x[u].w, cb.w); xc = fmaf(cw3.x, w0[u].w, xc); xc = fmaf(cw3.y, w1[u].w, xc); xc = fmaf(cw3.z, w2[u].w, xc); o.w = xc * sigmoid_tc(xc); }
-          float* wp = g.win + (size_t)rows[u] * 3 * g.E + nb;
-          *reinterpret_cast<float4*>(wp) = w1[u];
-          *reinterpret_cast<float4*>(wp + g.E) = w2[u];
-          *reinterpret_cast<float4*>(wp + 2 * g.E) = x[u];
-          *reinterpret_cast<float4*>(g.C + (size_t)rows[u] * g.ldc + nb) = o;
-          cut4_store(g.out_img, g.out_KB, rows[u], nb, o);
-        }
-      }
-    } else if (nb < g.n_valid) {
-      float4 osc = make_float4(1.f, 1.f, 1.f, 1.f);
-      if (EPI == EPI_RESID && g.out_scale) osc = *reinterpret_cast<const float4*>(g.out_scale + nb);
-#pragma unroll 1
-      for (int i0 = 0; i0 < NIT; i0 += 4) {
-        float4 o[4], q[4];
-        int rows[4];
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          const int r = (warp + 8 * (i0 + u)) * RPI + lane / LPR;
-          rows[u] = m0 + r;
-          o[u] = *reinterpret_cast<const float4*>(stile + r * LDS + col);
-          if (EPI == EPI_RESID) q[u] = *reinterpret_cast<const float4*>(g.C + (size_t)min(rows[u], g.M - 1) * g.ldc + nb);
-        }
-#pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          if (rows[u] >= g.M) continue;
-          if (EPI == EPI_RESID) {
-            // S9: the residual stream, and its image (times the consumer's RMSNorm weight) for the next contraction
-            o[u].x += q[u].x; o[u].y += q[u].y; o[u].z += q[u].z; o[u].w += q[u].w;
-            cut4_store(g.out_img, g.out_KB, rows[u], nb,
-                       make_float4(o[u].x * osc.x, o[u].y * osc.y, o[u].z * osc.z, o[u].w * osc.w));
+          for (int u = 0; u < 4; ++u) {
+            const int r = (warp + 8 * (i0 + u)) * RPI + lane / LPR;
+            rows[u] = m0 + r;
+            x[u] = *reinterpret_cast<const float4*>(stile + r * LDS + col);
+            const float* wp = g.win + (size_t)min(rows[u], g.M - 1) * 3 * g.E + nb;
+            w0[u] = *reinterpret_cast<const float4*>(wp);
+            w1[u] = *reinterpret_cast<const float4*>(wp + g.E);
+            w2[u] = *reinterpret_cast<const float4*>(wp + 2 * g.E);
           }
-          *reinterpret_cast<float4*>(g.C + (size_t)rows[u] * g.ldc + nb) = o[u];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            if (rows[u] >= g.M) continue;
+            float4 o;
+            { float xc = fmaf(cw0.w, x[u].x, cb.x); xc = fmaf(cw0.x, w0[u].x, xc); xc = fmaf(cw0.y, w1[u].x, xc); xc = fmaf(cw0.z, w2[u].x, xc); o.x = xc * sigmoid_tc(xc); }
+            { float xc = fmaf(cw1.w, x[u].y, cb.y); xc = fmaf(cw1.x, w0[u].y, xc); xc = fmaf(cw1.y, w1[u].y, xc); xc = fmaf(cw1.z, w2[u].y, xc); o.y = xc * sigmoid_tc(xc); }
+            { float xc = fmaf(cw2.w, x[u].z, cb.z); xc = fmaf(cw2.x, w0[u].z, xc); xc = fmaf(cw2.y, w1[u].z, xc); xc = fmaf(cw2.z, w2[u].z, xc); o.z = xc * sigmoid_tc(xc); }
+            { float xc = fmaf(cw3.w, x[u].w, cb.w); xc = fmaf(cw3.x, w0[u].w, xc); xc = fmaf(cw3.y, w1[u].w, xc); xc = fmaf(cw3.z, w2[u].w, xc); o.w = xc * sigmoid_tc(xc); }
+            float* wp = g.win + (size_t)rows[u] * 3 * g.E + nb;
+            *reinterpret_cast<float4*>(wp) = w1[u];
+            *reinterpret_cast<float4*>(wp + g.E) = w2[u];
+            *reinterpret_cast<float4*>(wp + 2 * g.E) = x[u];
+            *reinterpret_cast<float4*>(g.C + (size_t)rows[u] * g.ldc + nb) = o;
+            cut4_store(g.out_img, g.out_KB, rows[u], nb, o);
+          }
+        }
+      } else {
+        float4 osc = make_float4(1.f, 1.f, 1.f, 1.f);
+        if (EPI == EPI_RESID && g.out_scale) osc = *reinterpret_cast<const float4*>(g.out_scale + nb);
+        const bool cols_ok = nb < g.n_valid;
+#pragma unroll 1
+        for (int i0 = 0; i0 < NIT; i0 += 4) {
+          float4 o[4], q[4];
+          int rows[4];
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int r = (warp + 8 * (i0 + u)) * RPI + lane / LPR;
+            rows[u] = m0 + r;
+            o[u] = *reinterpret_cast<const float4*>(stile + r * LDS + col);
+            if (EPI == EPI_RESID) q[u] = *reinterpret_cast<const float4*>(g.C + (size_t)min(rows[u], g.M - 1) * g.ldc + nb);
+          }
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const bool live = rows[u] < g.M && cols_ok;
+            if (EPI == EPI_RESID) {
+              // S9: the residual stream; its image (times the consumer's RMSNorm weight) for the next contraction;
+              // and the sum of its squares over this tile's 64 columns (x, y, z, w, then the xor butterfly 8, 4, 2, 1)
+              o[u].x += q[u].x; o[u].y += q[u].y; o[u].z += q[u].z; o[u].w += q[u].w;
+              float ss = o[u].x * o[u].x;
+              ss = fmaf(o[u].y, o[u].y, ss); ss = fmaf(o[u].z, o[u].z, ss); ss = fmaf(o[u].w, o[u].w, ss);
+#pragma unroll
+              for (int d = 8; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
+              if (live) {
+                cut4_store(g.out_img, g.out_KB, rows[u], nb,
+                           make_float4(o[u].x * osc.x, o[u].y * osc.y, o[u].z * osc.z, o[u].w * osc.w));
+                if ((lane % LPR) == 0) g.ssq_out[(size_t)rows[u] * g.out_KB + nt] = ss;
+              }
+            }
+            if (live) *reinterpret_cast<float4*>(g.C + (size_t)rows[u] * g.ldc + nb) = o[u];
+          }
         }
       }
+      asm volatile("bar.sync 1, 256;" ::: "memory");     // the staging tile is free for the next tile
     }
     if (tid == 0) TC_TRACE(4);
   }

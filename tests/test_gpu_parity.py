@@ -72,11 +72,12 @@ def _to_bf16(x):
     return u.astype(np.uint32).view(np.float32)
 
 
-@pytest.mark.parametrize("pieces,tile_n", [(3, 64), (3, 128), (1, 64), (1, 128)])
+@pytest.mark.parametrize("pieces,grid_ctas", [(3, 0), (3, 3), (1, 0), (1, 2)])
 @pytest.mark.parametrize("M,N,K", [(300, 48, 512), (128, 256, 64), (1, 64, 256), (517, 320, 1024)])
-def test_tensor_core_gemm_against_fp64(boa, pieces, tile_n, M, N, K):
+def test_tensor_core_gemm_against_fp64(boa, pieces, grid_ctas, M, N, K):
     """C = A W^T by tcgen05 on bf16 pieces (tc_gemm.cuh) against numpy fp64 matmul: every product is kept to
-    ~2^-24, so the error is bounded by a few ulp of sum_k |a||w| (several tiles, ragged M, padded N)."""
+    ~2^-24, so the error is bounded by a few ulp of sum_k |a||w| (several tiles, ragged M, padded N; grid_ctas > 0
+    makes each persistent CTA walk over several tiles, i.e. both TMEM accumulator buffers and the stage ring wrap)."""
     g = np.random.Generator(np.random.PCG64(M * 7 + N * 3 + K + pieces))
     a = (g.normal(0, 1.0, (M, K)) * np.exp(g.normal(0, 2.0, (M, 1)))).astype(np.float32)   # rows of very different scale
     w = g.normal(0, 0.05, (N, K)).astype(np.float32)
@@ -84,11 +85,11 @@ def test_tensor_core_gemm_against_fp64(boa, pieces, tile_n, M, N, K):
         w = _to_bf16(w)                                             # a bf16 blob: one exact piece
     want = a.astype(np.float64) @ w.astype(np.float64).T
     scale = np.abs(a).astype(np.float64) @ np.abs(w).astype(np.float64).T
-    got = _np(boa.debug_gemm(torch.from_numpy(a).cuda(), torch.from_numpy(w), pieces, tile_n)).astype(np.float64)
+    got = _np(boa.debug_gemm(torch.from_numpy(a).cuda(), torch.from_numpy(w), pieces, grid_ctas)).astype(np.float64)
     err = np.abs(got - want) / scale
     assert err.max() <= 2.0 ** -20, (err.max(), np.unravel_index(err.argmax(), err.shape))
     # and from host pointers
-    got_h = _np(boa.debug_gemm(torch.from_numpy(a), torch.from_numpy(w), pieces, tile_n))
+    got_h = _np(boa.debug_gemm(torch.from_numpy(a), torch.from_numpy(w), pieces, grid_ctas))
     assert np.array_equal(got_h.astype(np.float64), got)
 
 
