@@ -9,6 +9,7 @@
 #include <stdlib.h>
 
 #include <algorithm>
+#include <utility>
 #include <new>
 #include <vector>
 
@@ -200,11 +201,25 @@ int mark(StepCtx& c, int cls) {
 }
 
 // ---- tensor-core GEMM launch (tc_gemm.cuh).  The dynamic shared-memory opt-in is set once per instantiation.
+// Launch with the programmatic-serialization attribute (PDL, common.cuh): the kernel calls pdl_wait() before it
+// touches anything an earlier kernel of the stream wrote.
+bool g_pdl = true;   // BOA_NO_PDL=1 in the environment turns it off (read at boa_model_load)
+template <typename... KArgs, typename... Args>
+cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at; cfg.numAttrs = g_pdl ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+
 template <int NPW, int EPI>
 int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
   using C = tc::Cfg<NPW>;
   const int tiles = ((g.M + tc::BM - 1) / tc::BM) * g.NT;
-  tc::k_tc_gemm<NPW, EPI><<<std::min(tiles, n_sm), tc::NTHREADS, C::SMEM, st>>>(g);   // persistent: one CTA per SM
+  BOA_CUDA_TRY(launch_pdl(tc::k_tc_gemm<NPW, EPI>, dim3(std::min(tiles, n_sm)), dim3(tc::NTHREADS), C::SMEM, st, g));   // persistent: one CTA per SM
   return BOA_OK;
 }
 template <int NPW, int EPI>
@@ -284,10 +299,10 @@ int launch_step(StepCtx& c) {
       const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
       const dim3 grid(per_slice, slices);
       switch (m->R) {   // W_dt's row in registers when it is short enough
-        case 4: k_scan<4><<<grid, ec + 32, scan::smem_bytes(ec, m->ldj, 0), c.st>>>(sa); break;
-        case 8: k_scan<8><<<grid, ec + 32, scan::smem_bytes(ec, m->ldj, 0), c.st>>>(sa); break;
-        case 16: k_scan<16><<<grid, ec + 32, scan::smem_bytes(ec, m->ldj, 0), c.st>>>(sa); break;
-        default: k_scan<0><<<grid, ec + 32, scan::smem_bytes(ec, m->ldj, m->R), c.st>>>(sa); break;
+        case 4: BOA_CUDA_TRY(launch_pdl(k_scan<4>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
+        case 8: BOA_CUDA_TRY(launch_pdl(k_scan<8>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
+        case 16: BOA_CUDA_TRY(launch_pdl(k_scan<16>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
+        default: BOA_CUDA_TRY(launch_pdl(k_scan<0>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, m->R), c.st, sa)); break;
       }
       BOA_TRY(mark(c, BOA_K_SCAN));
     }
@@ -322,9 +337,11 @@ int launch_step(StepCtx& c) {
     k_coder_step<0, true><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, ea, c.dump_probs,
                                                    c.dump_cdf, c.dump_steps);
   } else if (c.mode == 0) {
-    k_coder_step<0, false><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, ea, nullptr, nullptr, 0);
+    BOA_CUDA_TRY(launch_pdl(k_coder_step<0, false>, dim3(cgrid), dim3(256), 0, c.st, (const float*)logits, c.data,
+                            c.chunk_bytes, c.ca, B, ea, (float*)nullptr, (uint32_t*)nullptr, 0u));
   } else {
-    k_coder_step<1, false><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, ea, nullptr, nullptr, 0);
+    BOA_CUDA_TRY(launch_pdl(k_coder_step<1, false>, dim3(cgrid), dim3(256), 0, c.st, (const float*)logits, c.data,
+                            c.chunk_bytes, c.ca, B, ea, (float*)nullptr, (uint32_t*)nullptr, 0u));
   }
   BOA_TRY(mark(c, BOA_K_CODER));
   return BOA_OK;
@@ -551,6 +568,7 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
   if (!m) return BOA_E_NOMEM;
   m->L = (int)L; m->D = (int)D; m->E = (int)E; m->R = (int)R; m->J = (int)J;
   m->blob_crc = crc32_ieee(p, nbytes);
+  g_pdl = getenv("BOA_NO_PDL") == nullptr;
   m->npw = dtype == 1 ? 1 : 3;         // a bf16 weight is one exact piece; an fp32 weight is cut into three
   m->ldj = J <= 64 ? 64 : 128;
   {

@@ -235,6 +235,8 @@ k_coder_step(const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes
              EmbedArgs ea, float* dump_probs, uint32_t* dump_cdf, uint32_t dump_steps) {
   const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
+  pdl_launch();
+  pdl_wait();                                     // logits, coder state and (decode) the output buffer come from earlier kernels
   if (i >= B) return;
   const uint32_t pos = ca.pos[i], len = ca.len[i];
   if (pos + 1u >= len) return;                    // finished stream: masked

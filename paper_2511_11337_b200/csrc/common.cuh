@@ -20,6 +20,13 @@ constexpr float kEps = 1e-5f;        // RMSNorm epsilon (R#10)
 // arithmetic (operation order, fusion, precision).
 constexpr uint32_t kArithVersion = 0x42320005u;
 
+// Programmatic dependent launch (PDL): a kernel launched with the programmatic-serialization attribute may start
+// while its predecessor in the stream is still draining; pdl_wait() blocks until the predecessor grid has completed
+// and its memory is visible (every thread that touches data produced upstream calls it first); pdl_launch() lets the
+// successor's CTAs be scheduled as soon as SMs free up.  Without the attribute both are no-ops.
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_launch() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // Last CUDA failure seen by this thread ("file:line: cudaErrorName"), for boa_last_cuda_error().
 inline char* last_cuda_error_buf() {
   static thread_local char buf[256] = "";

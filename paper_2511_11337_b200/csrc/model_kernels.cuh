@@ -164,6 +164,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
+  pdl_launch();
 
   if (tid >= EC) {
     // ===================================================================== copy warp
@@ -181,6 +182,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
       g2s(st + EC * 64 + EC * 4, a.xz + i * 2 * a.E + a.E + e0, (uint32_t)(EC * 4), bar);
       g2s(st + EC * 64 + 2 * EC * 4 + EC * 6, a.dbc + i * a.ldj, (uint32_t)(a.ldj * 4), bar);
     };
+    pdl_wait();                                    // the state, xz and the x_proj rows come from earlier kernels
     if (lane == 0)
       for (int k = 0; k < NSTG && k < nk; ++k) issue_load(k);
     const int nchunks = (EC >> 6) * 24;          // 16-byte chunks of the y pieces of one stream-slice

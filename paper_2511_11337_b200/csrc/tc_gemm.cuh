@@ -259,6 +259,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
   if (tid == 0) TC_TRACE(1);
+  pdl_launch();
+  pdl_wait();                                      // everything below reads what earlier kernels of the step wrote
 
   if (warp == 9) {
     // ===================================================================== copy warp

