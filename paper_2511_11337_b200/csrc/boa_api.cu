@@ -60,7 +60,8 @@ bool is_device_ptr(const void* p) {
 struct boa_model {
   int L = 0, D = 0, E = 0, R = 0, J = 0;
   int npw = 3;                 // bf16 pieces per weight: 3 for fp32 blobs, 1 for bf16 blobs (exact)
-  int ldj = 64;                // row stride of the x_proj output = its tile width (64 or 128)
+  int ldj = 64;                // row stride of the x_proj output = its padded width (64 or 128)
+  int ks_x = 1;                // k-splits of x_proj (a function of the model shape only: results must not depend on B)
   int n_sm = 148;              // SM count of the device (persistent grids)
   uint32_t blob_crc = 0;
   GrowBuf weights, wimg;
@@ -277,7 +278,7 @@ int launch_step(StepCtx& c) {
     float* winl = m->win.as<float>() + (size_t)l * m->Bcap * 3 * E;
     {  // S2-S4: xz = [SiLU(conv(W_in_x r)) ; W_in_z r],  r = RMSNorm(u);  xs also as the image for x_proj
       tc::GemmArgs g{};
-      g.A = u_img; g.M = B; g.KB = D / 64; g.W = w.img_in; g.NT = 2 * E / 64;
+      g.A = u_img; g.M = B; g.KB = D / 64; g.W = w.img_in; g.NT = 2 * E / 64; g.KS = 1;
       g.C = xz; g.ldc = 2 * E; g.n_valid = 2 * E;
       g.ssq_in = m->ssq.as<float>(); g.win = winl; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
@@ -288,6 +289,7 @@ int launch_step(StepCtx& c) {
       tc::GemmArgs g{};
       g.A = xs_img; g.M = B; g.KB = E / 64; g.W = w.img_x; g.NT = m->ldj / 64;
       g.C = dbc; g.ldc = m->ldj; g.n_valid = m->J;
+      g.KS = m->ks_x; g.split_stride = (size_t)m->Bcap * m->ldj;   // split over k: enough tiles to fill the SMs
       BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_CONVX));
     }
@@ -295,6 +297,7 @@ int launch_step(StepCtx& c) {
       ScanArgs sa{};
       sa.h = hl; sa.xz = xz; sa.dbc = dbc; sa.W_dtT = w.w_dtT; sa.b_dt = w.b_dt; sa.A4 = w.A4; sa.Dskip = w.d_skip;
       sa.y_img = y_img; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
+      sa.KS = m->ks_x; sa.dbc_split = (size_t)m->Bcap * m->ldj;
       const int ec = (E % 256 == 0) ? 256 : 128, slices = E / ec;
       const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
       const dim3 grid(per_slice, slices);
@@ -308,7 +311,7 @@ int launch_step(StepCtx& c) {
     }
     {  // S9: u += W_out y;  the new u also as the image for the next in_proj (times its RMSNorm weight) or the head
       tc::GemmArgs g{};
-      g.A = y_img; g.M = B; g.KB = E / 64; g.W = w.img_out; g.NT = D / 64;
+      g.A = y_img; g.M = B; g.KB = E / 64; g.W = w.img_out; g.NT = D / 64; g.KS = 1;
       g.C = u; g.ldc = D; g.n_valid = D;
       g.out_img = u_img; g.out_KB = D / 64; g.ssq_out = m->ssq.as<float>();
       g.out_scale = (l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
@@ -318,7 +321,7 @@ int launch_step(StepCtx& c) {
   }
   {  // S10: logits = Emb u
     tc::GemmArgs g{};
-    g.A = u_img; g.M = B; g.KB = D / 64; g.W = m->img_head; g.NT = 4;
+    g.A = u_img; g.M = B; g.KB = D / 64; g.W = m->img_head; g.NT = 4; g.KS = 1;
     g.C = logits; g.ldc = 256; g.n_valid = 256;
     BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
     BOA_TRY(mark(c, BOA_K_HEAD));
@@ -428,7 +431,7 @@ int reserve_workspace(boa_model* m, uint64_t B, size_t cap) {
     // state arrays are indexed [l][Bcap][...]: growing B invalidates nothing (state is reset per wave)
     BOA_TRY(m->u.reserve(B * D * 4));
     BOA_TRY(m->xz.reserve(B * 2 * E * 4));
-    BOA_TRY(m->dbc.reserve(B * (size_t)m->ldj * 4));
+    BOA_TRY(m->dbc.reserve((size_t)m->ks_x * B * m->ldj * 4));
     BOA_TRY(m->ssq.reserve(B * (D / 64) * 4));
     BOA_TRY(m->u_img.reserve(tc::img_bytes(B, D)));
     BOA_TRY(m->xs_img.reserve(tc::img_bytes(B, E)));
@@ -571,6 +574,7 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
   g_pdl = getenv("BOA_NO_PDL") == nullptr;
   m->npw = dtype == 1 ? 1 : 3;         // a bf16 weight is one exact piece; an fp32 weight is cut into three
   m->ldj = J <= 64 ? 64 : 128;
+  m->ks_x = ((E / 64) % 4 == 0) ? 4 : ((E / 64) % 2 == 0) ? 2 : 1;
   {
     int dev = 0, n_sm = 0;
     if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) == cudaSuccess && n_sm > 0)
@@ -984,7 +988,7 @@ int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N,
   g.A = static_cast<const uint8_t*>(aimg); g.M = (int)M; g.KB = (int)(K / 64);
   g.W = static_cast<const uint16_t*>(tw.dev);
   g.C = static_cast<float*>(cpad); g.ldc = (int)Np; g.n_valid = (int)Np;
-  g.NT = (int)(Np / 64);
+  g.NT = (int)(Np / 64); g.KS = 1;
   int n_sm = 148, dev = 0;
   if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
     (void)cudaGetLastError();

@@ -74,7 +74,9 @@ __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, con
 struct ScanArgs {
   float* h;                 // [B][E/EC][4][EC] float4 (this layer): the state of a stream and channel slice is one contiguous run
   const float* xz;          // [B][2E]: xs | z
-  const float* dbc;         // [B][ldj]: dlt[R] | Bv[16] | Cv[16]
+  const float* dbc;         // [KS][B][ldj] k-split partials of x_proj; their ascending sum is dlt[R] | Bv[16] | Cv[16]
+  int KS;                   // the copy warp adds the partials once per stream, ((p0+p1)+p2)+...
+  size_t dbc_split;         // elements between partials
   const float* W_dtT;       // [R][E]
   const float* b_dt;        // [E]
   const float4* A4;         // [4][E] float4: A * log2(e), A = -exp(A_log)
@@ -85,8 +87,9 @@ struct ScanArgs {
 
 namespace scan {
 constexpr int NSTG = 4;
-__host__ __device__ inline int stage_bytes(int EC, int ldj) { return EC * 64 + 2 * EC * 4 + EC * 6 + ldj * 4; }   // h | xs | z | y pieces | dbc
-__host__ __device__ inline int smem_bytes(int EC, int ldj, int R) { return NSTG * stage_bytes(EC, ldj) + R * EC * 4 + 2 * NSTG * 8 + 128; }   // R = 0 when W_dt sits in registers
+constexpr int KSMAX = 4;         // x_proj k-split partial rows per stage
+__host__ __device__ inline int stage_bytes(int EC, int ldj) { return EC * 64 + 2 * EC * 4 + EC * 6 + KSMAX * ldj * 4; }   // h | xs | z | y pieces | dbc partials
+__host__ __device__ inline int smem_bytes(int EC, int ldj, int R) { return NSTG * stage_bytes(EC, ldj) + R * EC * 4 + 3 * NSTG * 8 + 128; }   // R = 0 when W_dt sits in registers
 
 __device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void bar_init(uint32_t bar, uint32_t count) {
@@ -155,12 +158,16 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   const int SB = stage_bytes(EC, a.ldj);
   uint8_t* stages = scan_smem;
   float* wdt = reinterpret_cast<float*>(scan_smem + NSTG * SB);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(scan_smem + NSTG * SB + (RR ? 0 : a.R * EC * 4));   // full[NSTG], done[NSTG]
+  uint64_t* bars = reinterpret_cast<uint64_t*>(scan_smem + NSTG * SB + (RR ? 0 : a.R * EC * 4));   // full, done, ready [NSTG] each
   const int nk = (a.B - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // streams of this CTA
   if (nk <= 0) return;
 
   if (tid == 0) {
-    for (int s = 0; s < NSTG; ++s) { bar_init(s_u32(&bars[s]), 1); bar_init(s_u32(&bars[NSTG + s]), (uint32_t)EC); }
+    for (int s = 0; s < NSTG; ++s) {
+      bar_init(s_u32(&bars[s]), 1);                       // full: the bulk copies of a stage have landed
+      bar_init(s_u32(&bars[NSTG + s]), (uint32_t)EC);     // done: every channel thread has finished the stream
+      bar_init(s_u32(&bars[2 * NSTG + s]), 1);            // ready: the x_proj partial rows have been added up
+    }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   __syncthreads();
@@ -171,7 +178,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     const int lane = tid - EC;
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    const uint32_t tx = (uint32_t)(EC * 64 + 2 * EC * 4 + a.ldj * 4);
+    const uint32_t tx = (uint32_t)(EC * 64 + 2 * EC * 4 + a.KS * a.ldj * 4);
     auto issue_load = [&](int k) {   // lane 0
       const int s = k % NSTG;
       const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
@@ -180,15 +187,31 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
       g2s_hint(st, a.h + ((i * slices + sl) * 4) * (size_t)EC * 4, (uint32_t)(EC * 64), bar, pol);
       g2s(st + EC * 64, a.xz + i * 2 * a.E + e0, (uint32_t)(EC * 4), bar);
       g2s(st + EC * 64 + EC * 4, a.xz + i * 2 * a.E + a.E + e0, (uint32_t)(EC * 4), bar);
-      g2s(st + EC * 64 + 2 * EC * 4 + EC * 6, a.dbc + i * a.ldj, (uint32_t)(a.ldj * 4), bar);
+      for (int p = 0; p < a.KS; ++p)
+        g2s(st + EC * 64 + 2 * EC * 4 + EC * 6 + p * a.ldj * 4, a.dbc + p * a.dbc_split + i * a.ldj, (uint32_t)(a.ldj * 4), bar);
+    };
+    // S5, last step: the k-split partials of the x_proj row are added in ascending order, in place, once per stream
+    auto reduce_row = [&](int k) {   // whole warp
+      const int s = k % NSTG;
+      bar_wait(s_u32(&bars[s]), (uint32_t)((k / NSTG) & 1));
+      float* row = reinterpret_cast<float*>(stages + s * SB + EC * 64 + 2 * EC * 4 + EC * 6);
+      for (int c = lane; c < a.ldj; c += 32) {
+        float v = row[c];
+        for (int p = 1; p < a.KS; ++p) v += row[p * a.ldj + c];
+        row[c] = v;
+      }
+      __syncwarp();
+      if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(&bars[2 * NSTG + s])) : "memory");
     };
     pdl_wait();                                    // the state, xz and the x_proj rows come from earlier kernels
     if (lane == 0)
       for (int k = 0; k < NSTG && k < nk; ++k) issue_load(k);
     const int nchunks = (EC >> 6) * 24;          // 16-byte chunks of the y pieces of one stream-slice
+    reduce_row(0);
     for (int k = 0; k < nk; ++k) {
       const int s = k % NSTG;
       uint8_t* st = stages + s * SB;
+      if (k + 1 < nk) reduce_row(k + 1);           // its copies were issued at least one iteration ago
       bar_wait(s_u32(&bars[NSTG + s]), (uint32_t)((k / NSTG) & 1));      // every channel of stream k is done
       const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
       if (lane == 0) {
@@ -229,7 +252,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   for (int k = 0; k < nk; ++k) {
     const int s = k % NSTG;
     uint8_t* st = stages + s * SB;
-    bar_wait(s_u32(&bars[s]), (uint32_t)((k / NSTG) & 1));
+    bar_wait(s_u32(&bars[2 * NSTG + s]), (uint32_t)((k / NSTG) & 1));   // copies landed and the x_proj row added up
     float4* hs = reinterpret_cast<float4*>(st);
     const float* xs_s = reinterpret_cast<const float*>(st + EC * 64);
     const float* row = reinterpret_cast<const float*>(st + EC * 64 + 2 * EC * 4 + EC * 6);

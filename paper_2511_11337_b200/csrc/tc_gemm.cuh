@@ -51,6 +51,8 @@ struct GemmArgs {
   int M, KB;               // KB = K/64
   const uint16_t* W;       // weight image [N/64][K/64][NPW][64 x 64 bf16, swizzled]
   int NT;                  // column tiles (N/64, N padded with zero weight rows)
+  int KS;                  // k-splits (>= 1, divides KB): split s covers k-blocks [s*KB/KS, (s+1)*KB/KS) and writes its
+  size_t split_stride;     //   partial result to C + s*split_stride; the consumer adds the partials in ascending order
   float* C;                // [M][ldc] fp32 result (in_proj: xz = xs | z; out_proj: the residual stream u, updated)
   int ldc, n_valid;        // columns >= n_valid are not stored (zero-padded weight rows)
   // EPI_INPROJ only
@@ -234,8 +236,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   __shared__ uint32_t tmem_base_s;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-  const int KB = g.KB, NT = g.NT;
-  const int ntiles = ((g.M + BM - 1) / BM) * NT;
+  const int KB = g.KB / g.KS, NT = g.NT, KS = g.KS;     // KB: k-blocks of one work item
+  const int ntiles = ((g.M + BM - 1) / BM) * NT * KS;    // work item t -> (row tile, column tile, k-split), k-split fastest
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   if (tid == 0) TC_TRACE(0);
 
@@ -267,9 +269,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     if (lane == 0) {
       int kbc = 0;                                 // k-blocks issued so far: position in the stage ring
       for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int mt = tile / NT, nt = tile - mt * NT;
-        const uint8_t* asrc = g.A + img_block((size_t)mt, 0, (size_t)KB);
-        const uint16_t* wsrc = g.W + (size_t)nt * KB * (NPW * BN * 64);
+        const int ks = tile % KS, t2 = tile / KS, mt = t2 / NT, nt = t2 - mt * NT;
+        const uint8_t* asrc = g.A + img_block((size_t)mt, (size_t)ks * KB, (size_t)g.KB);
+        const uint16_t* wsrc = g.W + ((size_t)nt * g.KB + (size_t)ks * KB) * (NPW * BN * 64);
         for (int kb = 0; kb < KB; ++kb, ++kbc) {
           const int s = kbc % C::NST, round = kbc / C::NST;
           if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
@@ -330,18 +332,34 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     int it = 0;
     for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
       const int b = it & 1;
-      const int mt = tile / NT, nt = tile - mt * NT;
+      const int ks = tile % KS, t2 = tile / KS, mt = t2 / NT, nt = t2 - mt * NT;
       const int m0 = mt * BM, n0 = nt * BN;
+      float* Cout = g.C + (size_t)ks * g.split_stride;
       // Pass 1: TMEM -> registers (thread = stream row; warps w and w+4 share the 32 TMEM lanes of rows 32*(w%4)..
       // and take one 32-column half each) -> shared staging tile, so that pass 2 can run with lane = column and
       // every global access coalesced.
       const int r1 = (warp & 3) * 32 + lane;
       float rs = 1.0f;
       if (EPI == EPI_INPROJ) {                     // S2: RMSNorm row scale from the block sums of u^2, ascending
-        const float* sp = g.ssq_in + (size_t)min(m0 + r1, g.M - 1) * KB;
+        const float* sp = g.ssq_in + (size_t)min(m0 + r1, g.M - 1) * g.KB;
         float ss = 0.0f;
-        for (int q = 0; q < KB; ++q) ss += sp[q];
-        rs = 1.0f / sqrtf(ss / (float)(KB * BK) + kEps);
+        for (int q = 0; q < g.KB; ++q) ss += sp[q];
+        rs = 1.0f / sqrtf(ss / (float)(g.KB * BK) + kEps);
+      }
+      // The conv window of the first row batch does not depend on the accumulators: its loads (from HBM at large B)
+      // are issued now and fly while the main loop of this tile finishes.
+      const int nb = n0 + col;
+      const bool conv_tile = EPI == EPI_INPROJ && n0 < g.E;
+      float4 w0[4], w1[4], w2[4];
+      if (conv_tile) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const int r = (warp + 8 * u) * RPI + lane / LPR;
+          const float* wp = g.win + (size_t)min(m0 + r, g.M - 1) * 3 * g.E + nb;
+          w0[u] = *reinterpret_cast<const float4*>(wp);
+          w1[u] = *reinterpret_cast<const float4*>(wp + g.E);
+          w2[u] = *reinterpret_cast<const float4*>(wp + 2 * g.E);
+        }
       }
       mbar_wait(smem_u32(&acc_full[b]), (uint32_t)((it >> 1) & 1));
       tc_fence_after();
@@ -368,41 +386,49 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       asm volatile("bar.sync 1, 256;" ::: "memory");
       // Pass 2: 16 lanes own one 64-column row segment (4 consecutive columns per lane), two rows per warp
       // instruction; rows are processed four at a time with all loads issued first.
-      const int nb = n0 + col;
-      if (EPI == EPI_INPROJ && n0 < g.E) {
+      if (conv_tile) {
         // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU; the window moves one step (R#11).
         // The lane's four channels are fixed within a tile, so their taps and biases live in registers.  xs goes out
-        // twice: fp32 (the scan reads it) and cut into pieces in the image of x_proj's operand.
+        // twice: fp32 (the scan reads it) and cut into pieces in the image of x_proj's operand.  The window loads of
+        // the next row batch are issued before the current one is computed.
         const float4 cw0 = g.conv_w[nb], cw1 = g.conv_w[nb + 1], cw2 = g.conv_w[nb + 2], cw3 = g.conv_w[nb + 3];
         const float4 cb = *reinterpret_cast<const float4*>(g.conv_b + nb);
-#pragma unroll 1
+#pragma unroll
         for (int i0 = 0; i0 < NIT; i0 += 4) {
-          float4 x[4], w0[4], w1[4], w2[4];
+          float4 x[4], n0_[4], n1_[4], n2_[4];
           int rows[4];
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const int r = (warp + 8 * (i0 + u)) * RPI + lane / LPR;
             rows[u] = m0 + r;
             x[u] = *reinterpret_cast<const float4*>(stile + r * LDS + col);
-            const float* wp = g.win + (size_t)min(rows[u], g.M - 1) * 3 * g.E + nb;
-            w0[u] = *reinterpret_cast<const float4*>(wp);
-            w1[u] = *reinterpret_cast<const float4*>(wp + g.E);
-            w2[u] = *reinterpret_cast<const float4*>(wp + 2 * g.E);
+            if (i0 + 4 < NIT) {
+              const int rn = (warp + 8 * (i0 + 4 + u)) * RPI + lane / LPR;
+              const float* wp = g.win + (size_t)min(m0 + rn, g.M - 1) * 3 * g.E + nb;
+              n0_[u] = *reinterpret_cast<const float4*>(wp);
+              n1_[u] = *reinterpret_cast<const float4*>(wp + g.E);
+              n2_[u] = *reinterpret_cast<const float4*>(wp + 2 * g.E);
+            }
           }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
-            if (rows[u] >= g.M) continue;
-            float4 o;
-            { float xc = fmaf(cw0.w, x[u].x, cb.x); xc = fmaf(cw0.x, w0[u].x, xc); xc = fmaf(cw0.y, w1[u].x, xc); xc = fmaf(cw0.z, w2[u].x, xc); o.x = xc * sigmoid_tc(xc); }
-            { float xc = fmaf(cw1.w, x[u].y, cb.y); xc = fmaf(cw1.x, w0[u].y, xc); xc = fmaf(cw1.y, w1[u].y, xc); xc = fmaf(cw1.z, w2[u].y, xc); o.y = xc * sigmoid_tc(xc); }
-            { float xc = fmaf(cw2.w, x[u].z, cb.z); xc = fmaf(cw2.x, w0[u].z, xc); xc = fmaf(cw2.y, w1[u].z, xc); xc = fmaf(cw2.z, w2[u].z, xc); o.z = xc * sigmoid_tc(xc); }
-            { float xc = fmaf(cw3.w, x[u].w, cb.w); xc = fmaf(cw3.x, w0[u].w, xc); xc = fmaf(cw3.y, w1[u].w, xc); xc = fmaf(cw3.z, w2[u].w, xc); o.w = xc * sigmoid_tc(xc); }
-            float* wp = g.win + (size_t)rows[u] * 3 * g.E + nb;
-            *reinterpret_cast<float4*>(wp) = w1[u];
-            *reinterpret_cast<float4*>(wp + g.E) = w2[u];
-            *reinterpret_cast<float4*>(wp + 2 * g.E) = x[u];
-            *reinterpret_cast<float4*>(g.C + (size_t)rows[u] * g.ldc + nb) = o;
-            cut4_store(g.out_img, g.out_KB, rows[u], nb, o);
+            if (rows[u] < g.M) {
+              float4 o;
+              { float xc = fmaf(cw0.w, x[u].x, cb.x); xc = fmaf(cw0.x, w0[u].x, xc); xc = fmaf(cw0.y, w1[u].x, xc); xc = fmaf(cw0.z, w2[u].x, xc); o.x = xc * sigmoid_tc(xc); }
+              { float xc = fmaf(cw1.w, x[u].y, cb.y); xc = fmaf(cw1.x, w0[u].y, xc); xc = fmaf(cw1.y, w1[u].y, xc); xc = fmaf(cw1.z, w2[u].y, xc); o.y = xc * sigmoid_tc(xc); }
+              { float xc = fmaf(cw2.w, x[u].z, cb.z); xc = fmaf(cw2.x, w0[u].z, xc); xc = fmaf(cw2.y, w1[u].z, xc); xc = fmaf(cw2.z, w2[u].z, xc); o.z = xc * sigmoid_tc(xc); }
+              { float xc = fmaf(cw3.w, x[u].w, cb.w); xc = fmaf(cw3.x, w0[u].w, xc); xc = fmaf(cw3.y, w1[u].w, xc); xc = fmaf(cw3.z, w2[u].w, xc); o.w = xc * sigmoid_tc(xc); }
+              float* wp = g.win + (size_t)rows[u] * 3 * g.E + nb;
+              *reinterpret_cast<float4*>(wp) = w1[u];
+              *reinterpret_cast<float4*>(wp + g.E) = w2[u];
+              *reinterpret_cast<float4*>(wp + 2 * g.E) = x[u];
+              *reinterpret_cast<float4*>(Cout + (size_t)rows[u] * g.ldc + nb) = o;
+              cut4_store(g.out_img, g.out_KB, rows[u], nb, o);
+            }
+          }
+          if (i0 + 4 < NIT) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) { w0[u] = n0_[u]; w1[u] = n1_[u]; w2[u] = n2_[u]; }
           }
         }
       } else {
@@ -418,7 +444,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
             const int r = (warp + 8 * (i0 + u)) * RPI + lane / LPR;
             rows[u] = m0 + r;
             o[u] = *reinterpret_cast<const float4*>(stile + r * LDS + col);
-            if (EPI == EPI_RESID) q[u] = *reinterpret_cast<const float4*>(g.C + (size_t)min(rows[u], g.M - 1) * g.ldc + nb);
+            if (EPI == EPI_RESID) q[u] = *reinterpret_cast<const float4*>(Cout + (size_t)min(rows[u], g.M - 1) * g.ldc + nb);
           }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
@@ -437,7 +463,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
                 if ((lane % LPR) == 0) g.ssq_out[(size_t)rows[u] * g.out_KB + nt] = ss;
               }
             }
-            if (live) *reinterpret_cast<float4*>(g.C + (size_t)rows[u] * g.ldc + nb) = o[u];
+            if (live) *reinterpret_cast<float4*>(Cout + (size_t)rows[u] * g.ldc + nb) = o[u];
           }
         }
       }
