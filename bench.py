@@ -149,6 +149,12 @@ def run_reference(args, cfg):
     print(json.dumps(line))
 
 
+# DRAM bytes per launch (dram__bytes_read.sum + dram__bytes_write.sum) measured by ncu inside the running step, cache
+# state left as it is (profiles/r01_insitu_traffic.md): config name -> kernel class -> bytes.
+NCU_TRAFFIC = {"cfg2_kinematics_64MiB": {"scan": 145.8e6 + 120.7e6, "inproj": 26.2e6 + 16.7e6, "convx": 12.6e6,
+                                         "outproj": 12.6e6, "head": 6.3e6}}
+
+
 def kernel_work(cfg, B):
     """Algorithmic work of ONE launch of each kernel class for B streams."""
     s = cfg.shape
@@ -302,7 +308,9 @@ def run_ours(args, cfg):
         k = ranked[0]
         e = kernels[k]
         line["roofline"] = {"kernel": k, "bound": e["bound"], "achieved": e["achieved"], "peak": e["peak"], "unit": e["unit"],
-                            "frac": e["frac"], "traffic": None, "peak_source": peaks["source"], "share_of_step": e["share"]}
+                            "frac": e["frac"], "traffic": NCU_TRAFFIC.get(cfg.name, {}).get(k),
+                            "algorithmic": work[k][1], "traffic_unit": "bytes per launch (ncu, in situ)",
+                            "peak_source": peaks["source"], "share_of_step": e["share"]}
     else:
         line["roofline"] = None
     s = cfg.shape

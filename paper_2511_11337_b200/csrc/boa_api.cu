@@ -186,6 +186,19 @@ struct StepCtx {
   size_t ev_used = 0;
 };
 
+#ifdef BOA_DEV
+// development builds only: BOA_DEV_SKIP is a bit mask of kernel classes whose launches are skipped (timing experiments;
+// results are then wrong)
+inline unsigned dev_skip_mask() {
+  static int v = -1;
+  if (v < 0) { const char* e = getenv("BOA_DEV_SKIP"); v = e ? atoi(e) : 0; }
+  return (unsigned)v;
+}
+#define BOA_DEV_SKIPPED(cls) (dev_skip_mask() & (1u << (cls)))
+#else
+#define BOA_DEV_SKIPPED(cls) false
+#endif
+
 int mark(StepCtx& c, int cls) {
   ++c.launches;
   BOA_CUDA_TRY(cudaPeekAtLastError());
@@ -219,7 +232,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 template <int NPW, int EPI>
 int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
   using C = tc::Cfg<NPW>;
-  const int tiles = ((g.M + tc::BM - 1) / tc::BM) * g.NT;
+  const int tiles = ((g.M + tc::BM - 1) / tc::BM) * g.NT * g.KS;
   BOA_CUDA_TRY(launch_pdl(tc::k_tc_gemm<NPW, EPI>, dim3(std::min(tiles, n_sm)), dim3(tc::NTHREADS), C::SMEM, st, g));   // persistent: one CTA per SM
   return BOA_OK;
 }
@@ -282,7 +295,7 @@ int launch_step(StepCtx& c) {
       g.C = xz; g.ldc = 2 * E; g.n_valid = 2 * E;
       g.ssq_in = m->ssq.as<float>(); g.win = winl; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
-      BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
+      if (!BOA_DEV_SKIPPED(BOA_K_INPROJ)) BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_INPROJ));
     }
     {  // S5: [dlt;Bv;Cv] = W_x xs
@@ -290,7 +303,7 @@ int launch_step(StepCtx& c) {
       g.A = xs_img; g.M = B; g.KB = E / 64; g.W = w.img_x; g.NT = m->ldj / 64;
       g.C = dbc; g.ldc = m->ldj; g.n_valid = m->J;
       g.KS = m->ks_x; g.split_stride = (size_t)m->Bcap * m->ldj;   // split over k: enough tiles to fill the SMs
-      BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
+      if (!BOA_DEV_SKIPPED(BOA_K_CONVX)) BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_CONVX));
     }
     {  // S6-S8: persistent, two CTAs per SM, each walking over streams for one channel slice
@@ -301,6 +314,7 @@ int launch_step(StepCtx& c) {
       const int ec = (E % 256 == 0) ? 256 : 128, slices = E / ec;
       const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
       const dim3 grid(per_slice, slices);
+      if (!BOA_DEV_SKIPPED(BOA_K_SCAN))
       switch (m->R) {   // W_dt's row in registers when it is short enough
         case 4: BOA_CUDA_TRY(launch_pdl(k_scan<4>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
         case 8: BOA_CUDA_TRY(launch_pdl(k_scan<8>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
@@ -315,7 +329,7 @@ int launch_step(StepCtx& c) {
       g.C = u; g.ldc = D; g.n_valid = D;
       g.out_img = u_img; g.out_KB = D / 64; g.ssq_out = m->ssq.as<float>();
       g.out_scale = (l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
-      BOA_TRY((launch_tc_npw<tc::EPI_RESID>(m->npw, g, m->n_sm, c.st)));
+      if (!BOA_DEV_SKIPPED(BOA_K_OUTPROJ)) BOA_TRY((launch_tc_npw<tc::EPI_RESID>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_OUTPROJ));
     }
   }
@@ -323,7 +337,7 @@ int launch_step(StepCtx& c) {
     tc::GemmArgs g{};
     g.A = u_img; g.M = B; g.KB = D / 64; g.W = m->img_head; g.NT = 4; g.KS = 1;
     g.C = logits; g.ldc = 256; g.n_valid = 256;
-    BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
+    if (!BOA_DEV_SKIPPED(BOA_K_HEAD)) BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
     BOA_TRY(mark(c, BOA_K_HEAD));
   }
 
