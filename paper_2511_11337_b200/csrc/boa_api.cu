@@ -218,6 +218,7 @@ int mark(StepCtx& c, int cls) {
 // Launch with the programmatic-serialization attribute (PDL, common.cuh): the kernel calls pdl_wait() before it
 // touches anything an earlier kernel of the stream wrote.
 bool g_pdl = true;   // BOA_NO_PDL=1 in the environment turns it off (read at boa_model_load)
+bool g_cluster = true;   // BOA_NO_CLUSTER=1: launch the contraction kernels without 2-CTA clusters (same results)
 template <typename... KArgs, typename... Args>
 cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
   cudaLaunchConfig_t cfg{};
@@ -232,13 +233,31 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
 template <int NPW, int EPI>
 int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
   using C = tc::Cfg<NPW>;
-  const int tiles = ((g.M + tc::BM - 1) / tc::BM) * g.NT * g.KS;
-  BOA_CUDA_TRY(launch_pdl(tc::k_tc_gemm<NPW, EPI>, dim3(std::min(tiles, n_sm)), dim3(tc::NTHREADS), C::SMEM, st, g));   // persistent: one CTA per SM
+  const int mt = (g.M + tc::BM - 1) / tc::BM;
+  cudaLaunchConfig_t cfg{};
+  cfg.blockDim = dim3(tc::NTHREADS); cfg.dynamicSmemBytes = C::SMEM; cfg.stream = st;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = g_pdl ? 1 : 0;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  if (g_cluster && g.NT % 2 == 0) {
+    // clusters of two CTAs share the activation k-blocks of a row tile (multicast): persistent, one cluster per SM pair
+    const int items = mt * (g.NT / 2) * g.KS;
+    cfg.gridDim = dim3(2 * std::min(items, n_sm / 2));
+    at[1].id = cudaLaunchAttributeClusterDimension;
+    at[1].val.clusterDim.x = 2; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
+    cfg.numAttrs = 2;
+    BOA_CUDA_TRY(cudaLaunchKernelEx(&cfg, tc::k_tc_gemm<NPW, EPI, 2>, g));
+  } else {
+    cfg.gridDim = dim3(std::min(mt * g.NT * g.KS, n_sm));             // persistent: one CTA per SM
+    BOA_CUDA_TRY(cudaLaunchKernelEx(&cfg, tc::k_tc_gemm<NPW, EPI, 1>, g));
+  }
   return BOA_OK;
 }
 template <int NPW, int EPI>
 int optin_tc() {
-  BOA_CUDA_TRY(cudaFuncSetAttribute(tc::k_tc_gemm<NPW, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Cfg<NPW>::SMEM));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(tc::k_tc_gemm<NPW, EPI, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Cfg<NPW>::SMEM));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(tc::k_tc_gemm<NPW, EPI, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Cfg<NPW>::SMEM));
   return BOA_OK;
 }
 // Shared-memory opt-ins of every kernel instantiation the step can launch (called by boa_model_load, outside
@@ -586,6 +605,7 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
   m->L = (int)L; m->D = (int)D; m->E = (int)E; m->R = (int)R; m->J = (int)J;
   m->blob_crc = crc32_ieee(p, nbytes);
   g_pdl = getenv("BOA_NO_PDL") == nullptr;
+  g_cluster = getenv("BOA_NO_CLUSTER") == nullptr;
   m->npw = dtype == 1 ? 1 : 3;         // a bf16 weight is one exact piece; an fp32 weight is cut into three
   m->ldj = J <= 64 ? 64 : 128;
   m->ks_x = ((E / 64) % 4 == 0) ? 4 : ((E / 64) % 2 == 0) ? 2 : 1;

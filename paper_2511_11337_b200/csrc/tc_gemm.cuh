@@ -107,6 +107,20 @@ __device__ __forceinline__ void bulk_g2s(uint32_t dst, const void* src, uint32_t
   asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
 }
+// the same, delivered to the same shared-memory offset (and mbarrier) of every CTA of the cluster named in `mask`
+__device__ __forceinline__ void bulk_g2s_mc(uint32_t dst, const void* src, uint32_t bytes, uint32_t bar, uint16_t mask) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes.multicast::cluster [%0], [%1], %2, [%3], %4;"
+               ::"r"(dst), "l"(src), "r"(bytes), "r"(bar), "h"(mask) : "memory");
+}
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ void cluster_sync() {   // every thread of every CTA of the cluster
+  asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+  asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 // generic-proxy shared stores -> visible to the async proxy (tensor core operand reads)
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 __device__ __forceinline__ void tc_fence_before() { asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory"); }
@@ -132,6 +146,12 @@ __device__ __forceinline__ void umma(uint32_t d_tmem, uint64_t adesc, uint64_t b
 // arrive on the mbarrier when every MMA issued so far by this thread has completed
 __device__ __forceinline__ void umma_commit(uint32_t bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(bar) : "memory");
+}
+
+// the same arrival on the mbarrier at this offset in every CTA of the cluster named in `mask`
+__device__ __forceinline__ void umma_commit_mc(uint32_t bar, uint16_t mask) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+               ::"r"(bar), "h"(mask) : "memory");
 }
 
 // 32 consecutive fp32 columns of this thread's TMEM lane
@@ -227,17 +247,26 @@ constexpr int NTHREADS = NEPI + 64;
 // grid = min(tiles, SMs), block = 320.  Tile t -> (row tile t / NT, column tile t % NT); CTA c takes tiles c,
 // c + grid, ...  Warp 9 (one lane) streams the k-blocks of both operand images into the stage ring; warp 8 (one lane)
 // issues the MMAs into accumulator buffer (tile iteration & 1); warps 0-7 drain the other buffer and run the epilogue.
-template <int NPW, int EPI>
+// CS = 2: the kernel is launched in clusters of two CTAs that take the two column tiles 2j, 2j+1 of the same row tile in
+// lock-step and share its activation k-blocks: each CTA fetches one half of the 48 KB block and the bulk copy delivers
+// it to both (multicast), halving the L2 -> SM traffic of A; a stage is reused when the MMAs of BOTH CTAs have read it.
+template <int NPW, int EPI, int CS>
 __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   using C = Cfg<NPW>;
   static_assert(NPW == 1 || NPW == 3, "weight pieces");
+  static_assert(CS == 1 || CS == 2, "cluster size");
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t full_bar[C::NST], empty_bar[C::NST], acc_full[2], acc_empty[2];
   __shared__ uint32_t tmem_base_s;
 
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int KB = g.KB / g.KS, NT = g.NT, KS = g.KS;     // KB: k-blocks of one work item
-  const int ntiles = ((g.M + BM - 1) / BM) * NT * KS;    // work item t -> (row tile, column tile, k-split), k-split fastest
+  // work item t -> (row tile, column tile [pair], k-split), k-split fastest; with CS = 2 an item is a pair of column
+  // tiles and this CTA takes the one of its rank
+  const int NTI = NT / CS;
+  const int ntiles = ((g.M + BM - 1) / BM) * NTI * KS;
+  const int crank = CS == 2 ? (int)cluster_ctarank() : 0;
+  const int item0 = (int)blockIdx.x / CS, item_step = (int)gridDim.x / CS;
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   if (tid == 0) TC_TRACE(0);
 
@@ -245,7 +274,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     if (lane == 0) {
       for (int s = 0; s < C::NST; ++s) {
         mbar_init(smem_u32(&full_bar[s]), 1);     // the copy warp's arrive.expect_tx
-        mbar_init(smem_u32(&empty_bar[s]), 1);    // one tcgen05.commit
+        mbar_init(smem_u32(&empty_bar[s]), CS);   // one tcgen05.commit per CTA of the cluster
       }
       for (int b = 0; b < 2; ++b) {
         mbar_init(smem_u32(&acc_full[b]), 1);     // one tcgen05.commit
@@ -258,6 +287,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   }
   tc_fence_before();
   __syncthreads();
+  if (CS == 2) cluster_sync();                     // the peer's barriers are initialised before anything is sent to them
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
   if (tid == 0) TC_TRACE(1);
@@ -268,8 +298,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     // ===================================================================== copy warp
     if (lane == 0) {
       int kbc = 0;                                 // k-blocks issued so far: position in the stage ring
-      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-        const int ks = tile % KS, t2 = tile / KS, mt = t2 / NT, nt = t2 - mt * NT;
+      for (int tile = item0; tile < ntiles; tile += item_step) {
+        const int ks = tile % KS, t2 = tile / KS, mt = t2 / NTI, nt = (t2 - mt * NTI) * CS + crank;
         const uint8_t* asrc = g.A + img_block((size_t)mt, (size_t)ks * KB, (size_t)g.KB);
         const uint16_t* wsrc = g.W + ((size_t)nt * g.KB + (size_t)ks * KB) * (NPW * BN * 64);
         for (int kb = 0; kb < KB; ++kb, ++kbc) {
@@ -277,7 +307,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
           if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
           const uint32_t sA = sbase + (uint32_t)s * C::STAGE, fb = smem_u32(&full_bar[s]);
           mbar_arrive_expect_tx(fb, (uint32_t)C::STAGE);
-          bulk_g2s(sA, asrc + (size_t)kb * C::A_BYTES, (uint32_t)C::A_BYTES, fb);
+          if (CS == 2)                             // this CTA's half of the block, delivered to both CTAs
+            bulk_g2s_mc(sA + (uint32_t)crank * (C::A_BYTES / 2), asrc + (size_t)kb * C::A_BYTES + (size_t)crank * (C::A_BYTES / 2),
+                        (uint32_t)(C::A_BYTES / 2), fb, (uint16_t)3);
+          else
+            bulk_g2s(sA, asrc + (size_t)kb * C::A_BYTES, (uint32_t)C::A_BYTES, fb);
           bulk_g2s(sA + C::A_BYTES, wsrc + (size_t)kb * (NPW * BN * 64), (uint32_t)C::W_BYTES, fb);
         }
       }
@@ -286,7 +320,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     // ===================================================================== MMA issuer
     if (lane == 0) {
       int kbc = 0, it = 0;
-      for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+      for (int tile = item0; tile < ntiles; tile += item_step, ++it) {
         const int b = it & 1;
         if (it >= 2) {                             // the epilogue has drained this buffer (tile it-2)
           mbar_wait(smem_u32(&acc_empty[b]), (uint32_t)(((it >> 1) - 1) & 1));
@@ -315,7 +349,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
               umma(tacc + 64, A_(1), wd, idesc_bf16(64), 1u);
             }
           }
-          umma_commit(smem_u32(&empty_bar[s]));                      // stage free when these MMAs have read it
+          if (CS == 2) umma_commit_mc(smem_u32(&empty_bar[s]), (uint16_t)3);   // stage free in both CTAs when both have read it
+          else umma_commit(smem_u32(&empty_bar[s]));                 // stage free when these MMAs have read it
         }
         umma_commit(smem_u32(&acc_full[b]));                         // this tile's accumulators are complete
         if (it < 8) TC_TRACE(8 + it);
@@ -330,9 +365,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     constexpr int NIT = BM / (8 * RPI);            // row groups per warp
     const int col = (lane % LPR) * 4;
     int it = 0;
-    for (int tile = blockIdx.x; tile < ntiles; tile += gridDim.x, ++it) {
+    for (int tile = item0; tile < ntiles; tile += item_step, ++it) {
       const int b = it & 1;
-      const int ks = tile % KS, t2 = tile / KS, mt = t2 / NT, nt = t2 - mt * NT;
+      const int ks = tile % KS, t2 = tile / KS, mt = t2 / NTI, nt = (t2 - mt * NTI) * CS + crank;
       const int m0 = mt * BM, n0 = nt * BN;
       float* Cout = g.C + (size_t)ks * g.split_stride;
       // Pass 1: TMEM -> registers (thread = stream row; warps w and w+4 share the 32 TMEM lanes of rows 32*(w%4)..
@@ -474,6 +509,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
 
   tc_fence_before();
   __syncthreads();
+  if (CS == 2) cluster_sync();                     // no CTA leaves while its peer may still send to it
   if (warp == 8) {
     __syncwarp();
     tmem_dealloc(tmem, C::TMEM_COLS);
