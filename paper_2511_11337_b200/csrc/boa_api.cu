@@ -312,7 +312,7 @@ int launch_step(StepCtx& c) {
       tc::GemmArgs g{};
       g.A = u_img; g.M = B; g.KB = D / 64; g.W = w.img_in; g.NT = 2 * E / 64; g.KS = 1;
       g.C = xz; g.ldc = 2 * E; g.n_valid = 2 * E;
-      g.ssq_in = m->ssq.as<float>(); g.win = winl; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
+      g.ssq_in = m->ssq.as<float>(); g.win = winl; g.pos = c.ca.pos; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
       if (!BOA_DEV_SKIPPED(BOA_K_INPROJ)) BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_INPROJ));

@@ -207,6 +207,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     if (lane == 0)
       for (int k = 0; k < NSTG && k < nk; ++k) issue_load(k);
     const int nchunks = (EC >> 6) * 24;          // 16-byte chunks of the y pieces of one stream-slice
+    const uint64_t keep = tc::policy_evict_last();
     reduce_row(0);
     for (int k = 0; k < nk; ++k) {
       const int s = k % NSTG;
@@ -224,7 +225,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
         const int rowid = c >> 3, kt = rowid / 3, q = rowid - kt * 3;
         uint8_t* dst = a.y_img + tc::img_block(i >> 7, (size_t)(e0 >> 6) + kt, (size_t)(a.E >> 6)) + (size_t)q * tc::A_PLANE +
                        (r >> 3) * 1024 + (r & 7) * 128 + (c & 7) * 16;
-        *reinterpret_cast<uint4*>(dst) = *reinterpret_cast<const uint4*>(st + EC * 64 + 2 * EC * 4 + rowid * 128 + (c & 7) * 16);
+        tc::st_keep_v4(dst, *reinterpret_cast<const uint4*>(st + EC * 64 + 2 * EC * 4 + rowid * 128 + (c & 7) * 16), keep);
       }
       __syncwarp();
       if (lane == 0 && k >= 1 && k - 1 + NSTG < nk) {

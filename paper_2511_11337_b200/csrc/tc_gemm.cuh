@@ -58,7 +58,8 @@ struct GemmArgs {
   // EPI_INPROJ only
   const float* ssq_in;     // [M][KB]: sum of u^2 over each 64-column block of the residual stream (written by the
                            // producer of u in a fixed order); rstd = 1/sqrt(sum/K + eps) (R#10)
-  float* win;              // [M][3][E] conv window of this layer
+  float* win;              // [M][3][E] conv window of this layer, a ring: at step t slot t%3 holds x_{t-3} and receives x_t
+  const uint32_t* pos;     // [M] steps taken so far by each stream (the coder's position) = t
   const float4* conv_w;    // [E] taps (x = t-3 ... w = t)
   const float* conv_b;     // [E]
   int E;
@@ -197,12 +198,27 @@ __host__ __device__ inline size_t img_bytes(size_t M, size_t K) { return ((M + B
 __device__ __forceinline__ float trunc_bf16(float v) { return __uint_as_float(__float_as_uint(v) & 0xFFFF0000u); }
 __device__ __forceinline__ uint32_t pack_hi(float lo, float hi) { return __byte_perm(__float_as_uint(lo), __float_as_uint(hi), 0x7632); }
 
+// L2 policy for the activation images: they are written by one kernel and read by the next while hundreds of MB of
+// state stream through L2 in between, so their lines are marked evict-last (the state copies are evict-first).
+__device__ __forceinline__ uint64_t policy_evict_last() {
+  uint64_t pol;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(pol));
+  return pol;
+}
+__device__ __forceinline__ void st_keep_v2(void* p, uint32_t a, uint32_t b, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v2.b32 [%0], {%1, %2}, %3;" ::"l"(p), "r"(a), "r"(b), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_keep_v4(void* p, uint4 v, uint64_t pol) {
+  asm volatile("st.global.L2::cache_hint.v4.b32 [%0], {%1, %2, %3, %4}, %5;" ::"l"(p), "r"(v.x), "r"(v.y), "r"(v.z), "r"(v.w), "l"(pol) : "memory");
+}
+
 // Cut 4 consecutive values (row m, columns k..k+3, k % 4 == 0) and store the pieces into an image: 8 bytes per plane.
 __device__ __forceinline__ void cut4_store(uint8_t* img, int KB, int m, int k, float4 v) {
   uint8_t* p = img + img_block((size_t)(m >> 7), (size_t)(k >> 6), (size_t)KB) + plane_off(m & 127, k & 63);
+  const uint64_t pol = policy_evict_last();
 #pragma unroll
   for (int q = 0; q < NPA; ++q) {
-    *reinterpret_cast<uint2*>(p + q * A_PLANE) = make_uint2(pack_hi(v.x, v.y), pack_hi(v.z, v.w));
+    st_keep_v2(p + q * A_PLANE, pack_hi(v.x, v.y), pack_hi(v.z, v.w), pol);
     v.x = __fsub_rn(v.x, trunc_bf16(v.x)); v.y = __fsub_rn(v.y, trunc_bf16(v.y));
     v.z = __fsub_rn(v.z, trunc_bf16(v.z)); v.w = __fsub_rn(v.w, trunc_bf16(v.w));
   }
@@ -386,14 +402,17 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       const int nb = n0 + col;
       const bool conv_tile = EPI == EPI_INPROJ && n0 < g.E;
       float4 w0[4], w1[4], w2[4];
+      int slot[4];                                 // ring slot of x_{t-3} (and of x_t after this step)
       if (conv_tile) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           const int r = (warp + 8 * u) * RPI + lane / LPR;
-          const float* wp = g.win + (size_t)min(m0 + r, g.M - 1) * 3 * g.E + nb;
-          w0[u] = *reinterpret_cast<const float4*>(wp);
-          w1[u] = *reinterpret_cast<const float4*>(wp + g.E);
-          w2[u] = *reinterpret_cast<const float4*>(wp + 2 * g.E);
+          const int rc = min(m0 + r, g.M - 1);
+          slot[u] = (int)(g.pos[rc] % 3u);
+          const float* wp = g.win + (size_t)rc * 3 * g.E + nb;
+          w0[u] = *reinterpret_cast<const float4*>(wp + slot[u] * g.E);
+          w1[u] = *reinterpret_cast<const float4*>(wp + ((slot[u] + 1) % 3) * g.E);
+          w2[u] = *reinterpret_cast<const float4*>(wp + ((slot[u] + 2) % 3) * g.E);
         }
       }
       mbar_wait(smem_u32(&acc_full[b]), (uint32_t)((it >> 1) & 1));
@@ -422,7 +441,8 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       // Pass 2: 16 lanes own one 64-column row segment (4 consecutive columns per lane), two rows per warp
       // instruction; rows are processed four at a time with all loads issued first.
       if (conv_tile) {
-        // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU; the window moves one step (R#11).
+        // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU (R#11).  The window is a ring of three
+        // slots per stream: all three are read, only the oldest is overwritten with x_t.
         // The lane's four channels are fixed within a tile, so their taps and biases live in registers.  xs goes out
         // twice: fp32 (the scan reads it) and cut into pieces in the image of x_proj's operand.  The window loads of
         // the next row batch are issued before the current one is computed.
@@ -431,7 +451,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
 #pragma unroll
         for (int i0 = 0; i0 < NIT; i0 += 4) {
           float4 x[4], n0_[4], n1_[4], n2_[4];
-          int rows[4];
+          int rows[4], nslot[4];
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
             const int r = (warp + 8 * (i0 + u)) * RPI + lane / LPR;
@@ -439,10 +459,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
             x[u] = *reinterpret_cast<const float4*>(stile + r * LDS + col);
             if (i0 + 4 < NIT) {
               const int rn = (warp + 8 * (i0 + 4 + u)) * RPI + lane / LPR;
-              const float* wp = g.win + (size_t)min(m0 + rn, g.M - 1) * 3 * g.E + nb;
-              n0_[u] = *reinterpret_cast<const float4*>(wp);
-              n1_[u] = *reinterpret_cast<const float4*>(wp + g.E);
-              n2_[u] = *reinterpret_cast<const float4*>(wp + 2 * g.E);
+              const int rc = min(m0 + rn, g.M - 1);
+              nslot[u] = (int)(g.pos[rc] % 3u);
+              const float* wp = g.win + (size_t)rc * 3 * g.E + nb;
+              n0_[u] = *reinterpret_cast<const float4*>(wp + nslot[u] * g.E);
+              n1_[u] = *reinterpret_cast<const float4*>(wp + ((nslot[u] + 1) % 3) * g.E);
+              n2_[u] = *reinterpret_cast<const float4*>(wp + ((nslot[u] + 2) % 3) * g.E);
             }
           }
 #pragma unroll
@@ -453,17 +475,14 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
               { float xc = fmaf(cw1.w, x[u].y, cb.y); xc = fmaf(cw1.x, w0[u].y, xc); xc = fmaf(cw1.y, w1[u].y, xc); xc = fmaf(cw1.z, w2[u].y, xc); o.y = xc * sigmoid_tc(xc); }
               { float xc = fmaf(cw2.w, x[u].z, cb.z); xc = fmaf(cw2.x, w0[u].z, xc); xc = fmaf(cw2.y, w1[u].z, xc); xc = fmaf(cw2.z, w2[u].z, xc); o.z = xc * sigmoid_tc(xc); }
               { float xc = fmaf(cw3.w, x[u].w, cb.w); xc = fmaf(cw3.x, w0[u].w, xc); xc = fmaf(cw3.y, w1[u].w, xc); xc = fmaf(cw3.z, w2[u].w, xc); o.w = xc * sigmoid_tc(xc); }
-              float* wp = g.win + (size_t)rows[u] * 3 * g.E + nb;
-              *reinterpret_cast<float4*>(wp) = w1[u];
-              *reinterpret_cast<float4*>(wp + g.E) = w2[u];
-              *reinterpret_cast<float4*>(wp + 2 * g.E) = x[u];
+              *reinterpret_cast<float4*>(g.win + ((size_t)rows[u] * 3 + slot[u]) * g.E + nb) = x[u];
               *reinterpret_cast<float4*>(Cout + (size_t)rows[u] * g.ldc + nb) = o;
               cut4_store(g.out_img, g.out_KB, rows[u], nb, o);
             }
           }
           if (i0 + 4 < NIT) {
 #pragma unroll
-            for (int u = 0; u < 4; ++u) { w0[u] = n0_[u]; w1[u] = n1_[u]; w2[u] = n2_[u]; }
+            for (int u = 0; u < 4; ++u) { w0[u] = n0_[u]; w1[u] = n1_[u]; w2[u] = n2_[u]; slot[u] = nslot[u]; }
           }
         }
       } else {
