@@ -297,3 +297,27 @@ def test_full_size_cfg2_in_the_bench_configuration(boa):
     # eq. 1 on a sampled stream: payload within (0, 5) bytes of the ideal code length under the GPU's own tables
     _, _, _, _, payloads = container.unpack(_np(comp).tobytes(), gm.fingerprint)
     assert len(payloads) == B and all(len(p) >= 4 for p in payloads)
+
+
+def test_maximum_wave_65536_streams_cfg4_model(boa):
+    """The largest wave the library steps together (65,536 streams, SURVEY 8(d) cfg4 sweep end point) on the cfg4 model
+    (4 layers, D = 256, bf16 matrices): 512 row tiles per contraction, 10 GB of stream state.  Byte-exact round trip of
+    every stream, and sampled streams against the oracle (probabilities 1e-5, tables bit-exact)."""
+    cfg = synth.CONFIGS[4]
+    blob = synth.make_weights(cfg.shape, cfg.model_seed, synth.DTYPE_BF16, emb_std=0.25)
+    gm = boa.Model(blob)
+    w = model.load_weights(blob)
+    B, T = 65536, 24
+    data = synth.CONFIGS[2].data(B * T)
+    src = torch.frombuffer(bytearray(data), dtype=torch.uint8).cuda()
+    comp = gm.compress(src, T)
+    assert torch.equal(gm.decompress(comp), src)
+    d = gm.debug_step_dump(src, T, T - 1, want=("logits", "probs", "cdf"))
+    buf = np.frombuffer(data, np.uint8).reshape(B, T)
+    ids = [0, 1, 32767, 32768, 65535]
+    ref = quantise.softmax(model.logits_for_chunks(w, buf[ids]))
+    err = np.abs(_np(d["probs"][ids]).astype(np.float64) - ref).max()
+    print(f"[parity] cfg4 model, 65536 streams, streams {ids}: max |p_gpu - p_oracle| = {err:.3e}")
+    assert err <= PROB_TOL
+    lg = _np(d["logits"][ids])
+    assert np.array_equal(_np(d["cdf"][ids]).astype(np.int64).reshape(-1, 257), quantise.quantise(lg.reshape(-1, 256)))
