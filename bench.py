@@ -114,7 +114,7 @@ def time_oracle(cfg, n_streams=64, length=128):
 
 
 def workload_name(cfg):
-    return (f"{cfg.name}: {cfg.n_bytes >> 20} MiB, {cfg.n_bytes // cfg.chunk_bytes} chunks x {cfg.chunk_bytes >> 10} KiB, "
+    return (f"{cfg.name}: {cfg.n_bytes / MiB:g} MiB, {cfg.n_bytes // cfg.chunk_bytes} chunks x {cfg.chunk_bytes / 1024:g} KiB, "
             f"{cfg.shape.n_layer}-layer d_model={cfg.shape.d_model} {'bf16' if cfg.weight_dtype else 'fp32'} weights")
 
 
@@ -189,7 +189,8 @@ def run_ours(args, cfg):
 
     # weak scaling: every rank gets the full workload shape on its own seeded input
     n, chunk = cfg.n_bytes, cfg.chunk_bytes
-    rcfg = cfg if rank == 0 else type(cfg)(**{**cfg.__dict__, "data_seed": cfg.data_seed + 7919 * rank})
+    import dataclasses
+    rcfg = cfg if rank == 0 else dataclasses.replace(cfg, data_seed=cfg.data_seed + 7919 * rank)
     host = torch.frombuffer(bytearray(rcfg.data()), dtype=torch.uint8)
     m = boa.Model(cfg.weights())
     d_in = host.to(dev)
@@ -308,7 +309,7 @@ def run_ours(args, cfg):
         k = ranked[0]
         e = kernels[k]
         line["roofline"] = {"kernel": k, "bound": e["bound"], "achieved": e["achieved"], "peak": e["peak"], "unit": e["unit"],
-                            "frac": e["frac"], "traffic": NCU_TRAFFIC.get(cfg.name, {}).get(k),
+                            "frac": e["frac"], "traffic": NCU_TRAFFIC.get(cfg.name, {}).get(k) if B == 4096 else None,
                             "algorithmic": work[k][1], "traffic_unit": "bytes per launch (ncu, in situ)",
                             "peak_source": peaks["source"], "share_of_step": e["share"]}
     else:
@@ -335,9 +336,16 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--sample-every", type=int, default=48, help="event-bracket every k-th 32-step batch (roofline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--streams", type=int, default=0, help="run the config's model with this many chunks (streams per step) ...")
+    ap.add_argument("--chunk-bytes", type=int, default=0, help="... of this many bytes each (a sweep point, not the headline workload)")
     args = ap.parse_args()
     from paper_2511_11337_b200 import synth
     cfg = synth.CONFIGS[args.config]
+    if args.streams or args.chunk_bytes:
+        import dataclasses
+        chunk = args.chunk_bytes or cfg.chunk_bytes
+        streams = args.streams or cfg.n_bytes // cfg.chunk_bytes
+        cfg = dataclasses.replace(cfg, name=f"{cfg.name}[sweep: {streams} streams x {chunk} B]", n_bytes=streams * chunk, chunk_bytes=chunk)
     if args.impl == "reference":
         run_reference(args, cfg)
     else:

@@ -273,6 +273,7 @@ int init_kernels() {
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
   return BOA_OK;
 }
 
@@ -338,6 +339,7 @@ int launch_step(StepCtx& c) {
         case 4: BOA_CUDA_TRY(launch_pdl(k_scan<4>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
         case 8: BOA_CUDA_TRY(launch_pdl(k_scan<8>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
         case 16: BOA_CUDA_TRY(launch_pdl(k_scan<16>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
+        case 32: BOA_CUDA_TRY(launch_pdl(k_scan<32>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
         default: BOA_CUDA_TRY(launch_pdl(k_scan<0>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, m->R), c.st, sa)); break;
       }
       BOA_TRY(mark(c, BOA_K_SCAN));

@@ -147,7 +147,7 @@ __device__ __forceinline__ void scan_update4(float4& h, const float4 a2, const f
 
 // grid = (CTAs per slice, E / EC), block = EC + 32 threads (EC = 256 or 128), two CTAs per SM.
 // Warps 0..EC/32-1: one thread per channel of the slice.  The last warp drives the bulk copies and moves the y pieces.
-// RR = dt_rank when W_dt's row fits in registers (4, 8, 16), else 0 (row kept in shared memory).
+// RR = dt_rank when W_dt's row is held in registers (4, 8, 16, 32), else 0 (row kept in shared memory).
 template <int RR>
 __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   using namespace scan;
