@@ -263,14 +263,15 @@ constexpr int NTHREADS = NEPI + 64;
 // grid = min(tiles, SMs), block = 320.  Tile t -> (row tile t / NT, column tile t % NT); CTA c takes tiles c,
 // c + grid, ...  Warp 9 (one lane) streams the k-blocks of both operand images into the stage ring; warp 8 (one lane)
 // issues the MMAs into accumulator buffer (tile iteration & 1); warps 0-7 drain the other buffer and run the epilogue.
-// CS = 2: the kernel is launched in clusters of two CTAs that take the two column tiles 2j, 2j+1 of the same row tile in
-// lock-step and share its activation k-blocks: each CTA fetches one half of the 48 KB block and the bulk copy delivers
-// it to both (multicast), halving the L2 -> SM traffic of A; a stage is reused when the MMAs of BOTH CTAs have read it.
+// CS > 1: the kernel is launched in clusters of CS CTAs that take CS consecutive column tiles of the same row tile in
+// lock-step and share its activation k-blocks: each CTA fetches 1/CS of the 48 KB block and the bulk copy delivers
+// it to all of them (multicast); a stage is reused when the MMAs of ALL CTAs of the cluster have read it.
 template <int NPW, int EPI, int CS>
 __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   using C = Cfg<NPW>;
   static_assert(NPW == 1 || NPW == 3, "weight pieces");
-  static_assert(CS == 1 || CS == 2, "cluster size");
+  static_assert(CS == 1 || CS == 2 || CS == 4 || CS == 8, "cluster size");
+  constexpr uint16_t CMASK = (uint16_t)((1u << CS) - 1u);
   extern __shared__ uint8_t smem_raw[];
   __shared__ __align__(8) uint64_t full_bar[C::NST], empty_bar[C::NST], acc_full[2], acc_empty[2];
   __shared__ uint32_t tmem_base_s;
@@ -281,7 +282,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   // tiles and this CTA takes the one of its rank
   const int NTI = NT / CS;
   const int ntiles = ((g.M + BM - 1) / BM) * NTI * KS;
-  const int crank = CS == 2 ? (int)cluster_ctarank() : 0;
+  const int crank = CS > 1 ? (int)cluster_ctarank() : 0;
   const int item0 = (int)blockIdx.x / CS, item_step = (int)gridDim.x / CS;
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   if (tid == 0) TC_TRACE(0);
@@ -303,7 +304,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   }
   tc_fence_before();
   __syncthreads();
-  if (CS == 2) cluster_sync();                     // the peer's barriers are initialised before anything is sent to them
+  if (CS > 1) cluster_sync();                      // the peers' barriers are initialised before anything is sent to them
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
   if (tid == 0) TC_TRACE(1);
@@ -323,9 +324,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
           if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
           const uint32_t sA = sbase + (uint32_t)s * C::STAGE, fb = smem_u32(&full_bar[s]);
           mbar_arrive_expect_tx(fb, (uint32_t)C::STAGE);
-          if (CS == 2)                             // this CTA's half of the block, delivered to both CTAs
-            bulk_g2s_mc(sA + (uint32_t)crank * (C::A_BYTES / 2), asrc + (size_t)kb * C::A_BYTES + (size_t)crank * (C::A_BYTES / 2),
-                        (uint32_t)(C::A_BYTES / 2), fb, (uint16_t)3);
+          if (CS > 1)                              // this CTA's part of the block, delivered to every CTA of the cluster
+            bulk_g2s_mc(sA + (uint32_t)crank * (C::A_BYTES / CS), asrc + (size_t)kb * C::A_BYTES + (size_t)crank * (C::A_BYTES / CS),
+                        (uint32_t)(C::A_BYTES / CS), fb, CMASK);
           else
             bulk_g2s(sA, asrc + (size_t)kb * C::A_BYTES, (uint32_t)C::A_BYTES, fb);
           bulk_g2s(sA + C::A_BYTES, wsrc + (size_t)kb * (NPW * BN * 64), (uint32_t)C::W_BYTES, fb);
@@ -365,7 +366,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
               umma(tacc + 64, A_(1), wd, idesc_bf16(64), 1u);
             }
           }
-          if (CS == 2) umma_commit_mc(smem_u32(&empty_bar[s]), (uint16_t)3);   // stage free in both CTAs when both have read it
+          if (CS > 1) umma_commit_mc(smem_u32(&empty_bar[s]), CMASK);   // stage free in every CTA when all have read it
           else umma_commit(smem_u32(&empty_bar[s]));                 // stage free when these MMAs have read it
         }
         umma_commit(smem_u32(&acc_full[b]));                         // this tile's accumulators are complete
@@ -528,7 +529,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
 
   tc_fence_before();
   __syncthreads();
-  if (CS == 2) cluster_sync();                     // no CTA leaves while its peer may still send to it
+  if (CS > 1) cluster_sync();                      // no CTA leaves while a peer may still send to it
   if (warp == 8) {
     __syncwarp();
     tmem_dealloc(tmem, C::TMEM_COLS);
