@@ -54,7 +54,7 @@ typedef struct boa_model boa_model; /* opaque: device weights + workspace */
  * [256][D] (also the tied head), per layer norm_w, W_in, conv_w, conv_b, W_x, W_dt,
  * b_dt, A_log, D_skip, W_out (eq. 20-22) — copy it to the current CUDA device and
  * return a handle.  Supported: d_state = 16, d_conv = 4, expand = 2, d_model a multiple of 64 and
- * <= 512, dt_rank <= 64, tied head, fp32 or bf16 matrices; else BOA_E_UNSUPPORTED.
+ * <= 512, dt_rank a multiple of 4 and <= 64, tied head, fp32 or bf16 matrices; else BOA_E_UNSUPPORTED.
  * The blob is not referenced after the call returns. */
 int boa_model_load(const void* weights, size_t nbytes, boa_model** out);
 void boa_model_free(boa_model* m);
@@ -97,13 +97,13 @@ const char* boa_last_cuda_error(void);
 /* ---- measurement hooks ---------------------------------------------------------------------------
  * Kernel classes of the step: the order below is the launch order inside one step. */
 enum {
-  BOA_K_EMBED = 0,   /* S1  byte embedding gather                                 */
-  BOA_K_INPROJ = 1,  /* S2+S3  RMSNorm + in_proj                                  */
-  BOA_K_CONVX = 2,   /* S4-S6  conv1d+SiLU, x_proj, dt_proj+softplus              */
-  BOA_K_SCAN = 3,    /* S7+S8  selective-SSM recurrence + gate (state streamed)   */
-  BOA_K_OUTPROJ = 4, /* S9  out_proj + residual                                   */
-  BOA_K_HEAD = 5,    /* S10 tied head                                             */
-  BOA_K_CODER = 6,   /* S11-S14 softmax, table, range coder step                  */
+  BOA_K_EMBED = 0,   /* S1  byte embedding of the first step of a wave (later steps: in the coder) */
+  BOA_K_INPROJ = 1,  /* S2-S4  RMSNorm + in_proj + causal conv1d + SiLU (tensor cores)             */
+  BOA_K_CONVX = 2,   /* S5  x_proj (tensor cores, split over k)                                    */
+  BOA_K_SCAN = 3,    /* S6-S8  dt_proj + softplus, selective-SSM recurrence, gate (state streamed) */
+  BOA_K_OUTPROJ = 4, /* S9  out_proj + residual (tensor cores)                                     */
+  BOA_K_HEAD = 5,    /* S10 tied head (tensor cores)                                               */
+  BOA_K_CODER = 6,   /* S11-S14 softmax, table, range coder step; S1 of the next step              */
   BOA_K_FINISH = 7,  /* S15/S16 flush, compaction, init                           */
   BOA_K_COUNT = 8
 };

@@ -597,7 +597,7 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
                  K = get_u32(p + 24), ex = get_u32(p + 28), R = get_u32(p + 32), flags = get_u32(p + 36);
   if (dtype > 1) return BOA_E_FORMAT;
   if (N != (uint32_t)kNState || K != (uint32_t)kDConv || ex != 2 || !(flags & 1u) || (flags & ~1u) || L == 0 || L > 64 ||
-      D == 0 || D % 64 != 0 || D > 512 || R == 0 || R > 64)
+      D == 0 || D % 64 != 0 || D > 512 || R == 0 || R > 64 || R % 4 != 0)
     return BOA_E_UNSUPPORTED;
   BOA_TRY(check_device());
   const size_t E = 2 * (size_t)D, J = R + 2 * kNState;
