@@ -24,6 +24,8 @@ using namespace boa;
 namespace {
 
 constexpr int kStepsPerGraph = 32;       // model steps captured into one CUDA graph launch
+constexpr int kSlabT = 8;                // steps per encode-side time slab
+constexpr int kSlabsPerGraph = 4;        // slabs captured into one CUDA graph launch
 constexpr uint64_t kMaxWaveStreams = 65536;  // streams stepped together; more chunks run in waves
 
 struct GrowBuf {   // grow-only device buffer
@@ -70,7 +72,8 @@ struct boa_model {
   std::vector<LayerW> layers;
 
   // workspace (per wave of Bcap streams)
-  uint64_t Bcap = 0;
+  uint64_t Bcap = 0;           // streams the per-stream buffers (state, window, coder) are sized for
+  uint64_t rows_cap = 0;       // rows the per-row activation buffers are sized for (>= Bcap; Bcap * kSlabT for time slabs)
   GrowBuf u, xz, dbc, logits, h, win, ssq;
   GrowBuf u_img, xs_img, y_img;   // activation images: operands of the tensor-core contractions (tc_gemm.cuh)
   GrowBuf pos, len, low, range, pending, wpos, cache, started, v, rpos, off, size, scratch, first, err;
@@ -179,6 +182,7 @@ struct StepCtx {
   bool dump = false;
   float* dump_logits = nullptr; float* dump_probs = nullptr; uint32_t* dump_cdf = nullptr;
   uint32_t dump_steps = 0, dump_t = 0;
+  int slab_T = 1;           // > 1: one call of launch_step advances every stream by slab_T steps (encode only)
   // accounting
   uint64_t launches = 0;
   bool sample = false;      // record an event after every launch
@@ -283,20 +287,25 @@ int launch_tc_npw(int npw, const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
 }
 
 // S1 for the first step of a wave: u = Emb[byte 0] (later steps: fused into the coder step).
-int launch_embed(StepCtx& c) {
+int launch_embed(StepCtx& c, int T = 1) {
   boa_model* m = c.m;
-  const int total = c.B * (m->D / 4);
-  k_embed<<<(total + 255) / 256, 256, 0, c.st>>>(c.data, c.chunk_bytes, c.ca.pos, c.ca.len,
+  const long long total = (long long)c.B * T * (m->D / 4);
+  k_embed<<<(unsigned)((total + 255) / 256), 256, 0, c.st>>>(c.data, c.chunk_bytes, c.ca.pos, c.ca.len,
                                                   reinterpret_cast<const float4*>(m->emb), m->u.as<float4>(),
                                                   reinterpret_cast<const float4*>(m->layers[0].norm_w),
-                                                  m->u_img.as<uint8_t>(), m->ssq.as<float>(), c.B, m->D / 4);
+                                                  m->u_img.as<uint8_t>(), m->ssq.as<float>(), c.B, m->D / 4, T);
   return mark(c, BOA_K_EMBED);
 }
 
 // One model step + one coder step for all B streams of the wave (S2-S14, and S1 of the next step).
+// With c.slab_T = T > 1 (encode-side time slab) the same kernels advance every stream by T steps:
+// the contractions run on B*T rows (row t*B + i), the conv walks over the T steps with the window in registers
+// (k_conv_slab), the scan keeps the state in registers across the T steps, the coder codes T symbols per stream.
+// Per row / per step the arithmetic is that of the step path, so the decoder (always step by step) reproduces it.
 int launch_step(StepCtx& c) {
   boa_model* m = c.m;
   const int B = c.B, D = m->D, E = m->E;
+  const int T = c.slab_T, rows = B * T;
   float* u = m->u.as<float>();
   float* xz = m->xz.as<float>();
   float* dbc = m->dbc.as<float>();
@@ -311,18 +320,23 @@ int launch_step(StepCtx& c) {
     float* winl = m->win.as<float>() + (size_t)l * m->Bcap * 3 * E;
     {  // S2-S4: xz = [SiLU(conv(W_in_x r)) ; W_in_z r],  r = RMSNorm(u);  xs also as the image for x_proj
       tc::GemmArgs g{};
-      g.A = u_img; g.M = B; g.KB = D / 64; g.W = w.img_in; g.NT = 2 * E / 64; g.KS = 1;
+      g.A = u_img; g.M = rows; g.KB = D / 64; g.W = w.img_in; g.NT = 2 * E / 64; g.KS = 1;
       g.C = xz; g.ldc = 2 * E; g.n_valid = 2 * E;
-      g.ssq_in = m->ssq.as<float>(); g.win = winl; g.pos = c.ca.pos; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
+      g.ssq_in = m->ssq.as<float>(); g.win = T == 1 ? winl : nullptr; g.pos = c.ca.pos; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
       if (!BOA_DEV_SKIPPED(BOA_K_INPROJ)) BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_INPROJ));
+      if (T > 1) {   // S4 over the slab
+        const long long total = (long long)B * (E / 4);
+        tc::k_conv_slab<<<(unsigned)((total + 255) / 256), 256, 0, c.st>>>(xz, winl, c.ca.pos, w.conv_w, w.conv_b, xs_img, B, E, T);
+        BOA_TRY(mark(c, BOA_K_INPROJ));
+      }
     }
     {  // S5: [dlt;Bv;Cv] = W_x xs
       tc::GemmArgs g{};
-      g.A = xs_img; g.M = B; g.KB = E / 64; g.W = w.img_x; g.NT = m->ldj / 64;
+      g.A = xs_img; g.M = rows; g.KB = E / 64; g.W = w.img_x; g.NT = m->ldj / 64;
       g.C = dbc; g.ldc = m->ldj; g.n_valid = m->J;
-      g.KS = m->ks_x; g.split_stride = (size_t)m->Bcap * m->ldj;   // split over k: enough tiles to fill the SMs
+      g.KS = m->ks_x; g.split_stride = (size_t)m->rows_cap * m->ldj;   // split over k: enough tiles to fill the SMs
       if (!BOA_DEV_SKIPPED(BOA_K_CONVX)) BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_CONVX));
     }
@@ -330,7 +344,7 @@ int launch_step(StepCtx& c) {
       ScanArgs sa{};
       sa.h = hl; sa.xz = xz; sa.dbc = dbc; sa.W_dtT = w.w_dtT; sa.b_dt = w.b_dt; sa.A4 = w.A4; sa.Dskip = w.d_skip;
       sa.y_img = y_img; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
-      sa.KS = m->ks_x; sa.dbc_split = (size_t)m->Bcap * m->ldj;
+      sa.KS = m->ks_x; sa.dbc_split = (size_t)m->rows_cap * m->ldj; sa.T = T;
       const int ec = (E % 256 == 0) ? 256 : 128, slices = E / ec;
       const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
       const dim3 grid(per_slice, slices);
@@ -346,7 +360,7 @@ int launch_step(StepCtx& c) {
     }
     {  // S9: u += W_out y;  the new u also as the image for the next in_proj (times its RMSNorm weight) or the head
       tc::GemmArgs g{};
-      g.A = y_img; g.M = B; g.KB = E / 64; g.W = w.img_out; g.NT = D / 64; g.KS = 1;
+      g.A = y_img; g.M = rows; g.KB = E / 64; g.W = w.img_out; g.NT = D / 64; g.KS = 1;
       g.C = u; g.ldc = D; g.n_valid = D;
       g.out_img = u_img; g.out_KB = D / 64; g.ssq_out = m->ssq.as<float>();
       g.out_scale = (l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
@@ -356,7 +370,7 @@ int launch_step(StepCtx& c) {
   }
   {  // S10: logits = Emb u
     tc::GemmArgs g{};
-    g.A = u_img; g.M = B; g.KB = D / 64; g.W = m->img_head; g.NT = 4; g.KS = 1;
+    g.A = u_img; g.M = rows; g.KB = D / 64; g.W = m->img_head; g.NT = 4; g.KS = 1;
     g.C = logits; g.ldc = 256; g.n_valid = 256;
     if (!BOA_DEV_SKIPPED(BOA_K_HEAD)) BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
     BOA_TRY(mark(c, BOA_K_HEAD));
@@ -366,7 +380,10 @@ int launch_step(StepCtx& c) {
   EmbedArgs ea{};
   ea.emb = reinterpret_cast<const float4*>(m->emb); ea.norm_w = reinterpret_cast<const float4*>(m->layers[0].norm_w);
   ea.u = m->u.as<float4>(); ea.u_img = u_img; ea.ssq = m->ssq.as<float>(); ea.D4 = D / 4;
-  if (c.dump) {
+  if (T > 1) {
+    BOA_CUDA_TRY(launch_pdl(k_coder_slab, dim3(cgrid), dim3(256), 0, c.st, (const float*)logits, (const uint8_t*)c.data,
+                            c.chunk_bytes, c.ca, B, T));
+  } else if (c.dump) {
     if (c.dump_logits) {
       BOA_CUDA_TRY(cudaMemcpy2DAsync(c.dump_logits + (size_t)c.dump_t * 256, (size_t)c.dump_steps * 256 * sizeof(float),
                                      logits, 256 * sizeof(float), 256 * sizeof(float), B,
@@ -454,24 +471,70 @@ int run_steps(StepCtx& c, uint64_t steps) {
   return rc;
 }
 
-// ------------------------------------------------------------------------------------- workspace
-size_t bytes_per_stream(const boa_model* m, size_t cap) {
-  const size_t E = m->E, D = m->D;
-  return 4 * (D + 2 * E + 128 + 256) + 6 * (D + 2 * E) + (size_t)m->L * 4 * (E * kNState + 3 * E) + 64 + cap;
+// Encode-side time slabs: n_slabs times (embed kSlabT bytes per stream, one launch_step with slab_T = kSlabT),
+// CUDA-graph batches of kSlabsPerGraph slabs, remainder eager.
+int run_slabs(StepCtx& c, uint64_t n_slabs) {
+  if (n_slabs == 0) return BOA_OK;
+  const int saved_T = c.slab_T;
+  c.slab_T = kSlabT;
+  const uint64_t G = std::min<uint64_t>(kSlabsPerGraph, n_slabs);
+  const uint64_t n_batches = n_slabs / G, rem = n_slabs - n_batches * G;
+  cudaGraph_t graph = nullptr;
+  cudaGraphExec_t exec = nullptr;
+  int rc = BOA_OK;
+  const uint64_t before = c.launches;
+  cudaError_t e = cudaStreamBeginCapture(c.st, cudaStreamCaptureModeThreadLocal);
+  if (e != cudaSuccess) { c.slab_T = saved_T; return note_cuda_error(e, __FILE__, __LINE__); }
+  for (uint64_t s = 0; s < G && rc == BOA_OK; ++s) {
+    rc = launch_embed(c, kSlabT);
+    if (rc == BOA_OK) rc = launch_step(c);
+  }
+  e = cudaStreamEndCapture(c.st, &graph);
+  const uint64_t graph_nodes = c.launches - before;
+  c.launches = before;
+  if (rc == BOA_OK && e != cudaSuccess) rc = note_cuda_error(e, __FILE__, __LINE__);
+  if (rc == BOA_OK && (e = cudaGraphInstantiate(&exec, graph, 0)) != cudaSuccess) rc = note_cuda_error(e, __FILE__, __LINE__);
+  for (uint64_t b = 0; b < n_batches && rc == BOA_OK; ++b) {
+    if ((e = cudaGraphLaunch(exec, c.st)) != cudaSuccess) rc = note_cuda_error(e, __FILE__, __LINE__);
+    c.launches += graph_nodes;
+  }
+  for (uint64_t s = 0; s < rem && rc == BOA_OK; ++s) {
+    rc = launch_embed(c, kSlabT);
+    if (rc == BOA_OK) rc = launch_step(c);
+  }
+  if (exec) cudaGraphExecDestroy(exec);
+  if (graph) cudaGraphDestroy(graph);
+  c.slab_T = saved_T;
+  return rc;
 }
 
-int reserve_workspace(boa_model* m, uint64_t B, size_t cap) {
+// ------------------------------------------------------------------------------------- workspace
+size_t bytes_per_row(const boa_model* m) {   // activations of one stream-step
+  const size_t E = m->E, D = m->D;
+  return 4 * (D + 2 * E + (size_t)m->ks_x * m->ldj + 256 + D / 64) + 6 * (D + 2 * E);
+}
+size_t bytes_per_stream(const boa_model* m, size_t cap, size_t rows_per_stream = 1) {
+  const size_t E = m->E;
+  return rows_per_stream * bytes_per_row(m) + (size_t)m->L * 4 * (E * kNState + 3 * E) + 64 + cap;
+}
+
+// B streams; `rows` stream-steps of activations (= B on the step path, B * kSlabT for encode-side time slabs)
+int reserve_workspace(boa_model* m, uint64_t B, size_t cap, uint64_t rows = 0) {
   const size_t E = m->E, D = m->D, L = m->L;
+  rows = std::max(rows, B);
+  if (rows > m->rows_cap) {
+    BOA_TRY(m->u.reserve(rows * D * 4));
+    BOA_TRY(m->xz.reserve(rows * 2 * E * 4));
+    BOA_TRY(m->dbc.reserve((size_t)m->ks_x * rows * m->ldj * 4));
+    BOA_TRY(m->ssq.reserve(rows * (D / 64) * 4));
+    BOA_TRY(m->u_img.reserve(tc::img_bytes(rows, D)));
+    BOA_TRY(m->xs_img.reserve(tc::img_bytes(rows, E)));
+    BOA_TRY(m->y_img.reserve(tc::img_bytes(rows, E)));
+    BOA_TRY(m->logits.reserve(rows * 256 * 4));
+    m->rows_cap = rows;
+  }
   if (B > m->Bcap) {
     // state arrays are indexed [l][Bcap][...]: growing B invalidates nothing (state is reset per wave)
-    BOA_TRY(m->u.reserve(B * D * 4));
-    BOA_TRY(m->xz.reserve(B * 2 * E * 4));
-    BOA_TRY(m->dbc.reserve((size_t)m->ks_x * B * m->ldj * 4));
-    BOA_TRY(m->ssq.reserve(B * (D / 64) * 4));
-    BOA_TRY(m->u_img.reserve(tc::img_bytes(B, D)));
-    BOA_TRY(m->xs_img.reserve(tc::img_bytes(B, E)));
-    BOA_TRY(m->y_img.reserve(tc::img_bytes(B, E)));
-    BOA_TRY(m->logits.reserve(B * 256 * 4));
     BOA_TRY(m->h.reserve(L * B * E * kNState * 4));
     BOA_TRY(m->win.reserve(L * B * 3 * E * 4));
     BOA_TRY(m->pos.reserve(B * 4));
@@ -515,14 +578,15 @@ int reset_state(boa_model* m, cudaStream_t st) {
 
 uint32_t stream_cap(size_t chunk_bytes) { return (uint32_t)round_up(2 * chunk_bytes + 8, 16); }
 
-uint64_t wave_streams(const boa_model* m, uint64_t nc, size_t cap) {
+uint64_t wave_streams(const boa_model* m, uint64_t nc, size_t cap, size_t rows_per_stream = 1) {
   size_t free_b = 0, total_b = 0;
   uint64_t w = std::min<uint64_t>(nc, kMaxWaveStreams);
   if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
     // what the handle already holds can be reused
-    const size_t held = m->Bcap * bytes_per_stream(m, m->scratch.cap / std::max<uint64_t>(m->Bcap, 1));
+    const size_t held = m->Bcap * bytes_per_stream(m, m->scratch.cap / std::max<uint64_t>(m->Bcap, 1), 0) +
+                        m->rows_cap * bytes_per_row(m);
     const size_t budget = (size_t)((free_b + held) * 0.85);
-    const uint64_t fit = std::max<uint64_t>(1, budget / bytes_per_stream(m, cap));
+    const uint64_t fit = std::max<uint64_t>(1, budget / bytes_per_stream(m, cap, rows_per_stream));
     w = std::min(w, fit);
   } else {
     (void)cudaGetLastError();
@@ -760,12 +824,13 @@ int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, 
   const uint32_t cap = stream_cap(chunk_bytes);
   uint64_t launches = 0;
 
-  const uint64_t W = nc ? wave_streams(m, nc, cap) : 0;
+  const bool slab = getenv("BOA_NO_SLAB") == nullptr && chunk_bytes > (size_t)kSlabT;   // BOA_NO_SLAB=1: step path only (same bytes)
+  const uint64_t W = nc ? wave_streams(m, nc, cap, slab ? kSlabT : 1) : 0;
   for (uint64_t c0 = 0; c0 < nc; c0 += W) {
     const uint64_t B = std::min(W, nc - c0);
     const uint64_t wave_base = c0 * chunk_bytes;
     const uint64_t n_wave = std::min<uint64_t>(n - wave_base, B * chunk_bytes);
-    BOA_TRY(reserve_workspace(m, B, cap));
+    BOA_TRY(reserve_workspace(m, B, cap, slab ? B * kSlabT : B));
     BOA_TRY(reset_state(m, st));
     StepCtx c{};
     c.m = m; c.st = st; c.B = (int)B; c.mode = 0;
@@ -778,8 +843,17 @@ int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, 
     k_first_bytes<<<g, 256, 0, st>>>(c.data, chunk_bytes, m->first.as<uint8_t>(), (int)B);
     BOA_TRY(mark(c, BOA_K_FINISH));
     const uint64_t max_len = std::min<uint64_t>(chunk_bytes, n_wave);
-    if (max_len > 1) BOA_TRY(launch_embed(c));
-    BOA_TRY(run_steps(c, max_len - 1));
+    {
+      // the bytes are all known: advance kSlabT steps per pass over the state (time slabs), the rest step by step
+      const uint64_t steps = max_len - 1;
+      const uint64_t n_slabs = slab ? steps / kSlabT : 0;
+      BOA_TRY(run_slabs(c, n_slabs));
+      const uint64_t rest = steps - n_slabs * kSlabT;
+      if (rest) {
+        BOA_TRY(launch_embed(c));
+        BOA_TRY(run_steps(c, rest));
+      }
+    }
     m->prof.steps += max_len - 1;
     k_coder_finish<0><<<g, 256, 0, st>>>(c.ca, (int)B);
     BOA_TRY(mark(c, BOA_K_FINISH));

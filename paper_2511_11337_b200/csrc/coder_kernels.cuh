@@ -312,6 +312,45 @@ k_coder_step(const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes
   }
 }
 
+// Encode-side time slab: the T tables of a stream (logits rows t*B + i) are coded one after the
+// other by the stream's warp, the coder state staying in registers.  Per symbol this is the arithmetic of the step
+// kernel, so the bytes are the ones the step path writes.
+__global__ void __launch_bounds__(256)
+k_coder_slab(const float* __restrict__ logits, const uint8_t* __restrict__ data, size_t chunk_bytes, CoderArrays ca,
+             int B, int T) {
+  const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  pdl_launch();
+  pdl_wait();
+  if (i >= B) return;
+  const uint32_t pos = ca.pos[i], len = ca.len[i];
+  if (pos + 1u >= len) return;                    // finished stream: masked
+  EncState st;
+  st.low = ca.low[i]; st.range = ca.range[i]; st.pending = ca.pending[i]; st.wpos = ca.wpos[i];
+  st.cache = ca.cache[i]; st.started = ca.started[i];
+  const uint8_t* sdata = data + (size_t)i * chunk_bytes;
+  uint8_t* out = ca.scratch + (size_t)i * ca.cap;
+  uint32_t done = 0;
+  for (int t = 0; t < T && pos + 1u + (uint32_t)t < len; ++t) {
+    float l[8];
+    const float4* lp = reinterpret_cast<const float4*>(logits + ((size_t)t * B + i) * 256 + lane * 8);
+    const float4 a = lp[0], b = lp[1];
+    l[0] = a.x; l[1] = a.y; l[2] = a.z; l[3] = a.w; l[4] = b.x; l[5] = b.y; l[6] = b.z; l[7] = b.w;
+    WarpTable tb;
+    build_table(l, tb);
+    const uint32_t s = sdata[pos + 1u + (uint32_t)t];
+    uint32_t c_lo, c_hi;
+    table_interval(tb, s, c_lo, c_hi);
+    if (lane == 0) enc_symbol(st, c_lo, c_hi, out);
+    ++done;
+  }
+  if (lane == 0) {
+    ca.low[i] = st.low; ca.range[i] = st.range; ca.pending[i] = st.pending; ca.wpos[i] = st.wpos;
+    ca.cache[i] = st.cache; ca.started[i] = st.started;
+    ca.pos[i] = pos + done;
+  }
+}
+
 // S0 / S16: per-stream initialisation.  Encode: coder state reset.  Decode: first byte -> output,
 // V = first four payload bytes (big-endian).
 template <int MODE>

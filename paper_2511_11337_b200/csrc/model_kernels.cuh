@@ -37,11 +37,13 @@ __device__ __forceinline__ float softplusf_(float v) { return fmaxf(v, 0.0f) + l
 __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, const uint32_t* __restrict__ pos,
                         const uint32_t* __restrict__ len, const float4* __restrict__ emb, float4* __restrict__ u,
                         const float4* __restrict__ norm_w, uint8_t* __restrict__ u_img, float* __restrict__ ssq,
-                        int B, int D4) {
+                        int B, int D4, int T) {
+  // T > 1 (encode-side time slab): rows are time-major, row t*B + i is byte pos_i + t of stream i
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  const bool live = idx < B * D4;                 // B*D4 is a multiple of 16: a 16-thread block is live as a whole
-  const int i = live ? idx / D4 : 0, q = live ? idx - i * D4 : 0;
-  const uint32_t p = min(pos[i], len[i] - 1u);
+  const bool live = idx < B * T * D4;             // a multiple of 16: a 16-thread block is live as a whole
+  const int row = live ? idx / D4 : 0, q = live ? idx - row * D4 : 0;
+  const int t = row / B, i = row - t * B;
+  const uint32_t p = min(pos[i] + (uint32_t)t, len[i] - 1u);
   const uint32_t s = src[(size_t)i * chunk_bytes + p];
   const float4 v = emb[s * D4 + q];
   float ss = v.x * v.x;
@@ -50,9 +52,9 @@ __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, con
   for (int d = 8; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
   if (!live) return;
   u[idx] = v;
-  if ((q & 15) == 0) ssq[(size_t)i * (D4 >> 4) + (q >> 4)] = ss;
+  if ((q & 15) == 0) ssq[(size_t)row * (D4 >> 4) + (q >> 4)] = ss;
   const float4 w = norm_w[q];
-  tc::cut4_store(u_img, D4 >> 4, i, q * 4, make_float4(v.x * w.x, v.y * w.y, v.z * w.z, v.w * w.w));
+  tc::cut4_store(u_img, D4 >> 4, row, q * 4, make_float4(v.x * w.x, v.y * w.y, v.z * w.z, v.w * w.w));
 }
 
 // ---------------------------------------------------------------------------------------------------
@@ -83,6 +85,8 @@ struct ScanArgs {
   const float* Dskip;       // [E]
   uint8_t* y_img;           // image of y[B][E] for out_proj (tc_gemm.cuh)
   int ldj, B, E, R;
+  int T;                    // steps per launch (1 = the step path; > 1 = encode-side time slab, rows t*B + i): the state
+                            // of a stream is loaded before its first and stored after its last step of the slab
 };
 
 namespace scan {
@@ -178,22 +182,23 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     const int lane = tid - EC;
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    const uint32_t tx = (uint32_t)(EC * 64 + 2 * EC * 4 + a.KS * a.ldj * 4);
-    auto issue_load = [&](int k) {   // lane 0
-      const int s = k % NSTG;
+    const int T = a.T, niter = nk * T;             // iteration kk = (stream k of this CTA, step t of the slab)
+    auto issue_load = [&](int kk) {   // lane 0
+      const int s = kk % NSTG, k = kk / T, t = kk - k * T;
       const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+      const size_t row = (size_t)t * a.B + i;
       const uint32_t st = s_u32(stages + s * SB), bar = s_u32(&bars[s]);
-      bar_expect(bar, tx);
-      g2s_hint(st, a.h + ((i * slices + sl) * 4) * (size_t)EC * 4, (uint32_t)(EC * 64), bar, pol);
-      g2s(st + EC * 64, a.xz + i * 2 * a.E + e0, (uint32_t)(EC * 4), bar);
-      g2s(st + EC * 64 + EC * 4, a.xz + i * 2 * a.E + a.E + e0, (uint32_t)(EC * 4), bar);
+      bar_expect(bar, (uint32_t)((t == 0 ? EC * 64 : 0) + 2 * EC * 4 + a.KS * a.ldj * 4));
+      if (t == 0) g2s_hint(st, a.h + ((i * slices + sl) * 4) * (size_t)EC * 4, (uint32_t)(EC * 64), bar, pol);
+      g2s(st + EC * 64, a.xz + row * 2 * a.E + e0, (uint32_t)(EC * 4), bar);
+      g2s(st + EC * 64 + EC * 4, a.xz + row * 2 * a.E + a.E + e0, (uint32_t)(EC * 4), bar);
       for (int p = 0; p < a.KS; ++p)
-        g2s(st + EC * 64 + 2 * EC * 4 + EC * 6 + p * a.ldj * 4, a.dbc + p * a.dbc_split + i * a.ldj, (uint32_t)(a.ldj * 4), bar);
+        g2s(st + EC * 64 + 2 * EC * 4 + EC * 6 + p * a.ldj * 4, a.dbc + p * a.dbc_split + row * a.ldj, (uint32_t)(a.ldj * 4), bar);
     };
     // S5, last step: the k-split partials of the x_proj row are added in ascending order, in place, once per stream
-    auto reduce_row = [&](int k) {   // whole warp
-      const int s = k % NSTG;
-      bar_wait(s_u32(&bars[s]), (uint32_t)((k / NSTG) & 1));
+    auto reduce_row = [&](int kk) {   // whole warp
+      const int s = kk % NSTG;
+      bar_wait(s_u32(&bars[s]), (uint32_t)((kk / NSTG) & 1));
       float* row = reinterpret_cast<float*>(stages + s * SB + EC * 64 + 2 * EC * 4 + EC * 6);
       for (int c = lane; c < a.ldj; c += 32) {
         float v = row[c];
@@ -205,32 +210,33 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     };
     pdl_wait();                                    // the state, xz and the x_proj rows come from earlier kernels
     if (lane == 0)
-      for (int k = 0; k < NSTG && k < nk; ++k) issue_load(k);
+      for (int kk = 0; kk < NSTG && kk < niter; ++kk) issue_load(kk);
     const int nchunks = (EC >> 6) * 24;          // 16-byte chunks of the y pieces of one stream-slice
     const uint64_t keep = tc::policy_evict_last();
     reduce_row(0);
-    for (int k = 0; k < nk; ++k) {
-      const int s = k % NSTG;
+    for (int kk = 0; kk < niter; ++kk) {
+      const int s = kk % NSTG, k = kk / T, t = kk - k * T;
       uint8_t* st = stages + s * SB;
-      if (k + 1 < nk) reduce_row(k + 1);           // its copies were issued at least one iteration ago
-      bar_wait(s_u32(&bars[NSTG + s]), (uint32_t)((k / NSTG) & 1));      // every channel of stream k is done
+      if (kk + 1 < niter) reduce_row(kk + 1);      // its copies were issued at least one iteration ago
+      bar_wait(s_u32(&bars[NSTG + s]), (uint32_t)((kk / NSTG) & 1));     // every channel of this stream-step is done
       const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
+      const size_t row = (size_t)t * a.B + i;
       if (lane == 0) {
-        s2g_hint(a.h + ((i * slices + sl) * 4) * (size_t)EC * 4, s_u32(st), (uint32_t)(EC * 64), pol);
+        if (t == T - 1) s2g_hint(a.h + ((i * slices + sl) * 4) * (size_t)EC * 4, s_u32(st), (uint32_t)(EC * 64), pol);
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
       }
       // y pieces: row (c/8) = (64-channel block, piece), chunk c%8 of its 128-byte row in out_proj's operand image
-      const int r = (int)(i & 127);
+      const int r = (int)(row & 127);
       for (int c = lane; c < nchunks; c += 32) {
         const int rowid = c >> 3, kt = rowid / 3, q = rowid - kt * 3;
-        uint8_t* dst = a.y_img + tc::img_block(i >> 7, (size_t)(e0 >> 6) + kt, (size_t)(a.E >> 6)) + (size_t)q * tc::A_PLANE +
+        uint8_t* dst = a.y_img + tc::img_block(row >> 7, (size_t)(e0 >> 6) + kt, (size_t)(a.E >> 6)) + (size_t)q * tc::A_PLANE +
                        (r >> 3) * 1024 + (r & 7) * 128 + (c & 7) * 16;
         tc::st_keep_v4(dst, *reinterpret_cast<const uint4*>(st + EC * 64 + 2 * EC * 4 + rowid * 128 + (c & 7) * 16), keep);
       }
       __syncwarp();
-      if (lane == 0 && k >= 1 && k - 1 + NSTG < nk) {
-        asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the store of stream k-1 has left its stage
-        issue_load(k - 1 + NSTG);
+      if (lane == 0 && kk >= 1 && kk - 1 + NSTG < niter) {
+        asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the store of iteration kk-1 has left its stage
+        issue_load(kk - 1 + NSTG);
       }
     }
     if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
@@ -250,16 +256,18 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   const float dsk = a.Dskip[e];
   const float bdt = a.b_dt[e];
 
-  for (int k = 0; k < nk; ++k) {
-    const int s = k % NSTG;
+  const int T = a.T, niter = nk * T;
+  float4 h0, h1, h2, h3;                           // the channel's 16 state values: in registers across a slab
+  for (int kk = 0; kk < niter; ++kk) {
+    const int s = kk % NSTG, k = kk / T, t = kk - k * T;
     uint8_t* st = stages + s * SB;
-    bar_wait(s_u32(&bars[2 * NSTG + s]), (uint32_t)((k / NSTG) & 1));   // copies landed and the x_proj row added up
+    bar_wait(s_u32(&bars[2 * NSTG + s]), (uint32_t)((kk / NSTG) & 1));  // copies landed and the x_proj row added up
     float4* hs = reinterpret_cast<float4*>(st);
     const float* xs_s = reinterpret_cast<const float*>(st + EC * 64);
     const float* row = reinterpret_cast<const float*>(st + EC * 64 + 2 * EC * 4 + EC * 6);
     const float x = xs_s[tid];
     const float z = xs_s[EC + tid];
-    float4 h0 = hs[tid], h1 = hs[EC + tid], h2 = hs[2 * EC + tid], h3 = hs[3 * EC + tid];
+    if (t == 0) { h0 = hs[tid]; h1 = hs[EC + tid]; h2 = hs[2 * EC + tid]; h3 = hs[3 * EC + tid]; }
     float acc = bdt;
     if constexpr (RR > 0) {
 #pragma unroll
@@ -288,10 +296,10 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     scan_update4(h3, a3, bcp[3], bcp[7], dl, x, yv);
     yv = fmaf(dsk, x, yv);
     yv *= silu_fast(z);
-    hs[tid] = h0; hs[EC + tid] = h1; hs[2 * EC + tid] = h2; hs[3 * EC + tid] = h3;
+    if (t == T - 1) { hs[tid] = h0; hs[EC + tid] = h1; hs[2 * EC + tid] = h2; hs[3 * EC + tid] = h3; }
     {
       // y -> three bf16 pieces (truncation split, exact), staged as [64-channel block][piece][128-byte swizzled row]
-      const int i7 = (int)((blockIdx.x + (size_t)k * gridDim.x) & 7);
+      const int i7 = (int)(((size_t)t * a.B + blockIdx.x + (size_t)k * gridDim.x) & 7);
       uint8_t* yp = st + EC * 64 + 2 * EC * 4 + ((tid >> 6) * 3) * 128 + (((((tid & 63) >> 3) ^ i7) & 7) << 4) + (tid & 7) * 2;
 #pragma unroll
       for (int q = 0; q < 3; ++q) {

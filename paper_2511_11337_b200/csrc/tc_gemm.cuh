@@ -58,7 +58,8 @@ struct GemmArgs {
   // EPI_INPROJ only
   const float* ssq_in;     // [M][KB]: sum of u^2 over each 64-column block of the residual stream (written by the
                            // producer of u in a fixed order); rstd = 1/sqrt(sum/K + eps) (R#10)
-  float* win;              // [M][3][E] conv window of this layer, a ring: at step t slot t%3 holds x_{t-3} and receives x_t
+  float* win;              // [M][3][E] conv window of this layer, a ring: at step t slot t%3 holds x_{t-3} and receives x_t;
+                           // nullptr: no conv here, the x half is stored as it is (encode-side time slab, k_conv_slab)
   const uint32_t* pos;     // [M] steps taken so far by each stream (the coder's position) = t
   const float4* conv_w;    // [E] taps (x = t-3 ... w = t)
   const float* conv_b;     // [E]
@@ -256,6 +257,17 @@ struct Cfg {
 // sigmoid for the SiLU of the conv epilogue: fast forms (relative error ~1e-6; same code on encode and decode)
 __device__ __forceinline__ float sigmoid_tc(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
 
+// S4 for one channel: xc = b + w.x x_{t-3} + w.y x_{t-2} + w.z x_{t-1} + w.w x_t in this fixed FMA order (R#11), then SiLU.
+// The one definition shared by the step kernel (in_proj epilogue) and the encode-side time-slab kernel, so that both
+// produce the same bits.
+__device__ __forceinline__ float conv_silu1(float4 w, float b, float xm3, float xm2, float xm1, float x) {
+  float xc = fmaf(w.w, x, b);
+  xc = fmaf(w.x, xm3, xc);
+  xc = fmaf(w.y, xm2, xc);
+  xc = fmaf(w.z, xm1, xc);
+  return xc * sigmoid_tc(xc);
+}
+
 constexpr int NEPI = 256;        // epilogue threads (warps 0-7); warp 8 owns TMEM and issues the MMAs; warp 9 drives the copies
 constexpr int NTHREADS = NEPI + 64;
 
@@ -401,7 +413,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       // The conv window of the first row batch does not depend on the accumulators: its loads (from HBM at large B)
       // are issued now and fly while the main loop of this tile finishes.
       const int nb = n0 + col;
-      const bool conv_tile = EPI == EPI_INPROJ && n0 < g.E;
+      const bool conv_tile = EPI == EPI_INPROJ && n0 < g.E && g.win != nullptr;   // win == nullptr: x is stored raw (time slab)
       float4 w0[4], w1[4], w2[4];
       int slot[4];                                 // ring slot of x_{t-3} (and of x_t after this step)
       if (conv_tile) {
@@ -472,10 +484,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
           for (int u = 0; u < 4; ++u) {
             if (rows[u] < g.M) {
               float4 o;
-              { float xc = fmaf(cw0.w, x[u].x, cb.x); xc = fmaf(cw0.x, w0[u].x, xc); xc = fmaf(cw0.y, w1[u].x, xc); xc = fmaf(cw0.z, w2[u].x, xc); o.x = xc * sigmoid_tc(xc); }
-              { float xc = fmaf(cw1.w, x[u].y, cb.y); xc = fmaf(cw1.x, w0[u].y, xc); xc = fmaf(cw1.y, w1[u].y, xc); xc = fmaf(cw1.z, w2[u].y, xc); o.y = xc * sigmoid_tc(xc); }
-              { float xc = fmaf(cw2.w, x[u].z, cb.z); xc = fmaf(cw2.x, w0[u].z, xc); xc = fmaf(cw2.y, w1[u].z, xc); xc = fmaf(cw2.z, w2[u].z, xc); o.z = xc * sigmoid_tc(xc); }
-              { float xc = fmaf(cw3.w, x[u].w, cb.w); xc = fmaf(cw3.x, w0[u].w, xc); xc = fmaf(cw3.y, w1[u].w, xc); xc = fmaf(cw3.z, w2[u].w, xc); o.w = xc * sigmoid_tc(xc); }
+              o.x = conv_silu1(cw0, cb.x, w0[u].x, w1[u].x, w2[u].x, x[u].x);
+              o.y = conv_silu1(cw1, cb.y, w0[u].y, w1[u].y, w2[u].y, x[u].y);
+              o.z = conv_silu1(cw2, cb.z, w0[u].z, w1[u].z, w2[u].z, x[u].z);
+              o.w = conv_silu1(cw3, cb.w, w0[u].w, w1[u].w, w2[u].w, x[u].w);
               *reinterpret_cast<float4*>(g.win + ((size_t)rows[u] * 3 + slot[u]) * g.E + nb) = x[u];
               *reinterpret_cast<float4*>(Cout + (size_t)rows[u] * g.ldc + nb) = o;
               cut4_store(g.out_img, g.out_KB, rows[u], nb, o);
@@ -534,6 +546,44 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     __syncwarp();
     tmem_dealloc(tmem, C::TMEM_COLS);
   }
+}
+
+// ------------------------------------------------------------------------------------------ encode-side time slab
+// S4 over a slab of T consecutive steps of every stream (compression knows all bytes in advance).
+// Rows are time-major: row(t, i) = t*B + i.  One thread owns 4 channels of a stream, keeps the window in registers and
+// walks over the T steps: x (raw in_proj output, in xz) -> xs (in place, fp32) and its image for x_proj; the ring
+// window is read once before and written once after the slab.  Per step this is the arithmetic of the in_proj epilogue.
+__global__ void k_conv_slab(float* __restrict__ xz, float* __restrict__ win, const uint32_t* __restrict__ pos,
+                            const float4* __restrict__ conv_w, const float* __restrict__ conv_b,
+                            uint8_t* __restrict__ xs_img, int B, int E, int T) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  const int E4 = E >> 2;
+  if (idx >= B * E4) return;
+  const int i = idx / E4, e = (idx - i * E4) * 4;
+  const float4 cw0 = conv_w[e], cw1 = conv_w[e + 1], cw2 = conv_w[e + 2], cw3 = conv_w[e + 3];
+  const float4 cb = *reinterpret_cast<const float4*>(conv_b + e);
+  const uint32_t p0 = pos[i];
+  float* wp = win + (size_t)i * 3 * E + e;
+  float4 w0 = *reinterpret_cast<const float4*>(wp + (p0 % 3u) * E);            // x_{t-3}
+  float4 w1 = *reinterpret_cast<const float4*>(wp + ((p0 + 1u) % 3u) * E);     // x_{t-2}
+  float4 w2 = *reinterpret_cast<const float4*>(wp + ((p0 + 2u) % 3u) * E);     // x_{t-1}
+  for (int t = 0; t < T; ++t) {
+    const size_t row = (size_t)t * B + i;
+    float4* xp = reinterpret_cast<float4*>(xz + row * 2 * E + e);
+    const float4 x = *xp;
+    float4 o;
+    o.x = conv_silu1(cw0, cb.x, w0.x, w1.x, w2.x, x.x);
+    o.y = conv_silu1(cw1, cb.y, w0.y, w1.y, w2.y, x.y);
+    o.z = conv_silu1(cw2, cb.z, w0.z, w1.z, w2.z, x.z);
+    o.w = conv_silu1(cw3, cb.w, w0.w, w1.w, w2.w, x.w);
+    *xp = o;
+    cut4_store(xs_img, E / BK, (int)row, e, o);
+    w0 = w1; w1 = w2; w2 = x;
+  }
+  const uint32_t p1 = p0 + (uint32_t)T;          // after the slab slot (p1+j)%3 holds x_{p1-3+j}
+  *reinterpret_cast<float4*>(wp + (p1 % 3u) * E) = w0;
+  *reinterpret_cast<float4*>(wp + ((p1 + 1u) % 3u) * E) = w1;
+  *reinterpret_cast<float4*>(wp + ((p1 + 2u) % 3u) * E) = w2;
 }
 
 }  // namespace tc

@@ -321,3 +321,22 @@ def test_maximum_wave_65536_streams_cfg4_model(boa):
     assert err <= PROB_TOL
     lg = _np(d["logits"][ids])
     assert np.array_equal(_np(d["cdf"][ids]).astype(np.int64).reshape(-1, 257), quantise.quantise(lg.reshape(-1, 256)))
+
+
+def test_time_slab_encoder_writes_the_bytes_of_the_step_path(boa):
+    """Encode-side time slabs (compression advances 8 steps per pass over the stream state) must be
+    bit-identical to stepping one byte at a time - the decoder always steps - for ragged lengths around the slab size."""
+    import os
+    cfg = synth.CONFIGS[1]
+    for blob in (cfg.weights(emb_std=0.25), synth.make_weights(synth.CONFIGS[2].shape, 1, emb_std=0.25)):
+        gm = boa.Model(blob)
+        for n, chunk in [(150 * 41 + 13, 41), (300 * 9, 9), (5 * 200 + 10, 200), (130 * 17, 17)]:
+            data = cfg.data(n)
+            a = _np(gm.compress(data, chunk)).tobytes()
+            os.environ["BOA_NO_SLAB"] = "1"
+            try:
+                b = _np(gm.compress(data, chunk)).tobytes()
+            finally:
+                del os.environ["BOA_NO_SLAB"]
+            assert a == b, (n, chunk)
+            assert _np(gm.decompress(torch.frombuffer(bytearray(a), dtype=torch.uint8).cuda())).tobytes() == data
