@@ -314,6 +314,7 @@ int launch_step(StepCtx& c) {
   uint8_t* xs_img = m->xs_img.as<uint8_t>();
   uint8_t* y_img = m->y_img.as<uint8_t>();
 
+  const int ec = (E % 256 == 0) ? 256 : 128;     // channels per scan slice
   for (int l = 0; l < m->L; ++l) {
     const LayerW& w = m->layers[l];
     float* hl = m->h.as<float>() + (size_t)l * m->Bcap * E * kNState;
@@ -321,22 +322,22 @@ int launch_step(StepCtx& c) {
     {  // S2-S4: xz = [SiLU(conv(W_in_x r)) ; W_in_z r],  r = RMSNorm(u);  xs also as the image for x_proj
       tc::GemmArgs g{};
       g.A = u_img; g.M = rows; g.KB = D / 64; g.W = w.img_in; g.NT = 2 * E / 64; g.KS = 1;
-      g.C = xz; g.ldc = 2 * E; g.n_valid = 2 * E;
+      g.C = xz; g.ldc = 2 * E; g.n_valid = 2 * E; g.xz_ec = ec;
       g.ssq_in = m->ssq.as<float>(); g.win = T == 1 ? winl : nullptr; g.pos = c.ca.pos; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
       if (!BOA_DEV_SKIPPED(BOA_K_INPROJ)) BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_INPROJ));
       if (T > 1) {   // S4 over the slab
         const long long total = (long long)B * (E / 4);
-        tc::k_conv_slab<<<(unsigned)((total + 255) / 256), 256, 0, c.st>>>(xz, winl, c.ca.pos, w.conv_w, w.conv_b, xs_img, B, E, T);
+        tc::k_conv_slab<<<(unsigned)((total + 255) / 256), 256, 0, c.st>>>(xz, winl, c.ca.pos, w.conv_w, w.conv_b, xs_img, B, E, T, ec);
         BOA_TRY(mark(c, BOA_K_INPROJ));
       }
     }
     {  // S5: [dlt;Bv;Cv] = W_x xs
       tc::GemmArgs g{};
       g.A = xs_img; g.M = rows; g.KB = E / 64; g.W = w.img_x; g.NT = m->ldj / 64;
-      g.C = dbc; g.ldc = m->ldj; g.n_valid = m->J;
-      g.KS = m->ks_x; g.split_stride = (size_t)m->rows_cap * m->ldj;   // split over k: enough tiles to fill the SMs
+      g.C = dbc; g.ldc = m->ks_x * m->ldj; g.n_valid = m->J;           // row = [k-split][ldj]
+      g.KS = m->ks_x; g.split_stride = (size_t)m->ldj;                  // split over k: enough tiles to fill the SMs
       if (!BOA_DEV_SKIPPED(BOA_K_CONVX)) BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_CONVX));
     }
@@ -344,8 +345,8 @@ int launch_step(StepCtx& c) {
       ScanArgs sa{};
       sa.h = hl; sa.xz = xz; sa.dbc = dbc; sa.W_dtT = w.w_dtT; sa.b_dt = w.b_dt; sa.A4 = w.A4; sa.Dskip = w.d_skip;
       sa.y_img = y_img; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
-      sa.KS = m->ks_x; sa.dbc_split = (size_t)m->rows_cap * m->ldj; sa.T = T;
-      const int ec = (E % 256 == 0) ? 256 : 128, slices = E / ec;
+      sa.KS = m->ks_x; sa.T = T;
+      const int slices = E / ec;
       const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
       const dim3 grid(per_slice, slices);
       if (!BOA_DEV_SKIPPED(BOA_K_SCAN))

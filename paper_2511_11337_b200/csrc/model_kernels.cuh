@@ -75,10 +75,9 @@ __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, con
 // One thread per channel of the slice holds A[e][0..15] in registers; W_dt^T of the slice lives in shared memory.
 struct ScanArgs {
   float* h;                 // [B][E/EC][4][EC] float4 (this layer): the state of a stream and channel slice is one contiguous run
-  const float* xz;          // [B][2E]: xs | z
-  const float* dbc;         // [KS][B][ldj] k-split partials of x_proj; their ascending sum is dlt[R] | Bv[16] | Cv[16]
-  int KS;                   // the copy warp adds the partials once per stream, ((p0+p1)+p2)+...
-  size_t dbc_split;         // elements between partials
+  const float* xz;          // [rows][E/EC][xs of the slice | z of the slice] (tc::xz_col): one copy per stream-step and slice
+  const float* dbc;         // [rows][KS][ldj] k-split partials of x_proj; their ascending sum is dlt[R] | Bv[16] | Cv[16]
+  int KS;                   // the copy warp adds the partials once per stream-step, ((p0+p1)+p2)+...
   const float* W_dtT;       // [R][E]
   const float* b_dt;        // [E]
   const float4* A4;         // [4][E] float4: A * log2(e), A = -exp(A_log)
@@ -190,10 +189,8 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
       const uint32_t st = s_u32(stages + s * SB), bar = s_u32(&bars[s]);
       bar_expect(bar, (uint32_t)((t == 0 ? EC * 64 : 0) + 2 * EC * 4 + a.KS * a.ldj * 4));
       if (t == 0) g2s_hint(st, a.h + ((i * slices + sl) * 4) * (size_t)EC * 4, (uint32_t)(EC * 64), bar, pol);
-      g2s(st + EC * 64, a.xz + row * 2 * a.E + e0, (uint32_t)(EC * 4), bar);
-      g2s(st + EC * 64 + EC * 4, a.xz + row * 2 * a.E + a.E + e0, (uint32_t)(EC * 4), bar);
-      for (int p = 0; p < a.KS; ++p)
-        g2s(st + EC * 64 + 2 * EC * 4 + EC * 6 + p * a.ldj * 4, a.dbc + p * a.dbc_split + row * a.ldj, (uint32_t)(a.ldj * 4), bar);
+      g2s(st + EC * 64, a.xz + row * 2 * a.E + (size_t)sl * 2 * EC, (uint32_t)(2 * EC * 4), bar);          // xs | z
+      g2s(st + EC * 64 + 2 * EC * 4 + EC * 6, a.dbc + row * a.KS * a.ldj, (uint32_t)(a.KS * a.ldj * 4), bar);   // all partials
     };
     // S5, last step: the k-split partials of the x_proj row are added in ascending order, in place, once per stream
     auto reduce_row = [&](int kk) {   // whole warp

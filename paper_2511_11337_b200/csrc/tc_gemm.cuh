@@ -55,6 +55,8 @@ struct GemmArgs {
   size_t split_stride;     //   partial result to C + s*split_stride; the consumer adds the partials in ascending order
   float* C;                // [M][ldc] fp32 result (in_proj: xz = xs | z; out_proj: the residual stream u, updated)
   int ldc, n_valid;        // columns >= n_valid are not stored (zero-padded weight rows)
+  int xz_ec;               // EPI_INPROJ: > 0 = the result row is stored slice-interleaved for the scan: with E = N/2 and
+                           // slices of xz_ec channels, [slice][xs of the slice | z of the slice] (xz_col below); 0 = as is
   // EPI_INPROJ only
   const float* ssq_in;     // [M][KB]: sum of u^2 over each 64-column block of the residual stream (written by the
                            // producer of u in a fixed order); rstd = 1/sqrt(sum/K + eps) (R#10)
@@ -257,6 +259,12 @@ struct Cfg {
 // sigmoid for the SiLU of the conv epilogue: fast forms (relative error ~1e-6; same code on encode and decode)
 __device__ __forceinline__ float sigmoid_tc(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
 
+// Column of in_proj output n (x half: n < E, z half: n >= E) in the slice-interleaved xz row the scan copies in one go.
+__host__ __device__ inline int xz_col(int n, int E, int EC) {
+  const int half = n >= E, c = n - half * E;
+  return (c / EC) * 2 * EC + half * EC + c % EC;
+}
+
 // S4 for one channel: xc = b + w.x x_{t-3} + w.y x_{t-2} + w.z x_{t-1} + w.w x_t in this fixed FMA order (R#11), then SiLU.
 // The one definition shared by the step kernel (in_proj epilogue) and the encode-side time-slab kernel, so that both
 // produce the same bits.
@@ -413,6 +421,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       // The conv window of the first row batch does not depend on the accumulators: its loads (from HBM at large B)
       // are issued now and fly while the main loop of this tile finishes.
       const int nb = n0 + col;
+      const int ncol = (EPI == EPI_INPROJ && g.xz_ec > 0) ? xz_col(nb, g.E, g.xz_ec) : nb;   // column of the stored result
       const bool conv_tile = EPI == EPI_INPROJ && n0 < g.E && g.win != nullptr;   // win == nullptr: x is stored raw (time slab)
       float4 w0[4], w1[4], w2[4];
       int slot[4];                                 // ring slot of x_{t-3} (and of x_t after this step)
@@ -489,7 +498,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
               o.z = conv_silu1(cw2, cb.z, w0[u].z, w1[u].z, w2[u].z, x[u].z);
               o.w = conv_silu1(cw3, cb.w, w0[u].w, w1[u].w, w2[u].w, x[u].w);
               *reinterpret_cast<float4*>(g.win + ((size_t)rows[u] * 3 + slot[u]) * g.E + nb) = x[u];
-              *reinterpret_cast<float4*>(Cout + (size_t)rows[u] * g.ldc + nb) = o;
+              *reinterpret_cast<float4*>(Cout + (size_t)rows[u] * g.ldc + ncol) = o;
               cut4_store(g.out_img, g.out_KB, rows[u], nb, o);
             }
           }
@@ -511,7 +520,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
             const int r = (warp + 8 * (i0 + u)) * RPI + lane / LPR;
             rows[u] = m0 + r;
             o[u] = *reinterpret_cast<const float4*>(stile + r * LDS + col);
-            if (EPI == EPI_RESID) q[u] = *reinterpret_cast<const float4*>(Cout + (size_t)min(rows[u], g.M - 1) * g.ldc + nb);
+            if (EPI == EPI_RESID) q[u] = *reinterpret_cast<const float4*>(Cout + (size_t)min(rows[u], g.M - 1) * g.ldc + ncol);
           }
 #pragma unroll
           for (int u = 0; u < 4; ++u) {
@@ -530,7 +539,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
                 if ((lane % LPR) == 0) g.ssq_out[(size_t)rows[u] * g.out_KB + nt] = ss;
               }
             }
-            if (live) *reinterpret_cast<float4*>(Cout + (size_t)rows[u] * g.ldc + nb) = o[u];
+            if (live) *reinterpret_cast<float4*>(Cout + (size_t)rows[u] * g.ldc + ncol) = o[u];
           }
         }
       }
@@ -555,7 +564,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
 // window is read once before and written once after the slab.  Per step this is the arithmetic of the in_proj epilogue.
 __global__ void k_conv_slab(float* __restrict__ xz, float* __restrict__ win, const uint32_t* __restrict__ pos,
                             const float4* __restrict__ conv_w, const float* __restrict__ conv_b,
-                            uint8_t* __restrict__ xs_img, int B, int E, int T) {
+                            uint8_t* __restrict__ xs_img, int B, int E, int T, int xz_ec) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const int E4 = E >> 2;
   if (idx >= B * E4) return;
@@ -569,7 +578,7 @@ __global__ void k_conv_slab(float* __restrict__ xz, float* __restrict__ win, con
   float4 w2 = *reinterpret_cast<const float4*>(wp + ((p0 + 2u) % 3u) * E);     // x_{t-1}
   for (int t = 0; t < T; ++t) {
     const size_t row = (size_t)t * B + i;
-    float4* xp = reinterpret_cast<float4*>(xz + row * 2 * E + e);
+    float4* xp = reinterpret_cast<float4*>(xz + row * 2 * E + xz_col(e, E, xz_ec));
     const float4 x = *xp;
     float4 o;
     o.x = conv_silu1(cw0, cb.x, w0.x, w1.x, w2.x, x.x);
