@@ -89,10 +89,13 @@ struct ScanArgs {
 };
 
 namespace scan {
-constexpr int NSTG = 4;
+constexpr int NSB = 4;           // state buffers (one stream-slice state each): the ring the HBM traffic flows through
+constexpr int NSTG = 8;          // step stages (the small per-step inputs and outputs): deeper, a slab step is short
 constexpr int KSMAX = 4;         // x_proj k-split partial rows per stage
-__host__ __device__ inline int stage_bytes(int EC, int ldj) { return EC * 64 + 2 * EC * 4 + EC * 6 + KSMAX * ldj * 4; }   // h | xs | z | y pieces | dbc partials
-__host__ __device__ inline int smem_bytes(int EC, int ldj, int R) { return NSTG * stage_bytes(EC, ldj) + R * EC * 4 + 3 * NSTG * 8 + 128; }   // R = 0 when W_dt sits in registers
+__host__ __device__ inline int stage_bytes(int EC, int ldj) { return 2 * EC * 4 + EC * 6 + KSMAX * ldj * 4; }   // xs | z | y pieces | dbc partials
+__host__ __device__ inline int smem_bytes(int EC, int ldj, int R) {   // R = 0 when W_dt sits in registers
+  return NSB * EC * 64 + NSTG * stage_bytes(EC, ldj) + R * EC * 4 + 3 * NSTG * 8 + 128;
+}
 
 __device__ __forceinline__ uint32_t s_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void bar_init(uint32_t bar, uint32_t count) {
@@ -159,9 +162,12 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   const int slices = gridDim.y, sl = blockIdx.y;
   const int e0 = sl * EC;
   const int SB = stage_bytes(EC, a.ldj);
-  uint8_t* stages = scan_smem;
-  float* wdt = reinterpret_cast<float*>(scan_smem + NSTG * SB);
-  uint64_t* bars = reinterpret_cast<uint64_t*>(scan_smem + NSTG * SB + (RR ? 0 : a.R * EC * 4));   // full, done, ready [NSTG] each
+  uint8_t* sbufs = scan_smem;                      // [NSB][EC*64] state buffers
+  uint8_t* stages = scan_smem + NSB * EC * 64;     // [NSTG][SB] step stages
+  float* wdt = reinterpret_cast<float*>(stages + NSTG * SB);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(stages + NSTG * SB + (RR ? 0 : a.R * EC * 4));   // full, done, ready [NSTG] each
+  // copies run LA iterations ahead: all step stages when a slab gives the state buffers time to drain (LA <= 3T+1)
+  const int LA = a.T >= 3 ? NSTG : (a.T == 2 ? 7 : NSB);
   const int nk = (a.B - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // streams of this CTA
   if (nk <= 0) return;
 
@@ -182,21 +188,31 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
     const int T = a.T, niter = nk * T;             // iteration kk = (stream k of this CTA, step t of the slab)
-    auto issue_load = [&](int kk) {   // lane 0
-      const int s = kk % NSTG, k = kk / T, t = kk - k * T;
-      const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
-      const size_t row = (size_t)t * a.B + i;
+    // This warp is one serial instruction stream beside eight channel warps: indices advance incrementally (no
+    // divisions), per-lane offsets are computed once.
+    static_assert((NSTG & (NSTG - 1)) == 0 && (NSB & (NSB - 1)) == 0, "ring sizes are powers of two");
+    const size_t state_stride = (size_t)slices * 4 * EC * 4;        // floats between the states of consecutive streams
+    const float* h0p = a.h + (size_t)sl * 4 * EC * 4;
+    const float* xz0 = a.xz + (size_t)sl * 2 * EC;
+    const uint32_t xz_bytes = (uint32_t)(2 * EC * 4), dbc_bytes = (uint32_t)(a.KS * a.ldj * 4);
+    int ik = 0, it_ = 0, ikk = 0;                  // next copy to issue: stream, step, iteration
+    size_t ii = blockIdx.x;                        // its stream index in the wave
+    auto issue_next = [&]() {   // lane 0
+      const int s = ikk & (NSTG - 1);
+      const size_t row = (size_t)it_ * a.B + ii;
       const uint32_t st = s_u32(stages + s * SB), bar = s_u32(&bars[s]);
-      bar_expect(bar, (uint32_t)((t == 0 ? EC * 64 : 0) + 2 * EC * 4 + a.KS * a.ldj * 4));
-      if (t == 0) g2s_hint(st, a.h + ((i * slices + sl) * 4) * (size_t)EC * 4, (uint32_t)(EC * 64), bar, pol);
-      g2s(st + EC * 64, a.xz + row * 2 * a.E + (size_t)sl * 2 * EC, (uint32_t)(2 * EC * 4), bar);          // xs | z
-      g2s(st + EC * 64 + 2 * EC * 4 + EC * 6, a.dbc + row * a.KS * a.ldj, (uint32_t)(a.KS * a.ldj * 4), bar);   // all partials
+      bar_expect(bar, (it_ == 0 ? (uint32_t)(EC * 64) : 0u) + xz_bytes + dbc_bytes);
+      if (it_ == 0) g2s_hint(s_u32(sbufs + (ik & (NSB - 1)) * EC * 64), h0p + ii * state_stride, (uint32_t)(EC * 64), bar, pol);
+      g2s(st, xz0 + row * 2 * a.E, xz_bytes, bar);                                                  // xs | z
+      g2s(st + 2 * EC * 4 + EC * 6, a.dbc + row * a.KS * a.ldj, dbc_bytes, bar);                     // all partials
+      ++ikk;
+      if (++it_ == T) { it_ = 0; ++ik; ii += gridDim.x; }
     };
-    // S5, last step: the k-split partials of the x_proj row are added in ascending order, in place, once per stream
+    // S5, last step: the k-split partials of the x_proj row are added in ascending order, in place, once per stream-step
     auto reduce_row = [&](int kk) {   // whole warp
-      const int s = kk % NSTG;
+      const int s = kk & (NSTG - 1);
       bar_wait(s_u32(&bars[s]), (uint32_t)((kk / NSTG) & 1));
-      float* row = reinterpret_cast<float*>(stages + s * SB + EC * 64 + 2 * EC * 4 + EC * 6);
+      float* row = reinterpret_cast<float*>(stages + s * SB + 2 * EC * 4 + EC * 6);
       for (int c = lane; c < a.ldj; c += 32) {
         float v = row[c];
         for (int p = 1; p < a.KS; ++p) v += row[p * a.ldj + c];
@@ -207,34 +223,45 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     };
     pdl_wait();                                    // the state, xz and the x_proj rows come from earlier kernels
     if (lane == 0)
-      for (int kk = 0; kk < NSTG && kk < niter; ++kk) issue_load(kk);
-    const int nchunks = (EC >> 6) * 24;          // 16-byte chunks of the y pieces of one stream-slice
+      for (int kk = 0; kk < LA && kk < niter; ++kk) issue_next();
+    // y pieces: 16-byte chunk c of a stream-step = row (c/8) = (64-channel block, piece) of the staged pieces, chunk c%8
+    // of its 128-byte row in out_proj's operand image; this lane's (at most 3) chunks:
+    const int nchunks = (EC >> 6) * 24;
+    uint32_t ysrc[3], ydst[3];
+#pragma unroll
+    for (int j = 0; j < 3; ++j) {
+      const int c = lane + 32 * j, rowid = c >> 3, kt = rowid / 3, q = rowid - kt * 3;
+      ysrc[j] = (uint32_t)(2 * EC * 4 + rowid * 128 + (c & 7) * 16);
+      ydst[j] = (uint32_t)(kt * (tc::NPA * tc::A_PLANE) + q * tc::A_PLANE + (c & 7) * 16);
+    }
+    const size_t img_row_tile = (size_t)(a.E >> 6) * (tc::NPA * tc::A_PLANE);   // bytes of one 128-row tile of the image
+    uint8_t* yimg0 = a.y_img + (size_t)(e0 >> 6) * (tc::NPA * tc::A_PLANE);
     const uint64_t keep = tc::policy_evict_last();
     reduce_row(0);
+    int k = 0, t = 0;                              // this iteration's stream and step
+    size_t i = blockIdx.x;
     for (int kk = 0; kk < niter; ++kk) {
-      const int s = kk % NSTG, k = kk / T, t = kk - k * T;
+      const int s = kk & (NSTG - 1);
       uint8_t* st = stages + s * SB;
       if (kk + 1 < niter) reduce_row(kk + 1);      // its copies were issued at least one iteration ago
       bar_wait(s_u32(&bars[NSTG + s]), (uint32_t)((kk / NSTG) & 1));     // every channel of this stream-step is done
-      const size_t i = (size_t)blockIdx.x + (size_t)k * gridDim.x;
-      const size_t row = (size_t)t * a.B + i;
       if (lane == 0) {
-        if (t == T - 1) s2g_hint(a.h + ((i * slices + sl) * 4) * (size_t)EC * 4, s_u32(st), (uint32_t)(EC * 64), pol);
+        if (t == T - 1)
+          s2g_hint(const_cast<float*>(h0p) + i * state_stride, s_u32(sbufs + (k & (NSB - 1)) * EC * 64), (uint32_t)(EC * 64), pol);
         asm volatile("cp.async.bulk.commit_group;" ::: "memory");
       }
-      // y pieces: row (c/8) = (64-channel block, piece), chunk c%8 of its 128-byte row in out_proj's operand image
+      const size_t row = (size_t)t * a.B + i;
       const int r = (int)(row & 127);
-      for (int c = lane; c < nchunks; c += 32) {
-        const int rowid = c >> 3, kt = rowid / 3, q = rowid - kt * 3;
-        uint8_t* dst = a.y_img + tc::img_block(row >> 7, (size_t)(e0 >> 6) + kt, (size_t)(a.E >> 6)) + (size_t)q * tc::A_PLANE +
-                       (r >> 3) * 1024 + (r & 7) * 128 + (c & 7) * 16;
-        tc::st_keep_v4(dst, *reinterpret_cast<const uint4*>(st + EC * 64 + 2 * EC * 4 + rowid * 128 + (c & 7) * 16), keep);
-      }
+      uint8_t* ybase = yimg0 + (row >> 7) * img_row_tile + (r >> 3) * 1024 + (r & 7) * 128;
+#pragma unroll
+      for (int j = 0; j < 3; ++j)
+        if (lane + 32 * j < nchunks) tc::st_keep_v4(ybase + ydst[j], *reinterpret_cast<const uint4*>(st + ysrc[j]), keep);
       __syncwarp();
-      if (lane == 0 && kk >= 1 && kk - 1 + NSTG < niter) {
-        asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the store of iteration kk-1 has left its stage
-        issue_load(kk - 1 + NSTG);
+      if (lane == 0 && kk >= 1 && ikk < niter) {
+        asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // every state store but this iteration's has left its buffer
+        issue_next();                              // iteration kk - 1 + LA
       }
+      if (++t == T) { t = 0; ++k; i += gridDim.x; }
     }
     if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
     return;
@@ -255,13 +282,15 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
 
   const int T = a.T, niter = nk * T;
   float4 h0, h1, h2, h3;                           // the channel's 16 state values: in registers across a slab
+  int k = 0, t = 0;
+  size_t row_i = blockIdx.x;                       // this iteration's stream index in the wave
   for (int kk = 0; kk < niter; ++kk) {
-    const int s = kk % NSTG, k = kk / T, t = kk - k * T;
+    const int s = kk & (NSTG - 1);
     uint8_t* st = stages + s * SB;
     bar_wait(s_u32(&bars[2 * NSTG + s]), (uint32_t)((kk / NSTG) & 1));  // copies landed and the x_proj row added up
-    float4* hs = reinterpret_cast<float4*>(st);
-    const float* xs_s = reinterpret_cast<const float*>(st + EC * 64);
-    const float* row = reinterpret_cast<const float*>(st + EC * 64 + 2 * EC * 4 + EC * 6);
+    float4* hs = reinterpret_cast<float4*>(sbufs + (k % NSB) * EC * 64);
+    const float* xs_s = reinterpret_cast<const float*>(st);
+    const float* row = reinterpret_cast<const float*>(st + 2 * EC * 4 + EC * 6);
     const float x = xs_s[tid];
     const float z = xs_s[EC + tid];
     if (t == 0) { h0 = hs[tid]; h1 = hs[EC + tid]; h2 = hs[2 * EC + tid]; h3 = hs[3 * EC + tid]; }
@@ -296,16 +325,17 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     if (t == T - 1) { hs[tid] = h0; hs[EC + tid] = h1; hs[2 * EC + tid] = h2; hs[3 * EC + tid] = h3; }
     {
       // y -> three bf16 pieces (truncation split, exact), staged as [64-channel block][piece][128-byte swizzled row]
-      const int i7 = (int)(((size_t)t * a.B + blockIdx.x + (size_t)k * gridDim.x) & 7);
-      uint8_t* yp = st + EC * 64 + 2 * EC * 4 + ((tid >> 6) * 3) * 128 + (((((tid & 63) >> 3) ^ i7) & 7) << 4) + (tid & 7) * 2;
+      const int i7 = (int)(((size_t)t * a.B + row_i) & 7);
+      uint8_t* yp = st + 2 * EC * 4 + ((tid >> 6) * 3) * 128 + (((((tid & 63) >> 3) ^ i7) & 7) << 4) + (tid & 7) * 2;
 #pragma unroll
       for (int q = 0; q < 3; ++q) {
         *reinterpret_cast<uint16_t*>(yp + q * 128) = (uint16_t)(__float_as_uint(yv) >> 16);
         yv = __fsub_rn(yv, tc::trunc_bf16(yv));
       }
     }
-    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    if (t == T - 1) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the state leaves by a bulk store
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(&bars[NSTG + s])) : "memory");
+    if (++t == T) { t = 0; ++k; row_i += gridDim.x; }
   }
 }
 
