@@ -278,6 +278,11 @@ int init_kernels() {
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan_slab<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::slab_smem_bytes(256, 128, 64)));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan_slab<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::slab_smem_bytes(256, 128, 0)));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan_slab<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::slab_smem_bytes(256, 128, 0)));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan_slab<16>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::slab_smem_bytes(256, 128, 0)));
+  BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan_slab<32>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::slab_smem_bytes(256, 128, 0)));
   return BOA_OK;
 }
 
@@ -322,14 +327,17 @@ int launch_step(StepCtx& c) {
     {  // S2-S4: xz = [SiLU(conv(W_in_x r)) ; W_in_z r],  r = RMSNorm(u);  xs also as the image for x_proj
       tc::GemmArgs g{};
       g.A = u_img; g.M = rows; g.KB = D / 64; g.W = w.img_in; g.NT = 2 * E / 64; g.KS = 1;
-      g.C = xz; g.ldc = 2 * E; g.n_valid = 2 * E; g.xz_ec = ec;
+      g.n_valid = 2 * E; g.xz_ec = ec;
+      g.C = xz;           // step path: a row = [slice][xs | z]; time slab: [slice][row][xs | z] (one copy per stream-group)
+      g.ldc = T == 1 ? 2 * E : 2 * ec;
+      g.xz_slice = T == 1 ? (size_t)2 * ec : (size_t)rows * 2 * ec;
       g.ssq_in = m->ssq.as<float>(); g.win = T == 1 ? winl : nullptr; g.pos = c.ca.pos; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
       if (!BOA_DEV_SKIPPED(BOA_K_INPROJ)) BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_INPROJ));
       if (T > 1) {   // S4 over the slab
         const long long total = (long long)B * (E / 4);
-        tc::k_conv_slab<<<(unsigned)((total + 255) / 256), 256, 0, c.st>>>(xz, winl, c.ca.pos, w.conv_w, w.conv_b, xs_img, B, E, T, ec);
+        tc::k_conv_slab<<<(unsigned)((total + 255) / 256), 256, 0, c.st>>>(xz, 2 * ec, (size_t)rows * 2 * ec, winl, c.ca.pos, w.conv_w, w.conv_b, xs_img, B, E, T, ec);
         BOA_TRY(mark(c, BOA_K_INPROJ));
       }
     }
@@ -345,11 +353,24 @@ int launch_step(StepCtx& c) {
       ScanArgs sa{};
       sa.h = hl; sa.xz = xz; sa.dbc = dbc; sa.W_dtT = w.w_dtT; sa.b_dt = w.b_dt; sa.A4 = w.A4; sa.Dskip = w.d_skip;
       sa.y_img = y_img; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
-      sa.KS = m->ks_x; sa.T = T;
+      sa.KS = m->ks_x; sa.T = 1;
       const int slices = E / ec;
       const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
       const dim3 grid(per_slice, slices);
-      if (!BOA_DEV_SKIPPED(BOA_K_SCAN))
+      if (T > 1) {      // time slab: groups of 8 steps per iteration, state in registers across a stream's groups
+        ScanSlabArgs ss{};
+        ss.h = hl; ss.xz = xz; ss.dbc = dbc; ss.W_dtT = w.w_dtT; ss.b_dt = w.b_dt; ss.A4 = w.A4; ss.Dskip = w.d_skip;
+        ss.y_img = y_img; ss.KS = m->ks_x; ss.ldj = m->ldj; ss.B = B; ss.E = E; ss.R = m->R; ss.T = T;
+        const int regs = (m->R == 4 || m->R == 8 || m->R == 16 || m->R == 32) ? 0 : m->R;
+        const size_t smem = scan::slab_smem_bytes(ec, m->ldj, regs);
+        switch (m->R) {
+          case 4: BOA_CUDA_TRY(launch_pdl(k_scan_slab<4>, grid, dim3(ec + 32), smem, c.st, ss)); break;
+          case 8: BOA_CUDA_TRY(launch_pdl(k_scan_slab<8>, grid, dim3(ec + 32), smem, c.st, ss)); break;
+          case 16: BOA_CUDA_TRY(launch_pdl(k_scan_slab<16>, grid, dim3(ec + 32), smem, c.st, ss)); break;
+          case 32: BOA_CUDA_TRY(launch_pdl(k_scan_slab<32>, grid, dim3(ec + 32), smem, c.st, ss)); break;
+          default: BOA_CUDA_TRY(launch_pdl(k_scan_slab<0>, grid, dim3(ec + 32), smem, c.st, ss)); break;
+        }
+      } else if (!BOA_DEV_SKIPPED(BOA_K_SCAN))
       switch (m->R) {   // W_dt's row in registers when it is short enough
         case 4: BOA_CUDA_TRY(launch_pdl(k_scan<4>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
         case 8: BOA_CUDA_TRY(launch_pdl(k_scan<8>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;

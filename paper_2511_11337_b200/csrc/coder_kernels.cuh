@@ -312,7 +312,7 @@ k_coder_step(const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes
   }
 }
 
-// Encode-side time slab: the T tables of a stream (logits rows t*B + i) are coded one after the
+// Encode-side time slab: the T tables of a stream (logits rows i*T + t) are coded one after the
 // other by the stream's warp, the coder state staying in registers.  Per symbol this is the arithmetic of the step
 // kernel, so the bytes are the ones the step path writes.
 __global__ void __launch_bounds__(256)
@@ -333,7 +333,7 @@ k_coder_slab(const float* __restrict__ logits, const uint8_t* __restrict__ data,
   uint32_t done = 0;
   for (int t = 0; t < T && pos + 1u + (uint32_t)t < len; ++t) {
     float l[8];
-    const float4* lp = reinterpret_cast<const float4*>(logits + ((size_t)t * B + i) * 256 + lane * 8);
+    const float4* lp = reinterpret_cast<const float4*>(logits + ((size_t)i * T + t) * 256 + lane * 8);
     const float4 a = lp[0], b = lp[1];
     l[0] = a.x; l[1] = a.y; l[2] = a.z; l[3] = a.w; l[4] = b.x; l[5] = b.y; l[6] = b.z; l[7] = b.w;
     WarpTable tb;

@@ -38,11 +38,11 @@ __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, con
                         const uint32_t* __restrict__ len, const float4* __restrict__ emb, float4* __restrict__ u,
                         const float4* __restrict__ norm_w, uint8_t* __restrict__ u_img, float* __restrict__ ssq,
                         int B, int D4, int T) {
-  // T > 1 (encode-side time slab): rows are time-major, row t*B + i is byte pos_i + t of stream i
+  // T > 1 (encode-side time slab): rows are stream-major, row i*T + t is byte pos_i + t of stream i
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const bool live = idx < B * T * D4;             // a multiple of 16: a 16-thread block is live as a whole
   const int row = live ? idx / D4 : 0, q = live ? idx - row * D4 : 0;
-  const int t = row / B, i = row - t * B;
+  const int i = row / T, t = row - i * T;
   const uint32_t p = min(pos[i] + (uint32_t)t, len[i] - 1u);
   const uint32_t s = src[(size_t)i * chunk_bytes + p];
   const float4 v = emb[s * D4 + q];
@@ -149,6 +149,44 @@ __device__ __forceinline__ void scan_update4(float4& h, const float4 a2, const f
   h.y = fmaf(ex2_approx(dl * a2.y), h.y, dx * bv.y); y = fmaf(cv.y, h.y, y);
   h.z = fmaf(ex2_approx(dl * a2.z), h.z, dx * bv.z); y = fmaf(cv.z, h.z, y);
   h.w = fmaf(ex2_approx(dl * a2.w), h.w, dx * bv.w); y = fmaf(cv.w, h.w, y);
+}
+
+// S6-S8 of one channel for one step: dt_proj + softplus, the recurrence on the 16 state values, D skip and gate.
+// `row` = dlt[R] | Bv[16] | Cv[16] (shared memory, broadcast reads).  The one definition used by the step kernel and
+// by the encode-side slab kernel, so both produce the same bits.
+template <int RR>
+__device__ __forceinline__ float scan_channel_step(const float* row, int R, const float (&wr)[RR ? RR : 1], const float* wdt_col,
+                                                   int EC, float bdt, const float4 a0, const float4 a1, const float4 a2,
+                                                   const float4 a3, float dsk, float x, float z, float4& h0, float4& h1,
+                                                   float4& h2, float4& h3) {
+  float acc = bdt;
+  if constexpr (RR > 0) {
+#pragma unroll
+    for (int r = 0; r < RR; r += 4) {
+      const float4 d = *reinterpret_cast<const float4*>(row + r);
+      acc = fmaf(wr[r], d.x, acc);
+      acc = fmaf(wr[r + 1], d.y, acc);
+      acc = fmaf(wr[r + 2], d.z, acc);
+      acc = fmaf(wr[r + 3], d.w, acc);
+    }
+  } else {
+    for (int r = 0; r < R; r += 4) {
+      const float4 d = *reinterpret_cast<const float4*>(row + r);
+      acc = fmaf(wdt_col[(r + 0) * EC], d.x, acc);
+      acc = fmaf(wdt_col[(r + 1) * EC], d.y, acc);
+      acc = fmaf(wdt_col[(r + 2) * EC], d.z, acc);
+      acc = fmaf(wdt_col[(r + 3) * EC], d.w, acc);
+    }
+  }
+  const float dl = softplus_fast(acc);
+  const float4* bcp = reinterpret_cast<const float4*>(row + R);
+  float yv = 0.0f;
+  scan_update4(h0, a0, bcp[0], bcp[4], dl, x, yv);
+  scan_update4(h1, a1, bcp[1], bcp[5], dl, x, yv);
+  scan_update4(h2, a2, bcp[2], bcp[6], dl, x, yv);
+  scan_update4(h3, a3, bcp[3], bcp[7], dl, x, yv);
+  yv = fmaf(dsk, x, yv);
+  return yv * silu_fast(z);
 }
 
 // grid = (CTAs per slice, E / EC), block = EC + 32 threads (EC = 256 or 128), two CTAs per SM.
@@ -294,34 +332,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     const float x = xs_s[tid];
     const float z = xs_s[EC + tid];
     if (t == 0) { h0 = hs[tid]; h1 = hs[EC + tid]; h2 = hs[2 * EC + tid]; h3 = hs[3 * EC + tid]; }
-    float acc = bdt;
-    if constexpr (RR > 0) {
-#pragma unroll
-      for (int r = 0; r < RR; r += 4) {
-        const float4 d = *reinterpret_cast<const float4*>(row + r);
-        acc = fmaf(wr[r], d.x, acc);
-        acc = fmaf(wr[r + 1], d.y, acc);
-        acc = fmaf(wr[r + 2], d.z, acc);
-        acc = fmaf(wr[r + 3], d.w, acc);
-      }
-    } else {
-      for (int r = 0; r < a.R; r += 4) {
-        const float4 d = *reinterpret_cast<const float4*>(row + r);
-        acc = fmaf(wdt[(r + 0) * EC + tid], d.x, acc);
-        acc = fmaf(wdt[(r + 1) * EC + tid], d.y, acc);
-        acc = fmaf(wdt[(r + 2) * EC + tid], d.z, acc);
-        acc = fmaf(wdt[(r + 3) * EC + tid], d.w, acc);
-      }
-    }
-    const float dl = softplus_fast(acc);
-    const float4* bcp = reinterpret_cast<const float4*>(row + a.R);
-    float yv = 0.0f;
-    scan_update4(h0, a0, bcp[0], bcp[4], dl, x, yv);
-    scan_update4(h1, a1, bcp[1], bcp[5], dl, x, yv);
-    scan_update4(h2, a2, bcp[2], bcp[6], dl, x, yv);
-    scan_update4(h3, a3, bcp[3], bcp[7], dl, x, yv);
-    yv = fmaf(dsk, x, yv);
-    yv *= silu_fast(z);
+    float yv = scan_channel_step<RR>(row, a.R, wr, wdt + tid, EC, bdt, a0, a1, a2, a3, dsk, x, z, h0, h1, h2, h3);
     if (t == T - 1) { hs[tid] = h0; hs[EC + tid] = h1; hs[2 * EC + tid] = h2; hs[3 * EC + tid] = h3; }
     {
       // y -> three bf16 pieces (truncation split, exact), staged as [64-channel block][piece][128-byte swizzled row]
@@ -336,6 +347,175 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     if (t == T - 1) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the state leaves by a bulk store
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(&bars[NSTG + s])) : "memory");
     if (++t == T) { t = 0; ++k; row_i += gridDim.x; }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
+// S6-S8 over an encode-side time slab: rows are stream-major, row(i, t) = i*T + t, T a multiple
+// of G = 8.  One iteration of a CTA = one stream and one group of 8 consecutive steps: the copy warp brings in the 8
+// rows of xs | z (one copy: the slab's xz is laid out [slice][row][xs | z]) and of x_proj partials (one copy), plus the
+// state with the first group of a stream; the channel threads then run the 8 steps back to back with no
+// synchronisation in between, the state in registers across the groups of a stream; the 8 rows of y pieces of a
+// (64-channel block, piece) form one contiguous 1 KB block of out_proj's operand image and leave by bulk stores,
+// with the state after the last group.  Per step the arithmetic is scan_channel_step, as in k_scan.
+namespace scan {
+constexpr int G = 8;             // steps per iteration
+constexpr int NSL = 2;           // stages
+__host__ __device__ inline int slab_stage_bytes(int EC, int ldj) { return EC * 64 + G * 2 * EC * 4 + G * EC * 6 + G * KSMAX * ldj * 4; }
+__host__ __device__ inline int slab_smem_bytes(int EC, int ldj, int R) { return NSL * slab_stage_bytes(EC, ldj) + R * EC * 4 + 3 * NSL * 8 + 128; }
+}  // namespace scan
+
+struct ScanSlabArgs {
+  float* h;                 // [B][E/EC][4][EC] float4 (this layer)
+  const float* xz;          // [E/EC][rows][xs of the slice | z of the slice], rows = B*T
+  const float* dbc;         // [rows][KS][ldj]
+  const float* W_dtT; const float* b_dt; const float4* A4; const float* Dskip;
+  uint8_t* y_img;           // image of y[rows][E]
+  int KS, ldj, B, E, R, T;
+};
+
+template <int RR>
+__global__ void __launch_bounds__(288, 2) k_scan_slab(const ScanSlabArgs a) {
+  using namespace scan;
+  extern __shared__ __align__(128) uint8_t scan_smem[];
+  const int EC = blockDim.x - 32, tid = threadIdx.x;
+  const int slices = gridDim.y, sl = blockIdx.y;
+  const int e0 = sl * EC;
+  const int SB = slab_stage_bytes(EC, a.ldj);
+  const int XZ_OFF = EC * 64, Y_OFF = XZ_OFF + G * 2 * EC * 4, D_OFF = Y_OFF + G * EC * 6;
+  uint8_t* stages = scan_smem;
+  float* wdt = reinterpret_cast<float*>(stages + NSL * SB);
+  uint64_t* bars = reinterpret_cast<uint64_t*>(stages + NSL * SB + (RR ? 0 : a.R * EC * 4));   // full, done, ready [NSL] each
+  const int nk = (a.B - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // streams of this CTA
+  if (nk <= 0) return;
+  const int NG = a.T / G, niter = nk * NG;         // iteration kk = (stream k of this CTA, group g of 8 steps)
+  const size_t rows = (size_t)a.B * a.T;
+
+  if (tid == 0) {
+    for (int s = 0; s < NSL; ++s) {
+      bar_init(s_u32(&bars[s]), 1);
+      bar_init(s_u32(&bars[NSL + s]), (uint32_t)EC);
+      bar_init(s_u32(&bars[2 * NSL + s]), 1);
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  pdl_launch();
+  const size_t state_stride = (size_t)slices * 4 * EC * 4;
+  float* h0p = a.h + (size_t)sl * 4 * EC * 4;
+
+  if (tid >= EC) {
+    // ===================================================================== copy warp
+    const int lane = tid - EC;
+    uint64_t pol;
+    asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
+    const float* xz0 = a.xz + (size_t)sl * rows * 2 * EC;
+    const uint32_t xz_bytes = (uint32_t)(G * 2 * EC * 4), dbc_bytes = (uint32_t)(G * a.KS * a.ldj * 4);
+    int ig = 0, ikk = 0;                           // next copy to issue: group within the stream, iteration
+    size_t ii = blockIdx.x;
+    auto issue_next = [&]() {   // lane 0
+      const int s = ikk & (NSL - 1);
+      const size_t row = ii * a.T + (size_t)ig * G;
+      const uint32_t st = s_u32(stages + s * SB), bar = s_u32(&bars[s]);
+      bar_expect(bar, (ig == 0 ? (uint32_t)(EC * 64) : 0u) + xz_bytes + dbc_bytes);
+      if (ig == 0) g2s_hint(st, h0p + ii * state_stride, (uint32_t)(EC * 64), bar, pol);
+      g2s(st + XZ_OFF, xz0 + row * 2 * EC, xz_bytes, bar);
+      g2s(st + D_OFF, a.dbc + row * a.KS * a.ldj, dbc_bytes, bar);
+      ++ikk;
+      if (++ig == NG) { ig = 0; ii += gridDim.x; }
+    };
+    // S5, last step, for the 8 rows of an iteration: partials added in ascending order, in place
+    auto reduce_rows = [&](int kk) {   // whole warp
+      const int s = kk & (NSL - 1);
+      bar_wait(s_u32(&bars[s]), (uint32_t)((kk / NSL) & 1));
+      float* d = reinterpret_cast<float*>(stages + s * SB + D_OFF);
+      const int rl = a.KS * a.ldj;
+      for (int c = lane; c < G * a.ldj; c += 32) {
+        const int t = c / a.ldj, col = c - t * a.ldj;
+        float v = d[t * rl + col];
+        for (int p = 1; p < a.KS; ++p) v += d[t * rl + p * a.ldj + col];
+        d[t * rl + col] = v;
+      }
+      __syncwarp();
+      if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(&bars[2 * NSL + s])) : "memory");
+    };
+    pdl_wait();
+    if (lane == 0)
+      for (int kk = 0; kk < NSL && kk < niter; ++kk) issue_next();
+    const size_t img_row_tile = (size_t)(a.E >> 6) * (tc::NPA * tc::A_PLANE);
+    uint8_t* yimg0 = a.y_img + (size_t)(e0 >> 6) * (tc::NPA * tc::A_PLANE);
+    const int nblk = (EC >> 6) * 3;                // (64-channel block, piece) blocks of 1 KB per iteration
+    reduce_rows(0);
+    int g = 0;
+    size_t i = blockIdx.x;
+    for (int kk = 0; kk < niter; ++kk) {
+      const int s = kk & (NSL - 1);
+      uint8_t* st = stages + s * SB;
+      if (kk + 1 < niter) reduce_rows(kk + 1);
+      bar_wait(s_u32(&bars[NSL + s]), (uint32_t)((kk / NSL) & 1));       // the 8 steps of this iteration are done
+      if (lane == 0) {
+        const size_t row = i * a.T + (size_t)g * G;                       // a multiple of 8: one 8-row swizzle group
+        uint8_t* ybase = yimg0 + (row >> 7) * img_row_tile + ((row & 127) >> 3) * 1024;
+        for (int b = 0; b < nblk; ++b) {
+          const int kt = b / 3, q = b - kt * 3;
+          s2g(ybase + (size_t)kt * (tc::NPA * tc::A_PLANE) + (size_t)q * tc::A_PLANE, s_u32(st + Y_OFF + b * 1024), 1024u);
+        }
+        if (g == NG - 1) s2g_hint(h0p + i * state_stride, s_u32(st), (uint32_t)(EC * 64), pol);
+        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+        if (ikk < niter) {
+          asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the stage has been read out
+          issue_next();                                                   // iteration kk + NSL
+        }
+      }
+      __syncwarp();
+      if (++g == NG) { g = 0; i += gridDim.x; }
+    }
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+    return;
+  }
+
+  // ======================================================================= channel threads
+  const int e = e0 + tid;
+  float wr[RR ? RR : 1];
+  if constexpr (RR > 0) {
+#pragma unroll
+    for (int r = 0; r < RR; ++r) wr[r] = a.W_dtT[(size_t)r * a.E + e];
+  } else {
+    for (int r = 0; r < a.R; ++r) wdt[r * EC + tid] = a.W_dtT[(size_t)r * a.E + e];
+  }
+  const float4 a0 = a.A4[e], a1 = a.A4[a.E + e], a2 = a.A4[2 * a.E + e], a3 = a.A4[3 * a.E + e];
+  const float dsk = a.Dskip[e];
+  const float bdt = a.b_dt[e];
+  float4 h0, h1, h2, h3;
+  int g = 0;
+  const int rl = a.KS * a.ldj;
+  // y pieces of step t: block (64-channel block, piece) = 8 rows of 128 bytes; row t, chunk (c ^ t), bf16 (tid & 7)
+  const uint32_t yoff = (uint32_t)(((tid >> 6) * 3) * 1024 + (tid & 7) * 2);
+  const int ychunk = (tid & 63) >> 3;
+  for (int kk = 0; kk < niter; ++kk) {
+    const int s = kk & (NSL - 1);
+    uint8_t* st = stages + s * SB;
+    bar_wait(s_u32(&bars[2 * NSL + s]), (uint32_t)((kk / NSL) & 1));
+    float4* hs = reinterpret_cast<float4*>(st);
+    if (g == 0) { h0 = hs[tid]; h1 = hs[EC + tid]; h2 = hs[2 * EC + tid]; h3 = hs[3 * EC + tid]; }
+    const float* xz_s = reinterpret_cast<const float*>(st + XZ_OFF);
+    const float* d = reinterpret_cast<const float*>(st + D_OFF);
+#pragma unroll 1
+    for (int t = 0; t < G; ++t) {
+      const float x = xz_s[t * 2 * EC + tid];
+      const float z = xz_s[t * 2 * EC + EC + tid];
+      float yv = scan_channel_step<RR>(d + t * rl, a.R, wr, wdt + tid, EC, bdt, a0, a1, a2, a3, dsk, x, z, h0, h1, h2, h3);
+      uint8_t* yp = st + Y_OFF + yoff + t * 128 + (((ychunk ^ t) & 7) << 4);
+#pragma unroll
+      for (int q = 0; q < 3; ++q) {
+        *reinterpret_cast<uint16_t*>(yp + q * 1024) = (uint16_t)(__float_as_uint(yv) >> 16);
+        yv = __fsub_rn(yv, tc::trunc_bf16(yv));
+      }
+    }
+    if (g == NG - 1) { hs[tid] = h0; hs[EC + tid] = h1; hs[2 * EC + tid] = h2; hs[3 * EC + tid] = h3; }
+    asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // y pieces (and the state) leave by bulk stores
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(&bars[NSL + s])) : "memory");
+    if (++g == NG) g = 0;
   }
 }
 

@@ -55,8 +55,10 @@ struct GemmArgs {
   size_t split_stride;     //   partial result to C + s*split_stride; the consumer adds the partials in ascending order
   float* C;                // [M][ldc] fp32 result (in_proj: xz = xs | z; out_proj: the residual stream u, updated)
   int ldc, n_valid;        // columns >= n_valid are not stored (zero-padded weight rows)
-  int xz_ec;               // EPI_INPROJ: > 0 = the result row is stored slice-interleaved for the scan: with E = N/2 and
-                           // slices of xz_ec channels, [slice][xs of the slice | z of the slice] (xz_col below); 0 = as is
+  int xz_ec;               // EPI_INPROJ: > 0 = the result is stored for the scan in slices of xz_ec channels (E = N/2):
+  size_t xz_slice;         //   element (row, slice, xs|z half, c) at slice*xz_slice + row*ldc + half*xz_ec + c.  Step path:
+                           //   ldc = 2E, xz_slice = 2*xz_ec (a row = [slice][xs | z]); time slab: ldc = 2*xz_ec,
+                           //   xz_slice = rows*2*xz_ec ([slice][row][xs | z]).  xz_ec = 0: plain row-major
   // EPI_INPROJ only
   const float* ssq_in;     // [M][KB]: sum of u^2 over each 64-column block of the residual stream (written by the
                            // producer of u in a fixed order); rstd = 1/sqrt(sum/K + eps) (R#10)
@@ -259,10 +261,10 @@ struct Cfg {
 // sigmoid for the SiLU of the conv epilogue: fast forms (relative error ~1e-6; same code on encode and decode)
 __device__ __forceinline__ float sigmoid_tc(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
 
-// Column of in_proj output n (x half: n < E, z half: n >= E) in the slice-interleaved xz row the scan copies in one go.
-__host__ __device__ inline int xz_col(int n, int E, int EC) {
+// Offset (without the row term row*ldc) of in_proj output n (x half: n < E, z half: n >= E) in the sliced xz layout.
+__host__ __device__ inline size_t xz_col(int n, int E, int EC, size_t slice_stride) {
   const int half = n >= E, c = n - half * E;
-  return (c / EC) * 2 * EC + half * EC + c % EC;
+  return (size_t)(c / EC) * slice_stride + (size_t)(half * EC + c % EC);
 }
 
 // S4 for one channel: xc = b + w.x x_{t-3} + w.y x_{t-2} + w.z x_{t-1} + w.w x_t in this fixed FMA order (R#11), then SiLU.
@@ -421,7 +423,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       // The conv window of the first row batch does not depend on the accumulators: its loads (from HBM at large B)
       // are issued now and fly while the main loop of this tile finishes.
       const int nb = n0 + col;
-      const int ncol = (EPI == EPI_INPROJ && g.xz_ec > 0) ? xz_col(nb, g.E, g.xz_ec) : nb;   // column of the stored result
+      const size_t ncol = (EPI == EPI_INPROJ && g.xz_ec > 0) ? xz_col(nb, g.E, g.xz_ec, g.xz_slice) : (size_t)nb;   // offset of the stored result in its row
       const bool conv_tile = EPI == EPI_INPROJ && n0 < g.E && g.win != nullptr;   // win == nullptr: x is stored raw (time slab)
       float4 w0[4], w1[4], w2[4];
       int slot[4];                                 // ring slot of x_{t-3} (and of x_t after this step)
@@ -559,12 +561,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
 
 // ------------------------------------------------------------------------------------------ encode-side time slab
 // S4 over a slab of T consecutive steps of every stream (compression knows all bytes in advance).
-// Rows are time-major: row(t, i) = t*B + i.  One thread owns 4 channels of a stream, keeps the window in registers and
+// Rows are stream-major: row(i, t) = i*T + t.  One thread owns 4 channels of a stream, keeps the window in registers and
 // walks over the T steps: x (raw in_proj output, in xz) -> xs (in place, fp32) and its image for x_proj; the ring
 // window is read once before and written once after the slab.  Per step this is the arithmetic of the in_proj epilogue.
-__global__ void k_conv_slab(float* __restrict__ xz, float* __restrict__ win, const uint32_t* __restrict__ pos,
-                            const float4* __restrict__ conv_w, const float* __restrict__ conv_b,
-                            uint8_t* __restrict__ xs_img, int B, int E, int T, int xz_ec) {
+__global__ void k_conv_slab(float* __restrict__ xz, int ldc, size_t xz_slice, float* __restrict__ win,
+                            const uint32_t* __restrict__ pos, const float4* __restrict__ conv_w,
+                            const float* __restrict__ conv_b, uint8_t* __restrict__ xs_img, int B, int E, int T, int xz_ec) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   const int E4 = E >> 2;
   if (idx >= B * E4) return;
@@ -576,9 +578,10 @@ __global__ void k_conv_slab(float* __restrict__ xz, float* __restrict__ win, con
   float4 w0 = *reinterpret_cast<const float4*>(wp + (p0 % 3u) * E);            // x_{t-3}
   float4 w1 = *reinterpret_cast<const float4*>(wp + ((p0 + 1u) % 3u) * E);     // x_{t-2}
   float4 w2 = *reinterpret_cast<const float4*>(wp + ((p0 + 2u) % 3u) * E);     // x_{t-1}
+  float* xcol = xz + xz_col(e, E, xz_ec, xz_slice);
   for (int t = 0; t < T; ++t) {
-    const size_t row = (size_t)t * B + i;
-    float4* xp = reinterpret_cast<float4*>(xz + row * 2 * E + xz_col(e, E, xz_ec));
+    const size_t row = (size_t)i * T + t;          // stream-major rows
+    float4* xp = reinterpret_cast<float4*>(xcol + row * ldc);
     const float4 x = *xp;
     float4 o;
     o.x = conv_silu1(cw0, cb.x, w0.x, w1.x, w2.x, x.x);
