@@ -304,6 +304,9 @@ def run_ours(args, cfg):
             ent["frac"] = ent["achieved"] / ent["peak"]
         kernels[k] = ent
     line["kernels"] = kernels
+    line["kernels_note"] = ("CUDA events around eagerly launched sample batches of the STEP path (decompression, and the tail of "
+                            "compression); compression itself advances 16 steps per pass in time slabs (DESIGN.md 6c) and is "
+                            "not sampled per kernel")
     ranked = [k for k in sorted(kernels, key=lambda k: -kernels[k]["share"]) if "bound" in kernels[k]]
     if ranked:
         k = ranked[0]
