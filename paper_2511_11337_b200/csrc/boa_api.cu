@@ -331,15 +331,10 @@ int launch_step(StepCtx& c) {
       g.C = xz;           // step path: a row = [slice][xs | z]; time slab: [slice][row][xs | z] (one copy per stream-group)
       g.ldc = T == 1 ? 2 * E : 2 * ec;
       g.xz_slice = T == 1 ? (size_t)2 * ec : (size_t)rows * 2 * ec;
-      g.ssq_in = m->ssq.as<float>(); g.win = T == 1 ? winl : nullptr; g.pos = c.ca.pos; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
+      g.ssq_in = m->ssq.as<float>(); g.win = winl; g.pos = c.ca.pos; g.slab_T = T == 1 ? 0 : T; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
       if (!BOA_DEV_SKIPPED(BOA_K_INPROJ)) BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_INPROJ));
-      if (T > 1) {   // S4 over the slab
-        const long long total = (long long)B * (E / 4);
-        tc::k_conv_slab<<<(unsigned)((total + 255) / 256), 256, 0, c.st>>>(xz, 2 * ec, (size_t)rows * 2 * ec, winl, c.ca.pos, w.conv_w, w.conv_b, xs_img, B, E, T, ec);
-        BOA_TRY(mark(c, BOA_K_INPROJ));
-      }
     }
     {  // S5: [dlt;Bv;Cv] = W_x xs
       tc::GemmArgs g{};

@@ -62,9 +62,11 @@ struct GemmArgs {
   // EPI_INPROJ only
   const float* ssq_in;     // [M][KB]: sum of u^2 over each 64-column block of the residual stream (written by the
                            // producer of u in a fixed order); rstd = 1/sqrt(sum/K + eps) (R#10)
-  float* win;              // [M][3][E] conv window of this layer, a ring: at step t slot t%3 holds x_{t-3} and receives x_t;
-                           // nullptr: no conv here, the x half is stored as it is (encode-side time slab, k_conv_slab)
-  const uint32_t* pos;     // [M] steps taken so far by each stream (the coder's position) = t
+  float* win;              // [streams][3][E] conv window of this layer, a ring: at step t slot t%3 holds x_{t-3} and receives x_t
+  const uint32_t* pos;     // [streams] steps taken so far by each stream (the coder's position) = t
+  int slab_T;              // 0: one row per stream.  T > 0 (encode-side time slab, 128 % T == 0): rows are stream-major,
+                           // row i*T + t is step pos_i + t of stream i; the conv of a row reads the rows before it in the
+                           // tile (the window only for t < 3) and the last three rows of a stream go into the window
   const float4* conv_w;    // [E] taps (x = t-3 ... w = t)
   const float* conv_b;     // [E]
   int E;
@@ -424,10 +426,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       // are issued now and fly while the main loop of this tile finishes.
       const int nb = n0 + col;
       const size_t ncol = (EPI == EPI_INPROJ && g.xz_ec > 0) ? xz_col(nb, g.E, g.xz_ec, g.xz_slice) : (size_t)nb;   // offset of the stored result in its row
-      const bool conv_tile = EPI == EPI_INPROJ && n0 < g.E && g.win != nullptr;   // win == nullptr: x is stored raw (time slab)
+      const bool conv_tile = EPI == EPI_INPROJ && n0 < g.E;
+      const bool slab_tile = conv_tile && g.slab_T > 0;
       float4 w0[4], w1[4], w2[4];
       int slot[4];                                 // ring slot of x_{t-3} (and of x_t after this step)
-      if (conv_tile) {
+      if (conv_tile && !slab_tile) {
 #pragma unroll
         for (int u = 0; u < 4; ++u) {
           const int r = (warp + 8 * u) * RPI + lane / LPR;
@@ -464,7 +467,48 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       asm volatile("bar.sync 1, 256;" ::: "memory");
       // Pass 2: 16 lanes own one 64-column row segment (4 consecutive columns per lane), two rows per warp
       // instruction; rows are processed four at a time with all loads issued first.
-      if (conv_tile) {
+      if (slab_tile) {
+        // S4 over a time slab: the rows of a stream are consecutive in the tile, so x_{t-1..t-3} of row t are the rows
+        // before it in the staging tile; only the first three steps of the slab read the window ring (x before the
+        // slab) and the last three go into it - after a barrier, when every row of the tile has read it.
+        const float4 cw0 = g.conv_w[nb], cw1 = g.conv_w[nb + 1], cw2 = g.conv_w[nb + 2], cw3 = g.conv_w[nb + 3];
+        const float4 cb = *reinterpret_cast<const float4*>(g.conv_b + nb);
+        const int T = g.slab_T;
+#pragma unroll
+        for (int i = 0; i < NIT; ++i) {
+          const int r = (warp + 8 * i) * RPI + lane / LPR;
+          const int row = m0 + r;
+          const int rc = min(row, g.M - 1);
+          const int si = rc / T, t = rc - si * T;                 // stream and step of the row
+          const float4 x = *reinterpret_cast<const float4*>(stile + r * LDS + col);
+          float4 xm[3];                                           // x_{t-1}, x_{t-2}, x_{t-3}
+          const uint32_t p0 = g.pos[si];
+          const float* wp = g.win + (size_t)si * 3 * g.E + nb;
+#pragma unroll
+          for (int j = 1; j <= 3; ++j)
+            xm[j - 1] = (t >= j) ? *reinterpret_cast<const float4*>(stile + (r - j) * LDS + col)
+                                 : *reinterpret_cast<const float4*>(wp + ((p0 + 3u + (uint32_t)t - (uint32_t)j) % 3u) * g.E);
+          if (row < g.M) {
+            float4 o;
+            o.x = conv_silu1(cw0, cb.x, xm[2].x, xm[1].x, xm[0].x, x.x);
+            o.y = conv_silu1(cw1, cb.y, xm[2].y, xm[1].y, xm[0].y, x.y);
+            o.z = conv_silu1(cw2, cb.z, xm[2].z, xm[1].z, xm[0].z, x.z);
+            o.w = conv_silu1(cw3, cb.w, xm[2].w, xm[1].w, xm[0].w, x.w);
+            *reinterpret_cast<float4*>(Cout + (size_t)row * g.ldc + ncol) = o;
+            cut4_store(g.out_img, g.out_KB, row, nb, o);
+          }
+        }
+        asm volatile("bar.sync 1, 256;" ::: "memory");     // every row has read the window
+#pragma unroll
+        for (int i = 0; i < NIT; ++i) {                      // x_t of the last three steps -> ring slot (pos + t) % 3
+          const int r = (warp + 8 * i) * RPI + lane / LPR;
+          const int row = m0 + r;
+          const int si = row / T, t = row - si * T;
+          if (row < g.M && t >= T - 3)
+            *reinterpret_cast<float4*>(g.win + ((size_t)si * 3 + (g.pos[si] + (uint32_t)t) % 3u) * g.E + nb) =
+                *reinterpret_cast<const float4*>(stile + r * LDS + col);
+        }
+      } else if (conv_tile) {
         // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU (R#11).  The window is a ring of three
         // slots per stream: all three are read, only the oldest is overwritten with x_t.
         // The lane's four channels are fixed within a tile, so their taps and biases live in registers.  xs goes out
@@ -557,45 +601,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     __syncwarp();
     tmem_dealloc(tmem, C::TMEM_COLS);
   }
-}
-
-// ------------------------------------------------------------------------------------------ encode-side time slab
-// S4 over a slab of T consecutive steps of every stream (compression knows all bytes in advance).
-// Rows are stream-major: row(i, t) = i*T + t.  One thread owns 4 channels of a stream, keeps the window in registers and
-// walks over the T steps: x (raw in_proj output, in xz) -> xs (in place, fp32) and its image for x_proj; the ring
-// window is read once before and written once after the slab.  Per step this is the arithmetic of the in_proj epilogue.
-__global__ void k_conv_slab(float* __restrict__ xz, int ldc, size_t xz_slice, float* __restrict__ win,
-                            const uint32_t* __restrict__ pos, const float4* __restrict__ conv_w,
-                            const float* __restrict__ conv_b, uint8_t* __restrict__ xs_img, int B, int E, int T, int xz_ec) {
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  const int E4 = E >> 2;
-  if (idx >= B * E4) return;
-  const int i = idx / E4, e = (idx - i * E4) * 4;
-  const float4 cw0 = conv_w[e], cw1 = conv_w[e + 1], cw2 = conv_w[e + 2], cw3 = conv_w[e + 3];
-  const float4 cb = *reinterpret_cast<const float4*>(conv_b + e);
-  const uint32_t p0 = pos[i];
-  float* wp = win + (size_t)i * 3 * E + e;
-  float4 w0 = *reinterpret_cast<const float4*>(wp + (p0 % 3u) * E);            // x_{t-3}
-  float4 w1 = *reinterpret_cast<const float4*>(wp + ((p0 + 1u) % 3u) * E);     // x_{t-2}
-  float4 w2 = *reinterpret_cast<const float4*>(wp + ((p0 + 2u) % 3u) * E);     // x_{t-1}
-  float* xcol = xz + xz_col(e, E, xz_ec, xz_slice);
-  for (int t = 0; t < T; ++t) {
-    const size_t row = (size_t)i * T + t;          // stream-major rows
-    float4* xp = reinterpret_cast<float4*>(xcol + row * ldc);
-    const float4 x = *xp;
-    float4 o;
-    o.x = conv_silu1(cw0, cb.x, w0.x, w1.x, w2.x, x.x);
-    o.y = conv_silu1(cw1, cb.y, w0.y, w1.y, w2.y, x.y);
-    o.z = conv_silu1(cw2, cb.z, w0.z, w1.z, w2.z, x.z);
-    o.w = conv_silu1(cw3, cb.w, w0.w, w1.w, w2.w, x.w);
-    *xp = o;
-    cut4_store(xs_img, E / BK, (int)row, e, o);
-    w0 = w1; w1 = w2; w2 = x;
-  }
-  const uint32_t p1 = p0 + (uint32_t)T;          // after the slab slot (p1+j)%3 holds x_{p1-3+j}
-  *reinterpret_cast<float4*>(wp + (p1 % 3u) * E) = w0;
-  *reinterpret_cast<float4*>(wp + ((p1 + 1u) % 3u) * E) = w1;
-  *reinterpret_cast<float4*>(wp + ((p1 + 2u) % 3u) * E) = w2;
 }
 
 }  // namespace tc
