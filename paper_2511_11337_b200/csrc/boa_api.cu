@@ -348,7 +348,7 @@ int launch_step(StepCtx& c) {
       ScanArgs sa{};
       sa.h = hl; sa.xz = xz; sa.dbc = dbc; sa.W_dtT = w.w_dtT; sa.b_dt = w.b_dt; sa.A4 = w.A4; sa.Dskip = w.d_skip;
       sa.y_img = y_img; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
-      sa.KS = m->ks_x; sa.T = 1;
+      sa.KS = m->ks_x;
       const int slices = E / ec;
       const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
       const dim3 grid(per_slice, slices);

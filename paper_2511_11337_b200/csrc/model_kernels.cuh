@@ -84,8 +84,6 @@ struct ScanArgs {
   const float* Dskip;       // [E]
   uint8_t* y_img;           // image of y[B][E] for out_proj (tc_gemm.cuh)
   int ldj, B, E, R;
-  int T;                    // steps per launch (1 = the step path; > 1 = encode-side time slab, rows t*B + i): the state
-                            // of a stream is loaded before its first and stored after its last step of the slab
 };
 
 namespace scan {
@@ -204,8 +202,8 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   uint8_t* stages = scan_smem + NSB * EC * 64;     // [NSTG][SB] step stages
   float* wdt = reinterpret_cast<float*>(stages + NSTG * SB);
   uint64_t* bars = reinterpret_cast<uint64_t*>(stages + NSTG * SB + (RR ? 0 : a.R * EC * 4));   // full, done, ready [NSTG] each
-  // copies run LA iterations ahead: all step stages when a slab gives the state buffers time to drain (LA <= 3T+1)
-  const int LA = a.T >= 3 ? NSTG : (a.T == 2 ? 7 : NSB);
+  constexpr int T = 1;                             // steps per stream and launch (the time-slab form is k_scan_slab)
+  constexpr int LA = NSB;                          // copies run LA iterations ahead: one state buffer each
   const int nk = (a.B - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // streams of this CTA
   if (nk <= 0) return;
 
@@ -225,7 +223,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     const int lane = tid - EC;
     uint64_t pol;
     asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(pol));
-    const int T = a.T, niter = nk * T;             // iteration kk = (stream k of this CTA, step t of the slab)
+    const int niter = nk * T;                      // iteration kk = stream k of this CTA
     // This warp is one serial instruction stream beside eight channel warps: indices advance incrementally (no
     // divisions), per-lane offsets are computed once.
     static_assert((NSTG & (NSTG - 1)) == 0 && (NSB & (NSB - 1)) == 0, "ring sizes are powers of two");
@@ -318,7 +316,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   const float dsk = a.Dskip[e];
   const float bdt = a.b_dt[e];
 
-  const int T = a.T, niter = nk * T;
+  const int niter = nk * T;
   float4 h0, h1, h2, h3;                           // the channel's 16 state values: in registers across a slab
   int k = 0, t = 0;
   size_t row_i = blockIdx.x;                       // this iteration's stream index in the wave
