@@ -221,8 +221,11 @@ int mark(StepCtx& c, int cls) {
 // ---- tensor-core GEMM launch (tc_gemm.cuh).  The dynamic shared-memory opt-in is set once per instantiation.
 // Launch with the programmatic-serialization attribute (PDL, common.cuh): the kernel calls pdl_wait() before it
 // touches anything an earlier kernel of the stream wrote.
-bool g_pdl = true;   // BOA_NO_PDL=1 in the environment turns it off (read at boa_model_load)
-bool g_cluster = true;   // BOA_NO_CLUSTER=1: launch the contraction kernels without 2-CTA clusters (same results)
+// Debug switches, read once from the environment (results do not depend on them):
+//   BOA_NO_PDL=1      launch without the programmatic-serialization attribute
+//   BOA_NO_CLUSTER=1  launch the contraction kernels without 2-CTA clusters
+bool use_pdl() { static const bool v = getenv("BOA_NO_PDL") == nullptr; return v; }
+bool use_cluster() { static const bool v = getenv("BOA_NO_CLUSTER") == nullptr; return v; }
 template <typename... KArgs, typename... Args>
 cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
   cudaLaunchConfig_t cfg{};
@@ -230,7 +233,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = g_pdl ? 1 : 0;
+  cfg.attrs = at; cfg.numAttrs = use_pdl() ? 1 : 0;
   return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
 
@@ -242,9 +245,9 @@ int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
   cfg.blockDim = dim3(tc::NTHREADS); cfg.dynamicSmemBytes = C::SMEM; cfg.stream = st;
   cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = g_pdl ? 1 : 0;
+  at[0].val.programmaticStreamSerializationAllowed = use_pdl() ? 1 : 0;
   cfg.attrs = at; cfg.numAttrs = 1;
-  if (g_cluster && g.NT % 2 == 0) {
+  if (use_cluster() && g.NT % 2 == 0) {
     // clusters of two CTAs share the activation k-blocks of a row tile (multicast): persistent, one cluster per SM pair
     const int items = mt * (g.NT / 2) * g.KS;
     cfg.gridDim = dim3(2 * std::min(items, n_sm / 2));
@@ -687,8 +690,6 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
   if (!m) return BOA_E_NOMEM;
   m->L = (int)L; m->D = (int)D; m->E = (int)E; m->R = (int)R; m->J = (int)J;
   m->blob_crc = crc32_ieee(p, nbytes);
-  g_pdl = getenv("BOA_NO_PDL") == nullptr;
-  g_cluster = getenv("BOA_NO_CLUSTER") == nullptr;
   m->npw = dtype == 1 ? 1 : 3;         // a bf16 weight is one exact piece; an fp32 weight is cut into three
   m->ldj = J <= 64 ? 64 : 128;
   m->ks_x = ((E / 64) % 4 == 0) ? 4 : ((E / 64) % 2 == 0) ? 2 : 1;
