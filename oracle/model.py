@@ -9,6 +9,10 @@ Follows PAPER.md step by step:
 Readings: block = pre-RMSNorm -> mixer -> residual, no FFN (#1); no final norm (#2);
 B_bar = d*B (#3); no bias on B_t, C_t (#4); eps=1e-5, stable softplus, SiLU=x*sigmoid(x) (#10);
 conv tap K-1 multiplies the current input (#11).
+The paper's own block (blobs with FLAG_FFN): after the mixer and its residual,
+u <- LayerNorm(FFN(u)) as Alg. 1 l.4 (P:144) writes it - no residual around the FFN;
+FFN(u) = W2 GELU(W1 u + b1) + b2 with GELU(v) = v Phi(v) (erf form); LayerNorm over the D features with the
+biased variance, eps = 1e-5, affine (ln_w, ln_b); head untied when FLAG_TIED_HEAD is clear (#23).
 
 Streams are independent; every function below takes a leading "stream" axis S and
 treats the S rows independently — that axis is the only vectorisation.
@@ -35,6 +39,13 @@ class Layer:
     a_log: np.ndarray    # [E, N]
     d_skip: np.ndarray   # [E]
     w_out: np.ndarray    # [D, E]
+    # the paper's block only (FLAG_FFN), else None
+    ffn_w1: np.ndarray = None   # [F, D]
+    ffn_b1: np.ndarray = None   # [F]
+    ffn_w2: np.ndarray = None   # [D, F]
+    ffn_b2: np.ndarray = None   # [D]
+    ln_w: np.ndarray = None     # [D]
+    ln_b: np.ndarray = None     # [D]
 
 
 @dataclass
@@ -48,6 +59,8 @@ class Weights:
     emb: np.ndarray                      # [256, D]  (also the tied head)
     layers: list = field(default_factory=list)
     blob_crc: int = 0
+    d_ff: int = 0                        # > 0: FFN + LayerNorm after every mixer
+    head: np.ndarray = None              # [256, D] untied head, None = tied (Emb)
 
     @property
     def d_inner(self) -> int:
@@ -57,11 +70,11 @@ class Weights:
 def load_weights(blob: bytes) -> Weights:
     """Parse a BOAW v1 blob; stored fp32 / bf16 values are widened to fp64 exactly."""
     import zlib
-    magic, ver, dtype, nl, d, n, k, ex, r, flags = struct.unpack_from("<4s9I", blob, 0)
+    magic, ver, dtype, nl, d, n, k, ex, r, flags, f = struct.unpack_from("<4s10I", blob, 0)
     if magic != b"BOAW" or ver != 1:
         raise ValueError("not a BOAW v1 blob")
-    if not (flags & 1):
-        raise ValueError("untied head not supported")
+    if flags & ~3 or bool(flags & 2) != (f > 0):
+        raise ValueError("bad BOAW flags")
     e = ex * d
     off = 64
 
@@ -79,12 +92,23 @@ def load_weights(blob: bytes) -> Weights:
         return arr.reshape(shape)
 
     w = Weights(nl, d, n, k, ex, r, emb=take((256, d), True), blob_crc=zlib.crc32(blob) & 0xFFFFFFFF)
+    w.d_ff = f
     for _ in range(nl):
-        w.layers.append(Layer(
+        ly = Layer(
             norm_w=take((d,), False), w_in=take((2 * e, d), True), conv_w=take((e, k), False),
             conv_b=take((e,), False), w_x=take((r + 2 * n, e), True), w_dt=take((e, r), True),
             b_dt=take((e,), False), a_log=take((e, n), False), d_skip=take((e,), False),
-            w_out=take((d, e), True)))
+            w_out=take((d, e), True))
+        if f:
+            ly.ffn_w1 = take((f, d), True)
+            ly.ffn_b1 = take((f,), False)
+            ly.ffn_w2 = take((d, f), True)
+            ly.ffn_b2 = take((d,), False)
+            ly.ln_w = take((d,), False)
+            ly.ln_b = take((d,), False)
+        w.layers.append(ly)
+    if not (flags & 1):
+        w.head = take((256, d), True)
     if off != len(blob):
         raise ValueError("BOAW blob has trailing or missing bytes")
     return w
@@ -105,6 +129,26 @@ def softplus(v):
 
 def rmsnorm(u, w):
     return u * (1.0 / np.sqrt(np.mean(u * u, axis=-1, keepdims=True) + EPS)) * w
+
+
+_erf = np.vectorize(__import__("math").erf, otypes=[np.float64])
+
+
+def gelu(v):
+    """GELU(v) = v Phi(v) = v (1 + erf(v / sqrt 2)) / 2, Phi the standard normal CDF (reading #23)."""
+    return 0.5 * v * (1.0 + _erf(v / np.sqrt(2.0)))
+
+
+def layernorm(v, w, b):
+    """(v - mean) / sqrt(var + eps) * w + b over the last axis, var = the biased variance (reading #23)."""
+    mu = np.mean(v, axis=-1, keepdims=True)
+    var = np.mean((v - mu) * (v - mu), axis=-1, keepdims=True)
+    return (v - mu) / np.sqrt(var + EPS) * w + b
+
+
+def ffn(u, ly):
+    """Alg. 1 l.4's FFN: W2 GELU(W1 u + b1) + b2 (reading #23)."""
+    return gelu(u @ ly.ffn_w1.T + ly.ffn_b1) @ ly.ffn_w2.T + ly.ffn_b2
 
 
 @dataclass
@@ -158,7 +202,10 @@ def step(w: Weights, st: State, sym: np.ndarray):
         st.h[l], y = ssm_step(st.h[l], xs, delta, bv, cv, a, ly.d_skip)
         y = y * silu(z)
         u = u + y @ ly.w_out.T
-    return u @ w.emb.T                                     # Alg. 1 line 5 (tied head)
+        if w.d_ff:
+            u = layernorm(ffn(u, ly), ly.ln_w, ly.ln_b)   # Alg. 1 line 4
+    head = w.emb if w.head is None else w.head
+    return u @ head.T                                      # Alg. 1 line 5
 
 
 def logits_for_chunks(w: Weights, chunks: np.ndarray) -> np.ndarray:

@@ -22,7 +22,8 @@ BOAW_VERSION = 1
 BOAW_HEADER_BYTES = 64
 DTYPE_FP32 = 0
 DTYPE_BF16 = 1
-FLAG_TIED_HEAD = 1
+FLAG_TIED_HEAD = 1   # head = Emb^T (north_star's block); clear = a separate head matrix after the layers
+FLAG_FFN = 2         # every layer is followed by u <- LayerNorm(FFN(u)) (Alg. 1 l.4)
 
 
 @dataclass(frozen=True)
@@ -33,6 +34,8 @@ class ModelShape:
     d_conv: int = 4
     expand: int = 2
     dt_rank: int = 0  # 0 -> ceil(d_model / 16)
+    d_ff: int = 0     # > 0: the paper's block (Alg. 1 l.4): FFN of this hidden width + LayerNorm after every mixer
+    tied: bool = True # False: untied head matrix [256, D]
 
     @property
     def d_inner(self) -> int:
@@ -49,7 +52,11 @@ class ModelShape:
 
     def mac_per_byte(self) -> int:
         d, e, r, n = self.d_model, self.d_inner, self.rank, self.d_state
-        return self.n_layer * (d * 2 * e + e * (r + 2 * n) + r * e + e * d) + 256 * d
+        return self.n_layer * (d * 2 * e + e * (r + 2 * n) + r * e + e * d + 2 * d * self.d_ff) + 256 * d
+
+    @property
+    def flags(self) -> int:
+        return (FLAG_TIED_HEAD if self.tied else 0) | (FLAG_FFN if self.d_ff else 0)
 
 
 def _to_bf16_bits(a32: np.ndarray) -> np.ndarray:
@@ -85,28 +92,49 @@ def tensor_order(shape: ModelShape):
             (p + "d_skip", (e,), False),
             (p + "w_out", (d, e), True),
         ]
+        if shape.d_ff:
+            f = shape.d_ff
+            out += [
+                (p + "ffn_w1", (f, d), True),
+                (p + "ffn_b1", (f,), False),
+                (p + "ffn_w2", (d, f), True),
+                (p + "ffn_b2", (d,), False),
+                (p + "ln_w", (d,), False),
+                (p + "ln_b", (d,), False),
+            ]
+    if not shape.tied:
+        out.append(("head", (256, d), True))
     return out
 
 
 def make_weights(shape: ModelShape, seed: int, dtype: int = DTYPE_FP32,
-                 std: float = 0.02, emb_std: float | None = None) -> bytes:
+                 std: float = 0.02, emb_std: float | None = None, ffn_std: float | None = None) -> bytes:
     """Random-init BOAW blob.  Draw order = blob order, fp64 draws -> fp32 (-> bf16 for matrices).
 
     All matrices incl. emb and conv_w ~ N(0, std^2); norm_w = 1; conv_b = 0; d_skip = 1;
     a_log[e][n] = log(n+1); b_dt = softplus^-1(dt), dt = exp(U(log 1e-3, log 1e-1)).
     `emb_std` (e.g. 0.25) gives the "sharp" variant used to stress the quantiser and coder.
+    FFN variant (shape.d_ff > 0): ffn_w1, ffn_w2 ~ N(0, ffn_std^2) (default std); the FFN biases and ln_b
+    ~ N(0, std^2) and ln_w = 1 + N(0, std^2), so that a dropped bias or affine term changes the result;
+    untied head ~ N(0, emb_std^2).
     """
     g = np.random.Generator(np.random.PCG64(seed))
     emb_std = std if emb_std is None else emb_std
-    hdr = struct.pack("<4s9I", BOAW_MAGIC, BOAW_VERSION, dtype, shape.n_layer, shape.d_model,
-                      shape.d_state, shape.d_conv, shape.expand, shape.rank, FLAG_TIED_HEAD)
+    hdr = struct.pack("<4s10I", BOAW_MAGIC, BOAW_VERSION, dtype, shape.n_layer, shape.d_model,
+                      shape.d_state, shape.d_conv, shape.expand, shape.rank, shape.flags, shape.d_ff)
     parts = [hdr + b"\0" * (BOAW_HEADER_BYTES - len(hdr))]
     for name, dims, is_mat in tensor_order(shape):
         base = name.split(".")[-1]
-        if base == "emb":
+        if base == "emb" or base == "head":
             a = g.normal(0.0, emb_std, dims)
         elif base in ("w_in", "w_x", "w_dt", "w_out", "conv_w"):
             a = g.normal(0.0, std, dims)
+        elif base in ("ffn_w1", "ffn_w2"):
+            a = g.normal(0.0, ffn_std if ffn_std is not None else std, dims)
+        elif base in ("ffn_b1", "ffn_b2", "ln_b"):
+            a = g.normal(0.0, std, dims)
+        elif base == "ln_w":
+            a = 1.0 + g.normal(0.0, std, dims)
         elif base == "norm_w" or base == "d_skip":
             a = np.ones(dims)
         elif base == "conv_b":
@@ -127,10 +155,10 @@ def make_weights(shape: ModelShape, seed: int, dtype: int = DTYPE_FP32,
 
 
 def parse_header(blob: bytes):
-    magic, ver, dtype, nl, d, n, k, ex, r, flags = struct.unpack_from("<4s9I", blob, 0)
+    magic, ver, dtype, nl, d, n, k, ex, r, flags, d_ff = struct.unpack_from("<4s10I", blob, 0)
     if magic != BOAW_MAGIC or ver != BOAW_VERSION:
         raise ValueError("not a BOAW v1 blob")
-    return ModelShape(nl, d, n, k, ex, r), dtype, flags
+    return ModelShape(nl, d, n, k, ex, r, d_ff if flags & FLAG_FFN else 0, bool(flags & FLAG_TIED_HEAD)), dtype, flags
 
 
 # --------------------------------------------------------------------------- byte workloads
@@ -226,4 +254,8 @@ CONFIGS = {
     3: Config("cfg3_records_256MiB", ModelShape(2, 256, dt_rank=16), DTYPE_FP32, 1, 1003, 256 * MiB, 16384, "records"),
     4: Config("cfg4_kinematics_1GiB", ModelShape(4, 256, dt_rank=16), DTYPE_BF16, 2, 1004, 1024 * MiB, 16384, "kinematics"),
     5: Config("cfg5_mix_512MiB", ModelShape(8, 512, dt_rank=32), DTYPE_BF16, 3, 1005, 512 * MiB, 65536, "mix"),
+    # not a BASELINE.json config: the paper's own block (d_m = 256, n_l = 1, FFN +
+    # LayerNorm after the mixer, untied head, ~4.4 MB of fp32 weights) on the input of config 2
+    6: Config("next2_paper_block_64MiB", ModelShape(1, 256, dt_rank=16, d_ff=1024, tied=False), DTYPE_FP32, 4, 1002,
+              64 * MiB, 16384, "kinematics"),
 }

@@ -141,7 +141,11 @@ def _sequence_mode_logits(blob, chunks):
         y = torch.einsum("sten,stn->ste", h, cv) + tens[p + "d_skip"] * xs
         y = y * F.silu(z)
         u = u + torch.einsum("ste,de->std", y, tens[p + "w_out"])
-    return torch.einsum("std,vd->stv", u, tens["emb"]).numpy()
+        if shape.d_ff:                                                # Alg. 1 l.4 with library routines
+            hid = F.gelu(F.linear(u, tens[p + "ffn_w1"], tens[p + "ffn_b1"]))
+            u = F.layer_norm(F.linear(hid, tens[p + "ffn_w2"], tens[p + "ffn_b2"]), (D,),
+                             tens[p + "ln_w"], tens[p + "ln_b"], eps=1e-5)
+    return torch.einsum("std,vd->stv", u, tens["emb" if shape.tied else "head"]).numpy()
 
 
 @pytest.mark.parametrize("dtype,emb_std", [(synth.DTYPE_FP32, None), (synth.DTYPE_BF16, 0.25)])
@@ -153,6 +157,86 @@ def test_step_mode_against_sequence_mode(dtype, emb_std):
     ref = _sequence_mode_logits(blob, chunks)
     assert np.max(np.abs(ref)) > 0.05          # non-trivial logits
     np.testing.assert_allclose(got, ref, rtol=1e-10, atol=1e-11)
+
+
+@pytest.mark.parametrize("tied", [True, False])
+def test_paper_block_step_mode_against_sequence_mode(tied):
+    # FFN + LayerNorm after every mixer (Alg. 1 l.4), tied and untied head
+    shape = synth.ModelShape(2, 32, dt_rank=2, d_ff=96, tied=tied)
+    blob = synth.make_weights(shape, 11, synth.DTYPE_FP32, std=0.2, emb_std=0.3)
+    chunks = rng(6).integers(0, 256, (3, 17), dtype=np.uint8)
+    w = model.load_weights(blob)
+    got = model.logits_for_chunks(w, chunks)
+    ref = _sequence_mode_logits(blob, chunks)
+    assert np.max(np.abs(ref)) > 0.05
+    np.testing.assert_allclose(got, ref, rtol=1e-10, atol=1e-11)
+    # the block is not the north_star block in disguise: dropping the FFN flag's tensors changes the logits
+    plain = synth.make_weights(synth.ModelShape(2, 32, dt_rank=2), 11, synth.DTYPE_FP32, std=0.2, emb_std=0.3)
+    other = model.logits_for_chunks(model.load_weights(plain), chunks)
+    assert np.max(np.abs(other - got)) > 1e-3
+
+
+def test_gelu_against_library_and_identities():
+    from scipy.stats import norm
+    x = rng(8).normal(0, 2.5, 500)
+    x[:3] = [0.0, 30.0, -30.0]
+    # (the erf form cancels in the far negative tail: absolute, not relative, agreement there)
+    np.testing.assert_allclose(model.gelu(x), x * norm.cdf(x), rtol=1e-12, atol=1e-15)         # v Phi(v)
+    np.testing.assert_allclose(model.gelu(x), F.gelu(torch.tensor(x)).numpy(), rtol=1e-12, atol=1e-15)
+    np.testing.assert_allclose(model.gelu(x) - model.gelu(-x), x, rtol=1e-12, atol=1e-15)      # Phi(v) + Phi(-v) = 1
+    assert model.gelu(np.array([0.0]))[0] == 0.0 and model.gelu(np.array([30.0]))[0] == 30.0
+    assert abs(model.gelu(np.array([1.0]))[0] - 0.8413447460685429) < 1e-15                   # Phi(1)
+
+
+def test_layernorm_against_torch_and_invariants():
+    g = rng(9)
+    v, w, b = g.normal(3, 2, (5, 48)), g.normal(1, 0.2, 48), g.normal(0, 0.3, 48)
+    ref = F.layer_norm(torch.tensor(v), (48,), torch.tensor(w), torch.tensor(b), eps=1e-5).numpy()
+    np.testing.assert_allclose(model.layernorm(v, w, b), ref, rtol=1e-12, atol=1e-14)
+    plain = model.layernorm(v, np.ones(48), np.zeros(48))
+    np.testing.assert_allclose(plain.mean(axis=1), 0.0, atol=1e-14)
+    var = v.var(axis=1)                                                   # biased
+    np.testing.assert_allclose(plain.var(axis=1), var / (var + 1e-5), rtol=1e-12)
+    # invariant to a shift of the input, scales out a positive factor (up to eps)
+    np.testing.assert_allclose(model.layernorm(v + 7.0, w, b), model.layernorm(v, w, b), rtol=1e-9, atol=1e-12)
+
+
+def test_ffn_against_direct_sum():
+    import math
+    g = rng(10)
+    D, Fh = 6, 10
+    ly = model.Layer(*[None] * 10)
+    ly.ffn_w1, ly.ffn_b1 = g.normal(0, 1, (Fh, D)), g.normal(0, 1, Fh)
+    ly.ffn_w2, ly.ffn_b2 = g.normal(0, 1, (D, Fh)), g.normal(0, 1, D)
+    u = g.normal(0, 1, (2, D))
+    got = model.ffn(u, ly)
+    for s in range(2):
+        for d in range(D):
+            acc = ly.ffn_b2[d]
+            for j in range(Fh):
+                pre = ly.ffn_b1[j] + sum(ly.ffn_w1[j, k] * u[s, k] for k in range(D))
+                acc += ly.ffn_w2[d, j] * 0.5 * pre * (1.0 + math.erf(pre / math.sqrt(2.0)))
+            assert abs(acc - got[s, d]) < 1e-12
+
+
+def test_load_weights_slots_paper_block():
+    shape = synth.ModelShape(1, 16, dt_rank=1, d_ff=24, tied=False)
+    D, E, N, K, R, Fh = 16, 32, 16, 4, 1, 24
+    total = sum(int(np.prod(d)) for _, d, _ in synth.tensor_order(shape))
+    import struct
+    hdr = struct.pack("<4s10I", b"BOAW", 1, 0, 1, D, N, K, 2, R, 2, Fh).ljust(64, b"\0")
+    w = model.load_weights(hdr + np.arange(total, dtype="<f4").tobytes())
+    ly = w.layers[0]
+    off = 256 * D + D + 2 * E * D + E * K + E + (R + 2 * N) * E + E * R + E + E * N + E + D * E
+    for arr, shp in [(ly.ffn_w1, (Fh, D)), (ly.ffn_b1, (Fh,)), (ly.ffn_w2, (D, Fh)), (ly.ffn_b2, (D,)),
+                     (ly.ln_w, (D,)), (ly.ln_b, (D,)), (w.head, (256, D))]:
+        assert arr.shape == shp and arr.reshape(-1)[0] == off and arr.reshape(-1)[-1] == off + arr.size - 1
+        off += arr.size
+    assert off == total
+    # flag and width must agree
+    bad = struct.pack("<4s10I", b"BOAW", 1, 0, 1, D, N, K, 2, R, 2, 0).ljust(64, b"\0")
+    with pytest.raises(ValueError):
+        model.load_weights(bad + np.arange(total, dtype="<f4").tobytes())
 
 
 def test_load_weights_slots():
