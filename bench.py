@@ -115,14 +115,15 @@ def time_oracle(cfg, n_streams=64, length=128):
 
 def workload_name(cfg):
     return (f"{cfg.name}: {cfg.n_bytes / MiB:g} MiB, {cfg.n_bytes // cfg.chunk_bytes} chunks x {cfg.chunk_bytes / 1024:g} KiB, "
-            f"{cfg.shape.n_layer}-layer d_model={cfg.shape.d_model} {'bf16' if cfg.weight_dtype else 'fp32'} weights")
+            f"{cfg.shape.n_layer}-layer d_model={cfg.shape.d_model} {'bf16' if cfg.weight_dtype else 'fp32'} weights"
+            + (f", FFN {cfg.shape.d_ff} + LayerNorm per layer, untied head (the paper's block)" if cfg.shape.d_ff else ""))
 
 
 def base_line(args, cfg, world):
     return {"metric": "compress+decompress throughput (input bytes), mean of the two directions = 2n/(Tc+Td)",
             "unit": "MiB/s", "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-            "config": {"workload": workload_name(cfg), "baseline_config_index": args.config - 1,
+            "config": {"workload": workload_name(cfg), "baseline_config_index": args.config - 1 if args.config <= 5 else None,
                        "streams_per_gpu": cfg.n_bytes // cfg.chunk_bytes, "chunk_bytes": cfg.chunk_bytes,
                        "l2": "inputs larger than L2: the per-step working set is the stream state "
                              f"({cfg.shape.state_bytes_per_stream() * (cfg.n_bytes // cfg.chunk_bytes) / 1e9:.2f} GB) "
@@ -162,13 +163,18 @@ def kernel_work(cfg, B):
     # A contraction is computed as `mm` bf16 MMAs per fp32 product (tc_gemm.cuh: 6 for fp32 weights, 3 for bf16
     # weights): its algorithmic tensor work is mm * 2*M*N*K bf16 flops.
     mm = 3 if cfg.weight_dtype else 6
-    return {
+    work = {
         "scan": ("hbm", B * 2 * E * N * 4),                 # h read + written once, fp32
         "convx": ("tensor", mm * 2 * B * E * (R + 2 * N)),  # x_proj
         "inproj": ("tensor", mm * 2 * B * D * 2 * E),
         "outproj": ("tensor", mm * 2 * B * E * D),
         "head": ("tensor", mm * 2 * B * D * 256),
     }
+    if s.d_ff:   # the paper's block: two more contractions and a LayerNorm per layer
+        work["ffn1"] = ("tensor", mm * 2 * B * D * s.d_ff)
+        work["ffn2"] = ("tensor", mm * 2 * B * s.d_ff * D)
+        work["lnorm"] = ("hbm", B * D * (4 + 4 + 6))        # v read, u and its image written
+    return work
 
 
 def run_ours(args, cfg):
@@ -335,7 +341,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[] number, 1-based (2 = the metric's config)")
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs[] number, 1-based (2 = the metric's config; 6 = the paper's own block on config 2's input, SURVEY 8(f) NEXT-2)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--sample-every", type=int, default=48, help="event-bracket every k-th 32-step batch (roofline)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

@@ -53,8 +53,13 @@ typedef struct boa_model boa_model; /* opaque: device weights + workspace */
  * boa_model_load: parse a BOAW v1 blob (HOST pointer; layout in DESIGN.md "BOAW") — byte embedding
  * [256][D] (also the tied head), per layer norm_w, W_in, conv_w, conv_b, W_x, W_dt,
  * b_dt, A_log, D_skip, W_out (eq. 20-22) — copy it to the current CUDA device and
- * return a handle.  Supported: d_state = 16, d_conv = 4, expand = 2, d_model a multiple of 64 and
- * <= 512, dt_rank a multiple of 4 and <= 64, tied head, fp32 or bf16 matrices; else BOA_E_UNSUPPORTED.
+ * return a handle.  Header flags (offset 36): bit 0 = tied head; bit 1 = the paper's own block
+ * (Alg. 1 l.4; R#23): every layer is followed by u <- LayerNorm(W2 GELU(W1 u + b1) + b2)
+ * with hidden width d_ff (u32 at offset 40) and the per-layer tensors ffn_w1 [d_ff][D], ffn_b1, ffn_w2
+ * [D][d_ff], ffn_b2, ln_w, ln_b after W_out; with bit 0 clear an untied head [256][D] follows the layers.
+ * Supported: d_state = 16, d_conv = 4, expand = 2, d_model a multiple of 64 and <= 512, dt_rank a
+ * multiple of 4 and <= 64, d_ff a multiple of 64 and <= 4096, fp32 or bf16 matrices; else
+ * BOA_E_UNSUPPORTED.  Flag bits beyond 0-1, or bit 1 disagreeing with d_ff > 0: BOA_E_FORMAT.
  * The blob is not referenced after the call returns. */
 int boa_model_load(const void* weights, size_t nbytes, boa_model** out);
 void boa_model_free(boa_model* m);
@@ -105,7 +110,11 @@ enum {
   BOA_K_HEAD = 5,    /* S10 tied head (tensor cores)                                               */
   BOA_K_CODER = 6,   /* S11-S14 softmax, table, range coder step; S1 of the next step              */
   BOA_K_FINISH = 7,  /* S15/S16 flush, compaction, init                           */
-  BOA_K_COUNT = 8
+  /* the paper's block only (Alg. 1 l.4), after out_proj of every layer: */
+  BOA_K_FFN1 = 8,    /* hidden = GELU(W1 u + b1) (tensor cores; writes the operand image of FFN2)   */
+  BOA_K_FFN2 = 9,    /* v = W2 hidden + b2 (tensor cores)                                          */
+  BOA_K_LNORM = 10,  /* u = LayerNorm(v); image and block sums of u^2 for the next contraction     */
+  BOA_K_COUNT = 11
 };
 typedef struct boa_profile {
   uint64_t launches_total;            /* kernels launched by the last compress/decompress call       */

@@ -16,8 +16,8 @@ from . import build as _build
 
 OK = 0
 E_ARG, E_FORMAT, E_CRC, E_MODEL_MISMATCH, E_CAPACITY, E_CORRUPT, E_CUDA, E_NOMEM, E_UNSUPPORTED = range(-1, -10, -1)
-K_NAMES = ("embed", "inproj", "convx", "scan", "outproj", "head", "coder", "finish")
-K_COUNT = 8
+K_NAMES = ("embed", "inproj", "convx", "scan", "outproj", "head", "coder", "finish", "ffn1", "ffn2", "lnorm")
+K_COUNT = len(K_NAMES)
 
 EXPORTS = ("boa_model_load", "boa_model_free", "boa_model_fingerprint", "boa_compress_bound", "boa_compress",
            "boa_decompressed_size", "boa_decompress", "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",

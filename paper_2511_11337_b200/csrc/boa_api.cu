@@ -48,6 +48,9 @@ struct LayerW {
   const float *norm_w, *conv_b, *w_dtT, *b_dt, *d_skip;
   const float4 *conv_w, *A4;
   const uint16_t *img_in, *img_x, *img_out;   // tensor-core weight images (tc_gemm.cuh)
+  // the paper's block (FLAG_FFN; Alg. 1 l.4, R#23) only
+  const float *ffn_b1 = nullptr, *ffn_b2 = nullptr, *ln_w = nullptr, *ln_b = nullptr;
+  const uint16_t *img_ffn1 = nullptr, *img_ffn2 = nullptr;
 };
 
 bool is_device_ptr(const void* p) {
@@ -61,6 +64,7 @@ bool is_device_ptr(const void* p) {
 
 struct boa_model {
   int L = 0, D = 0, E = 0, R = 0, J = 0;
+  int F = 0;                   // > 0: the paper's block - every mixer is followed by u <- LayerNorm(FFN(u)), hidden width F
   int npw = 3;                 // bf16 pieces per weight: 3 for fp32 blobs, 1 for bf16 blobs (exact)
   int ldj = 64;                // row stride of the x_proj output = its padded width (64 or 128)
   int ks_x = 1;                // k-splits of x_proj (a function of the model shape only: results must not depend on B)
@@ -76,6 +80,7 @@ struct boa_model {
   uint64_t rows_cap = 0;       // rows the per-row activation buffers are sized for (>= Bcap; Bcap * kSlabT for time slabs)
   GrowBuf u, xz, dbc, logits, h, win, ssq;
   GrowBuf u_img, xs_img, y_img;   // activation images: operands of the tensor-core contractions (tc_gemm.cuh)
+  GrowBuf f_img, ffn_v;           // F > 0: image of the FFN's hidden layer; the FFN's output [rows][D] before LayerNorm
   GrowBuf pos, len, low, range, pending, wpos, cache, started, v, rpos, off, size, scratch, first, err;
   GrowBuf stage_in, stage_out;
 
@@ -90,7 +95,7 @@ struct boa_model {
   std::vector<cudaEvent_t> events;
 
   ~boa_model() {
-    for (GrowBuf* b : {&weights, &wimg, &u, &xz, &dbc, &u_img, &xs_img, &y_img, &logits, &h, &win, &ssq, &pos, &len, &low, &range,
+    for (GrowBuf* b : {&weights, &wimg, &u, &xz, &dbc, &u_img, &xs_img, &y_img, &f_img, &ffn_v, &logits, &h, &win, &ssq, &pos, &len, &low, &range,
                        &pending, &wpos, &cache, &started, &v, &rpos, &off, &size, &scratch, &first, &err,
                        &stage_in, &stage_out})
       b->release();
@@ -237,12 +242,12 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
   return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
 
-template <int NPW, int EPI>
+template <int NPW, int EPI, bool SLAB = false>
 int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
   using C = tc::Cfg<NPW>;
   const int mt = (g.M + tc::BM - 1) / tc::BM;
   cudaLaunchConfig_t cfg{};
-  cfg.blockDim = dim3(tc::NTHREADS); cfg.dynamicSmemBytes = C::SMEM; cfg.stream = st;
+  cfg.blockDim = dim3(tc::NTHREADS); cfg.dynamicSmemBytes = SLAB ? C::SMEM_SLAB : C::SMEM; cfg.stream = st;
   cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = use_pdl() ? 1 : 0;
@@ -254,17 +259,18 @@ int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
     at[1].id = cudaLaunchAttributeClusterDimension;
     at[1].val.clusterDim.x = 2; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
     cfg.numAttrs = 2;
-    BOA_CUDA_TRY(cudaLaunchKernelEx(&cfg, tc::k_tc_gemm<NPW, EPI, 2>, g));
+    BOA_CUDA_TRY(cudaLaunchKernelEx(&cfg, tc::k_tc_gemm<NPW, EPI, 2, SLAB>, g));
   } else {
     cfg.gridDim = dim3(std::min(mt * g.NT * g.KS, n_sm));             // persistent: one CTA per SM
-    BOA_CUDA_TRY(cudaLaunchKernelEx(&cfg, tc::k_tc_gemm<NPW, EPI, 1>, g));
+    BOA_CUDA_TRY(cudaLaunchKernelEx(&cfg, tc::k_tc_gemm<NPW, EPI, 1, SLAB>, g));
   }
   return BOA_OK;
 }
-template <int NPW, int EPI>
+template <int NPW, int EPI, bool SLAB = false>
 int optin_tc() {
-  BOA_CUDA_TRY(cudaFuncSetAttribute(tc::k_tc_gemm<NPW, EPI, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Cfg<NPW>::SMEM));
-  BOA_CUDA_TRY(cudaFuncSetAttribute(tc::k_tc_gemm<NPW, EPI, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Cfg<NPW>::SMEM));
+  constexpr int smem = SLAB ? tc::Cfg<NPW>::SMEM_SLAB : tc::Cfg<NPW>::SMEM;
+  BOA_CUDA_TRY((cudaFuncSetAttribute(tc::k_tc_gemm<NPW, EPI, 1, SLAB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)));
+  BOA_CUDA_TRY((cudaFuncSetAttribute(tc::k_tc_gemm<NPW, EPI, 2, SLAB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)));
   return BOA_OK;
 }
 // Shared-memory opt-ins of every kernel instantiation the step can launch (called by boa_model_load, outside
@@ -272,10 +278,14 @@ int optin_tc() {
 int init_kernels() {
   BOA_TRY((optin_tc<1, tc::EPI_INPROJ>()));
   BOA_TRY((optin_tc<3, tc::EPI_INPROJ>()));
+  BOA_TRY((optin_tc<1, tc::EPI_INPROJ, true>()));
+  BOA_TRY((optin_tc<3, tc::EPI_INPROJ, true>()));
   BOA_TRY((optin_tc<1, tc::EPI_STORE>()));
   BOA_TRY((optin_tc<3, tc::EPI_STORE>()));
   BOA_TRY((optin_tc<1, tc::EPI_RESID>()));
   BOA_TRY((optin_tc<3, tc::EPI_RESID>()));
+  BOA_TRY((optin_tc<1, tc::EPI_FFN1>()));
+  BOA_TRY((optin_tc<3, tc::EPI_FFN1>()));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 64)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
@@ -336,7 +346,12 @@ int launch_step(StepCtx& c) {
       g.xz_slice = T == 1 ? (size_t)2 * ec : (size_t)rows * 2 * ec;
       g.ssq_in = m->ssq.as<float>(); g.win = winl; g.pos = c.ca.pos; g.slab_T = T == 1 ? 0 : T; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
-      if (!BOA_DEV_SKIPPED(BOA_K_INPROJ)) BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
+      if (BOA_DEV_SKIPPED(BOA_K_INPROJ)) {
+      } else if (T > 1) {   // the time-slab form of the conv epilogue
+        BOA_TRY((m->npw == 1 ? launch_tc<1, tc::EPI_INPROJ, true>(g, m->n_sm, c.st) : launch_tc<3, tc::EPI_INPROJ, true>(g, m->n_sm, c.st)));
+      } else {
+        BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
+      }
       BOA_TRY(mark(c, BOA_K_INPROJ));
     }
     {  // S5: [dlt;Bv;Cv] = W_x xs
@@ -383,9 +398,33 @@ int launch_step(StepCtx& c) {
       g.A = y_img; g.M = rows; g.KB = E / 64; g.W = w.img_out; g.NT = D / 64; g.KS = 1;
       g.C = u; g.ldc = D; g.n_valid = D;
       g.out_img = u_img; g.out_KB = D / 64; g.ssq_out = m->ssq.as<float>();
-      g.out_scale = (l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
+      // (the paper's block: the FFN reads u itself, not a normalised u)
+      g.out_scale = (m->F == 0 && l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
       if (!BOA_DEV_SKIPPED(BOA_K_OUTPROJ)) BOA_TRY((launch_tc_npw<tc::EPI_RESID>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_OUTPROJ));
+    }
+    if (m->F > 0) {  // the paper's block (Alg. 1 l.4, R#23): u <- LayerNorm(W2 GELU(W1 u + b1) + b2)
+      const int F = m->F;
+      uint8_t* f_img = m->f_img.as<uint8_t>();
+      float* ffn_v = m->ffn_v.as<float>();
+      {
+        tc::GemmArgs g{};
+        g.A = u_img; g.M = rows; g.KB = D / 64; g.W = w.img_ffn1; g.NT = F / 64; g.KS = 1;
+        g.n_valid = F; g.bias = w.ffn_b1; g.out_img = f_img; g.out_KB = F / 64;
+        BOA_TRY((launch_tc_npw<tc::EPI_FFN1>(m->npw, g, m->n_sm, c.st)));
+        BOA_TRY(mark(c, BOA_K_FFN1));
+      }
+      {
+        tc::GemmArgs g{};
+        g.A = f_img; g.M = rows; g.KB = F / 64; g.W = w.img_ffn2; g.NT = D / 64; g.KS = 1;
+        g.C = ffn_v; g.ldc = D; g.n_valid = D; g.bias = w.ffn_b2;
+        BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
+        BOA_TRY(mark(c, BOA_K_FFN2));
+      }
+      BOA_CUDA_TRY(launch_pdl(k_layernorm, dim3((unsigned)(((size_t)rows * 32 + 255) / 256)), dim3(256), 0, c.st,
+                              (const float*)ffn_v, w.ln_w, w.ln_b, u, (l + 1 < m->L) ? m->layers[l + 1].norm_w : (const float*)nullptr,
+                              u_img, m->ssq.as<float>(), rows, D));
+      BOA_TRY(mark(c, BOA_K_LNORM));
     }
   }
   {  // S10: logits = Emb u
@@ -531,7 +570,7 @@ int run_slabs(StepCtx& c, uint64_t n_slabs) {
 // ------------------------------------------------------------------------------------- workspace
 size_t bytes_per_row(const boa_model* m) {   // activations of one stream-step
   const size_t E = m->E, D = m->D;
-  return 4 * (D + 2 * E + (size_t)m->ks_x * m->ldj + 256 + D / 64) + 6 * (D + 2 * E);
+  return 4 * (D + 2 * E + (size_t)m->ks_x * m->ldj + 256 + D / 64) + 6 * (D + 2 * E) + (m->F ? 6 * (size_t)m->F + 4 * D : 0);
 }
 size_t bytes_per_stream(const boa_model* m, size_t cap, size_t rows_per_stream = 1) {
   const size_t E = m->E;
@@ -550,6 +589,10 @@ int reserve_workspace(boa_model* m, uint64_t B, size_t cap, uint64_t rows = 0) {
     BOA_TRY(m->u_img.reserve(tc::img_bytes(rows, D)));
     BOA_TRY(m->xs_img.reserve(tc::img_bytes(rows, E)));
     BOA_TRY(m->y_img.reserve(tc::img_bytes(rows, E)));
+    if (m->F > 0) {
+      BOA_TRY(m->f_img.reserve(tc::img_bytes(rows, (size_t)m->F)));
+      BOA_TRY(m->ffn_v.reserve(rows * D * 4));
+    }
     BOA_TRY(m->logits.reserve(rows * 256 * 4));
     m->rows_cap = rows;
   }
@@ -678,17 +721,20 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
   const uint8_t* p = static_cast<const uint8_t*>(weights);
   if (memcmp(p, "BOAW", 4) != 0 || get_u32(p + 4) != 1) return BOA_E_FORMAT;
   const uint32_t dtype = get_u32(p + 8), L = get_u32(p + 12), D = get_u32(p + 16), N = get_u32(p + 20),
-                 K = get_u32(p + 24), ex = get_u32(p + 28), R = get_u32(p + 32), flags = get_u32(p + 36);
-  if (dtype > 1) return BOA_E_FORMAT;
-  if (N != (uint32_t)kNState || K != (uint32_t)kDConv || ex != 2 || !(flags & 1u) || (flags & ~1u) || L == 0 || L > 64 ||
-      D == 0 || D % 64 != 0 || D > 512 || R == 0 || R > 64 || R % 4 != 0)
+                 K = get_u32(p + 24), ex = get_u32(p + 28), R = get_u32(p + 32), flags = get_u32(p + 36),
+                 F = get_u32(p + 40);
+  // flags: bit 0 = tied head (Emb^T); bit 1 = the paper's block, FFN of hidden width F + LayerNorm after every mixer
+  const bool tied = (flags & 1u) != 0, ffn = (flags & 2u) != 0;
+  if (dtype > 1 || (flags & ~3u) || ffn != (F > 0)) return BOA_E_FORMAT;
+  if (N != (uint32_t)kNState || K != (uint32_t)kDConv || ex != 2 || L == 0 || L > 64 ||
+      D == 0 || D % 64 != 0 || D > 512 || R == 0 || R > 64 || R % 4 != 0 || F % 64 != 0 || F > 4096)
     return BOA_E_UNSUPPORTED;
   BOA_TRY(check_device());
   const size_t E = 2 * (size_t)D, J = R + 2 * kNState;
 
   boa_model* m = new (std::nothrow) boa_model();
   if (!m) return BOA_E_NOMEM;
-  m->L = (int)L; m->D = (int)D; m->E = (int)E; m->R = (int)R; m->J = (int)J;
+  m->L = (int)L; m->D = (int)D; m->E = (int)E; m->R = (int)R; m->J = (int)J; m->F = (int)F;
   m->blob_crc = crc32_ieee(p, nbytes);
   m->npw = dtype == 1 ? 1 : 3;         // a bf16 weight is one exact piece; an fp32 weight is cut into three
   m->ldj = J <= 64 ? 64 : 128;
@@ -706,20 +752,21 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
   std::vector<float> img;
   std::vector<uint16_t> wimg;
   img.reserve(256 * D + L * per_layer + 64);
-  wimg.reserve(((size_t)256 * D + L * (2 * E * D + (size_t)m->ldj * E + D * E)) * m->npw + 64);
+  wimg.reserve(((size_t)(tied ? 256 : 512) * D + L * (2 * E * D + (size_t)m->ldj * E + D * E + 2 * (size_t)F * D)) * m->npw + 64);
   auto append = [&](const std::vector<float>& v) {
     size_t o = img.size();
     img.insert(img.end(), v.begin(), v.end());
     while (img.size() % 4) img.push_back(0.0f);   // keep every tensor 16-byte aligned
     return o;
   };
-  struct Off { size_t norm_w, conv_w, conv_b, w_dtT, b_dt, A4, d_skip, img_in, img_x, img_out; };
+  struct Off { size_t norm_w, conv_w, conv_b, w_dtT, b_dt, A4, d_skip, img_in, img_x, img_out,
+               ffn_b1, ffn_b2, ln_w, ln_b, img_ffn1, img_ffn2; };
   std::vector<Off> offs(L);
   BlobReader br{p, nbytes, 64, (int)dtype};
   std::vector<float> t, t2;
   bool ok = br.take(256 * (size_t)D, true, t);
   size_t emb_off = 0, head_off = 0;
-  if (ok) { emb_off = append(t); head_off = append_w_image(t.data(), 256, D, 64, m->npw, wimg); }
+  if (ok) { emb_off = append(t); if (tied) head_off = append_w_image(t.data(), 256, D, 64, m->npw, wimg); }
   for (uint32_t l = 0; l < L && ok; ++l) {
     Off& o = offs[l];
     ok = ok && br.take(D, false, t); if (ok) o.norm_w = append(t);
@@ -745,6 +792,18 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
     }
     ok = ok && br.take(E, false, t); if (ok) o.d_skip = append(t);
     ok = ok && br.take(D * E, true, t); if (ok) o.img_out = append_w_image(t.data(), D, E, 64, m->npw, wimg);
+    if (ffn) {
+      ok = ok && br.take((size_t)F * D, true, t); if (ok) o.img_ffn1 = append_w_image(t.data(), F, D, 64, m->npw, wimg);
+      ok = ok && br.take(F, false, t); if (ok) o.ffn_b1 = append(t);
+      ok = ok && br.take((size_t)D * F, true, t); if (ok) o.img_ffn2 = append_w_image(t.data(), D, F, 64, m->npw, wimg);
+      ok = ok && br.take(D, false, t); if (ok) o.ffn_b2 = append(t);
+      ok = ok && br.take(D, false, t); if (ok) o.ln_w = append(t);
+      ok = ok && br.take(D, false, t); if (ok) o.ln_b = append(t);
+    }
+  }
+  if (!tied) {   // untied head [256][D] after the layers
+    ok = ok && br.take(256 * (size_t)D, true, t);
+    if (ok) head_off = append_w_image(t.data(), 256, D, 64, m->npw, wimg);
   }
   if (!ok || br.off != nbytes) { delete m; return BOA_E_FORMAT; }
 
@@ -777,6 +836,10 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
     w.conv_b = base + o.conv_b; w.w_dtT = base + o.w_dtT; w.b_dt = base + o.b_dt;
     w.A4 = reinterpret_cast<const float4*>(base + o.A4); w.d_skip = base + o.d_skip;
     w.img_in = wbase + o.img_in; w.img_x = wbase + o.img_x; w.img_out = wbase + o.img_out;
+    if (ffn) {
+      w.ffn_b1 = base + o.ffn_b1; w.ffn_b2 = base + o.ffn_b2; w.ln_w = base + o.ln_w; w.ln_b = base + o.ln_b;
+      w.img_ffn1 = wbase + o.img_ffn1; w.img_ffn2 = wbase + o.img_ffn2;
+    }
   }
   *out = m;
   return BOA_OK;

@@ -58,6 +58,62 @@ __global__ void k_embed(const uint8_t* __restrict__ src, size_t chunk_bytes, con
 }
 
 // ---------------------------------------------------------------------------------------------------
+// The paper's block only (Alg. 1 l.4; R#23): u = LayerNorm(v), v = FFN(u) as written by
+// the second FFN contraction.  One warp per row; lane l holds columns 128 j + 4 l .. + 3.
+//   mean = (sum v) / D ;  var = (sum (v - mean)^2) / D (biased) ;  u = (v - mean) / sqrt(var + eps) * ln_w + ln_b
+// Both sums: per lane j ascending over x, y, z, w, then the xor butterfly 16, 8, 4, 2, 1.  Like the residual epilogue
+// of out_proj it also writes what the next contraction needs: the image of u (times the next layer's RMSNorm weight,
+// or plain for the head) and the sums of u^2 over each 64-column block (x, y, z, w, then the butterfly 8, 4, 2, 1
+// over the 16 lanes of the block).  D <= 512 (4 float4 per lane).
+__global__ void k_layernorm(const float* __restrict__ v, const float* __restrict__ ln_w, const float* __restrict__ ln_b,
+                            float* __restrict__ u, const float* __restrict__ next_scale, uint8_t* __restrict__ u_img,
+                            float* __restrict__ ssq, int rows, int D) {
+  pdl_wait();
+  const int row = (int)((blockIdx.x * blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+  if (row >= rows) return;                         // warp-uniform
+  float4 x[4];
+  float s = 0.0f;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const int c = 128 * j + 4 * lane;
+    x[j] = c < D ? *reinterpret_cast<const float4*>(v + (size_t)row * D + c) : make_float4(0.f, 0.f, 0.f, 0.f);
+    s += x[j].x; s += x[j].y; s += x[j].z; s += x[j].w;
+  }
+  const float mean = warp_sum(s) / (float)D;
+  float q = 0.0f;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    if (128 * j + 4 * lane < D) {
+      x[j].x -= mean; x[j].y -= mean; x[j].z -= mean; x[j].w -= mean;
+      q = fmaf(x[j].x, x[j].x, q); q = fmaf(x[j].y, x[j].y, q); q = fmaf(x[j].z, x[j].z, q); q = fmaf(x[j].w, x[j].w, q);
+    }
+  }
+  const float rstd = 1.0f / sqrtf(warp_sum(q) / (float)D + kEps);
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    const int c = 128 * j + 4 * lane;
+    const bool live = c < D;                       // uniform over each group of 16 lanes (D % 64 == 0)
+    float4 o = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (live) {
+      const float4 w = *reinterpret_cast<const float4*>(ln_w + c), b = *reinterpret_cast<const float4*>(ln_b + c);
+      o.x = fmaf(x[j].x * rstd, w.x, b.x); o.y = fmaf(x[j].y * rstd, w.y, b.y);
+      o.z = fmaf(x[j].z * rstd, w.z, b.z); o.w = fmaf(x[j].w * rstd, w.w, b.w);
+    }
+    float ss = o.x * o.x;
+    ss = fmaf(o.y, o.y, ss); ss = fmaf(o.z, o.z, ss); ss = fmaf(o.w, o.w, ss);
+#pragma unroll
+    for (int d = 8; d > 0; d >>= 1) ss += __shfl_xor_sync(0xffffffffu, ss, d);
+    if (live) {
+      *reinterpret_cast<float4*>(u + (size_t)row * D + c) = o;
+      if ((lane & 15) == 0) ssq[(size_t)row * (D >> 6) + (c >> 6)] = ss;
+      float4 sc = make_float4(1.f, 1.f, 1.f, 1.f);
+      if (next_scale) sc = *reinterpret_cast<const float4*>(next_scale + c);
+      tc::cut4_store(u_img, D >> 6, row, c, make_float4(o.x * sc.x, o.y * sc.y, o.z * sc.z, o.w * sc.w));
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------
 // S6-S8, the kernel that streams the SSM state (the only large object of the path) through the SM.
 //   delta = softplus(b_dt[e] + sum_r W_dt[e][r] dlt[r])                      (sequential fp32 FMA chain, r ascending)
 //   h[n] = exp(delta*A[n]) * h[n] + (delta*Bv[n]) * xs ;  y = sum_n Cv[n] h[n] + D xs ;  y *= SiLU(z)

@@ -4,6 +4,7 @@
 //   x_proj    [dlt;Bv;Cv] = W_x xs          S5                                         eq. 21-22
 //   out_proj  u += W_out y                  S9                                         Alg. 1 l.3
 //   head      logits = Emb u                S10                                        Alg. 1 l.5
+//   FFN       f = GELU(W1 u + b1); v = W2 f + b2   (the paper's block only)   Alg. 1 l.4; R#23
 //
 // A tile is 128 streams x 64 columns:  C[m][n] = sum_k A[m][k] * W[n][k].  The kernel is persistent: one CTA per SM
 // walks over tiles; the TMEM accumulators are double-buffered so the epilogue of tile i overlaps the copies and MMAs
@@ -44,7 +45,7 @@ constexpr int BK = 64;           // k per stage: 64 bf16 = one 128-byte swizzle 
 constexpr int NPA = 3;           // bf16 pieces of an activation
 constexpr int A_PLANE = BM * 128;  // bytes of one activation piece tile
 
-enum { EPI_STORE = 0, EPI_RESID = 1, EPI_INPROJ = 2 };
+enum { EPI_STORE = 0, EPI_RESID = 1, EPI_INPROJ = 2, EPI_FFN1 = 3 };
 
 struct GemmArgs {
   const uint8_t* A;        // activation image of A[M][K]: [ceil(M/128)][K/64][3 pieces][128 x 64 bf16, swizzled]
@@ -75,6 +76,8 @@ struct GemmArgs {
   int out_KB;              // k-blocks per row tile of that image
   const float* out_scale;  // EPI_RESID: the consumer's RMSNorm weight (applied before cutting) or nullptr
   float* ssq_out;          // EPI_RESID: [M][out_KB] sum of the new u^2 over this tile's 64 columns
+  const float* bias;       // EPI_STORE (or nullptr), EPI_FFN1: [NT*64] added to the result.  EPI_FFN1 (the paper's block,
+                           // Alg. 1 l.4) then applies GELU and writes only the image of the hidden layer (out_img, out_KB)
 #ifdef BOA_TC_TRACE
   long long* trace;        // [gridDim.x*gridDim.y][64] SM-clock timestamps (development builds only)
 #endif
@@ -246,6 +249,17 @@ __global__ void k_cut_rows(const float* __restrict__ X, int ldx, int M, int K, c
   cut4_store(img, K >> 6, m, k, v);
 }
 
+// Asynchronous global -> shared copies of single words (LDGSTS): the epilogue's prefetches, which must not hold registers.
+__device__ __forceinline__ void cp_async4(uint32_t dst, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
 template <int NPW>
 struct Cfg {
   static constexpr int W_BYTES = NPW * BN * 128;
@@ -254,7 +268,13 @@ struct Cfg {
   static constexpr int LDS = BN + 4;                          // staging row, padded: conflict-free column stores
   static constexpr int STILE_BYTES = BM * LDS * 4;
   static constexpr int NST = (3 * STAGE + STILE_BYTES <= 220 * 1024) ? 3 : 2;
-  static constexpr int SMEM = NST * STAGE + STILE_BYTES + 1024;   // + alignment slack
+  // epilogue prefetch area (cp.async, no registers): [NSQ][BM] block sums of u^2 of the next tile's rows, and
+  // [4][NEPI] float4 of conv-window values of a time-slab tile (three for the row group at t = 0, 1; one for t = 2)
+  static constexpr int NSQ = 8;
+  static constexpr int SQ_BYTES = NSQ * BM * 4;
+  static constexpr int PW_BYTES = 4 * 256 * 16;
+  static constexpr int SMEM = NST * STAGE + STILE_BYTES + 1024;                  // + alignment slack
+  static constexpr int SMEM_SLAB = SMEM + SQ_BYTES + PW_BYTES;                  // the time-slab form of in_proj
   static constexpr int NACC = NPW == 3 ? 3 : 2;               // accumulators (magnitude classes)
   static constexpr int ACC_COLS = NACC * BN;                  // TMEM columns of one accumulator buffer
   static constexpr int TMEM_COLS = (2 * ACC_COLS <= 256) ? 256 : 512;   // two buffers
@@ -262,6 +282,9 @@ struct Cfg {
 
 // sigmoid for the SiLU of the conv epilogue: fast forms (relative error ~1e-6; same code on encode and decode)
 __device__ __forceinline__ float sigmoid_tc(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
+
+// GELU(v) = v Phi(v), erf form (R#23); erff is within a few ulp, the same code on encode and decode
+__device__ __forceinline__ float gelu_tc(float v) { return 0.5f * v * (1.0f + erff(v * 0.70710678118654752440f)); }
 
 // Offset (without the row term row*ldc) of in_proj output n (x half: n < E, z half: n >= E) in the sliced xz layout.
 __host__ __device__ inline size_t xz_col(int n, int E, int EC, size_t slice_stride) {
@@ -290,7 +313,10 @@ constexpr int NTHREADS = NEPI + 64;
 // CS > 1: the kernel is launched in clusters of CS CTAs that take CS consecutive column tiles of the same row tile in
 // lock-step and share its activation k-blocks: each CTA fetches 1/CS of the 48 KB block and the bulk copy delivers
 // it to all of them (multicast); a stage is reused when the MMAs of ALL CTAs of the cluster have read it.
-template <int NPW, int EPI, int CS>
+// SLAB (EPI_INPROJ with g.slab_T > 0 only): the time-slab form of the conv epilogue, whose tiles are epilogue-bound;
+// it fetches what the epilogue reads from global memory (block sums of u^2, window values) ahead of time with
+// cp.async into shared memory.  The step form (SLAB = false) is bound by its main loop and reads them directly.
+template <int NPW, int EPI, int CS, bool SLAB = false>
 __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   using C = Cfg<NPW>;
   static_assert(NPW == 1 || NPW == 3, "weight pieces");
@@ -405,7 +431,29 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     constexpr int RPI = 32 / LPR;                  // rows per warp instruction
     constexpr int NIT = BM / (8 * RPI);            // row groups per warp
     const int col = (lane % LPR) * 4;
+    static_assert(NIT == 8 && RPI == 2, "slab_row below assumes 128 x 64 tiles");
     int it = 0;
+    const int r1 = (warp & 3) * 32 + lane;         // pass 1: thread = stream row
+    // S2: the block sums of u^2 of this thread's row (the first 8 of them) are fetched one tile ahead, all loads in
+    // flight together, and summed in ascending order when the tile starts (absent blocks read as 0: x + 0 = x).
+    constexpr int NSQ = C::NSQ;
+    float* sqs = stile + BM * LDS;                 // [NSQ][BM]
+    float4* pws = reinterpret_cast<float4*>(sqs + NSQ * BM);   // [4][NEPI]
+    auto fetch_sq = [&](int tile) {                // by warps 0-3 (one thread per row); read by all after a barrier
+      if (warp < 4) {
+        const int mt = (tile / KS) / NTI;
+        const float* sp = g.ssq_in + (size_t)min(mt * BM + r1, g.M - 1) * g.KB;
+#pragma unroll
+        for (int q = 0; q < NSQ; ++q)
+          if (q < g.KB) cp_async4(smem_u32(sqs + q * BM + r1), sp + q);
+      }
+      cp_async_commit();
+    };
+    if (SLAB) {
+      if (item0 < ntiles) fetch_sq(item0);
+      cp_async_wait<0>();
+      asm volatile("bar.sync 1, 256;" ::: "memory");
+    }
     for (int tile = item0; tile < ntiles; tile += item_step, ++it) {
       const int b = it & 1;
       const int ks = tile % KS, t2 = tile / KS, mt = t2 / NTI, nt = (t2 - mt * NTI) * CS + crank;
@@ -414,12 +462,18 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       // Pass 1: TMEM -> registers (thread = stream row; warps w and w+4 share the 32 TMEM lanes of rows 32*(w%4)..
       // and take one 32-column half each) -> shared staging tile, so that pass 2 can run with lane = column and
       // every global access coalesced.
-      const int r1 = (warp & 3) * 32 + lane;
       float rs = 1.0f;
       if (EPI == EPI_INPROJ) {                     // S2: RMSNorm row scale from the block sums of u^2, ascending
         const float* sp = g.ssq_in + (size_t)min(m0 + r1, g.M - 1) * g.KB;
         float ss = 0.0f;
-        for (int q = 0; q < g.KB; ++q) ss += sp[q];
+        if (SLAB) {
+#pragma unroll
+          for (int q = 0; q < NSQ; ++q)
+            if (q < g.KB) ss += sqs[q * BM + r1];
+          for (int q = NSQ; q < g.KB; ++q) ss += sp[q];
+        } else {
+          for (int q = 0; q < g.KB; ++q) ss += sp[q];
+        }
         rs = 1.0f / sqrtf(ss / (float)(g.KB * BK) + kEps);
       }
       // The conv window of the first row batch does not depend on the accumulators: its loads (from HBM at large B)
@@ -427,7 +481,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       const int nb = n0 + col;
       const size_t ncol = (EPI == EPI_INPROJ && g.xz_ec > 0) ? xz_col(nb, g.E, g.xz_ec, g.xz_slice) : (size_t)nb;   // offset of the stored result in its row
       const bool conv_tile = EPI == EPI_INPROJ && n0 < g.E;
-      const bool slab_tile = conv_tile && g.slab_T > 0;
+      const bool slab_tile = SLAB && conv_tile;
       float4 w0[4], w1[4], w2[4];
       int slot[4];                                 // ring slot of x_{t-3} (and of x_t after this step)
       if (conv_tile && !slab_tile) {
@@ -442,6 +496,35 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
           w2[u] = *reinterpret_cast<const float4*>(wp + ((slot[u] + 2) % 3) * g.E);
         }
       }
+      // Time slab: row group i of a warp is rows 16 i + ((2 warp + 2 i) mod 16) + {0, 1}, so every warp meets every step
+      // t of a 16-step slab once and the rows that read the window (t < 3) are spread evenly over the warps.  Their
+      // window loads (at most two row groups per warp when T = 16) are issued here too.
+      auto slab_row = [&](int i) { return 16 * i + ((2 * warp + 2 * i) & 15) + lane / LPR; };
+      int ia = -1, ib = -1;                        // row groups whose window values sit in pws[0..2] / pws[3]
+      if (slab_tile) {
+        const int T = g.slab_T;
+#pragma unroll
+        for (int i = 0; i < NIT; ++i) {
+          const int rc = min(m0 + slab_row(i), g.M - 1);
+          const int si = rc / T, t = rc - si * T;
+          // (decided per warp so that ia, ib are uniform: the two rows of a group are t and t + 1)
+          if (__any_sync(0xffffffffu, t < 3)) {
+            const bool only3 = __all_sync(0xffffffffu, t >= 2);      // only x_{t-3} comes from the window
+            const int use = (only3 && ib < 0) ? 1 : (ia < 0) ? 0 : -1;
+            if (use >= 0) {
+              const uint32_t p0 = g.pos[si];
+              const float* wp = g.win + (size_t)si * 3 * g.E + nb;
+#pragma unroll
+              for (int j = 1; j <= 3; ++j)
+                if (t < j && (use == 0 || j == 3))
+                  cp_async16(smem_u32(pws + (use == 0 ? j - 1 : 3) * NEPI + tid),
+                             wp + ((p0 + 3u + (uint32_t)t - (uint32_t)j) % 3u) * g.E);
+              if (use == 0) ia = i; else ib = i;
+            }
+          }
+        }
+      }
+      if (SLAB) cp_async_commit();
       mbar_wait(smem_u32(&acc_full[b]), (uint32_t)((it >> 1) & 1));
       tc_fence_after();
       if (tid == 0 && it < 8) TC_TRACE(24 + it);
@@ -465,6 +548,10 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
                                     (v[j + 3] + w[j + 3]) * rs);
       }
       asm volatile("bar.sync 1, 256;" ::: "memory");
+      if (SLAB) {
+        if (tile + item_step < ntiles) fetch_sq(tile + item_step); else cp_async_commit();   // flies during pass 2
+        cp_async_wait<1>();                        // this tile's window values have landed (own thread's only)
+      }
       // Pass 2: 16 lanes own one 64-column row segment (4 consecutive columns per lane), two rows per warp
       // instruction; rows are processed four at a time with all loads issued first.
       if (slab_tile) {
@@ -476,18 +563,20 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
         const int T = g.slab_T;
 #pragma unroll
         for (int i = 0; i < NIT; ++i) {
-          const int r = (warp + 8 * i) * RPI + lane / LPR;
+          const int r = slab_row(i);
           const int row = m0 + r;
           const int rc = min(row, g.M - 1);
           const int si = rc / T, t = rc - si * T;                 // stream and step of the row
           const float4 x = *reinterpret_cast<const float4*>(stile + r * LDS + col);
           float4 xm[3];                                           // x_{t-1}, x_{t-2}, x_{t-3}
-          const uint32_t p0 = g.pos[si];
-          const float* wp = g.win + (size_t)si * 3 * g.E + nb;
 #pragma unroll
-          for (int j = 1; j <= 3; ++j)
-            xm[j - 1] = (t >= j) ? *reinterpret_cast<const float4*>(stile + (r - j) * LDS + col)
-                                 : *reinterpret_cast<const float4*>(wp + ((p0 + 3u + (uint32_t)t - (uint32_t)j) % 3u) * g.E);
+          for (int j = 1; j <= 3; ++j) {
+            if (t >= j) xm[j - 1] = *reinterpret_cast<const float4*>(stile + (r - j) * LDS + col);
+            else if (i == ia) xm[j - 1] = pws[(j - 1) * NEPI + tid];
+            else if (i == ib) xm[j - 1] = pws[3 * NEPI + tid];
+            else xm[j - 1] = *reinterpret_cast<const float4*>(g.win + (size_t)si * 3 * g.E + nb +
+                                                              ((g.pos[si] + 3u + (uint32_t)t - (uint32_t)j) % 3u) * g.E);
+          }
           if (row < g.M) {
             float4 o;
             o.x = conv_silu1(cw0, cb.x, xm[2].x, xm[1].x, xm[0].x, x.x);
@@ -501,7 +590,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
         asm volatile("bar.sync 1, 256;" ::: "memory");     // every row has read the window
 #pragma unroll
         for (int i = 0; i < NIT; ++i) {                      // x_t of the last three steps -> ring slot (pos + t) % 3
-          const int r = (warp + 8 * i) * RPI + lane / LPR;
+          const int r = slab_row(i);
           const int row = m0 + r;
           const int si = row / T, t = row - si * T;
           if (row < g.M && t >= T - 3)
@@ -557,6 +646,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
         float4 osc = make_float4(1.f, 1.f, 1.f, 1.f);
         if (EPI == EPI_RESID && g.out_scale) osc = *reinterpret_cast<const float4*>(g.out_scale + nb);
         const bool cols_ok = nb < g.n_valid;
+        float4 bs = make_float4(0.f, 0.f, 0.f, 0.f);
+        const bool has_bias = (EPI == EPI_STORE || EPI == EPI_FFN1) && g.bias != nullptr;
+        if (has_bias) bs = *reinterpret_cast<const float4*>(g.bias + nb);
 #pragma unroll 1
         for (int i0 = 0; i0 < NIT; i0 += 4) {
           float4 o[4], q[4];
@@ -585,10 +677,18 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
                 if ((lane % LPR) == 0) g.ssq_out[(size_t)rows[u] * g.out_KB + nt] = ss;
               }
             }
-            if (live) *reinterpret_cast<float4*>(Cout + (size_t)rows[u] * g.ldc + ncol) = o[u];
+            if (has_bias) { o[u].x += bs.x; o[u].y += bs.y; o[u].z += bs.z; o[u].w += bs.w; }
+            if (EPI == EPI_FFN1) {
+              if (live)
+                cut4_store(g.out_img, g.out_KB, rows[u], nb,
+                           make_float4(gelu_tc(o[u].x), gelu_tc(o[u].y), gelu_tc(o[u].z), gelu_tc(o[u].w)));
+            } else if (live) {
+              *reinterpret_cast<float4*>(Cout + (size_t)rows[u] * g.ldc + ncol) = o[u];
+            }
           }
         }
       }
+      if (SLAB) cp_async_wait<0>();                      // the next tile's block sums
       asm volatile("bar.sync 1, 256;" ::: "memory");     // the staging tile is free for the next tile
     }
     if (tid == 0) TC_TRACE(4);

@@ -39,6 +39,12 @@ def _cases():
         # the cfg4 / cfg5 model shapes (bf16 matrices): 4 layers at D = 256; D = 512, dt_rank 32, four scan slices
         "cfg4_shape_sharp": (synth.make_weights(synth.CONFIGS[4].shape, 2, synth.DTYPE_BF16, emb_std=0.25), s2),
         "cfg5_shape_l2_sharp": (synth.make_weights(synth.ModelShape(2, 512, dt_rank=32), 3, synth.DTYPE_BF16, emb_std=0.25), s2),
+        # SURVEY 8(f) NEXT-2, the paper's own block (Alg. 1 l.4): FFN + LayerNorm after every mixer.  The paper's
+        # shape (1 layer, D = 256, hidden 1024, untied head, fp32), and two layers with bf16 matrices, a tied head and
+        # a hidden width that is not a power of two
+        "paper_block_sharp": (synth.make_weights(synth.CONFIGS[6].shape, 4, emb_std=0.25, ffn_std=0.1), s2),
+        "paper_block_l2_d128_bf16_sharp": (synth.make_weights(synth.ModelShape(2, 128, dt_rank=8, d_ff=320), 9, synth.DTYPE_BF16,
+                                                              emb_std=0.25, ffn_std=0.1), s1),
     }
 
 
@@ -238,6 +244,12 @@ def test_errors(boa):
     assert code(lambda: gm.decompress_into(comp, dst[:100])) == boa.E_CAPACITY
     small = torch.empty(60, dtype=torch.uint8, device="cuda")
     assert code(lambda: gm.compress_into(torch.zeros(2000, dtype=torch.uint8, device="cuda"), 250, small)) == boa.E_CAPACITY
+    # BOAW header: the FFN flag and the hidden width must agree; unknown flag bits are refused
+    import struct
+    blob = bytearray(synth.make_weights(synth.ModelShape(1, 64, dt_rank=4, d_ff=64), 1))
+    for flags, d_ff in [(1, 64), (3, 0), (7, 64)]:
+        bad_blob = bytearray(blob); struct.pack_into("<2I", bad_blob, 36, flags, d_ff)
+        assert code(lambda: boa.Model(bytes(bad_blob))) == boa.E_FORMAT
     # payload corruption: either detected (BOA_E_CORRUPT) or decodes to different bytes, never a crash
     bad = comp.clone(); bad[-40:] = 0xFF
     try:
@@ -328,7 +340,8 @@ def test_time_slab_encoder_writes_the_bytes_of_the_step_path(boa):
     bit-identical to stepping one byte at a time - the decoder always steps - for ragged lengths around the slab size."""
     import os
     cfg = synth.CONFIGS[1]
-    for blob in (cfg.weights(emb_std=0.25), synth.make_weights(synth.CONFIGS[2].shape, 1, emb_std=0.25)):
+    for blob in (cfg.weights(emb_std=0.25), synth.make_weights(synth.CONFIGS[2].shape, 1, emb_std=0.25),
+                 synth.make_weights(synth.CONFIGS[6].shape, 4, emb_std=0.25, ffn_std=0.1)):
         gm = boa.Model(blob)
         for n, chunk in [(150 * 41 + 13, 41), (300 * 9, 9), (5 * 200 + 10, 200), (130 * 17, 17)]:
             data = cfg.data(n)
