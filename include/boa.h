@@ -95,6 +95,26 @@ int boa_decompressed_size(const uint8_t* in, size_t in_len, size_t* n);
 int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len,
                    uint8_t* out, size_t* out_len, void* cuda_stream);
 
+/* ---- streaming front end (PAPER Fig. 2) ------------------------------
+ * The input is cut into groups of `group_chunks` chunks; every group is compressed into one complete BOA1
+ * container (a shard) exactly as boa_compress would, and the shards are concatenated in `out`.  While the
+ * step kernels work on group k, a second CUDA stream pre-loads group k+1 from pinned host memory into the
+ * other device lane and brings shard k-1 back ("buffer / compress / pre-load", Fig. 2).
+ *   in, out      HOST pointers (device pointers: BOA_E_ARG); out_len = capacity on entry, bytes written on return;
+ *                boa_stream_bound(n, chunk_bytes, group_chunks) is always enough
+ *   shard_len    NULL, or HOST array receiving the byte length of every shard; *n_shards = its capacity on
+ *                entry (BOA_E_CAPACITY if < ceil(n / (chunk_bytes * group_chunks))), the shard count on return
+ * boa_stream_decompress walks the concatenated shards (each validated like boa_decompress: header, index
+ * CRC, fingerprint) with the same two-lane overlap and writes the original bytes; boa_stream_decompressed_size
+ * reads only the headers and size indices (HOST pointer) and returns the total length and the shard count.
+ * Errors: those of boa_compress / boa_decompress; BOA_E_FORMAT if the buffer is not a whole number of shards. */
+size_t boa_stream_bound(size_t n, size_t chunk_bytes, size_t group_chunks);
+int boa_stream_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, size_t group_chunks,
+                        uint8_t* out, size_t* out_len, uint64_t* shard_len, size_t* n_shards, void* cuda_stream);
+int boa_stream_decompressed_size(const uint8_t* in, size_t in_len, size_t* n, size_t* n_shards);
+int boa_stream_decompress(boa_model* m, const uint8_t* in, size_t in_len, uint8_t* out, size_t* out_len,
+                          void* cuda_stream);
+
 const char* boa_strerror(int code);
 /* "file:line: cudaErrorName" of the last CUDA failure seen by the calling thread ("" if none).  Diagnostic only. */
 const char* boa_last_cuda_error(void);

@@ -87,6 +87,18 @@ def decompress(w: model.Weights, blob: bytes) -> bytes:
     return out.tobytes()
 
 
+def stream_compress(w: model.Weights, data: bytes, chunk_bytes: int, group_chunks: int) -> list:
+    """Streaming pipeline (PAPER Fig. 2): the distributor cuts the sequence into groups of `group_chunks`
+    fixed-size chunks and every group is compressed into its own shard (a complete container).  Returns the shards
+    in order; the stream is their concatenation."""
+    g = chunk_bytes * group_chunks
+    return [compress(w, data[o: o + g], chunk_bytes) for o in range(0, len(data), g)]
+
+
+def stream_decompress(w: model.Weights, blob: bytes) -> bytes:
+    return b"".join(decompress(w, s) for s in container.split_shards(blob))
+
+
 def probabilities(w: model.Weights, chunks: np.ndarray) -> np.ndarray:
     """eq. 6 on the oracle's logits: chunks [S,T] -> p [S,T-1,256] (fp64)."""
     return quantise.softmax(model.logits_for_chunks(w, chunks))

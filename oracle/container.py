@@ -72,3 +72,25 @@ def unpack(buf: bytes, fingerprint: int | None = None):
         payloads.append(bytes(buf[off: off + s]))
         off += s
     return n, cb, last, first, payloads
+
+
+def split_shards(buf: bytes) -> list:
+    """Streaming output (PAPER Fig. 2): a concatenation of complete containers, one per group of chunks.
+    Returns the shards; each one's length follows from its own header and size index.  Raises FormatError."""
+    shards, off = [], 0
+    while off < len(buf):
+        if len(buf) - off < HEADER_BYTES + 4:
+            raise FormatError("truncated shard header")
+        magic, _ver, _n, _cb, _last, nc, _fb, _fp = struct.unpack_from("<4sIQIIIIQ", buf, off)
+        if magic != MAGIC:
+            raise FormatError("bad shard magic")
+        ib = index_bytes(nc)
+        if len(buf) - off < ib:
+            raise FormatError("truncated shard index")
+        sizes = struct.unpack_from(f"<{nc}I", buf, off + HEADER_BYTES + nc + ((-nc) % 4))
+        total = ib + sum(sizes)
+        if total > len(buf) - off:
+            raise FormatError("truncated shard payload")
+        shards.append(bytes(buf[off: off + total]))
+        off += total
+    return shards

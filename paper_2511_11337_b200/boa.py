@@ -20,7 +20,8 @@ K_NAMES = ("embed", "inproj", "convx", "scan", "outproj", "head", "coder", "fini
 K_COUNT = len(K_NAMES)
 
 EXPORTS = ("boa_model_load", "boa_model_free", "boa_model_fingerprint", "boa_compress_bound", "boa_compress",
-           "boa_decompressed_size", "boa_decompress", "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",
+           "boa_decompressed_size", "boa_decompress", "boa_stream_bound", "boa_stream_compress",
+           "boa_stream_decompressed_size", "boa_stream_decompress", "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",
            "boa_debug_gemm", "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
 
 
@@ -66,6 +67,14 @@ def lib() -> C.CDLL:
     l.boa_decompressed_size.restype = C.c_int
     l.boa_decompress.argtypes = [vp, u8p, sz, u8p, C.POINTER(sz), vp]
     l.boa_decompress.restype = C.c_int
+    l.boa_stream_bound.argtypes = [sz, sz, sz]
+    l.boa_stream_bound.restype = sz
+    l.boa_stream_compress.argtypes = [vp, u8p, sz, sz, sz, u8p, C.POINTER(sz), vp, C.POINTER(sz), vp]
+    l.boa_stream_compress.restype = C.c_int
+    l.boa_stream_decompressed_size.argtypes = [u8p, sz, C.POINTER(sz), C.POINTER(sz)]
+    l.boa_stream_decompressed_size.restype = C.c_int
+    l.boa_stream_decompress.argtypes = [vp, u8p, sz, u8p, C.POINTER(sz), vp]
+    l.boa_stream_decompress.restype = C.c_int
     l.boa_strerror.argtypes = [C.c_int]
     l.boa_strerror.restype = C.c_char_p
     l.boa_last_cuda_error.argtypes = []
@@ -180,6 +189,29 @@ class Model:
         self.decompress_into(src, dst)
         return dst
 
+    # -- streaming front end (Fig. 2): host buffers in, concatenated shards out --------------------------
+    def stream_compress(self, data, chunk_bytes: int, group_chunks: int):
+        """boa_stream_compress: returns (CPU uint8 tensor of the concatenated shards, list of shard lengths)."""
+        src = as_u8(data)
+        dst = torch.empty(stream_bound(src.numel(), chunk_bytes, group_chunks), dtype=torch.uint8)
+        groups = -(-src.numel() // (chunk_bytes * group_chunks)) if src.numel() else 0
+        lens = (C.c_uint64 * max(groups, 1))()
+        n, ns = C.c_size_t(dst.numel()), C.c_size_t(groups)
+        _check(lib().boa_stream_compress(self._h, _ptr(src), src.numel(), chunk_bytes, group_chunks, _ptr(dst), C.byref(n),
+                                         C.cast(lens, C.c_void_p), C.byref(ns), _stream()), "boa_stream_compress")
+        return dst[: n.value], [int(lens[i]) for i in range(ns.value)]
+
+    def stream_decompress(self, blob) -> torch.Tensor:
+        src = as_u8(blob)
+        total, ns = C.c_size_t(0), C.c_size_t(0)
+        _check(lib().boa_stream_decompressed_size(_ptr(src), src.numel(), C.byref(total), C.byref(ns)),
+               "boa_stream_decompressed_size")
+        dst = torch.empty(total.value, dtype=torch.uint8)
+        n = C.c_size_t(dst.numel())
+        _check(lib().boa_stream_decompress(self._h, _ptr(src), src.numel(), _ptr(dst) or 0, C.byref(n), _stream()),
+               "boa_stream_decompress")
+        return dst
+
     # -- test-only -----------------------------------------------------------------------------------
     def debug_step_dump(self, data, chunk_bytes: int, n_steps: int, want=("logits", "probs", "cdf"), device="cuda"):
         src = as_u8(data, device)
@@ -195,6 +227,10 @@ class Model:
                                          _ptr(out.get("probs")), _ptr(out.get("cdf")), _stream()), "boa_debug_step_dump")
         b = src.numel() // chunk_bytes
         return {k: v.view(b, n_steps, -1) for k, v in out.items()}
+
+
+def stream_bound(n: int, chunk_bytes: int, group_chunks: int) -> int:
+    return lib().boa_stream_bound(n, chunk_bytes, group_chunks)
 
 
 def compress_bound(n: int, chunk_bytes: int) -> int:

@@ -353,3 +353,42 @@ def test_time_slab_encoder_writes_the_bytes_of_the_step_path(boa):
                 del os.environ["BOA_NO_SLAB"]
             assert a == b, (n, chunk)
             assert _np(gm.decompress(torch.frombuffer(bytearray(a), dtype=torch.uint8).cuda())).tobytes() == data
+
+
+def test_streaming_front_end(boa):
+    """Fig. 2: groups of chunks -> concatenated shards through the two-lane
+    pre-load / compress / collect pipeline.  Every shard must be the bytes boa_compress writes for its group alone, the
+    stream must round-trip, parse with the oracle's reader, and match the oracle's stream size within 0.5 %."""
+    cfg = synth.CONFIGS[1]
+    blob = cfg.weights(emb_std=0.25)
+    gm, w = boa.Model(blob), model.load_weights(blob)
+    chunk, group = 100, 3
+    data = cfg.data(10 * chunk + 37)                               # 11 chunks: groups of 3, 3, 3, 2 (ragged tail)
+    stream, lens = gm.stream_compress(data, chunk, group)
+    assert stream.device.type == "cpu" and len(lens) == 4 and sum(lens) == stream.numel()
+    assert stream.numel() <= boa.stream_bound(len(data), chunk, group)
+    raw = _np(stream).tobytes()
+    shards = container.split_shards(raw)
+    assert [len(s) for s in shards] == lens
+    for k, s in enumerate(shards):
+        part = data[k * chunk * group:(k + 1) * chunk * group]
+        assert s == _np(gm.compress(part, chunk)).tobytes(), k
+        assert container.unpack(s, gm.fingerprint)[0] == len(part)
+    assert _np(gm.stream_decompress(stream)).tobytes() == data
+    ref = b"".join(codec.stream_compress(w, data, chunk, group))
+    assert abs(len(raw) - len(ref)) <= SIZE_TOL * len(ref)
+    # many groups (both lanes reused several times), one group, empty input
+    data = cfg.data(64 * 40)
+    for group in (1, 5, 64, 1000):
+        s2, l2 = gm.stream_compress(data, 40, group)
+        assert len(l2) == -(-64 // group) and _np(gm.stream_decompress(s2)).tobytes() == data
+    s0, l0 = gm.stream_compress(b"", 40, 4)
+    assert s0.numel() == 0 and l0 == [] and gm.stream_decompress(s0).numel() == 0
+    # errors: a cut stream, a stream from another model
+    with pytest.raises(boa.BoaError) as e:
+        gm.stream_decompress(stream[:-5])
+    assert e.value.code == boa.E_FORMAT
+    with pytest.raises(boa.BoaError) as e:
+        boa.Model(cfg.weights()).stream_decompress(stream)
+    assert e.value.code == boa.E_MODEL_MISMATCH
+

@@ -78,6 +78,40 @@ def test_edge_cases():
         codec.decompress(other, codec.compress(w, b"hello world", 4))
 
 
+def test_streaming_shards_by_hand():
+    """Fig. 2: groups of chunks become independent shards.  Pinned by hand-assembled bytes: the shard
+    boundaries are where the groups end, each shard is a container of its own group, and the chunks of a group do not
+    depend on other groups (streams are independent), so a shard equals the container of the group alone."""
+    cfg = synth.CONFIGS[1]
+    w = model.load_weights(cfg.weights(emb_std=0.25))
+    data = cfg.data(5 * 12 + 7)                       # chunks of 12 bytes, groups of 2 chunks: 3 groups, ragged tail
+    shards = codec.stream_compress(w, data, 12, 2)
+    assert len(shards) == 3
+    for k, s in enumerate(shards):
+        n, cb, last, first, payloads = container.unpack(s, codec.fingerprint(w))
+        part = data[24 * k: 24 * (k + 1)]
+        assert (n, cb) == (len(part), 12) and first == bytes(part[i] for i in range(0, len(part), 12))
+        assert len(payloads) == -(-len(part) // 12) and last == len(part) - 12 * (len(payloads) - 1)
+    # hand-split of the concatenation at the lengths the indices give
+    blob = b"".join(shards)
+    cut, off = [], 0
+    for s in shards:
+        nc = struct.unpack_from("<I", blob, off + 24)[0]          # header field n_chunks
+        sizes = struct.unpack_from(f"<{nc}I", blob, off + 40 + nc + (-nc) % 4)
+        ln = 40 + nc + (-nc) % 4 + 4 * nc + 4 + sum(sizes)
+        cut.append(blob[off: off + ln]); off += ln
+    assert off == len(blob) and cut == shards == container.split_shards(blob)
+    assert codec.stream_decompress(w, blob) == data
+    # the payload of a chunk is the same whether its group or the whole input is compressed
+    whole = container.unpack(codec.compress(w, data, 12))[4]
+    assert [p for s in shards for p in container.unpack(s)[4]] == whole
+    assert codec.stream_compress(w, b"", 12, 2) == [] and codec.stream_decompress(w, b"") == b""
+    with pytest.raises(container.FormatError):
+        container.split_shards(blob[:-1])
+    with pytest.raises(container.FormatError):
+        container.split_shards(blob + b"BOA1")
+
+
 def test_table1_pins_the_ssr_formula():
     ok = 0
     for line in open(os.path.join(HERE, "golden", "table1.txt")):
