@@ -255,7 +255,7 @@ int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
   if (use_cluster() && g.NT % 2 == 0) {
     // clusters of two CTAs share the activation k-blocks of a row tile (multicast): persistent, one cluster per SM pair
     const int items = mt * (g.NT / 2) * g.KS;
-    cfg.gridDim = dim3(2 * std::min(items, n_sm / 2));
+    cfg.gridDim = dim3(2 * std::min(items, std::max(1, n_sm / 2)));
     at[1].id = cudaLaunchAttributeClusterDimension;
     at[1].val.clusterDim.x = 2; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
     cfg.numAttrs = 2;

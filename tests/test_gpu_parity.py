@@ -282,11 +282,13 @@ def test_more_chunks_than_one_wave(boa):
     assert _np(gm.decompress(comp)).tobytes() == data
 
 
-def test_full_size_cfg2_in_the_bench_configuration(boa):
+@pytest.mark.parametrize("config", [2, 6])
+def test_full_size_in_the_bench_configuration(boa, config):
     """BASELINE.json configs[1] at full size, exactly as bench.py runs it (64 MiB, 4096 chunks x 16 KiB, B = 4096 streams
     per step): byte-exact round trip of the whole input, and - on sampled streams the oracle can compute one by one -
-    probabilities within 1e-5 and tables bit-exact for the first steps of the same full-width launch."""
-    cfg = synth.CONFIGS[2]
+    probabilities within 1e-5 and tables bit-exact for the first steps of the same full-width launch.  Config 6 is the
+    paper's own block on the same input, as `bench.py --config 6` runs it."""
+    cfg = synth.CONFIGS[config]
     blob = cfg.weights()
     gm = boa.Model(blob)
     w = model.load_weights(blob)
@@ -302,7 +304,7 @@ def test_full_size_cfg2_in_the_bench_configuration(boa):
     ref = quantise.softmax(model.logits_for_chunks(w, buf[ids, :T]))
     got = _np(d["probs"][ids]).astype(np.float64)
     err = np.abs(got - ref).max()
-    print(f"[parity] cfg2 full size, streams {ids}: max |p_gpu - p_oracle| = {err:.3e}")
+    print(f"[parity] {cfg.name} full size, streams {ids}: max |p_gpu - p_oracle| = {err:.3e}")
     assert err <= PROB_TOL
     lg = _np(d["logits"][ids])
     assert np.array_equal(_np(d["cdf"][ids]).astype(np.int64).reshape(-1, 257), quantise.quantise(lg.reshape(-1, 256)))
