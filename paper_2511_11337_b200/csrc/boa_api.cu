@@ -24,7 +24,7 @@ using namespace boa;
 namespace {
 
 constexpr int kStepsPerGraph = 32;       // model steps captured into one CUDA graph launch
-constexpr int kSlabT = 16;               // steps per encode-side time slab
+constexpr int kSlabT = tc::SLAB_T;       // steps per encode-side time slab
 constexpr int kSlabsPerGraph = 4;        // slabs captured into one CUDA graph launch
 constexpr uint64_t kMaxWaveStreams = 65536;  // streams stepped together; more chunks run in waves
 

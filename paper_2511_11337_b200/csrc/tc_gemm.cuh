@@ -46,6 +46,7 @@ constexpr int NPA = 3;           // bf16 pieces of an activation
 constexpr int A_PLANE = BM * 128;  // bytes of one activation piece tile
 
 enum { EPI_STORE = 0, EPI_RESID = 1, EPI_INPROJ = 2, EPI_FFN1 = 3 };
+constexpr int SLAB_T = 16;       // steps per encode-side time slab in the slab form of in_proj (rows i*16 + t)
 
 struct GemmArgs {
   const uint8_t* A;        // activation image of A[M][K]: [ceil(M/128)][K/64][3 pieces][128 x 64 bf16, swizzled]
@@ -65,7 +66,7 @@ struct GemmArgs {
                            // producer of u in a fixed order); rstd = 1/sqrt(sum/K + eps) (R#10)
   float* win;              // [streams][3][E] conv window of this layer, a ring: at step t slot t%3 holds x_{t-3} and receives x_t
   const uint32_t* pos;     // [streams] steps taken so far by each stream (the coder's position) = t
-  int slab_T;              // 0: one row per stream.  T > 0 (encode-side time slab, 128 % T == 0): rows are stream-major,
+  int slab_T;              // 0: one row per stream.  T = SLAB_T (encode-side time slab, the SLAB instantiation): rows are stream-major,
                            // row i*T + t is step pos_i + t of stream i; the conv of a row reads the rows before it in the
                            // tile (the window only for t < 3) and the last three rows of a stream go into the window
   const float4* conv_w;    // [E] taps (x = t-3 ... w = t)
@@ -496,31 +497,24 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
           w2[u] = *reinterpret_cast<const float4*>(wp + ((slot[u] + 2) % 3) * g.E);
         }
       }
-      // Time slab: row group i of a warp is rows 16 i + ((2 warp + 2 i) mod 16) + {0, 1}, so every warp meets every step
-      // t of a 16-step slab once and the rows that read the window (t < 3) are spread evenly over the warps.  Their
-      // window loads (at most two row groups per warp when T = 16) are issued here too.
-      auto slab_row = [&](int i) { return 16 * i + ((2 * warp + 2 * i) & 15) + lane / LPR; };
-      int ia = -1, ib = -1;                        // row groups whose window values sit in pws[0..2] / pws[3]
+      // Time slab (T = SLAB_T = 16 steps, rows i*16 + t, tiles start at a multiple of 16): row group i of a warp is rows
+      // 16 i + g0 + {0, 1} with g0 = (2 warp + 2 i) mod 16, so every warp meets every step t of a slab once and the
+      // rows that read the window (t < 3: the groups g0 = 0 and g0 = 2) are spread evenly over the warps.  Their window
+      // values are fetched here, into pws[0..2] (g0 = 0: x_{t-1}, x_{t-2}, x_{t-3}) and pws[3] (g0 = 2, t = 2: x_{t-3}).
+      auto slab_g0 = [&](int i) { return (2 * warp + 2 * i) & 15; };
+      auto slab_row = [&](int i) { return 16 * i + slab_g0(i) + lane / LPR; };
       if (slab_tile) {
-        const int T = g.slab_T;
 #pragma unroll
         for (int i = 0; i < NIT; ++i) {
-          const int rc = min(m0 + slab_row(i), g.M - 1);
-          const int si = rc / T, t = rc - si * T;
-          // (decided per warp so that ia, ib are uniform: the two rows of a group are t and t + 1)
-          if (__any_sync(0xffffffffu, t < 3)) {
-            const bool only3 = __all_sync(0xffffffffu, t >= 2);      // only x_{t-3} comes from the window
-            const int use = (only3 && ib < 0) ? 1 : (ia < 0) ? 0 : -1;
-            if (use >= 0) {
-              const uint32_t p0 = g.pos[si];
-              const float* wp = g.win + (size_t)si * 3 * g.E + nb;
+          const int g0 = slab_g0(i);
+          if (g0 <= 2) {                           // warp-uniform
+            const int si = min(m0 + slab_row(i), g.M - 1) / SLAB_T, t = g0 + lane / LPR;
+            const uint32_t p0 = g.pos[si];
+            const float* wp = g.win + (size_t)si * 3 * g.E + nb;
 #pragma unroll
-              for (int j = 1; j <= 3; ++j)
-                if (t < j && (use == 0 || j == 3))
-                  cp_async16(smem_u32(pws + (use == 0 ? j - 1 : 3) * NEPI + tid),
-                             wp + ((p0 + 3u + (uint32_t)t - (uint32_t)j) % 3u) * g.E);
-              if (use == 0) ia = i; else ib = i;
-            }
+            for (int j = 1; j <= 3; ++j)
+              if (t < j) cp_async16(smem_u32(pws + (g0 == 0 ? j - 1 : 3) * NEPI + tid),
+                                    wp + ((p0 + 3u + (uint32_t)t - (uint32_t)j) % 3u) * g.E);
           }
         }
       }
@@ -560,23 +554,16 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
         // slab) and the last three go into it - after a barrier, when every row of the tile has read it.
         const float4 cw0 = g.conv_w[nb], cw1 = g.conv_w[nb + 1], cw2 = g.conv_w[nb + 2], cw3 = g.conv_w[nb + 3];
         const float4 cb = *reinterpret_cast<const float4*>(g.conv_b + nb);
-        const int T = g.slab_T;
 #pragma unroll
         for (int i = 0; i < NIT; ++i) {
-          const int r = slab_row(i);
-          const int row = m0 + r;
-          const int rc = min(row, g.M - 1);
-          const int si = rc / T, t = rc - si * T;                 // stream and step of the row
+          const int g0 = slab_g0(i);
+          const int r = slab_row(i), row = m0 + r, t = g0 + lane / LPR;   // step of the row within its slab
           const float4 x = *reinterpret_cast<const float4*>(stile + r * LDS + col);
           float4 xm[3];                                           // x_{t-1}, x_{t-2}, x_{t-3}
 #pragma unroll
-          for (int j = 1; j <= 3; ++j) {
-            if (t >= j) xm[j - 1] = *reinterpret_cast<const float4*>(stile + (r - j) * LDS + col);
-            else if (i == ia) xm[j - 1] = pws[(j - 1) * NEPI + tid];
-            else if (i == ib) xm[j - 1] = pws[3 * NEPI + tid];
-            else xm[j - 1] = *reinterpret_cast<const float4*>(g.win + (size_t)si * 3 * g.E + nb +
-                                                              ((g.pos[si] + 3u + (uint32_t)t - (uint32_t)j) % 3u) * g.E);
-          }
+          for (int j = 1; j <= 3; ++j)
+            xm[j - 1] = (t >= j) ? *reinterpret_cast<const float4*>(stile + (r - j) * LDS + col)
+                                 : pws[(g0 == 0 ? j - 1 : 3) * NEPI + tid];
           if (row < g.M) {
             float4 o;
             o.x = conv_silu1(cw0, cb.x, xm[2].x, xm[1].x, xm[0].x, x.x);
@@ -590,12 +577,13 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
         asm volatile("bar.sync 1, 256;" ::: "memory");     // every row has read the window
 #pragma unroll
         for (int i = 0; i < NIT; ++i) {                      // x_t of the last three steps -> ring slot (pos + t) % 3
-          const int r = slab_row(i);
-          const int row = m0 + r;
-          const int si = row / T, t = row - si * T;
-          if (row < g.M && t >= T - 3)
-            *reinterpret_cast<float4*>(g.win + ((size_t)si * 3 + (g.pos[si] + (uint32_t)t) % 3u) * g.E + nb) =
-                *reinterpret_cast<const float4*>(stile + r * LDS + col);
+          const int g0 = slab_g0(i);
+          if (g0 >= 12) {                                    // warp-uniform
+            const int r = slab_row(i), row = m0 + r, t = g0 + lane / LPR, si = row / SLAB_T;
+            if (row < g.M && t >= SLAB_T - 3)
+              *reinterpret_cast<float4*>(g.win + ((size_t)si * 3 + (g.pos[si] + (uint32_t)t) % 3u) * g.E + nb) =
+                  *reinterpret_cast<const float4*>(stile + r * LDS + col);
+          }
         }
       } else if (conv_tile) {
         // S4: causal depthwise conv over (x_{t-3}, x_{t-2}, x_{t-1}, x_t) + SiLU (R#11).  The window is a ring of three
