@@ -35,6 +35,28 @@ def test_host_only_entry_points(boa):
     assert lib.boa_decompressed_size(ctypes.cast(buf, ctypes.c_void_p), 64, ctypes.byref(n)) == boa.E_FORMAT
 
 
+def test_streaming_host_only_entry_points(boa):
+    """boa_stream_bound and boa_stream_decompressed_size work on host memory only (Fig. 2 shards)."""
+    import struct
+    import zlib
+    lib = boa.lib()
+    # 10 bytes in chunks of 4, groups of 2 chunks: shards of 8 and 2 bytes
+    assert boa.stream_bound(10, 4, 2) == boa.compress_bound(8, 4) + boa.compress_bound(2, 4)
+    assert boa.stream_bound(16, 4, 2) == 2 * boa.compress_bound(8, 4) and boa.stream_bound(0, 4, 2) == 0
+    # two hand-assembled shards (BOA1 header, first bytes, sizes, CRC, payload): 5 bytes in one chunk, then 1 byte
+    def shard(n, payload):
+        head = struct.pack("<4sIQIIIIQ", b"BOA1", 1, n, 8, n, 1, 16, 0x1234) + b"A\0\0\0" + struct.pack("<I", len(payload))
+        return head + struct.pack("<I", zlib.crc32(head) & 0xFFFFFFFF) + payload
+    blob = shard(5, b"\x01\x02\x03\x04\x05\x06") + shard(1, b"\0\0\0\0")
+    buf = ctypes.create_string_buffer(blob, len(blob))
+    n, ns = ctypes.c_size_t(), ctypes.c_size_t()
+    assert lib.boa_stream_decompressed_size(ctypes.cast(buf, ctypes.c_void_p), len(blob), ctypes.byref(n), ctypes.byref(ns)) == 0
+    assert (n.value, ns.value) == (6, 2)
+    assert lib.boa_stream_decompressed_size(ctypes.cast(buf, ctypes.c_void_p), len(blob) - 1, ctypes.byref(n), ctypes.byref(ns)) == boa.E_FORMAT
+    assert lib.boa_stream_decompressed_size(None, 0, ctypes.byref(n), ctypes.byref(ns)) == 0 and n.value == 0 and ns.value == 0
+    assert lib.boa_stream_compress(None, None, 0, 0, 0, None, None, None, None, None) == boa.E_ARG
+
+
 def test_model_load_rejects_bad_blobs_before_touching_the_gpu(boa):
     with pytest.raises(boa.BoaError) as e:
         boa.Model(b"NOPE" + b"\0" * 100)
