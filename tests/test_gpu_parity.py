@@ -45,6 +45,11 @@ def _cases():
         "paper_block_sharp": (synth.make_weights(synth.CONFIGS[6].shape, 4, emb_std=0.25, ffn_std=0.1), s2),
         "paper_block_l2_d128_bf16_sharp": (synth.make_weights(synth.ModelShape(2, 128, dt_rank=8, d_ff=320), 9, synth.DTYPE_BF16,
                                                               emb_std=0.25, ffn_std=0.1), s1),
+        # the ends of k_layernorm's lane map: D = 64 (half a warp holds the row) and D = 512 (four float4 per lane)
+        "paper_block_d64_sharp": (synth.make_weights(synth.ModelShape(1, 64, dt_rank=4, d_ff=64, tied=False), 12,
+                                                     emb_std=0.25, ffn_std=0.1), s1),
+        "paper_block_d512_bf16_sharp": (synth.make_weights(synth.ModelShape(1, 512, dt_rank=32, d_ff=128), 13, synth.DTYPE_BF16,
+                                                           emb_std=0.25, ffn_std=0.1), s2),
     }
 
 
