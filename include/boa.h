@@ -74,7 +74,8 @@ uint64_t boa_model_fingerprint(const boa_model* m);
  * model is stepped on byte t and byte t+1 is range-coded with the resulting table (len-1 symbols),
  * all streams in lock-step.  Writes a BOA1 container to `out`.
  *   in        host|device pointer, n bytes (may be NULL iff n == 0)
- *   chunk_bytes  >= 1 and < 2^31
+ *   chunk_bytes  >= 1 and <= 2^30 (stream positions and the per-stream payload scratch, 2*chunk_bytes + 8, are
+ *             32-bit; boa_decompress rejects a header with a larger value as BOA_E_FORMAT)
  *   out       host|device pointer; *out_len = its capacity on entry, bytes written on return.
  *             boa_compress_bound(n, chunk_bytes) is always enough (f >= 1 with total 2^16 bounds a
  *             symbol at 16 bits: payload <= 2*(len-1) + 4 flush bytes).
@@ -166,6 +167,12 @@ int boa_get_profile(const boa_model* m, boa_profile* out);
  *   `weight_pieces` (1 or 3) bf16 pieces exactly as boa_model_load does; A is cut into its three pieces by the same
  *   device routine the step kernels use.  grid_ctas = 0 launches one persistent CTA per SM as the step does; a small
  *   positive value forces several tiles per CTA (the accumulator double-buffering path).  K % 64 == 0. */
+/* boa_debug_set_slab: enabled = 0 makes boa_compress step one byte at a time, exactly as boa_decompress must, instead
+ *   of advancing 16 bytes per pass over the stream state; the container bytes must not change (test).
+ * boa_debug_set_max_wave: streams > 0 caps the number of streams stepped together (more chunks then run in waves), as
+ *   a small free-memory budget would; 0 restores the default.  Results must not depend on it (test). */
+int boa_debug_set_slab(boa_model* m, int enabled);
+int boa_debug_set_max_wave(boa_model* m, size_t streams);
 int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N, int weight_pieces, int grid_ctas,
                    float* C, void* cuda_stream);
 int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, size_t n_steps,

@@ -22,7 +22,7 @@ K_COUNT = len(K_NAMES)
 EXPORTS = ("boa_model_load", "boa_model_free", "boa_model_fingerprint", "boa_compress_bound", "boa_compress",
            "boa_decompressed_size", "boa_decompress", "boa_stream_bound", "boa_stream_compress",
            "boa_stream_decompressed_size", "boa_stream_decompress", "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",
-           "boa_debug_gemm", "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
+           "boa_debug_set_slab", "boa_debug_set_max_wave", "boa_debug_gemm", "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
 
 
 class Profile(C.Structure):
@@ -83,6 +83,10 @@ def lib() -> C.CDLL:
     l.boa_set_profiling.restype = C.c_int
     l.boa_get_profile.argtypes = [vp, C.POINTER(Profile)]
     l.boa_get_profile.restype = C.c_int
+    l.boa_debug_set_slab.argtypes = [vp, C.c_int]
+    l.boa_debug_set_slab.restype = C.c_int
+    l.boa_debug_set_max_wave.argtypes = [vp, sz]
+    l.boa_debug_set_max_wave.restype = C.c_int
     l.boa_debug_gemm.argtypes = [vp, sz, sz, vp, sz, C.c_int, C.c_int, vp, vp]
     l.boa_debug_gemm.restype = C.c_int
     l.boa_debug_step_dump.argtypes = [vp, u8p, sz, sz, sz, vp, vp, vp, vp]
@@ -213,6 +217,12 @@ class Model:
         return dst
 
     # -- test-only -----------------------------------------------------------------------------------
+    def debug_set_slab(self, enabled: bool):
+        _check(lib().boa_debug_set_slab(self._h, 1 if enabled else 0), "boa_debug_set_slab")
+
+    def debug_set_max_wave(self, streams: int):
+        _check(lib().boa_debug_set_max_wave(self._h, streams), "boa_debug_set_max_wave")
+
     def debug_step_dump(self, data, chunk_bytes: int, n_steps: int, want=("logits", "probs", "cdf"), device="cuda"):
         src = as_u8(data, device)
         rows = (src.numel() // chunk_bytes) * n_steps

@@ -13,7 +13,10 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libboa.so")
 SOURCES = ["boa_api.cu", "boa_stream.cu"]
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+# -fmad=false: the kernels spell every fused multiply-add as fmaf and every separately rounded operation as
+# __fmul_rn / __fadd_rn; with contraction off the compiler cannot fuse a plain a*b+c differently in the slab and the
+# step instantiations of a shared helper, so encoder and decoder keep identical per-step arithmetic.
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-fmad=false",
               "-shared", "-Xcompiler", "-fPIC"]
 
 

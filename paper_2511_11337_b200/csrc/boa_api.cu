@@ -89,6 +89,10 @@ struct boa_model {
   cudaStream_t own = nullptr;
   cudaEvent_t user_ev = nullptr;
 
+  // test-only switches (boa_debug_set_slab / boa_debug_set_max_wave): results do not depend on them
+  bool use_slab = true;        // false: boa_compress steps one byte at a time like the decoder (same bytes)
+  uint64_t max_wave = 0;       // > 0: at most this many streams are stepped together (more chunks run in waves)
+
   // profiling
   int sample_every = 0;
   boa_profile prof{};
@@ -195,19 +199,6 @@ struct StepCtx {
   size_t ev_used = 0;
 };
 
-#ifdef BOA_DEV
-// development builds only: BOA_DEV_SKIP is a bit mask of kernel classes whose launches are skipped (timing experiments;
-// results are then wrong)
-inline unsigned dev_skip_mask() {
-  static int v = -1;
-  if (v < 0) { const char* e = getenv("BOA_DEV_SKIP"); v = e ? atoi(e) : 0; }
-  return (unsigned)v;
-}
-#define BOA_DEV_SKIPPED(cls) (dev_skip_mask() & (1u << (cls)))
-#else
-#define BOA_DEV_SKIPPED(cls) false
-#endif
-
 int mark(StepCtx& c, int cls) {
   ++c.launches;
   BOA_CUDA_TRY(cudaPeekAtLastError());
@@ -226,11 +217,6 @@ int mark(StepCtx& c, int cls) {
 // ---- tensor-core GEMM launch (tc_gemm.cuh).  The dynamic shared-memory opt-in is set once per instantiation.
 // Launch with the programmatic-serialization attribute (PDL, common.cuh): the kernel calls pdl_wait() before it
 // touches anything an earlier kernel of the stream wrote.
-// Debug switches, read once from the environment (results do not depend on them):
-//   BOA_NO_PDL=1      launch without the programmatic-serialization attribute
-//   BOA_NO_CLUSTER=1  launch the contraction kernels without 2-CTA clusters
-bool use_pdl() { static const bool v = getenv("BOA_NO_PDL") == nullptr; return v; }
-bool use_cluster() { static const bool v = getenv("BOA_NO_CLUSTER") == nullptr; return v; }
 template <typename... KArgs, typename... Args>
 cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t st, Args&&... args) {
   cudaLaunchConfig_t cfg{};
@@ -238,7 +224,7 @@ cudaError_t launch_pdl(void (*kernel)(KArgs...), dim3 grid, dim3 block, size_t s
   cudaLaunchAttribute at[1];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
-  cfg.attrs = at; cfg.numAttrs = use_pdl() ? 1 : 0;
+  cfg.attrs = at; cfg.numAttrs = 1;
   return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
 
@@ -250,9 +236,9 @@ int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
   cfg.blockDim = dim3(tc::NTHREADS); cfg.dynamicSmemBytes = SLAB ? C::SMEM_SLAB : C::SMEM; cfg.stream = st;
   cudaLaunchAttribute at[2];
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-  at[0].val.programmaticStreamSerializationAllowed = use_pdl() ? 1 : 0;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at; cfg.numAttrs = 1;
-  if (use_cluster() && g.NT % 2 == 0) {
+  if (g.NT % 2 == 0) {
     // clusters of two CTAs share the activation k-blocks of a row tile (multicast): persistent, one cluster per SM pair
     const int items = mt * (g.NT / 2) * g.KS;
     cfg.gridDim = dim3(2 * std::min(items, std::max(1, n_sm / 2)));
@@ -317,8 +303,9 @@ int launch_embed(StepCtx& c, int T = 1) {
 
 // One model step + one coder step for all B streams of the wave (S2-S14, and S1 of the next step).
 // With c.slab_T = T > 1 (encode-side time slab) the same kernels advance every stream by T steps:
-// the contractions run on B*T rows (row t*B + i), the conv walks over the T steps with the window in registers
-// (k_conv_slab), the scan keeps the state in registers across the T steps, the coder codes T symbols per stream.
+// the contractions run on B*T rows (stream-major: row i*T + t), the conv of a row reads the rows before it in its
+// tile (the slab form of in_proj's epilogue), the scan keeps the state in registers across the T steps
+// (k_scan_slab), the coder codes T symbols per stream (k_coder_slab).
 // Per row / per step the arithmetic is that of the step path, so the decoder (always step by step) reproduces it.
 int launch_step(StepCtx& c) {
   boa_model* m = c.m;
@@ -346,8 +333,7 @@ int launch_step(StepCtx& c) {
       g.xz_slice = T == 1 ? (size_t)2 * ec : (size_t)rows * 2 * ec;
       g.ssq_in = m->ssq.as<float>(); g.win = winl; g.pos = c.ca.pos; g.slab_T = T == 1 ? 0 : T; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
-      if (BOA_DEV_SKIPPED(BOA_K_INPROJ)) {
-      } else if (T > 1) {   // the time-slab form of the conv epilogue
+      if (T > 1) {   // the time-slab form of the conv epilogue
         BOA_TRY((m->npw == 1 ? launch_tc<1, tc::EPI_INPROJ, true>(g, m->n_sm, c.st) : launch_tc<3, tc::EPI_INPROJ, true>(g, m->n_sm, c.st)));
       } else {
         BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
@@ -359,7 +345,7 @@ int launch_step(StepCtx& c) {
       g.A = xs_img; g.M = rows; g.KB = E / 64; g.W = w.img_x; g.NT = m->ldj / 64;
       g.C = dbc; g.ldc = m->ks_x * m->ldj; g.n_valid = m->J;           // row = [k-split][ldj]
       g.KS = m->ks_x; g.split_stride = (size_t)m->ldj;                  // split over k: enough tiles to fill the SMs
-      if (!BOA_DEV_SKIPPED(BOA_K_CONVX)) BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
+      BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_CONVX));
     }
     {  // S6-S8: persistent, two CTAs per SM, each walking over streams for one channel slice
@@ -383,7 +369,7 @@ int launch_step(StepCtx& c) {
           case 32: BOA_CUDA_TRY(launch_pdl(k_scan_slab<32>, grid, dim3(ec + 32), smem, c.st, ss)); break;
           default: BOA_CUDA_TRY(launch_pdl(k_scan_slab<0>, grid, dim3(ec + 32), smem, c.st, ss)); break;
         }
-      } else if (!BOA_DEV_SKIPPED(BOA_K_SCAN))
+      } else
       switch (m->R) {   // W_dt's row in registers when it is short enough
         case 4: BOA_CUDA_TRY(launch_pdl(k_scan<4>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
         case 8: BOA_CUDA_TRY(launch_pdl(k_scan<8>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
@@ -400,7 +386,7 @@ int launch_step(StepCtx& c) {
       g.out_img = u_img; g.out_KB = D / 64; g.ssq_out = m->ssq.as<float>();
       // (the paper's block: the FFN reads u itself, not a normalised u)
       g.out_scale = (m->F == 0 && l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
-      if (!BOA_DEV_SKIPPED(BOA_K_OUTPROJ)) BOA_TRY((launch_tc_npw<tc::EPI_RESID>(m->npw, g, m->n_sm, c.st)));
+      BOA_TRY((launch_tc_npw<tc::EPI_RESID>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_OUTPROJ));
     }
     if (m->F > 0) {  // the paper's block (Alg. 1 l.4, R#23): u <- LayerNorm(W2 GELU(W1 u + b1) + b2)
@@ -431,7 +417,7 @@ int launch_step(StepCtx& c) {
     tc::GemmArgs g{};
     g.A = u_img; g.M = rows; g.KB = D / 64; g.W = m->img_head; g.NT = 4; g.KS = 1;
     g.C = logits; g.ldc = 256; g.n_valid = 256;
-    if (!BOA_DEV_SKIPPED(BOA_K_HEAD)) BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
+    BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
     BOA_TRY(mark(c, BOA_K_HEAD));
   }
 
@@ -639,11 +625,14 @@ int reset_state(boa_model* m, cudaStream_t st) {
   return BOA_OK;
 }
 
+// Per-stream payload scratch: f >= 1 of 2^16 bounds a symbol at 2 bytes, + 4 flush bytes.  chunk_bytes <= kMaxChunkBytes
+// (2^30) keeps this below 2^32.
 uint32_t stream_cap(size_t chunk_bytes) { return (uint32_t)round_up(2 * chunk_bytes + 8, 16); }
 
 uint64_t wave_streams(const boa_model* m, uint64_t nc, size_t cap, size_t rows_per_stream = 1) {
   size_t free_b = 0, total_b = 0;
   uint64_t w = std::min<uint64_t>(nc, kMaxWaveStreams);
+  if (m->max_wave) w = std::min(w, m->max_wave);
   if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) {
     // what the handle already holds can be reused
     const size_t held = m->Bcap * bytes_per_stream(m, m->scratch.cap / std::max<uint64_t>(m->Bcap, 1), 0) +
@@ -872,7 +861,7 @@ int boa_get_profile(const boa_model* m, boa_profile* out) {
 
 int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, uint8_t* out, size_t* out_len,
                  void* cuda_stream) {
-  if (!m || !out || !out_len || chunk_bytes == 0 || chunk_bytes >= (1ull << 31) || (n && !in)) return BOA_E_ARG;
+  if (!m || !out || !out_len || chunk_bytes == 0 || chunk_bytes > kMaxChunkBytes || (n && !in)) return BOA_E_ARG;
   cudaStream_t st;
   BOA_TRY(enter(m, cuda_stream, &st));
   const uint64_t nc = n_chunks_of(n, chunk_bytes);
@@ -905,7 +894,7 @@ int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, 
   const uint32_t cap = stream_cap(chunk_bytes);
   uint64_t launches = 0;
 
-  const bool slab = getenv("BOA_NO_SLAB") == nullptr && chunk_bytes > (size_t)kSlabT;   // BOA_NO_SLAB=1: step path only (same bytes)
+  const bool slab = m->use_slab && chunk_bytes > (size_t)kSlabT;
   const uint64_t W = nc ? wave_streams(m, nc, cap, slab ? kSlabT : 1) : 0;
   for (uint64_t c0 = 0; c0 < nc; c0 += W) {
     const uint64_t B = std::min(W, nc - c0);
@@ -1111,6 +1100,18 @@ struct TmpDev {   // device view of a user buffer for the debug entry points
   ~TmpDev() { if (owned && dev) cudaFree(dev); }
 };
 }  // namespace
+
+int boa_debug_set_slab(boa_model* m, int enabled) {
+  if (!m) return BOA_E_ARG;
+  m->use_slab = enabled != 0;
+  return BOA_OK;
+}
+
+int boa_debug_set_max_wave(boa_model* m, size_t streams) {
+  if (!m || streams > kMaxWaveStreams) return BOA_E_ARG;
+  m->max_wave = streams;
+  return BOA_OK;
+}
 
 int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, size_t n_steps,
                         float* logits, float* probs, uint32_t* cdf, void* cuda_stream) {

@@ -93,7 +93,7 @@ extern "C" size_t boa_stream_bound(size_t n, size_t chunk_bytes, size_t group_ch
 
 extern "C" int boa_stream_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, size_t group_chunks,
                                    uint8_t* out, size_t* out_len, uint64_t* shard_len, size_t* n_shards, void* cuda_stream) {
-  if (!m || !out_len || chunk_bytes == 0 || chunk_bytes >= (1ull << 31) || group_chunks == 0 || (n && (!in || !out)))
+  if (!m || !out_len || chunk_bytes == 0 || chunk_bytes > boa::kMaxChunkBytes || group_chunks == 0 || (n && (!in || !out)))
     return BOA_E_ARG;
   if (on_device(in) || on_device(out)) return BOA_E_ARG;     // the streaming entry points take host buffers
   const size_t group_bytes = chunk_bytes * group_chunks;

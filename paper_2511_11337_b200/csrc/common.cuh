@@ -18,7 +18,7 @@ constexpr float kEps = 1e-5f;        // RMSNorm epsilon (R#10)
 // are only reproducible with the same per-step floating-point arithmetic.
 // 'B2' + generation number.  Bump whenever any kernel upstream of the quantiser changes its
 // arithmetic (operation order, fusion, precision).
-constexpr uint32_t kArithVersion = 0x42320007u;
+constexpr uint32_t kArithVersion = 0x42320008u;
 
 // Programmatic dependent launch (PDL): a kernel launched with the programmatic-serialization attribute may start
 // while its predecessor in the stream is still draining; pdl_wait() blocks until the predecessor grid has completed

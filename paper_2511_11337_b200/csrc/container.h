@@ -18,20 +18,24 @@ namespace boa {
 
 constexpr size_t kHeaderBytes = 40;
 constexpr uint32_t kContainerVersion = 1;
+constexpr size_t kMaxChunkBytes = (size_t)1 << 30;   // encoder and decoder limit (per-stream scratch and positions are 32-bit)
 
-inline uint32_t crc32_ieee(const uint8_t* p, size_t n, uint32_t crc = 0) {
-  static uint32_t table[256];
-  static bool init = false;
-  if (!init) {
+struct Crc32Table {
+  uint32_t v[256];
+  constexpr Crc32Table() : v{} {
     for (uint32_t i = 0; i < 256; ++i) {
       uint32_t c = i;
       for (int k = 0; k < 8; ++k) c = (c & 1u) ? (0xEDB88320u ^ (c >> 1)) : (c >> 1);
-      table[i] = c;
+      v[i] = c;
     }
-    init = true;
   }
+};
+
+// built at compile time: different handles may run on different threads (boa.h)
+inline uint32_t crc32_ieee(const uint8_t* p, size_t n, uint32_t crc = 0) {
+  static constexpr Crc32Table table{};
   crc = ~crc;
-  for (size_t i = 0; i < n; ++i) crc = table[(crc ^ p[i]) & 0xFFu] ^ (crc >> 8);
+  for (size_t i = 0; i < n; ++i) crc = table.v[(crc ^ p[i]) & 0xFFu] ^ (crc >> 8);
   return ~crc;
 }
 
@@ -70,7 +74,7 @@ inline bool parse_header(const uint8_t* p, Header& h) {
   h.n_chunks = get_u32(p + 24);
   h.freq_bits = get_u32(p + 28);
   h.fingerprint = get_u64(p + 32);
-  if (h.freq_bits != 16 || h.chunk_bytes == 0) return false;
+  if (h.freq_bits != 16 || h.chunk_bytes == 0 || h.chunk_bytes > kMaxChunkBytes) return false;
   const uint64_t nc = n_chunks_of(h.n, h.chunk_bytes);
   if (nc != h.n_chunks) return false;
   if (nc ? (h.last_len != h.n - (nc - 1) * (uint64_t)h.chunk_bytes) : (h.last_len != 0)) return false;

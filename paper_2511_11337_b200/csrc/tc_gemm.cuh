@@ -79,16 +79,7 @@ struct GemmArgs {
   float* ssq_out;          // EPI_RESID: [M][out_KB] sum of the new u^2 over this tile's 64 columns
   const float* bias;       // EPI_STORE (or nullptr), EPI_FFN1: [NT*64] added to the result.  EPI_FFN1 (the paper's block,
                            // Alg. 1 l.4) then applies GELU and writes only the image of the hidden layer (out_img, out_KB)
-#ifdef BOA_TC_TRACE
-  long long* trace;        // [gridDim.x*gridDim.y][64] SM-clock timestamps (development builds only)
-#endif
 };
-
-#ifdef BOA_TC_TRACE
-#define TC_TRACE(slot) do { g.trace[(size_t)(blockIdx.y * gridDim.x + blockIdx.x) * 64 + (slot)] = clock64(); } while (0)
-#else
-#define TC_TRACE(slot) do { } while (0)
-#endif
 
 // ------------------------------------------------------------------------------------------ PTX wrappers
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -336,7 +327,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   const int crank = CS > 1 ? (int)cluster_ctarank() : 0;
   const int item0 = (int)blockIdx.x / CS, item_step = (int)gridDim.x / CS;
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
-  if (tid == 0) TC_TRACE(0);
 
   if (warp == 8) {
     if (lane == 0) {
@@ -358,7 +348,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   if (CS > 1) cluster_sync();                      // the peers' barriers are initialised before anything is sent to them
   tc_fence_after();
   const uint32_t tmem = tmem_base_s;
-  if (tid == 0) TC_TRACE(1);
   pdl_launch();
   pdl_wait();                                      // everything below reads what earlier kernels of the step wrote
 
@@ -421,7 +410,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
           else umma_commit(smem_u32(&empty_bar[s]));                 // stage free when these MMAs have read it
         }
         umma_commit(smem_u32(&acc_full[b]));                         // this tile's accumulators are complete
-        if (it < 8) TC_TRACE(8 + it);
       }
     }
   } else {
@@ -521,7 +509,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       if (SLAB) cp_async_commit();
       mbar_wait(smem_u32(&acc_full[b]), (uint32_t)((it >> 1) & 1));
       tc_fence_after();
-      if (tid == 0 && it < 8) TC_TRACE(24 + it);
       {
         const uint32_t tl = tmem + (uint32_t)(b * C::ACC_COLS) + ((uint32_t)((warp & 3) * 32) << 16) + (uint32_t)((warp >> 2) * 32);
         float v[32], w[32];
@@ -679,7 +666,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
       if (SLAB) cp_async_wait<0>();                      // the next tile's block sums
       asm volatile("bar.sync 1, 256;" ::: "memory");     // the staging tile is free for the next tile
     }
-    if (tid == 0) TC_TRACE(4);
   }
 
   tc_fence_before();

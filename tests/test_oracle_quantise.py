@@ -104,3 +104,52 @@ def test_find_symbol_brute_force_and_division_free_identity():
                 lhs = C[r, a] <= x
                 rhs = a <= x and int(G[r, a]) * 65280 < (x - a + 1) * int(T[r])
                 assert lhs == rhs
+
+
+def test_exp2_coefficients_in_exact_arithmetic():
+    """Pins EXP2_COEF independently of both transcriptions of the EXP recipe (oracle/quantise.py, coder_kernels.cuh):
+    the seven binary32 constants, evaluated as EXACT rationals (no fp32 rounding anywhere), against 2^r at 50 digits
+    on a dense grid of r in [-1/2, 1/2].  A wrong hex digit in c0..c4 breaks the bound; c0 = 1 makes EXP(0) = 1 exact
+    (the arg-max gets g = 2^23, R#5); c1 is the binary32 nearest to ln 2; and the whole polynomial stays within 2e-8
+    (relative) of the continuous least-squares fit of 2^r with c0 fixed, which is how such a table is regenerated."""
+    from fractions import Fraction
+    import mpmath as mp
+    mp.mp.dps = 50
+    c = [Fraction(float(v)) for v in q.EXP2_COEF]               # binary32 -> exact rational
+    assert len(c) == 7 and c[0] == 1
+    ln2 = mp.log(2)
+    c1 = np.float32(float(ln2))
+    assert q.EXP2_COEF[1] == c1 and abs(mp.mpf(float(c1)) - ln2) <= mp.mpf(2) ** -25   # nearest binary32 to ln 2
+    assert q.LOG2E == np.float32(float(1 / ln2))
+
+    def poly(r):
+        p = c[6]
+        for j in range(5, -1, -1):
+            p = p * r + c[j]
+        return p
+
+    worst = mp.mpf(0)
+    for i in range(-4096, 4097):
+        p = poly(Fraction(i, 8192))
+        rel = abs(mp.mpf(p.numerator) / mp.mpf(p.denominator) / mp.power(2, mp.mpf(i) / 8192) - 1)
+        worst = max(worst, rel)
+    assert worst <= mp.mpf("1.6e-8"), worst                     # documented: 1.0e-7 incl. the fp32 rounding of Horner
+    # independent derivation: least squares of (sum_{k>=1} c_k r^k - (2^r - 1)) * 2^-r over [-1/2, 1/2] (c0 = 1 fixed)
+    ks = range(1, 7)
+    A, b = mp.matrix(6, 6), mp.matrix(6, 1)
+    for a_, ka in enumerate(ks):
+        for b_, kb in enumerate(ks):
+            A[a_, b_] = mp.quad(lambda x: 4 ** (-x) * x ** (ka + kb), [-0.5, 0.5])
+        b[a_] = mp.quad(lambda x: 4 ** (-x) * x ** ka * (2 ** x - 1), [-0.5, 0.5])
+    fit = mp.lu_solve(A, b)
+    for i in range(-64, 65):
+        r = mp.mpf(i) / 128
+        d = sum((mp.mpf(float(q.EXP2_COEF[k])) - fit[k - 1]) * r ** k for k in ks)
+        assert abs(d) <= mp.mpf("2e-8"), (i, d)
+    # sensitivity: the bound does notice a single wrong hex digit (16 ulp) in c2
+    bad = list(c)
+    bad[2] = Fraction(float(np.array(0x3E75FDFE, np.uint32).view(np.float32)))
+    pb = bad[6]
+    for j in range(5, -1, -1):
+        pb = pb * Fraction(1, 2) + bad[j]
+    assert abs(mp.mpf(pb.numerator) / mp.mpf(pb.denominator) / mp.sqrt(2) - 1) > mp.mpf("1.6e-8")
