@@ -96,6 +96,37 @@ int boa_decompressed_size(const uint8_t* in, size_t in_len, size_t* n);
 int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len,
                    uint8_t* out, size_t* out_len, void* cuda_stream);
 
+/* ---- one container from several GPUs (chunks are independent) ------------------------
+ * The chunks of one input are cut into contiguous ranges, one per GPU (weights replicated, no data-path collective).
+ * boa_compress_shard: compress a range given as its own bytes - `in` (host|device) points at the first byte of the range's
+ *   first chunk, `n` is the byte length of the range (a multiple of chunk_bytes except for the range that holds the end of
+ *   the input) - exactly as boa_compress would, but return the parts instead of a container: the range-coder streams back
+ *   to back in `payload` (host|device; *payload_len = capacity on entry - 2*n + 4*ceil(n/chunk_bytes) is always enough -
+ *   bytes written on return), the per-chunk sizes in `sizes` and first bytes in `first` (HOST arrays of
+ *   ceil(n/chunk_bytes) entries; device pointers: BOA_E_ARG).
+ * boa_container_assemble: write ONE BOA1 container (fingerprint = boa_model_fingerprint of the model the parts were
+ *   compressed with) for the input of `n` bytes from `n_parts` consecutive parts:
+ *   header + first bytes + size index + CRC (built on the host from the HOST arrays first[p], sizes[p] of part_chunks[p]
+ *   entries) followed by the payload blocks.  `out` is host|device, *out_len capacity on entry (boa_compress_bound is
+ *   enough), bytes written on return.  payload[p] (host|device, payload_len[p] bytes = the sum of the part's sizes, else
+ *   BOA_E_FORMAT) is copied to its place; a block that already sits there (payload[p] == out + payload_off[p], e.g.
+ *   received there from its GPU) is left alone; `payload` may be NULL (index only: the caller places the blocks at
+ *   payload_off[p], an optional HOST array of n_parts + 1 byte offsets into `out`; boa_container_index_bytes(n,
+ *   chunk_bytes) = payload_off[0]).  The result is byte-identical to boa_compress of the whole input on one GPU.
+ *   With host pointers only it is plain host code (no CUDA call; it also runs on a machine without a GPU).
+ * boa_decompress_shard: validate the whole container like boa_decompress (header, index CRC, fingerprint) and decode only
+ *   chunks [first_chunk, first_chunk + n_chunks_local) into `out` (host|device; byte 0 of chunk first_chunk at out[0];
+ *   *out_len capacity on entry, bytes written on return).  A range beyond the container's chunks: BOA_E_ARG.
+ * Errors otherwise those of boa_compress / boa_decompress. */
+int boa_compress_shard(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, uint8_t* payload, size_t* payload_len,
+                       uint32_t* sizes, uint8_t* first, void* cuda_stream);
+size_t boa_container_index_bytes(size_t n, size_t chunk_bytes);
+int boa_container_assemble(uint64_t fingerprint, size_t n, size_t chunk_bytes, size_t n_parts, const size_t* part_chunks,
+                           const uint8_t* const* first, const uint32_t* const* sizes, const uint8_t* const* payload,
+                           const size_t* payload_len, uint8_t* out, size_t* out_len, uint64_t* payload_off, void* cuda_stream);
+int boa_decompress_shard(boa_model* m, const uint8_t* in, size_t in_len, size_t first_chunk, size_t n_chunks_local,
+                         uint8_t* out, size_t* out_len, void* cuda_stream);
+
 /* ---- streaming front end (PAPER Fig. 2) ------------------------------
  * The input is cut into groups of `group_chunks` chunks; every group is compressed into one complete BOA1
  * container (a shard) exactly as boa_compress would, and the shards are concatenated in `out`.  While the

@@ -20,7 +20,8 @@ K_NAMES = ("embed", "inproj", "convx", "scan", "outproj", "head", "coder", "fini
 K_COUNT = len(K_NAMES)
 
 EXPORTS = ("boa_model_load", "boa_model_free", "boa_model_fingerprint", "boa_compress_bound", "boa_compress",
-           "boa_decompressed_size", "boa_decompress", "boa_stream_bound", "boa_stream_compress",
+           "boa_decompressed_size", "boa_decompress", "boa_compress_shard", "boa_container_index_bytes", "boa_container_assemble",
+           "boa_decompress_shard", "boa_stream_bound", "boa_stream_compress",
            "boa_stream_decompressed_size", "boa_stream_decompress", "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",
            "boa_debug_set_slab", "boa_debug_set_max_wave", "boa_debug_gemm", "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
 
@@ -67,6 +68,14 @@ def lib() -> C.CDLL:
     l.boa_decompressed_size.restype = C.c_int
     l.boa_decompress.argtypes = [vp, u8p, sz, u8p, C.POINTER(sz), vp]
     l.boa_decompress.restype = C.c_int
+    l.boa_compress_shard.argtypes = [vp, u8p, sz, sz, u8p, C.POINTER(sz), vp, vp, vp]
+    l.boa_compress_shard.restype = C.c_int
+    l.boa_container_index_bytes.argtypes = [sz, sz]
+    l.boa_container_index_bytes.restype = sz
+    l.boa_container_assemble.argtypes = [C.c_uint64, sz, sz, sz, vp, vp, vp, vp, vp, u8p, C.POINTER(sz), vp, vp]
+    l.boa_container_assemble.restype = C.c_int
+    l.boa_decompress_shard.argtypes = [vp, u8p, sz, sz, sz, u8p, C.POINTER(sz), vp]
+    l.boa_decompress_shard.restype = C.c_int
     l.boa_stream_bound.argtypes = [sz, sz, sz]
     l.boa_stream_bound.restype = sz
     l.boa_stream_compress.argtypes = [vp, u8p, sz, sz, sz, u8p, C.POINTER(sz), vp, C.POINTER(sz), vp]
@@ -193,6 +202,27 @@ class Model:
         self.decompress_into(src, dst)
         return dst
 
+    # -- one container from several GPUs ---------------------------------------------------
+    def compress_shard(self, src: torch.Tensor, chunk_bytes: int, payload: torch.Tensor):
+        """boa_compress_shard: src = the bytes of a contiguous chunk range (CUDA or CPU), payload = uint8 buffer (CUDA or
+        CPU).  Returns (payload bytes written, sizes [chunks] int32 CPU tensor, first [chunks] uint8 CPU tensor)."""
+        nc = -(-src.numel() // chunk_bytes) if src.numel() else 0
+        sizes = torch.zeros(max(nc, 1), dtype=torch.int32)
+        first = torch.zeros(max(nc, 1), dtype=torch.uint8)
+        n = C.c_size_t(payload.numel())
+        _check(lib().boa_compress_shard(self._h, _ptr(src), src.numel(), chunk_bytes, _ptr(payload) or 0, C.byref(n),
+                                        sizes.data_ptr(), first.data_ptr(), _stream()), "boa_compress_shard")
+        return n.value, sizes[:nc], first[:nc]
+
+    def container_assemble(self, n: int, chunk_bytes: int, parts, out: torch.Tensor, payloads=None):
+        return container_assemble(self.fingerprint, n, chunk_bytes, parts, out, payloads)
+
+    def decompress_shard(self, src: torch.Tensor, first_chunk: int, n_chunks: int, dst: torch.Tensor) -> int:
+        n = C.c_size_t(dst.numel())
+        _check(lib().boa_decompress_shard(self._h, _ptr(src), src.numel(), first_chunk, n_chunks, _ptr(dst) or 0, C.byref(n),
+                                          _stream()), "boa_decompress_shard")
+        return n.value
+
     # -- streaming front end (Fig. 2): host buffers in, concatenated shards out --------------------------
     def stream_compress(self, data, chunk_bytes: int, group_chunks: int):
         """boa_stream_compress: returns (CPU uint8 tensor of the concatenated shards, list of shard lengths)."""
@@ -241,6 +271,33 @@ class Model:
 
 def stream_bound(n: int, chunk_bytes: int, group_chunks: int) -> int:
     return lib().boa_stream_bound(n, chunk_bytes, group_chunks)
+
+
+def container_assemble(fingerprint: int, n: int, chunk_bytes: int, parts, out: torch.Tensor, payloads=None):
+    """boa_container_assemble: parts = [(sizes int32 CPU tensor, first uint8 CPU tensor), ...] in chunk order;
+    payloads = matching list of uint8 tensors (CUDA or CPU) or None (index only).  Returns (bytes written, offsets).
+    Host-only when every tensor is a CPU tensor (no GPU needed)."""
+    k = len(parts)
+    sizes = [p[0].contiguous() for p in parts]
+    first = [p[1].contiguous() for p in parts]
+    counts = (C.c_size_t * max(k, 1))(*[int(z.numel()) for z in sizes])
+    fp = (C.c_void_p * max(k, 1))(*[f.data_ptr() if f.numel() else None for f in first])
+    zp = (C.c_void_p * max(k, 1))(*[z.data_ptr() if z.numel() else None for z in sizes])
+    offs = (C.c_uint64 * (k + 1))()
+    pp = pl = None
+    if payloads is not None:
+        pp = (C.c_void_p * max(k, 1))(*[_ptr(p) for p in payloads])
+        pl = (C.c_size_t * max(k, 1))(*[int(p.numel()) for p in payloads])
+    ln = C.c_size_t(out.numel())
+    _check(lib().boa_container_assemble(fingerprint, n, chunk_bytes, k, C.cast(counts, C.c_void_p), C.cast(fp, C.c_void_p),
+                                        C.cast(zp, C.c_void_p), C.cast(pp, C.c_void_p) if pp is not None else None,
+                                        C.cast(pl, C.c_void_p) if pl is not None else None, _ptr(out), C.byref(ln),
+                                        C.cast(offs, C.c_void_p), _stream() if out.is_cuda else 0), "boa_container_assemble")
+    return ln.value, [int(o) for o in offs]
+
+
+def container_index_bytes(n: int, chunk_bytes: int) -> int:
+    return lib().boa_container_index_bytes(n, chunk_bytes)
 
 
 def compress_bound(n: int, chunk_bytes: int) -> int:

@@ -44,6 +44,21 @@ struct GrowBuf {   // grow-only device buffer
   template <class T> T* as() const { return reinterpret_cast<T*>(p); }
 };
 
+struct PinBuf {    // grow-only pinned host buffer
+  void* p = nullptr;
+  size_t cap = 0;
+  int reserve(size_t bytes) {
+    if (bytes <= cap) return BOA_OK;
+    if (p) { cudaFreeHost(p); p = nullptr; cap = 0; }
+    const size_t want = round_up(bytes, 4096);
+    if (cudaHostAlloc(&p, want, cudaHostAllocDefault) != cudaSuccess) { (void)cudaGetLastError(); p = nullptr; return BOA_E_NOMEM; }
+    cap = want;
+    return BOA_OK;
+  }
+  void release() { if (p) cudaFreeHost(p); p = nullptr; cap = 0; }
+  template <class T> T* as() const { return reinterpret_cast<T*>(p); }
+};
+
 struct LayerW {
   const float *norm_w, *conv_b, *w_dtT, *b_dt, *d_skip;
   const float4 *conv_w, *A4;
@@ -83,6 +98,8 @@ struct boa_model {
   GrowBuf f_img, ffn_v;           // F > 0: image of the FFN's hidden layer; the FFN's output [rows][D] before LayerNorm
   GrowBuf pos, len, low, range, pending, wpos, cache, started, v, rpos, off, size, scratch, first, err;
   GrowBuf stage_in, stage_out;
+  GrowBuf total;               // [0] u64 payload bytes of the waves so far, [2] int: a payload would not fit (k_wave_offsets, k_compact)
+  PinBuf pin;                  // pinned host staging: payload total, per-chunk sizes and first bytes of a compress call
 
   // the library's own stream (capturable, unlike the legacy default stream) and the event that orders it
   // after the caller's stream
@@ -101,8 +118,9 @@ struct boa_model {
   ~boa_model() {
     for (GrowBuf* b : {&weights, &wimg, &u, &xz, &dbc, &u_img, &xs_img, &y_img, &f_img, &ffn_v, &logits, &h, &win, &ssq, &pos, &len, &low, &range,
                        &pending, &wpos, &cache, &started, &v, &rpos, &off, &size, &scratch, &first, &err,
-                       &stage_in, &stage_out})
+                       &stage_in, &stage_out, &total})
       b->release();
+    pin.release();
     for (cudaEvent_t e : events) cudaEventDestroy(e);
     if (user_ev) cudaEventDestroy(user_ev);
     if (own) cudaStreamDestroy(own);
@@ -859,43 +877,28 @@ int boa_get_profile(const boa_model* m, boa_profile* out) {
   return BOA_OK;
 }
 
-int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, uint8_t* out, size_t* out_len,
-                 void* cuda_stream) {
-  if (!m || !out || !out_len || chunk_bytes == 0 || chunk_bytes > kMaxChunkBytes || (n && !in)) return BOA_E_ARG;
-  cudaStream_t st;
-  BOA_TRY(enter(m, cuda_stream, &st));
+namespace {
+
+// Compress the chunks of d_in[0..n) (DEVICE) into d_payload (DEVICE, capacity payload_cap): the range-coder streams back to
+// back; per-chunk sizes and first bytes go to the HOST arrays sizes[nc], first[nc].  Waves of streams; per wave the
+// sizes -> offsets exclusive scan and the compaction run on the device (k_wave_offsets, k_compact), the sizes and first
+// bytes leave through pinned memory, and the host synchronises once, after the last wave.
+int compress_parts(boa_model* m, const uint8_t* d_in, size_t n, size_t chunk_bytes, uint8_t* d_payload, size_t payload_cap,
+                   uint32_t* sizes, uint8_t* first, uint64_t* payload_total, cudaStream_t st, uint64_t* launches_out) {
   const uint64_t nc = n_chunks_of(n, chunk_bytes);
-  if (nc >= (1ull << 32)) return BOA_E_ARG;
-  const size_t ib = index_bytes(nc);
-  const size_t capacity = *out_len;
-  if (capacity < ib) return BOA_E_CAPACITY;
-  prof_begin(m);
-  CallTimer timer(st);
-
-  // device views of the user buffers
-  const bool in_dev = (n == 0) || is_device_ptr(in), out_dev = is_device_ptr(out);
-  const uint8_t* d_in = in;
-  if (!in_dev) {
-    BOA_TRY(m->stage_in.reserve(n));
-    BOA_CUDA_TRY(cudaMemcpyAsync(m->stage_in.p, in, n, cudaMemcpyHostToDevice, st));
-    d_in = m->stage_in.as<uint8_t>();
-  }
-  uint8_t* d_out = out;
-  const size_t out_cap = std::min(capacity, boa_compress_bound(n, chunk_bytes));
-  if (!out_dev) {
-    BOA_TRY(m->stage_out.reserve(out_cap));
-    d_out = m->stage_out.as<uint8_t>();
-  }
-
-  std::vector<uint8_t> index(ib, 0);
-  std::vector<uint32_t> sizes((size_t)nc);
-  std::vector<uint64_t> offs;
-  uint64_t payload_total = 0;
+  *payload_total = 0;
+  if (nc == 0) return BOA_OK;
   const uint32_t cap = stream_cap(chunk_bytes);
+  BOA_TRY(m->pin.reserve(16 + 5 * (size_t)nc));
+  uint8_t* pin = m->pin.as<uint8_t>();
+  uint32_t* pin_sizes = reinterpret_cast<uint32_t*>(pin + 16);
+  uint8_t* pin_first = pin + 16 + 4 * (size_t)nc;
+  BOA_TRY(m->total.reserve(16));                   // [0] u64 running payload total, [1] int capacity overflow flag
+  BOA_CUDA_TRY(cudaMemsetAsync(m->total.p, 0, 16, st));
   uint64_t launches = 0;
 
   const bool slab = m->use_slab && chunk_bytes > (size_t)kSlabT;
-  const uint64_t W = nc ? wave_streams(m, nc, cap, slab ? kSlabT : 1) : 0;
+  const uint64_t W = wave_streams(m, nc, cap, slab ? kSlabT : 1);
   for (uint64_t c0 = 0; c0 < nc; c0 += W) {
     const uint64_t B = std::min(W, nc - c0);
     const uint64_t wave_base = c0 * chunk_bytes;
@@ -927,28 +930,169 @@ int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, 
     m->prof.steps += max_len - 1;
     k_coder_finish<0><<<g, 256, 0, st>>>(c.ca, (int)B);
     BOA_TRY(mark(c, BOA_K_FINISH));
-    BOA_CUDA_TRY(cudaMemcpyAsync(sizes.data() + c0, m->wpos.p, B * 4, cudaMemcpyDeviceToHost, st));
-    BOA_CUDA_TRY(cudaMemcpyAsync(index.data() + kHeaderBytes + c0, m->first.p, B, cudaMemcpyDeviceToHost, st));
-    BOA_CUDA_TRY(cudaStreamSynchronize(st));
-    offs.resize((size_t)B);
-    for (uint64_t i = 0; i < B; ++i) { offs[i] = payload_total; payload_total += sizes[c0 + i]; }
-    if (ib + payload_total > out_cap) return BOA_E_CAPACITY;
-    BOA_CUDA_TRY(cudaMemcpyAsync(m->off.p, offs.data(), B * 8, cudaMemcpyHostToDevice, st));
-    k_compact<<<(int)((B * 32 + 255) / 256), 256, 0, st>>>(m->scratch.as<uint8_t>(), cap, m->wpos.as<uint32_t>(),
-                                                          m->off.as<uint64_t>(), d_out + ib, (int)B);
+    // S15: sizes -> offsets (exclusive scan on the device, continuing from the waves before), then pack the payloads
+    k_wave_offsets<<<1, 1024, 0, st>>>(m->wpos.as<uint32_t>(), m->off.as<uint64_t>(), (int)B, m->total.as<uint64_t>());
     BOA_TRY(mark(c, BOA_K_FINISH));
-    BOA_CUDA_TRY(cudaStreamSynchronize(st));   // offs is reused by the next wave
+    k_compact<<<(int)((B * 32 + 255) / 256), 256, 0, st>>>(m->scratch.as<uint8_t>(), cap, m->wpos.as<uint32_t>(),
+                                                          m->off.as<uint64_t>(), d_payload, (uint64_t)payload_cap,
+                                                          m->total.as<int>() + 2, (int)B);
+    BOA_TRY(mark(c, BOA_K_FINISH));
+    BOA_CUDA_TRY(cudaMemcpyAsync(pin_sizes + c0, m->wpos.p, B * 4, cudaMemcpyDeviceToHost, st));
+    BOA_CUDA_TRY(cudaMemcpyAsync(pin_first + c0, m->first.p, B, cudaMemcpyDeviceToHost, st));
     launches += c.launches;
   }
+  BOA_CUDA_TRY(cudaMemcpyAsync(pin, m->total.p, 16, cudaMemcpyDeviceToHost, st));
+  BOA_CUDA_TRY(cudaStreamSynchronize(st));        // the one host synchronisation of the call's device work
+  uint64_t total = 0;
+  int overflow = 0;
+  memcpy(&total, pin, 8);
+  memcpy(&overflow, pin + 8, 4);
+  if (overflow || total > payload_cap) return BOA_E_CAPACITY;
+  memcpy(sizes, pin_sizes, 4 * (size_t)nc);
+  memcpy(first, pin_first, (size_t)nc);
+  *payload_total = total;
+  if (launches_out) *launches_out += launches;
+  return BOA_OK;
+}
 
+// BOA1 header + first bytes + size index + CRC into index[0 .. index_bytes(nc))
+void write_index(uint8_t* index, uint64_t fingerprint, size_t n, size_t chunk_bytes, uint64_t nc, const uint8_t* first,
+                 const uint32_t* sizes) {
+  const size_t ib = index_bytes(nc);
+  memset(index, 0, ib);
   Header h{};
   h.n = n; h.chunk_bytes = (uint32_t)chunk_bytes; h.n_chunks = (uint32_t)nc; h.freq_bits = 16;
   h.last_len = nc ? (uint32_t)(n - (nc - 1) * chunk_bytes) : 0;
-  h.fingerprint = boa_model_fingerprint(m);
-  write_header(index.data(), h);
-  uint8_t* sp = index.data() + kHeaderBytes + first_padded(nc);
+  h.fingerprint = fingerprint;
+  write_header(index, h);
+  if (nc) memcpy(index + kHeaderBytes, first, (size_t)nc);
+  uint8_t* sp = index + kHeaderBytes + first_padded(nc);
   for (uint64_t i = 0; i < nc; ++i) put_u32(sp + 4 * i, sizes[i]);
-  put_u32(index.data() + ib - 4, crc32_ieee(index.data(), ib - 4));
+  put_u32(index + ib - 4, crc32_ieee(index, ib - 4));
+}
+
+// A validated container index: header, per-chunk sizes and payload offsets.
+struct Index {
+  Header h{};
+  size_t ib = 0;
+  std::vector<uint8_t> bytes;
+  std::vector<uint32_t> sizes;
+  std::vector<uint64_t> offs;
+  uint64_t payload_total = 0;
+};
+
+// S16: read and validate header, index CRC, fingerprint and total length of a container (host|device pointer).
+int read_index(const boa_model* m, const uint8_t* in, size_t in_len, bool in_dev, cudaStream_t st, Index& ix) {
+  if (in_len < kHeaderBytes + 4) return BOA_E_FORMAT;
+  uint8_t hb[kHeaderBytes];
+  if (in_dev) {
+    BOA_CUDA_TRY(cudaMemcpyAsync(hb, in, kHeaderBytes, cudaMemcpyDeviceToHost, st));
+    BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  } else {
+    memcpy(hb, in, kHeaderBytes);
+  }
+  if (!parse_header(hb, ix.h)) return BOA_E_FORMAT;
+  const uint64_t nc = ix.h.n_chunks;
+  ix.ib = index_bytes(nc);
+  if (in_len < ix.ib) return BOA_E_FORMAT;
+  ix.bytes.resize(ix.ib);
+  if (in_dev) {
+    BOA_CUDA_TRY(cudaMemcpyAsync(ix.bytes.data(), in, ix.ib, cudaMemcpyDeviceToHost, st));
+    BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  } else {
+    memcpy(ix.bytes.data(), in, ix.ib);
+  }
+  if (get_u32(ix.bytes.data() + ix.ib - 4) != crc32_ieee(ix.bytes.data(), ix.ib - 4)) return BOA_E_CRC;
+  if (ix.h.fingerprint != boa_model_fingerprint(m)) return BOA_E_MODEL_MISMATCH;
+  const uint8_t* sp = ix.bytes.data() + kHeaderBytes + first_padded(nc);
+  ix.sizes.resize((size_t)nc);
+  ix.offs.resize((size_t)nc);
+  ix.payload_total = 0;
+  for (uint64_t i = 0; i < nc; ++i) { ix.sizes[i] = get_u32(sp + 4 * i); ix.offs[i] = ix.payload_total; ix.payload_total += ix.sizes[i]; }
+  if (ix.ib + ix.payload_total != in_len) return BOA_E_FORMAT;
+  return BOA_OK;
+}
+
+// Decode chunks [c_lo, c_hi) of a validated container whose bytes are at d_in (DEVICE) into d_out (DEVICE; byte 0 of
+// chunk c_lo at d_out[0]).  Waves of streams, the same step kernels as the encoder.
+int decompress_range(boa_model* m, const Index& ix, const uint8_t* d_in, uint64_t c_lo, uint64_t c_hi, uint8_t* d_out,
+                     cudaStream_t st, uint64_t* launches_out) {
+  const size_t chunk_bytes = ix.h.chunk_bytes;
+  const uint64_t n_range = std::min<uint64_t>(ix.h.n, c_hi * chunk_bytes) - c_lo * chunk_bytes;
+  uint64_t launches = 0;
+  const uint64_t nc = c_hi - c_lo;
+  const uint64_t W = wave_streams(m, nc, 0);
+  for (uint64_t c0 = 0; c0 < nc; c0 += W) {
+    const uint64_t B = std::min(W, nc - c0);
+    const uint64_t wave_base = c0 * chunk_bytes;
+    const uint64_t n_wave = std::min<uint64_t>(n_range - wave_base, B * chunk_bytes);
+    BOA_TRY(reserve_workspace(m, B, 0));
+    BOA_TRY(reset_state(m, st));
+    if (c0 == 0) BOA_CUDA_TRY(cudaMemsetAsync(m->err.p, 0, 4, st));
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->off.p, ix.offs.data() + c_lo + c0, B * 8, cudaMemcpyHostToDevice, st));
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->size.p, ix.sizes.data() + c_lo + c0, B * 4, cudaMemcpyHostToDevice, st));
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->first.p, ix.bytes.data() + kHeaderBytes + c_lo + c0, B, cudaMemcpyHostToDevice, st));
+    StepCtx c{};
+    c.m = m; c.st = st; c.B = (int)B; c.mode = 1;
+    c.data = d_out + wave_base;
+    c.chunk_bytes = chunk_bytes;
+    c.ca = coder_arrays(m, 0);
+    c.ca.payload = d_in + ix.ib;
+    const int g = (int)((B + 255) / 256);
+    k_coder_init<1><<<g, 256, 0, st>>>(c.ca, (int)B, chunk_bytes, n_wave, m->first.as<uint8_t>(), c.data);
+    BOA_TRY(mark(c, BOA_K_FINISH));
+    const uint64_t max_len = std::min<uint64_t>(chunk_bytes, n_wave);
+    if (max_len > 1) BOA_TRY(launch_embed(c));
+    BOA_TRY(run_steps(c, max_len - 1));
+    m->prof.steps += max_len - 1;
+    k_coder_finish<1><<<g, 256, 0, st>>>(c.ca, (int)B);
+    BOA_TRY(mark(c, BOA_K_FINISH));
+    launches += c.launches;
+  }
+  // one host synchronisation: the error flag accumulates over the waves (the index arrays live until the call returns)
+  int err = 0;
+  BOA_CUDA_TRY(cudaMemcpyAsync(&err, m->err.p, 4, cudaMemcpyDeviceToHost, st));
+  BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  if (err) return BOA_E_CORRUPT;
+  if (launches_out) *launches_out += launches;
+  return BOA_OK;
+}
+
+}  // namespace
+
+int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, uint8_t* out, size_t* out_len,
+                 void* cuda_stream) {
+  if (!m || !out || !out_len || chunk_bytes == 0 || chunk_bytes > kMaxChunkBytes || (n && !in)) return BOA_E_ARG;
+  cudaStream_t st;
+  BOA_TRY(enter(m, cuda_stream, &st));
+  const uint64_t nc = n_chunks_of(n, chunk_bytes);
+  if (nc >= (1ull << 32)) return BOA_E_ARG;
+  const size_t ib = index_bytes(nc);
+  const size_t capacity = *out_len;
+  if (capacity < ib) return BOA_E_CAPACITY;
+  prof_begin(m);
+  CallTimer timer(st);
+
+  // device views of the user buffers
+  const bool in_dev = (n == 0) || is_device_ptr(in), out_dev = is_device_ptr(out);
+  const uint8_t* d_in = in;
+  if (!in_dev) {
+    BOA_TRY(m->stage_in.reserve(n));
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->stage_in.p, in, n, cudaMemcpyHostToDevice, st));
+    d_in = m->stage_in.as<uint8_t>();
+  }
+  uint8_t* d_out = out;
+  const size_t out_cap = std::min(capacity, boa_compress_bound(n, chunk_bytes));
+  if (!out_dev) {
+    BOA_TRY(m->stage_out.reserve(out_cap));
+    d_out = m->stage_out.as<uint8_t>();
+  }
+
+  std::vector<uint8_t> index(ib, 0), first((size_t)nc);
+  std::vector<uint32_t> sizes((size_t)nc);
+  uint64_t payload_total = 0, launches = 0;
+  BOA_TRY(compress_parts(m, d_in, n, chunk_bytes, d_out + ib, out_cap - ib, sizes.data(), first.data(), &payload_total, st, &launches));
+  write_index(index.data(), boa_model_fingerprint(m), n, chunk_bytes, nc, first.data(), sizes.data());
   const size_t total = ib + payload_total;
   if (out_dev) {
     BOA_CUDA_TRY(cudaMemcpyAsync(out, index.data(), ib, cudaMemcpyHostToDevice, st));
@@ -961,6 +1105,93 @@ int boa_compress(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, 
   m->prof.launches_total = launches;
   m->prof.streams = nc;
   m->prof.total_ms = timer.stop();
+  return BOA_OK;
+}
+
+int boa_compress_shard(boa_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, uint8_t* payload, size_t* payload_len,
+                       uint32_t* sizes, uint8_t* first, void* cuda_stream) {
+  if (!m || !payload_len || chunk_bytes == 0 || chunk_bytes > kMaxChunkBytes || (n && (!in || !payload || !sizes || !first)))
+    return BOA_E_ARG;
+  if (is_device_ptr(sizes) || is_device_ptr(first)) return BOA_E_ARG;
+  cudaStream_t st;
+  BOA_TRY(enter(m, cuda_stream, &st));
+  const uint64_t nc = n_chunks_of(n, chunk_bytes);
+  if (nc >= (1ull << 32)) return BOA_E_ARG;
+  prof_begin(m);
+  CallTimer timer(st);
+  const size_t capacity = *payload_len;
+  const size_t cap_used = std::min(capacity, 2 * n + 4 * (size_t)nc);
+  const bool in_dev = (n == 0) || is_device_ptr(in), out_dev = is_device_ptr(payload);
+  const uint8_t* d_in = in;
+  if (!in_dev) {
+    BOA_TRY(m->stage_in.reserve(n));
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->stage_in.p, in, n, cudaMemcpyHostToDevice, st));
+    d_in = m->stage_in.as<uint8_t>();
+  }
+  uint8_t* d_pay = payload;
+  if (!out_dev && nc) {
+    BOA_TRY(m->stage_out.reserve(cap_used));
+    d_pay = m->stage_out.as<uint8_t>();
+  }
+  uint64_t payload_total = 0, launches = 0;
+  BOA_TRY(compress_parts(m, d_in, n, chunk_bytes, d_pay, cap_used, sizes, first, &payload_total, st, &launches));
+  if (!out_dev && payload_total) {
+    BOA_CUDA_TRY(cudaMemcpyAsync(payload, d_pay, payload_total, cudaMemcpyDeviceToHost, st));
+    BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  }
+  *payload_len = payload_total;
+  m->prof.launches_total = launches;
+  m->prof.streams = nc;
+  m->prof.total_ms = timer.stop();
+  return BOA_OK;
+}
+
+size_t boa_container_index_bytes(size_t n, size_t chunk_bytes) {
+  return chunk_bytes ? index_bytes(n_chunks_of(n, chunk_bytes)) : 0;
+}
+
+int boa_container_assemble(uint64_t fingerprint, size_t n, size_t chunk_bytes, size_t n_parts, const size_t* part_chunks,
+                           const uint8_t* const* first, const uint32_t* const* sizes, const uint8_t* const* payload,
+                           const size_t* payload_len, uint8_t* out, size_t* out_len, uint64_t* payload_off, void* cuda_stream) {
+  if (!out || !out_len || chunk_bytes == 0 || chunk_bytes > kMaxChunkBytes || (n_parts && (!part_chunks || !first || !sizes)))
+    return BOA_E_ARG;
+  const uint64_t nc = n_chunks_of(n, chunk_bytes);
+  uint64_t have = 0;
+  for (size_t p = 0; p < n_parts; ++p) have += part_chunks[p];
+  if (have != nc || nc >= (1ull << 32)) return BOA_E_ARG;
+  const size_t ib = index_bytes(nc);
+  std::vector<uint8_t> f((size_t)nc), index(ib);
+  std::vector<uint32_t> z((size_t)nc);
+  uint64_t c = 0, total = 0;
+  std::vector<uint64_t> offs(n_parts + 1, 0);
+  for (size_t p = 0; p < n_parts; ++p) {
+    if (part_chunks[p] && (!first[p] || !sizes[p])) return BOA_E_ARG;
+    uint64_t part_total = 0;
+    for (size_t i = 0; i < part_chunks[p]; ++i, ++c) { f[c] = first[p][i]; z[c] = sizes[p][i]; part_total += sizes[p][i]; }
+    if (payload_len && payload_len[p] != part_total) return BOA_E_FORMAT;   // a part's payload is the sum of its sizes
+    offs[p] = ib + total;
+    total += part_total;
+  }
+  offs[n_parts] = ib + total;
+  if (payload_off) memcpy(payload_off, offs.data(), (n_parts + 1) * sizeof(uint64_t));
+  if (*out_len < ib + total) return BOA_E_CAPACITY;
+  write_index(index.data(), fingerprint, n, chunk_bytes, nc, f.data(), z.data());
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const bool out_dev = is_device_ptr(out);
+  bool async = false;                              // pure host assembly touches no CUDA call (it also runs without a GPU)
+  if (out_dev) { BOA_CUDA_TRY(cudaMemcpyAsync(out, index.data(), ib, cudaMemcpyHostToDevice, st)); async = true; }
+  else memcpy(out, index.data(), ib);
+  if (payload) {
+    for (size_t p = 0; p < n_parts; ++p) {
+      const uint64_t len = offs[p + 1] - offs[p];
+      if (!len || payload[p] == out + offs[p]) continue;        // already in place (received there)
+      if (!payload[p]) return BOA_E_ARG;
+      if (!out_dev && !is_device_ptr(payload[p])) memcpy(out + offs[p], payload[p], len);
+      else { BOA_CUDA_TRY(cudaMemcpyAsync(out + offs[p], payload[p], len, cudaMemcpyDefault, st)); async = true; }
+    }
+  }
+  if (async) BOA_CUDA_TRY(cudaStreamSynchronize(st));
+  *out_len = ib + total;
   return BOA_OK;
 }
 
@@ -978,7 +1209,10 @@ int boa_decompressed_size(const uint8_t* in, size_t in_len, size_t* n) {
   return BOA_OK;
 }
 
-int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len, uint8_t* out, size_t* out_len, void* cuda_stream) {
+namespace {
+// boa_decompress and boa_decompress_shard: chunks [c_lo, c_lo + count) of the container (count = SIZE_MAX: all of them)
+int decompress_entry(boa_model* m, const uint8_t* in, size_t in_len, uint64_t c_lo, uint64_t count, uint8_t* out,
+                     size_t* out_len, void* cuda_stream) {
   if (!m || !in || !out_len) return BOA_E_ARG;
   if (in_len < kHeaderBytes + 4) return BOA_E_FORMAT;
   cudaStream_t st;
@@ -986,44 +1220,24 @@ int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len, uint8_t* out,
   const bool in_dev = is_device_ptr(in);
   prof_begin(m);
   CallTimer timer(st);
-
-  uint8_t hb[kHeaderBytes];
-  if (in_dev) {
-    BOA_CUDA_TRY(cudaMemcpyAsync(hb, in, kHeaderBytes, cudaMemcpyDeviceToHost, st));
-    BOA_CUDA_TRY(cudaStreamSynchronize(st));
-  } else {
-    memcpy(hb, in, kHeaderBytes);
-  }
-  Header h;
-  if (!parse_header(hb, h)) return BOA_E_FORMAT;
-  const uint64_t nc = h.n_chunks;
-  const size_t ib = index_bytes(nc);
-  if (in_len < ib) return BOA_E_FORMAT;
-  std::vector<uint8_t> index(ib);
-  if (in_dev) {
-    BOA_CUDA_TRY(cudaMemcpyAsync(index.data(), in, ib, cudaMemcpyDeviceToHost, st));
-    BOA_CUDA_TRY(cudaStreamSynchronize(st));
-  } else {
-    memcpy(index.data(), in, ib);
-  }
-  if (get_u32(index.data() + ib - 4) != crc32_ieee(index.data(), ib - 4)) return BOA_E_CRC;
-  if (h.fingerprint != boa_model_fingerprint(m)) return BOA_E_MODEL_MISMATCH;
-  const uint8_t* sp = index.data() + kHeaderBytes + first_padded(nc);
-  std::vector<uint32_t> sizes((size_t)nc);
-  std::vector<uint64_t> offs((size_t)nc);
-  uint64_t payload_total = 0;
-  for (uint64_t i = 0; i < nc; ++i) { sizes[i] = get_u32(sp + 4 * i); offs[i] = payload_total; payload_total += sizes[i]; }
-  if (ib + payload_total != in_len) return BOA_E_FORMAT;
-  const size_t n = (size_t)h.n;
+  Index ix;
+  BOA_TRY(read_index(m, in, in_len, in_dev, st, ix));
+  const uint64_t nc = ix.h.n_chunks;
+  if (count == SIZE_MAX) count = nc - std::min(nc, c_lo);
+  if (c_lo > nc || count > nc - c_lo) return BOA_E_ARG;
+  const uint64_t c_hi = c_lo + count;
+  const size_t chunk_bytes = ix.h.chunk_bytes;
+  const size_t n = count ? (size_t)(std::min<uint64_t>(ix.h.n, c_hi * chunk_bytes) - c_lo * chunk_bytes) : 0;
   if (*out_len < n) return BOA_E_CAPACITY;
   if (n && !out) return BOA_E_ARG;
   if (n == 0) { *out_len = 0; m->prof.total_ms = timer.stop(); return BOA_OK; }
 
-  const size_t chunk_bytes = h.chunk_bytes;
   const uint8_t* d_in = in;
   if (!in_dev) {
     BOA_TRY(m->stage_in.reserve(in_len));
-    BOA_CUDA_TRY(cudaMemcpyAsync(m->stage_in.p, in, in_len, cudaMemcpyHostToDevice, st));
+    // only the index and this range's payload bytes are needed on the device
+    const uint64_t p_lo = ix.ib + ix.offs[c_lo], p_hi = ix.ib + ix.offs[c_hi - 1] + ix.sizes[c_hi - 1];
+    BOA_CUDA_TRY(cudaMemcpyAsync(m->stage_in.as<uint8_t>() + p_lo, in + p_lo, p_hi - p_lo, cudaMemcpyHostToDevice, st));
     d_in = m->stage_in.as<uint8_t>();
   }
   const bool out_dev = is_device_ptr(out);
@@ -1032,49 +1246,28 @@ int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len, uint8_t* out,
     BOA_TRY(m->stage_out.reserve(n));
     d_out = m->stage_out.as<uint8_t>();
   }
-
   uint64_t launches = 0;
-  const uint64_t W = wave_streams(m, nc, 0);
-  for (uint64_t c0 = 0; c0 < nc; c0 += W) {
-    const uint64_t B = std::min(W, nc - c0);
-    const uint64_t wave_base = c0 * chunk_bytes;
-    const uint64_t n_wave = std::min<uint64_t>(n - wave_base, B * chunk_bytes);
-    BOA_TRY(reserve_workspace(m, B, 0));
-    BOA_TRY(reset_state(m, st));
-    BOA_CUDA_TRY(cudaMemsetAsync(m->err.p, 0, 4, st));
-    BOA_CUDA_TRY(cudaMemcpyAsync(m->off.p, offs.data() + c0, B * 8, cudaMemcpyHostToDevice, st));
-    BOA_CUDA_TRY(cudaMemcpyAsync(m->size.p, sizes.data() + c0, B * 4, cudaMemcpyHostToDevice, st));
-    BOA_CUDA_TRY(cudaMemcpyAsync(m->first.p, index.data() + kHeaderBytes + c0, B, cudaMemcpyHostToDevice, st));
-    StepCtx c{};
-    c.m = m; c.st = st; c.B = (int)B; c.mode = 1;
-    c.data = d_out + wave_base;
-    c.chunk_bytes = chunk_bytes;
-    c.ca = coder_arrays(m, 0);
-    c.ca.payload = d_in + ib;
-    const int g = (int)((B + 255) / 256);
-    k_coder_init<1><<<g, 256, 0, st>>>(c.ca, (int)B, chunk_bytes, n_wave, m->first.as<uint8_t>(), c.data);
-    BOA_TRY(mark(c, BOA_K_FINISH));
-    const uint64_t max_len = std::min<uint64_t>(chunk_bytes, n_wave);
-    if (max_len > 1) BOA_TRY(launch_embed(c));
-    BOA_TRY(run_steps(c, max_len - 1));
-    m->prof.steps += max_len - 1;
-    k_coder_finish<1><<<g, 256, 0, st>>>(c.ca, (int)B);
-    BOA_TRY(mark(c, BOA_K_FINISH));
-    int err = 0;
-    BOA_CUDA_TRY(cudaMemcpyAsync(&err, m->err.p, 4, cudaMemcpyDeviceToHost, st));
-    BOA_CUDA_TRY(cudaStreamSynchronize(st));
-    launches += c.launches;
-    if (err) return BOA_E_CORRUPT;
-  }
+  BOA_TRY(decompress_range(m, ix, d_in, c_lo, c_hi, d_out, st, &launches));
   if (!out_dev) {
     BOA_CUDA_TRY(cudaMemcpyAsync(out, d_out, n, cudaMemcpyDeviceToHost, st));
     BOA_CUDA_TRY(cudaStreamSynchronize(st));
   }
   *out_len = n;
   m->prof.launches_total = launches;
-  m->prof.streams = nc;
+  m->prof.streams = count;
   m->prof.total_ms = timer.stop();
   return BOA_OK;
+}
+}  // namespace
+
+int boa_decompress(boa_model* m, const uint8_t* in, size_t in_len, uint8_t* out, size_t* out_len, void* cuda_stream) {
+  return decompress_entry(m, in, in_len, 0, SIZE_MAX, out, out_len, cuda_stream);
+}
+
+int boa_decompress_shard(boa_model* m, const uint8_t* in, size_t in_len, size_t first_chunk, size_t n_chunks_local,
+                         uint8_t* out, size_t* out_len, void* cuda_stream) {
+  if (n_chunks_local == SIZE_MAX) return BOA_E_ARG;
+  return decompress_entry(m, in, in_len, first_chunk, n_chunks_local, out, out_len, cuda_stream);
 }
 
 // ------------------------------------------------------------------------------------ test-only

@@ -394,16 +394,69 @@ __global__ void k_coder_finish(CoderArrays ca, int B) {
   }
 }
 
-// S15: pack the per-stream scratch payloads back to back.  One warp per stream.
+// S15: per-stream sizes -> payload offsets.  off[i] = total + sum_{j<i} sizes[j] (exclusive scan), then total += the
+// wave's sum, so the next wave continues where this one ends and the host never sees the sizes in between.
+// One block of 1024 threads (B <= 65,536: at most 64 consecutive streams per thread); integer sums: order-free.
+__global__ void __launch_bounds__(1024) k_wave_offsets(const uint32_t* __restrict__ sizes, uint64_t* __restrict__ off, int B,
+                                                       uint64_t* __restrict__ total) {
+  __shared__ uint64_t warp_sum[32];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int per = (B + 1023) / 1024, i0 = tid * per, i1 = min(B, i0 + per);
+  uint64_t mine = 0;
+  for (int i = i0; i < i1; ++i) mine += sizes[i];
+  uint64_t inc = mine;                             // inclusive scan over the warp, then over the 32 warp sums
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    const uint64_t v = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += v;
+  }
+  if (lane == 31) warp_sum[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    uint64_t w = warp_sum[lane], winc = w;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const uint64_t v = __shfl_up_sync(0xffffffffu, winc, o);
+      if (lane >= o) winc += v;
+    }
+    warp_sum[lane] = winc - w;                     // exclusive
+  }
+  __syncthreads();
+  const uint64_t base = *total;
+  uint64_t run = base + warp_sum[warp] + (inc - mine);
+  for (int i = i0; i < i1; ++i) { off[i] = run; run += sizes[i]; }
+  __syncthreads();                                 // every thread has read *total
+  if (tid == 1023) *total = run;                   // the last thread's running sum is the new total (empty ranges add 0)
+}
+
+// S15: pack the per-stream scratch payloads back to back.  One warp per stream; the body moves 16 bytes per lane and
+// instruction with stores aligned in the destination (the scratch rows start 16-byte aligned, the packed position does
+// not: each 16-byte block is funnel-shifted together from five aligned source words); byte loops for head and tail.
+// A payload that would end beyond dst_cap is not written and raises *overflow (BOA_E_CAPACITY).
 __global__ void k_compact(const uint8_t* __restrict__ scratch, uint32_t cap, const uint32_t* __restrict__ sizes,
-                          const uint64_t* __restrict__ off, uint8_t* __restrict__ dst, int B) {
+                          const uint64_t* __restrict__ off, uint8_t* __restrict__ dst, uint64_t dst_cap,
+                          int* __restrict__ overflow, int B) {
   const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   if (i >= B) return;
   const uint8_t* s = scratch + (size_t)i * cap;
-  uint8_t* d = dst + off[i];
   const uint32_t n = sizes[i];
-  for (uint32_t k = lane; k < n; k += 32) d[k] = s[k];
+  const uint64_t o = off[i];
+  if (o + n > dst_cap) { if (lane == 0) *overflow = 1; return; }
+  uint8_t* d = dst + o;
+  const uint32_t head = min(n, (uint32_t)((16u - (uint32_t)(reinterpret_cast<uintptr_t>(d) & 15u)) & 15u));
+  for (uint32_t k = lane; k < head; k += 32) d[k] = s[k];
+  const uint32_t nblk = (n - head) >> 4;
+  const uint32_t sh = (head & 3u) * 8u;            // misalignment of the source of a block, in bits
+  const uint32_t* sw = reinterpret_cast<const uint32_t*>(s + (head & ~3u));
+  uint4* dv = reinterpret_cast<uint4*>(d + head);
+  for (uint32_t b = lane; b < nblk; b += 32) {
+    const uint32_t* p = sw + 4 * b;
+    const uint32_t w0 = p[0], w1 = p[1], w2 = p[2], w3 = p[3], w4 = sh ? p[4] : 0u;   // p[4] stays inside the row: cap >= n + 4
+    dv[b] = make_uint4(__funnelshift_r(w0, w1, sh), __funnelshift_r(w1, w2, sh), __funnelshift_r(w2, w3, sh),
+                       __funnelshift_r(w3, w4, sh));
+  }
+  for (uint32_t k = head + (nblk << 4) + lane; k < n; k += 32) d[k] = s[k];
 }
 
 // first byte of each stream

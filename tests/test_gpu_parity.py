@@ -441,6 +441,53 @@ def test_time_slab_encoder_writes_the_bytes_of_the_step_path(boa):
             assert _np(gm.decompress(torch.frombuffer(bytearray(a), dtype=torch.uint8).cuda())).tobytes() == data
 
 
+@pytest.mark.parametrize("world", [2, 3, 5])
+def test_one_container_from_several_gpus_run_one_after_the_other(boa, world):
+    """contiguous chunk ranges per GPU, parts -> ONE container.  The ranks are run one after
+    the other on this GPU (chunks are independent, so that is what N GPUs compute): boa_compress_shard of every
+    range + boa_container_assemble must be byte-identical to boa_compress of the whole input, and boa_decompress_shard
+    of every range of that container must give back the range's bytes."""
+    from paper_2511_11337_b200 import shard
+    cfg = synth.CONFIGS[1]
+    gm = boa.Model(cfg.weights(emb_std=0.25))
+    chunk = 150
+    data = cfg.data(11 * chunk + 77)                               # 12 chunks, ragged tail
+    n = len(data)
+    src = torch.frombuffer(bytearray(data), dtype=torch.uint8).cuda()
+    whole = gm.compress(src, chunk)
+    parts, pays = [], []
+    for r in range(world):
+        lo, hi = shard.byte_range(n, chunk, r, world)
+        buf = torch.empty(2 * (hi - lo) + 4 * 12, dtype=torch.uint8, device="cuda" if r % 2 == 0 else "cpu")
+        plen, sizes, first = gm.compress_shard(src[lo:hi] if r % 2 == 0 else src[lo:hi].cpu(), chunk, buf)
+        assert plen == int(sizes.sum()) and sizes.numel() == -(-(hi - lo) // chunk)
+        parts.append((sizes, first)); pays.append(buf[:plen])
+    for dev in ("cuda", "cpu"):
+        out = torch.zeros(boa.compress_bound(n, chunk), dtype=torch.uint8, device=dev)
+        ln, offs = gm.container_assemble(n, chunk, parts, out, pays)
+        assert ln == whole.numel() and torch.equal(out[:ln].cpu(), whole.cpu()), dev
+        assert offs[0] == boa.container_index_bytes(n, chunk) and offs[-1] == ln
+    # index only + blocks placed by the caller (what the NCCL exchange does: blocks are received in place)
+    out = torch.zeros(boa.compress_bound(n, chunk), dtype=torch.uint8, device="cuda")
+    _, offs = gm.container_assemble(n, chunk, parts, out, None)
+    for r in range(world):
+        out[offs[r]: offs[r + 1]] = pays[r].cuda()
+    ln2, _ = gm.container_assemble(n, chunk, parts, out, [out[offs[r]: offs[r + 1]] for r in range(world)])
+    assert torch.equal(out[:ln2], whole)
+    # decode: every rank its own chunk range of the shared container
+    back = torch.zeros(n, dtype=torch.uint8, device="cuda")
+    for r in range(world):
+        c_lo, c_hi = shard.chunk_range(12, r, world)
+        lo, hi = shard.byte_range(n, chunk, r, world)
+        got = gm.decompress_shard(whole if r % 2 == 0 else whole.cpu(), c_lo, c_hi - c_lo, back[lo:hi])
+        assert got == hi - lo
+    assert torch.equal(back, src)
+    with pytest.raises(boa.BoaError) as e:
+        gm.decompress_shard(whole, 11, 2, back)
+    assert e.value.code == boa.E_ARG
+    assert gm.decompress_shard(whole, 12, 0, back) == 0
+
+
 def test_streaming_front_end(boa):
     """Fig. 2: groups of chunks -> concatenated shards through the two-lane
     pre-load / compress / collect pipeline.  Every shard must be the bytes boa_compress writes for its group alone, the
