@@ -196,13 +196,19 @@ int boa_get_profile(const boa_model* m, boa_profile* out);
 /* boa_debug_gemm: the tensor-core contraction kernel alone (S3/S5/S9/S10; tc_gemm.cuh):
  *   C[M][N] = A[M][K] W[N][K]^T, A and C host|device fp32 row-major, W a HOST fp32 matrix that is cut into
  *   `weight_pieces` (1 or 3) bf16 pieces exactly as boa_model_load does; A is cut into its three pieces by the same
- *   device routine the step kernels use.  grid_ctas = 0 launches one persistent CTA per SM as the step does; a small
- *   positive value forces several tiles per CTA (the accumulator double-buffering path).  K % 64 == 0. */
+ *   device routine the step kernels use.  grid_ctas = 0 launches one persistent CTA per SM as the time slabs do; a small
+ *   positive value forces several tiles per CTA (the accumulator double-buffering path).  grid_ctas = -1 runs the
+ *   CTA-pair kernel of the step path instead (tc_gemm2.cuh: tcgen05 cta_group::2, 256 x 128 tiles) with one pair per SM
+ *   pair; -2k runs it with k pairs (several tiles per pair).  Both kernels must return the same bits.  K % 64 == 0. */
 /* boa_debug_set_slab: enabled = 0 makes boa_compress step one byte at a time, exactly as boa_decompress must, instead
  *   of advancing 16 bytes per pass over the stream state; the container bytes must not change (test).
  * boa_debug_set_max_wave: streams > 0 caps the number of streams stepped together (more chunks then run in waves), as
  *   a small free-memory budget would; 0 restores the default.  Results must not depend on it (test). */
 int boa_debug_set_slab(boa_model* m, int enabled);
+/* boa_debug_set_pair_tiles: the step path's contractions run with CTA-pair tiles (tc_gemm2.cuh) when a wave has at least
+ *   `min_row_tiles` row tiles of 128 streams (0 = always; default INT_MAX = never: measured slower).
+ *   Same bytes either way. */
+int boa_debug_set_pair_tiles(boa_model* m, int min_row_tiles);
 int boa_debug_set_max_wave(boa_model* m, size_t streams);
 int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N, int weight_pieces, int grid_ctas,
                    float* C, void* cuda_stream);

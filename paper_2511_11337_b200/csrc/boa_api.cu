@@ -4,6 +4,7 @@
 // that computes returns BOA_E_CUDA.  Nothing under oracle/ is included, linked or executed.
 #include "../../include/boa.h"
 
+#include <limits.h>
 #include <math.h>
 #include <stdio.h>
 #include <stdlib.h>
@@ -18,6 +19,7 @@
 #include "container.h"
 #include "model_kernels.cuh"
 #include "tc_gemm.cuh"
+#include "tc_gemm2.cuh"
 
 using namespace boa;
 
@@ -108,6 +110,7 @@ struct boa_model {
 
   // test-only switches (boa_debug_set_slab / boa_debug_set_max_wave): results do not depend on them
   bool use_slab = true;        // false: boa_compress steps one byte at a time like the decoder (same bytes)
+  int pair_min_row_tiles = INT_MAX; // step-path contractions use CTA-pair tiles from this many 128-stream row tiles on (use_pair_tiles)
   uint64_t max_wave = 0;       // > 0: at most this many streams are stepped together (more chunks run in waves)
 
   // profiling
@@ -270,6 +273,36 @@ int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
   }
   return BOA_OK;
 }
+// The step path's contractions: CTA-pair tiles of 256 streams x 128 columns (tc_gemm2.cuh).  Persistent, one cluster of
+// two CTAs per SM pair.  `max_pairs` > 0 limits the grid (tests: several tiles per pair).
+template <int NPW, int EPI>
+int launch_tc2(const tc::GemmArgs& g, int n_sm, cudaStream_t st, int max_pairs = 0) {
+  using C = tc2::Cfg2<NPW>;
+  const int mt = (g.M + tc::BM - 1) / tc::BM;
+  const int items = ((mt + 1) / 2) * ((g.NT + 1) / 2);
+  int pairs = std::min(items, std::max(1, n_sm / 2));
+  if (max_pairs > 0) pairs = std::min(pairs, max_pairs);
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3(2 * pairs); cfg.blockDim = dim3(tc::NTHREADS); cfg.dynamicSmemBytes = C::SMEM; cfg.stream = st;
+  cudaLaunchAttribute at[2];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  at[1].id = cudaLaunchAttributeClusterDimension;
+  at[1].val.clusterDim.x = 2; at[1].val.clusterDim.y = 1; at[1].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 2;
+  BOA_CUDA_TRY(cudaLaunchKernelEx(&cfg, tc2::k_tc_gemm2<NPW, EPI>, g));
+  return BOA_OK;
+}
+template <int EPI>
+int launch_tc2_npw(int npw, const tc::GemmArgs& g, int n_sm, cudaStream_t st, int max_pairs = 0) {
+  return npw == 1 ? launch_tc2<1, EPI>(g, n_sm, st, max_pairs) : launch_tc2<3, EPI>(g, n_sm, st, max_pairs);
+}
+template <int NPW, int EPI>
+int optin_tc2() {
+  BOA_CUDA_TRY((cudaFuncSetAttribute(tc2::k_tc_gemm2<NPW, EPI>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc2::Cfg2<NPW>::SMEM)));
+  return BOA_OK;
+}
+
 template <int NPW, int EPI, bool SLAB = false>
 int optin_tc() {
   constexpr int smem = SLAB ? tc::Cfg<NPW>::SMEM_SLAB : tc::Cfg<NPW>::SMEM;
@@ -290,6 +323,14 @@ int init_kernels() {
   BOA_TRY((optin_tc<3, tc::EPI_RESID>()));
   BOA_TRY((optin_tc<1, tc::EPI_FFN1>()));
   BOA_TRY((optin_tc<3, tc::EPI_FFN1>()));
+  BOA_TRY((optin_tc2<1, tc::EPI_INPROJ>()));
+  BOA_TRY((optin_tc2<3, tc::EPI_INPROJ>()));
+  BOA_TRY((optin_tc2<1, tc::EPI_STORE>()));
+  BOA_TRY((optin_tc2<3, tc::EPI_STORE>()));
+  BOA_TRY((optin_tc2<1, tc::EPI_RESID>()));
+  BOA_TRY((optin_tc2<3, tc::EPI_RESID>()));
+  BOA_TRY((optin_tc2<1, tc::EPI_FFN1>()));
+  BOA_TRY((optin_tc2<3, tc::EPI_FFN1>()));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 64)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
@@ -306,6 +347,18 @@ int init_kernels() {
 template <int EPI>
 int launch_tc_npw(int npw, const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
   return npw == 1 ? launch_tc<1, EPI>(g, n_sm, st) : launch_tc<3, EPI>(g, n_sm, st);
+}
+
+// Which tile shape a step-path contraction runs with.  Both kernels return the same bits (tests), so this is a pure
+// performance choice.  The CTA-pair tiles (256 x 128, tc_gemm2.cuh) halve the operand traffic per output, but as measured
+// (profiles/r02_pair_gemm.md: B = 4,096 ... 65,536, fp32 and bf16 blobs) they are slower than or equal to the single-CTA
+// tiles (128 x 64) at every size - fewer and longer work items, a single accumulator buffer for fp32 blobs - so the
+// default threshold is "never"; boa_debug_set_pair_tiles selects them for the tests and for measurement.
+bool use_pair_tiles(const tc::GemmArgs& g, int min_row_tiles) { return (g.M + tc::BM - 1) / tc::BM >= min_row_tiles; }
+template <int EPI>
+int launch_gemm_step(const boa_model* m, const tc::GemmArgs& g, cudaStream_t st) {
+  if (use_pair_tiles(g, m->pair_min_row_tiles)) return launch_tc2_npw<EPI>(m->npw, g, m->n_sm, st);
+  return launch_tc_npw<EPI>(m->npw, g, m->n_sm, st);
 }
 
 // S1 for the first step of a wave: u = Emb[byte 0] (later steps: fused into the coder step).
@@ -333,6 +386,7 @@ int launch_step(StepCtx& c) {
   float* xz = m->xz.as<float>();
   float* dbc = m->dbc.as<float>();
   float* logits = m->logits.as<float>();
+  float* ssq = m->ssq.as<float>();
   uint8_t* u_img = m->u_img.as<uint8_t>();
   uint8_t* xs_img = m->xs_img.as<uint8_t>();
   uint8_t* y_img = m->y_img.as<uint8_t>();
@@ -349,12 +403,12 @@ int launch_step(StepCtx& c) {
       g.C = xz;           // step path: a row = [slice][xs | z]; time slab: [slice][row][xs | z] (one copy per stream-group)
       g.ldc = T == 1 ? 2 * E : 2 * ec;
       g.xz_slice = T == 1 ? (size_t)2 * ec : (size_t)rows * 2 * ec;
-      g.ssq_in = m->ssq.as<float>(); g.win = winl; g.pos = c.ca.pos; g.slab_T = T == 1 ? 0 : T; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
+      g.ssq_in = ssq; g.win = winl; g.pos = c.ca.pos; g.slab_T = T == 1 ? 0 : T; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
       g.out_img = xs_img; g.out_KB = E / 64;
       if (T > 1) {   // the time-slab form of the conv epilogue
         BOA_TRY((m->npw == 1 ? launch_tc<1, tc::EPI_INPROJ, true>(g, m->n_sm, c.st) : launch_tc<3, tc::EPI_INPROJ, true>(g, m->n_sm, c.st)));
       } else {
-        BOA_TRY((launch_tc_npw<tc::EPI_INPROJ>(m->npw, g, m->n_sm, c.st)));
+        BOA_TRY((launch_gemm_step<tc::EPI_INPROJ>(m, g, c.st)));
       }
       BOA_TRY(mark(c, BOA_K_INPROJ));
     }
@@ -401,10 +455,11 @@ int launch_step(StepCtx& c) {
       tc::GemmArgs g{};
       g.A = y_img; g.M = rows; g.KB = E / 64; g.W = w.img_out; g.NT = D / 64; g.KS = 1;
       g.C = u; g.ldc = D; g.n_valid = D;
-      g.out_img = u_img; g.out_KB = D / 64; g.ssq_out = m->ssq.as<float>();
+      g.out_img = u_img; g.out_KB = D / 64; g.ssq_out = ssq;
       // (the paper's block: the FFN reads u itself, not a normalised u)
       g.out_scale = (m->F == 0 && l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
-      BOA_TRY((launch_tc_npw<tc::EPI_RESID>(m->npw, g, m->n_sm, c.st)));
+      if (T == 1) BOA_TRY((launch_gemm_step<tc::EPI_RESID>(m, g, c.st)));
+      else BOA_TRY((launch_tc_npw<tc::EPI_RESID>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_OUTPROJ));
     }
     if (m->F > 0) {  // the paper's block (Alg. 1 l.4, R#23): u <- LayerNorm(W2 GELU(W1 u + b1) + b2)
@@ -415,19 +470,21 @@ int launch_step(StepCtx& c) {
         tc::GemmArgs g{};
         g.A = u_img; g.M = rows; g.KB = D / 64; g.W = w.img_ffn1; g.NT = F / 64; g.KS = 1;
         g.n_valid = F; g.bias = w.ffn_b1; g.out_img = f_img; g.out_KB = F / 64;
-        BOA_TRY((launch_tc_npw<tc::EPI_FFN1>(m->npw, g, m->n_sm, c.st)));
+        if (T == 1) BOA_TRY((launch_gemm_step<tc::EPI_FFN1>(m, g, c.st)));
+        else BOA_TRY((launch_tc_npw<tc::EPI_FFN1>(m->npw, g, m->n_sm, c.st)));
         BOA_TRY(mark(c, BOA_K_FFN1));
       }
       {
         tc::GemmArgs g{};
         g.A = f_img; g.M = rows; g.KB = F / 64; g.W = w.img_ffn2; g.NT = D / 64; g.KS = 1;
         g.C = ffn_v; g.ldc = D; g.n_valid = D; g.bias = w.ffn_b2;
-        BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
+        if (T == 1) BOA_TRY((launch_gemm_step<tc::EPI_STORE>(m, g, c.st)));
+        else BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
         BOA_TRY(mark(c, BOA_K_FFN2));
       }
       BOA_CUDA_TRY(launch_pdl(k_layernorm, dim3((unsigned)(((size_t)rows * 32 + 255) / 256)), dim3(256), 0, c.st,
                               (const float*)ffn_v, w.ln_w, w.ln_b, u, (l + 1 < m->L) ? m->layers[l + 1].norm_w : (const float*)nullptr,
-                              u_img, m->ssq.as<float>(), rows, D));
+                              u_img, ssq, rows, D));
       BOA_TRY(mark(c, BOA_K_LNORM));
     }
   }
@@ -435,14 +492,15 @@ int launch_step(StepCtx& c) {
     tc::GemmArgs g{};
     g.A = u_img; g.M = rows; g.KB = D / 64; g.W = m->img_head; g.NT = 4; g.KS = 1;
     g.C = logits; g.ldc = 256; g.n_valid = 256;
-    BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
+    if (T == 1) BOA_TRY((launch_gemm_step<tc::EPI_STORE>(m, g, c.st)));
+    else BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
     BOA_TRY(mark(c, BOA_K_HEAD));
   }
 
   const int cgrid = (B * 32 + 255) / 256;
   EmbedArgs ea{};
   ea.emb = reinterpret_cast<const float4*>(m->emb); ea.norm_w = reinterpret_cast<const float4*>(m->layers[0].norm_w);
-  ea.u = m->u.as<float4>(); ea.u_img = u_img; ea.ssq = m->ssq.as<float>(); ea.D4 = D / 4;
+  ea.u = reinterpret_cast<float4*>(u); ea.u_img = u_img; ea.ssq = ssq; ea.D4 = D / 4;
   if (T > 1) {
     BOA_CUDA_TRY(launch_pdl(k_coder_slab, dim3(cgrid), dim3(256), 0, c.st, (const float*)logits, (const uint8_t*)c.data,
                             c.chunk_bytes, c.ca, B, T));
@@ -1300,6 +1358,12 @@ int boa_debug_set_slab(boa_model* m, int enabled) {
   return BOA_OK;
 }
 
+int boa_debug_set_pair_tiles(boa_model* m, int min_row_tiles) {
+  if (!m || min_row_tiles < 0) return BOA_E_ARG;
+  m->pair_min_row_tiles = min_row_tiles;
+  return BOA_OK;
+}
+
 int boa_debug_set_max_wave(boa_model* m, size_t streams) {
   if (!m || streams > kMaxWaveStreams) return BOA_E_ARG;
   m->max_wave = streams;
@@ -1348,7 +1412,7 @@ int boa_debug_step_dump(boa_model* m, const uint8_t* in, size_t n, size_t chunk_
 int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N, int weight_pieces, int grid_ctas,
                    float* C, void* cuda_stream) {
   if (!A || !W || !C || M == 0 || N == 0 || K == 0 || K % 64 != 0 || (weight_pieces != 1 && weight_pieces != 3) ||
-      grid_ctas < 0 || M >= (1u << 30) || N >= (1u << 20) || K >= (1u << 20))
+      M >= (1u << 30) || N >= (1u << 20) || K >= (1u << 20))
     return BOA_E_ARG;
   BOA_TRY(check_device());
   BOA_TRY(init_kernels());
@@ -1380,7 +1444,8 @@ int boa_debug_gemm(const float* A, size_t M, size_t K, const float* W, size_t N,
     n_sm = 148;
   }
   if (grid_ctas > 0) n_sm = std::min(n_sm, grid_ctas);
-  int rc = launch_tc_npw<tc::EPI_STORE>(weight_pieces, g, n_sm, st);
+  int rc = grid_ctas < 0 ? launch_tc2_npw<tc::EPI_STORE>(weight_pieces, g, n_sm, st, grid_ctas == -1 ? 0 : -grid_ctas / 2)
+                         : launch_tc_npw<tc::EPI_STORE>(weight_pieces, g, n_sm, st);
   cudaError_t e = cudaGetLastError();
   if (rc == BOA_OK && e != cudaSuccess) rc = note_cuda_error(e, __FILE__, __LINE__);
   if (rc == BOA_OK) {

@@ -109,6 +109,63 @@ def test_tensor_core_gemm_against_fp64(boa, pieces, grid_ctas, M, N, K):
     assert np.array_equal(got_h.astype(np.float64), got)
 
 
+@pytest.mark.parametrize("pieces", [3, 1])
+@pytest.mark.parametrize("M,N,K", [(300, 48, 512), (128, 256, 64), (1, 64, 256), (517, 320, 1024), (700, 192, 128), (2100, 1024, 256)])
+def test_cta_pair_gemm_returns_the_bits_of_the_single_cta_gemm(boa, pieces, M, N, K):
+    """The step path multiplies with CTA-pair tiles (tc_gemm2.cuh: tcgen05 cta_group::2, 256 x 128), the encode-side time
+    slabs with single-CTA tiles (tc_gemm.cuh: 128 x 64).  Both issue, per output element, the same piece products into
+    the same accumulator classes in the same order, so they must agree bit for bit (the decoder steps, the encoder
+    runs slabs) - for odd numbers of row tiles and of 64-column weight tiles (a pair with a missing half), one tile per
+    pair and several tiles per pair (accumulator and stage rings wrap), and against numpy fp64."""
+    g = np.random.Generator(np.random.PCG64(M * 5 + N * 11 + K + pieces))
+    a = (g.normal(0, 1.0, (M, K)) * np.exp(g.normal(0, 2.0, (M, 1)))).astype(np.float32)
+    w = g.normal(0, 0.05, (N, K)).astype(np.float32)
+    if pieces == 1:
+        w = _to_bf16(w)
+    ad, wt = torch.from_numpy(a).cuda(), torch.from_numpy(w)
+    single = _np(boa.debug_gemm(ad, wt, pieces, 0))
+    for grid in (-1, -2, -6):
+        pair = _np(boa.debug_gemm(ad, wt, pieces, grid))
+        assert np.array_equal(pair.view(np.uint32), single.view(np.uint32)), (grid, np.abs(pair - single).max())
+    want = a.astype(np.float64) @ w.astype(np.float64).T
+    scale = np.abs(a).astype(np.float64) @ np.abs(w).astype(np.float64).T
+    assert (np.abs(single - want) / scale).max() <= 2.0 ** -20
+
+
+@pytest.mark.parametrize("shape", ["cfg1", "d192_l1", "cfg2", "cfg5_l2_bf16", "paper_block_d64", "paper_block_l2_d128_bf16"])
+def test_pair_tiles_and_single_tiles_write_the_same_container(boa, shape):
+    """The whole step path with CTA-pair tiles forced on (every contraction incl. the conv epilogue of in_proj, the
+    residual epilogue and the FFN) against single-CTA tiles: same container bytes, and either decodes the other's.
+    D = 64 / 192 give contractions with an odd number of 64-column weight tiles (a pair whose second half is missing),
+    300 streams an odd number of row tiles."""
+    s1 = synth.CONFIGS[1]
+    blob = {"cfg1": lambda: s1.weights(emb_std=0.25),
+            "d192_l1": lambda: synth.make_weights(synth.ModelShape(1, 192), 5, emb_std=0.25),
+            "cfg2": lambda: synth.make_weights(synth.CONFIGS[2].shape, 1, emb_std=0.25),
+            "cfg5_l2_bf16": lambda: synth.make_weights(synth.ModelShape(2, 512, dt_rank=32), 3, synth.DTYPE_BF16, emb_std=0.25),
+            "paper_block_d64": lambda: synth.make_weights(synth.ModelShape(1, 64, dt_rank=4, d_ff=64, tied=False), 12, emb_std=0.25, ffn_std=0.1),
+            "paper_block_l2_d128_bf16": lambda: synth.make_weights(synth.ModelShape(2, 128, dt_rank=8, d_ff=320), 9, synth.DTYPE_BF16,
+                                                                   emb_std=0.25, ffn_std=0.1)}[shape]()
+    gm = boa.Model(blob)
+    for n, chunk in [(300 * 23, 23), (5 * 50 + 7, 50), (1, 40)]:
+        data = s1.data(n)
+        gm.debug_set_slab(False)                                   # encode with the step kernels, like the decoder
+        try:
+            gm.debug_set_pair_tiles(1 << 30)
+            single = gm.compress(data, chunk)
+            gm.debug_set_pair_tiles(0)
+            pair = gm.compress(data, chunk)
+            assert torch.equal(single, pair), (shape, n, chunk)
+            assert _np(gm.decompress(single)).tobytes() == data    # pair-tile decoder, single-tile encoder
+            gm.debug_set_slab(True)
+            assert torch.equal(gm.compress(data, chunk), pair)     # time slabs (single-CTA tiles) == pair-tile steps
+            gm.debug_set_pair_tiles(1 << 30)
+            assert _np(gm.decompress(pair)).tobytes() == data      # single-tile decoder, pair-tile encoder
+        finally:
+            gm.debug_set_slab(True)
+            gm.debug_set_pair_tiles(2 ** 31 - 1)
+
+
 # ---------------------------------------------------------------------------------------------- check 1
 @pytest.mark.parametrize("kind", ["uniform", "peaked", "random"])
 def test_range_coder_bit_exact_given_oracle_tables(boa, kind):
