@@ -368,6 +368,8 @@ def run_ours(args, cfg):
     m = boa.Model(cfg.weights())
     if args.pair_tiles >= 0:
         m.debug_set_pair_tiles(args.pair_tiles)
+    if args.persist_max >= 0:
+        m.debug_set_persist(args.persist_max, args.persist_cluster)
     d_in = host.to(dev)
     d_comp = torch.empty(boa.compress_bound(n, chunk), dtype=torch.uint8, device=dev)
     d_out = torch.empty(n, dtype=torch.uint8, device=dev)
@@ -567,6 +569,8 @@ def main():
     ap.add_argument("--no-sweep", action="store_true", help="skip the once-only sweep points and the largest configuration")
     ap.add_argument("--no-largest", action="store_true", help="skip the 1 GiB configs[3] pass (about two minutes)")
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"], help="N > 1: independent replicas (weak) or one input / one container sharded over the ranks (strong)")
+    ap.add_argument("--persist-max", type=int, default=-1, help="measurement only: waves up to this many streams run the persistent step kernel (boa_debug_set_persist; -1 = library default, 0 = never)")
+    ap.add_argument("--persist-cluster", type=int, default=0, help="measurement only: CTAs per row tile in the persistent step kernel (0 = library default)")
     ap.add_argument("--pair-tiles", type=int, default=-1, help="measurement only: row-tile threshold from which the step path uses CTA-pair tiles (boa_debug_set_pair_tiles; -1 = library default)")
     ap.add_argument("--streams", type=int, default=0, help="run the config's model with this many chunks (streams per step) ...")
     ap.add_argument("--chunk-bytes", type=int, default=0, help="... of this many bytes each (a sweep point, not the headline workload)")

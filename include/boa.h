@@ -205,6 +205,10 @@ int boa_get_profile(const boa_model* m, boa_profile* out);
  * boa_debug_set_max_wave: streams > 0 caps the number of streams stepped together (more chunks then run in waves), as
  *   a small free-memory budget would; 0 restores the default.  Results must not depend on it (test). */
 int boa_debug_set_slab(boa_model* m, int enabled);
+/* boa_debug_set_persist: waves of at most `max_streams` streams step inside one launch of the persistent step kernel
+ *   (step_persist.cuh; 0 = never, i.e. always the graph of one kernel per phase), with `cluster_ctas` CTAs per row tile of
+ *   128 streams (1, 2, 4, 8 or 16; 0 = keep).  Same bytes either way (test). */
+int boa_debug_set_persist(boa_model* m, size_t max_streams, int cluster_ctas);
 /* boa_debug_set_pair_tiles: the step path's contractions run with CTA-pair tiles (tc_gemm2.cuh) when a wave has at least
  *   `min_row_tiles` row tiles of 128 streams (0 = always; default INT_MAX = never: measured slower).
  *   Same bytes either way. */

@@ -20,6 +20,7 @@
 #include "model_kernels.cuh"
 #include "tc_gemm.cuh"
 #include "tc_gemm2.cuh"
+#include "step_persist.cuh"
 
 using namespace boa;
 
@@ -110,6 +111,9 @@ struct boa_model {
 
   // test-only switches (boa_debug_set_slab / boa_debug_set_max_wave): results do not depend on them
   bool use_slab = true;        // false: boa_compress steps one byte at a time like the decoder (same bytes)
+  uint64_t persist_max_streams = 0;     // waves up to this many streams step inside ONE persistent launch (step_persist.cuh)
+  int persist_cluster = 8;              // CTAs per row tile of 128 streams in that launch (8 = the portable maximum)
+  GrowBuf persist_layers;               // device copy of the per-layer arguments of that launch
   int pair_min_row_tiles = INT_MAX; // step-path contractions use CTA-pair tiles from this many 128-stream row tiles on (use_pair_tiles)
   uint64_t max_wave = 0;       // > 0: at most this many streams are stepped together (more chunks run in waves)
 
@@ -121,7 +125,7 @@ struct boa_model {
   ~boa_model() {
     for (GrowBuf* b : {&weights, &wimg, &u, &xz, &dbc, &u_img, &xs_img, &y_img, &f_img, &ffn_v, &logits, &h, &win, &ssq, &pos, &len, &low, &range,
                        &pending, &wpos, &cache, &started, &v, &rpos, &off, &size, &scratch, &first, &err,
-                       &stage_in, &stage_out, &total})
+                       &stage_in, &stage_out, &total, &persist_layers})
       b->release();
     pin.release();
     for (cudaEvent_t e : events) cudaEventDestroy(e);
@@ -523,10 +527,72 @@ int launch_step(StepCtx& c) {
   return BOA_OK;
 }
 
+// Small waves: all `steps` iterations inside ONE launch of the persistent step kernel (step_persist.cuh) - a cluster of
+// CTAs per row tile of 128 streams, cluster barriers between the phases of a step.  Same device code per phase as
+// launch_step's kernels, same bytes (test).  The argument structs are those launch_step builds for T = 1.
+template <int NPW>
+int launch_persist(StepCtx& c, uint64_t steps) {
+  boa_model* m = c.m;
+  const int B = c.B, D = m->D, E = m->E;
+  const int ec = (E % 256 == 0) ? 256 : 128;
+  std::vector<persist::LayerArgs> la((size_t)m->L);
+  for (int l = 0; l < m->L; ++l) {
+    const LayerW& w = m->layers[l];
+    float* hl = m->h.as<float>() + (size_t)l * m->Bcap * E * kNState;
+    float* winl = m->win.as<float>() + (size_t)l * m->Bcap * 3 * E;
+    tc::GemmArgs& gi = la[l].inproj;
+    gi = tc::GemmArgs{};
+    gi.A = m->u_img.as<uint8_t>(); gi.M = B; gi.KB = D / 64; gi.W = w.img_in; gi.NT = 2 * E / 64; gi.KS = 1;
+    gi.n_valid = 2 * E; gi.xz_ec = ec; gi.C = m->xz.as<float>(); gi.ldc = 2 * E; gi.xz_slice = (size_t)2 * ec;
+    gi.ssq_in = m->ssq.as<float>(); gi.win = winl; gi.pos = c.ca.pos; gi.slab_T = 0; gi.conv_w = w.conv_w; gi.conv_b = w.conv_b; gi.E = E;
+    gi.out_img = m->xs_img.as<uint8_t>(); gi.out_KB = E / 64;
+    tc::GemmArgs& gx = la[l].xproj;
+    gx = tc::GemmArgs{};
+    gx.A = m->xs_img.as<uint8_t>(); gx.M = B; gx.KB = E / 64; gx.W = w.img_x; gx.NT = m->ldj / 64;
+    gx.C = m->dbc.as<float>(); gx.ldc = m->ks_x * m->ldj; gx.n_valid = m->J; gx.KS = m->ks_x; gx.split_stride = (size_t)m->ldj;
+    ScanArgs& sa = la[l].scan;
+    sa = ScanArgs{};
+    sa.h = hl; sa.xz = m->xz.as<float>(); sa.dbc = m->dbc.as<float>(); sa.W_dtT = w.w_dtT; sa.b_dt = w.b_dt; sa.A4 = w.A4; sa.Dskip = w.d_skip;
+    sa.y_img = m->y_img.as<uint8_t>(); sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R; sa.KS = m->ks_x;
+    tc::GemmArgs& go = la[l].outproj;
+    go = tc::GemmArgs{};
+    go.A = m->y_img.as<uint8_t>(); go.M = B; go.KB = E / 64; go.W = w.img_out; go.NT = D / 64; go.KS = 1;
+    go.C = m->u.as<float>(); go.ldc = D; go.n_valid = D;
+    go.out_img = m->u_img.as<uint8_t>(); go.out_KB = D / 64; go.ssq_out = m->ssq.as<float>();
+    go.out_scale = (l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
+  }
+  BOA_TRY(m->persist_layers.reserve(la.size() * sizeof(persist::LayerArgs)));
+  BOA_CUDA_TRY(cudaMemcpyAsync(m->persist_layers.p, la.data(), la.size() * sizeof(persist::LayerArgs), cudaMemcpyHostToDevice, c.st));
+  BOA_CUDA_TRY(cudaStreamSynchronize(c.st));      // `la` is pageable host memory: the copy has left it
+  persist::Args p{};
+  p.layers = m->persist_layers.as<persist::LayerArgs>(); p.L = m->L;
+  p.head = tc::GemmArgs{};
+  p.head.A = m->u_img.as<uint8_t>(); p.head.M = B; p.head.KB = D / 64; p.head.W = m->img_head; p.head.NT = 4; p.head.KS = 1;
+  p.head.C = m->logits.as<float>(); p.head.ldc = 256; p.head.n_valid = 256;
+  p.logits = m->logits.as<float>(); p.data = c.data; p.chunk_bytes = c.chunk_bytes; p.ca = c.ca;
+  p.ea.emb = reinterpret_cast<const float4*>(m->emb); p.ea.norm_w = reinterpret_cast<const float4*>(m->layers[0].norm_w);
+  p.ea.u = m->u.as<float4>(); p.ea.u_img = m->u_img.as<uint8_t>(); p.ea.ssq = m->ssq.as<float>(); p.ea.D4 = D / 4;
+  p.B = B; p.mode = c.mode; p.n_steps = (uint32_t)steps; p.ec = ec;
+  const int cs = m->persist_cluster, row_tiles = (B + tc::BM - 1) / tc::BM;
+  const int smem = persist::smem_bytes<NPW>(ec, m->ldj, m->R);
+  BOA_CUDA_TRY(cudaFuncSetAttribute(persist::k_step_persist<NPW>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  if (cs > 8) BOA_CUDA_TRY(cudaFuncSetAttribute(persist::k_step_persist<NPW>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = dim3((unsigned)(row_tiles * cs)); cfg.blockDim = dim3(persist::NTHREADS); cfg.dynamicSmemBytes = (size_t)smem; cfg.stream = c.st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = (unsigned)cs; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = 1;
+  BOA_CUDA_TRY(cudaLaunchKernelEx(&cfg, persist::k_step_persist<NPW>, p));
+  return mark(c, BOA_K_CODER);
+}
+
 // Run `steps` lock-step iterations: CUDA-graph batches of kStepsPerGraph steps, remainder eager.
 int run_steps(StepCtx& c, uint64_t steps) {
   boa_model* m = c.m;
   if (steps == 0) return BOA_OK;
+  if (!c.dump && m->sample_every == 0 && m->F == 0 && c.slab_T == 1 && (uint64_t)c.B <= m->persist_max_streams)
+    return m->npw == 1 ? launch_persist<1>(c, steps) : launch_persist<3>(c, steps);
   const uint64_t S = std::min<uint64_t>(kStepsPerGraph, steps);
   const uint64_t n_batches = steps / S;
   const uint64_t rem = steps - n_batches * S;
@@ -1361,6 +1427,14 @@ int boa_debug_set_slab(boa_model* m, int enabled) {
 int boa_debug_set_pair_tiles(boa_model* m, int min_row_tiles) {
   if (!m || min_row_tiles < 0) return BOA_E_ARG;
   m->pair_min_row_tiles = min_row_tiles;
+  return BOA_OK;
+}
+
+int boa_debug_set_persist(boa_model* m, size_t max_streams, int cluster_ctas) {
+  if (!m || (cluster_ctas != 0 && cluster_ctas != 1 && cluster_ctas != 2 && cluster_ctas != 4 && cluster_ctas != 8 && cluster_ctas != 16))
+    return BOA_E_ARG;
+  m->persist_max_streams = max_streams;
+  if (cluster_ctas) m->persist_cluster = cluster_ctas;
   return BOA_OK;
 }
 

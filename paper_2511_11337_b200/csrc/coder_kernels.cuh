@@ -229,15 +229,13 @@ __device__ __forceinline__ void embed_row(const EmbedArgs& ea, int i, uint32_t s
 // MODE 0 = encode, 1 = decode.  One warp per stream.  `data` is the input (encode) or output (decode)
 // buffer of this wave: stream i, byte t at data[i*chunk + t].
 // DUMP: additionally write logits-derived probabilities / the whole CDF for row i*dump_steps + pos.
+// One coder step of stream i by one warp (all 32 lanes call): table from the stream's logits, the symbol's interval
+// (encode) or the search for the decoder's target (decode), the coder update by lane 0, the embedding of the next byte.
+// Shared by k_coder_step (one launch per step) and the persistent step kernel (step_persist.cuh).
 template <int MODE, bool DUMP>
-__global__ void __launch_bounds__(256)
-k_coder_step(const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes, CoderArrays ca, int B,
-             EmbedArgs ea, float* dump_probs, uint32_t* dump_cdf, uint32_t dump_steps) {
-  const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  pdl_launch();
-  pdl_wait();                                     // logits, coder state and (decode) the output buffer come from earlier kernels
-  if (i >= B) return;
+__device__ __forceinline__ void coder_step_one(int i, int lane, const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes,
+                                               const CoderArrays& ca, const EmbedArgs& ea, float* dump_probs, uint32_t* dump_cdf,
+                                               uint32_t dump_steps) {
   const uint32_t pos = ca.pos[i], len = ca.len[i];
   if (pos + 1u >= len) return;                    // finished stream: masked
 
@@ -310,6 +308,18 @@ k_coder_step(const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes
       if (corrupt) *ca.err = 1;
     }
   }
+}
+
+template <int MODE, bool DUMP>
+__global__ void __launch_bounds__(256)
+k_coder_step(const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes, CoderArrays ca, int B,
+             EmbedArgs ea, float* dump_probs, uint32_t* dump_cdf, uint32_t dump_steps) {
+  const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
+  const int lane = threadIdx.x & 31;
+  pdl_launch();
+  pdl_wait();                                     // logits, coder state and (decode) the output buffer come from earlier kernels
+  if (i >= B) return;
+  coder_step_one<MODE, DUMP>(i, lane, logits, data, chunk_bytes, ca, ea, dump_probs, dump_cdf, dump_steps);
 }
 
 // Encode-side time slab: the T tables of a stream (logits rows i*T + t) are coded one after the

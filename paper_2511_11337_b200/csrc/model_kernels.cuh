@@ -243,15 +243,16 @@ __device__ __forceinline__ float scan_channel_step(const float* row, int R, cons
   return yv * silu_fast(z);
 }
 
-// grid = (CTAs per slice, E / EC), block = EC + 32 threads (EC = 256 or 128), two CTAs per SM.
-// Warps 0..EC/32-1: one thread per channel of the slice.  The last warp drives the bulk copies and moves the y pieces.
+// The roles of a scan CTA over the streams i_begin + bx, + gx, ... < i_end of channel slice `sl` (EC channels):
+// threads 0..EC-1 = one thread per channel, the warp after them drives the bulk copies and moves the y pieces; later
+// threads (if the block is larger) only take part in the block barrier.  Initialises its own barriers in `scan_smem`.
+// Shared by k_scan (one launch per layer and step) and the persistent step kernel (step_persist.cuh).
 // RR = dt_rank when W_dt's row is held in registers (4, 8, 16, 32), else 0 (row kept in shared memory).
 template <int RR>
-__global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
+__device__ __forceinline__ void scan_roles(const ScanArgs& a, uint8_t* scan_smem, int EC, int sl, int slices, int bx, int gx,
+                                           int i_begin, int i_end) {
   using namespace scan;
-  extern __shared__ __align__(128) uint8_t scan_smem[];
-  const int EC = blockDim.x - 32, tid = threadIdx.x;
-  const int slices = gridDim.y, sl = blockIdx.y;
+  const int tid = threadIdx.x;
   const int e0 = sl * EC;
   const int SB = stage_bytes(EC, a.ldj);
   uint8_t* sbufs = scan_smem;                      // [NSB][EC*64] state buffers
@@ -260,7 +261,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   uint64_t* bars = reinterpret_cast<uint64_t*>(stages + NSTG * SB + (RR ? 0 : a.R * EC * 4));   // full, done, ready [NSTG] each
   constexpr int T = 1;                             // steps per stream and launch (the time-slab form is k_scan_slab)
   constexpr int LA = NSB;                          // copies run LA iterations ahead: one state buffer each
-  const int nk = (a.B - (int)blockIdx.x + (int)gridDim.x - 1) / (int)gridDim.x;   // streams of this CTA
+  const int nk = (i_end - i_begin - bx + gx - 1) / gx;   // streams of this CTA
   if (nk <= 0) return;
 
   if (tid == 0) {
@@ -273,6 +274,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   }
   __syncthreads();
   pdl_launch();
+  if (tid >= EC + 32) return;
 
   if (tid >= EC) {
     // ===================================================================== copy warp
@@ -288,7 +290,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     const float* xz0 = a.xz + (size_t)sl * 2 * EC;
     const uint32_t xz_bytes = (uint32_t)(2 * EC * 4), dbc_bytes = (uint32_t)(a.KS * a.ldj * 4);
     int ik = 0, it_ = 0, ikk = 0;                  // next copy to issue: stream, step, iteration
-    size_t ii = blockIdx.x;                        // its stream index in the wave
+    size_t ii = (size_t)(i_begin + bx);                        // its stream index in the wave
     auto issue_next = [&]() {   // lane 0
       const int s = ikk & (NSTG - 1);
       const size_t row = (size_t)it_ * a.B + ii;
@@ -298,7 +300,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
       g2s(st, xz0 + row * 2 * a.E, xz_bytes, bar);                                                  // xs | z
       g2s(st + 2 * EC * 4 + EC * 6, a.dbc + row * a.KS * a.ldj, dbc_bytes, bar);                     // all partials
       ++ikk;
-      if (++it_ == T) { it_ = 0; ++ik; ii += gridDim.x; }
+      if (++it_ == T) { it_ = 0; ++ik; ii += gx; }
     };
     // S5, last step: the k-split partials of the x_proj row are added in ascending order, in place, once per stream-step
     auto reduce_row = [&](int kk) {   // whole warp
@@ -331,7 +333,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     const uint64_t keep = tc::policy_evict_last();
     reduce_row(0);
     int k = 0, t = 0;                              // this iteration's stream and step
-    size_t i = blockIdx.x;
+    size_t i = (size_t)(i_begin + bx);
     for (int kk = 0; kk < niter; ++kk) {
       const int s = kk & (NSTG - 1);
       uint8_t* st = stages + s * SB;
@@ -353,10 +355,10 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
         asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // every state store but this iteration's has left its buffer
         issue_next();                              // iteration kk - 1 + LA
       }
-      if (++t == T) { t = 0; ++k; i += gridDim.x; }
+      if (++t == T) { t = 0; ++k; i += gx; }
     }
-    if (lane == 0) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
-    return;
+    if (lane == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");   // the state stores are complete (the persistent
+    return;                                                                     // step kernel reads them back in the next step)
   }
 
   // ======================================================================= channel threads
@@ -375,7 +377,7 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
   const int niter = nk * T;
   float4 h0, h1, h2, h3;                           // the channel's 16 state values: in registers across a slab
   int k = 0, t = 0;
-  size_t row_i = blockIdx.x;                       // this iteration's stream index in the wave
+  size_t row_i = (size_t)(i_begin + bx);                       // this iteration's stream index in the wave
   for (int kk = 0; kk < niter; ++kk) {
     const int s = kk & (NSTG - 1);
     uint8_t* st = stages + s * SB;
@@ -400,8 +402,15 @@ __global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
     }
     if (t == T - 1) asm volatile("fence.proxy.async.shared::cta;" ::: "memory");   // the state leaves by a bulk store
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(&bars[NSTG + s])) : "memory");
-    if (++t == T) { t = 0; ++k; row_i += gridDim.x; }
+    if (++t == T) { t = 0; ++k; row_i += gx; }
   }
+}
+
+// grid = (CTAs per slice, E / EC), block = EC + 32 threads (EC = 256 or 128), two CTAs per SM.
+template <int RR>
+__global__ void __launch_bounds__(288, 2) k_scan(const ScanArgs a) {
+  extern __shared__ __align__(128) uint8_t scan_smem[];
+  scan_roles<RR>(a, scan_smem, (int)blockDim.x - 32, (int)blockIdx.y, (int)gridDim.y, (int)blockIdx.x, (int)gridDim.x, 0, a.B);
 }
 
 // ---------------------------------------------------------------------------------------------------

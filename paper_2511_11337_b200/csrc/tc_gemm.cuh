@@ -298,58 +298,45 @@ __device__ __forceinline__ float conv_silu1(float4 w, float b, float xm3, float 
 constexpr int NEPI = 256;        // epilogue threads (warps 0-7); warp 8 owns TMEM and issues the MMAs; warp 9 drives the copies
 constexpr int NTHREADS = NEPI + 64;
 
-// ------------------------------------------------------------------------------------------ the kernel
-// grid = min(tiles, SMs), block = 320.  Tile t -> (row tile t / NT, column tile t % NT); CTA c takes tiles c,
-// c + grid, ...  Warp 9 (one lane) streams the k-blocks of both operand images into the stage ring; warp 8 (one lane)
-// issues the MMAs into accumulator buffer (tile iteration & 1); warps 0-7 drain the other buffer and run the epilogue.
-// CS > 1: the kernel is launched in clusters of CS CTAs that take CS consecutive column tiles of the same row tile in
-// lock-step and share its activation k-blocks: each CTA fetches 1/CS of the 48 KB block and the bulk copy delivers
-// it to all of them (multicast); a stage is reused when the MMAs of ALL CTAs of the cluster have read it.
-// SLAB (EPI_INPROJ with g.slab_T > 0 only): the time-slab form of the conv epilogue, whose tiles are epilogue-bound;
-// it fetches what the epilogue reads from global memory (block sums of u^2, window values) ahead of time with
-// cp.async into shared memory.  The step form (SLAB = false) is bound by its main loop and reads them directly.
-template <int NPW, int EPI, int CS, bool SLAB = false>
-__global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
-  using C = Cfg<NPW>;
-  static_assert(NPW == 1 || NPW == 3, "weight pieces");
-  static_assert(CS == 1 || CS == 2 || CS == 4 || CS == 8, "cluster size");
-  constexpr uint16_t CMASK = (uint16_t)((1u << CS) - 1u);
-  extern __shared__ uint8_t smem_raw[];
-  __shared__ __align__(8) uint64_t full_bar[C::NST], empty_bar[C::NST], acc_full[2], acc_empty[2];
-  __shared__ uint32_t tmem_base_s;
+// ------------------------------------------------------------------------------------------ the contraction
+// Shared-memory objects of a contraction CTA: the stage ring, its barriers, the TMEM accumulators.
+struct GemmShared {
+  uint8_t* raw;            // dynamic shared memory (stage ring + staging tile [+ prefetch area])
+  uint64_t *full_bar, *empty_bar, *acc_full, *acc_empty;
+  uint32_t tmem;           // TMEM base address of the accumulators
+};
+// (Re-)initialise the barriers of the ring: one thread; the caller fences and synchronises the block (and cluster).
+template <int NPW, int CS>
+__device__ __forceinline__ void gemm_init_barriers(const GemmShared& sh) {
+  for (int s = 0; s < Cfg<NPW>::NST; ++s) {
+    mbar_init(smem_u32(&sh.full_bar[s]), 1);     // the copy warp's arrive.expect_tx
+    mbar_init(smem_u32(&sh.empty_bar[s]), CS);   // one tcgen05.commit per CTA of the cluster
+  }
+  for (int b = 0; b < 2; ++b) {
+    mbar_init(smem_u32(&sh.acc_full[b]), 1);     // one tcgen05.commit
+    mbar_init(smem_u32(&sh.acc_empty[b]), NEPI); // every epilogue thread has drained its part
+  }
+  fence_barrier_init();
+}
 
+// The three roles of a contraction CTA over its work items tile_begin + item0, + item_step, ... < tile_end (item index ->
+// (row tile, column tile [pair], k-split), k-split fastest).  Called by all NTHREADS threads with freshly initialised
+// barriers; returns when this CTA's copies are issued, its MMAs committed and its epilogues done (the caller
+// synchronises).  Shared by k_tc_gemm (one launch per contraction) and the persistent step kernel (step_persist.cuh).
+template <int NPW, int EPI, int CS, bool SLAB>
+__device__ __forceinline__ void gemm_roles(const GemmArgs& g, const GemmShared& sh, int item0, int item_step, int tile_begin,
+                                           int tile_end, int crank) {
+  using C = Cfg<NPW>;
+  constexpr uint16_t CMASK = (uint16_t)((1u << CS) - 1u);
+  uint8_t* smem_raw = sh.raw;
+  uint64_t *full_bar = sh.full_bar, *empty_bar = sh.empty_bar, *acc_full = sh.acc_full, *acc_empty = sh.acc_empty;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int KB = g.KB / g.KS, NT = g.NT, KS = g.KS;     // KB: k-blocks of one work item
-  // work item t -> (row tile, column tile [pair], k-split), k-split fastest; with CS = 2 an item is a pair of column
-  // tiles and this CTA takes the one of its rank
   const int NTI = NT / CS;
-  const int ntiles = ((g.M + BM - 1) / BM) * NTI * KS;
-  const int crank = CS > 1 ? (int)cluster_ctarank() : 0;
-  const int item0 = (int)blockIdx.x / CS, item_step = (int)gridDim.x / CS;
+  const int ntiles = tile_end;
+  item0 += tile_begin;
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
-
-  if (warp == 8) {
-    if (lane == 0) {
-      for (int s = 0; s < C::NST; ++s) {
-        mbar_init(smem_u32(&full_bar[s]), 1);     // the copy warp's arrive.expect_tx
-        mbar_init(smem_u32(&empty_bar[s]), CS);   // one tcgen05.commit per CTA of the cluster
-      }
-      for (int b = 0; b < 2; ++b) {
-        mbar_init(smem_u32(&acc_full[b]), 1);     // one tcgen05.commit
-        mbar_init(smem_u32(&acc_empty[b]), NEPI); // every epilogue thread has drained its part
-      }
-      fence_barrier_init();
-    }
-    __syncwarp();
-    tmem_alloc(smem_u32(&tmem_base_s), C::TMEM_COLS);
-  }
-  tc_fence_before();
-  __syncthreads();
-  if (CS > 1) cluster_sync();                      // the peers' barriers are initialised before anything is sent to them
-  tc_fence_after();
-  const uint32_t tmem = tmem_base_s;
-  pdl_launch();
-  pdl_wait();                                      // everything below reads what earlier kernels of the step wrote
+  const uint32_t tmem = sh.tmem;
 
   if (warp == 9) {
     // ===================================================================== copy warp
@@ -668,12 +655,50 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
     }
   }
 
+}
+
+// ------------------------------------------------------------------------------------------ the kernel
+// grid = min(tiles, SMs), block = 320.  Tile t -> (row tile t / NT, column tile t % NT); CTA c takes tiles c,
+// c + grid, ...  Warp 9 (one lane) streams the k-blocks of both operand images into the stage ring; warp 8 (one lane)
+// issues the MMAs into accumulator buffer (tile iteration & 1); warps 0-7 drain the other buffer and run the epilogue.
+// CS > 1: the kernel is launched in clusters of CS CTAs that take CS consecutive column tiles of the same row tile in
+// lock-step and share its activation k-blocks: each CTA fetches 1/CS of the 48 KB block and the bulk copy delivers
+// it to all of them (multicast); a stage is reused when the MMAs of ALL CTAs of the cluster have read it.
+// SLAB (EPI_INPROJ with g.slab_T > 0 only): the time-slab form of the conv epilogue, whose tiles are epilogue-bound;
+// it fetches what the epilogue reads from global memory (block sums of u^2, window values) ahead of time with
+// cp.async into shared memory.  The step form (SLAB = false) is bound by its main loop and reads them directly.
+template <int NPW, int EPI, int CS, bool SLAB = false>
+__global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
+  using C = Cfg<NPW>;
+  static_assert(NPW == 1 || NPW == 3, "weight pieces");
+  static_assert(CS == 1 || CS == 2 || CS == 4 || CS == 8, "cluster size");
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t full_bar[C::NST], empty_bar[C::NST], acc_full[2], acc_empty[2];
+  __shared__ uint32_t tmem_base_s;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  GemmShared sh{smem_raw, full_bar, empty_bar, acc_full, acc_empty, 0u};
+  if (warp == 8) {
+    if (lane == 0) gemm_init_barriers<NPW, CS>(sh);
+    __syncwarp();
+    tmem_alloc(smem_u32(&tmem_base_s), C::TMEM_COLS);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (CS > 1) cluster_sync();                      // the peers' barriers are initialised before anything is sent to them
+  tc_fence_after();
+  sh.tmem = tmem_base_s;
+  pdl_launch();
+  pdl_wait();                                      // everything below reads what earlier kernels of the step wrote
+
+  const int ntiles = ((g.M + BM - 1) / BM) * (g.NT / CS) * g.KS;
+  gemm_roles<NPW, EPI, CS, SLAB>(g, sh, (int)blockIdx.x / CS, (int)gridDim.x / CS, 0, ntiles, CS > 1 ? (int)cluster_ctarank() : 0);
+
   tc_fence_before();
   __syncthreads();
   if (CS > 1) cluster_sync();                      // no CTA leaves while a peer may still send to it
   if (warp == 8) {
     __syncwarp();
-    tmem_dealloc(tmem, C::TMEM_COLS);
+    tmem_dealloc(sh.tmem, C::TMEM_COLS);
   }
 }
 

@@ -166,6 +166,36 @@ def test_pair_tiles_and_single_tiles_write_the_same_container(boa, shape):
             gm.debug_set_pair_tiles(2 ** 31 - 1)
 
 
+@pytest.mark.parametrize("shape", ["cfg1", "d192_l1", "cfg2", "cfg4_bf16", "cfg5_l2_bf16"])
+def test_persistent_step_kernel_writes_the_bytes_of_the_graph_path(boa, shape):
+    """north_star's persistent decode-step kernel (step_persist.cuh: one launch steps a small wave for all of its bytes,
+    a cluster of CTAs per row tile, cluster barriers between the phases) against the graph of one kernel per phase: same
+    container when encoding step by step, and each decodes the other's - for 1, 5, 64, 130 (two row tiles) and 300
+    streams, clusters of 8, 4 and 1 CTAs (fewer CTAs than scan slices), ragged tails, 1 to 4 layers."""
+    s1 = synth.CONFIGS[1]
+    blob = {"cfg1": lambda: s1.weights(emb_std=0.25),
+            "d192_l1": lambda: synth.make_weights(synth.ModelShape(1, 192), 5, emb_std=0.25),
+            "cfg2": lambda: synth.make_weights(synth.CONFIGS[2].shape, 1, emb_std=0.25),
+            "cfg4_bf16": lambda: synth.make_weights(synth.CONFIGS[4].shape, 2, synth.DTYPE_BF16, emb_std=0.25),
+            "cfg5_l2_bf16": lambda: synth.make_weights(synth.ModelShape(2, 512, dt_rank=32), 3, synth.DTYPE_BF16, emb_std=0.25)}[shape]()
+    gm = boa.Model(blob)
+    gm.debug_set_slab(False)                                       # encode with the step path, like the decoder
+    try:
+        for n, chunk, cluster in [(1 * 37, 37, 8), (5 * 41 + 13, 41, 8), (64 * 29, 29, 4), (130 * 23, 23, 8), (300 * 19 + 5, 19, 1), (9, 40, 8)]:
+            data = s1.data(n)
+            gm.debug_set_persist(0)
+            graph = gm.compress(data, chunk)
+            gm.debug_set_persist(1 << 20, cluster)
+            pers = gm.compress(data, chunk)
+            assert torch.equal(graph, pers), (shape, n, chunk, cluster)
+            assert _np(gm.decompress(graph)).tobytes() == data     # persistent decoder
+            gm.debug_set_persist(0)
+            assert _np(gm.decompress(pers)).tobytes() == data      # graph decoder
+    finally:
+        gm.debug_set_slab(True)
+        gm.debug_set_persist(0, 8)
+
+
 # ---------------------------------------------------------------------------------------------- check 1
 @pytest.mark.parametrize("kind", ["uniform", "peaked", "random"])
 def test_range_coder_bit_exact_given_oracle_tables(boa, kind):
