@@ -67,10 +67,10 @@ __device__ __forceinline__ void phase_sync() {
 template <int NPW, int EPI>
 __device__ __forceinline__ void gemm_phase(const tc::GemmArgs& g, const tc::GemmShared& sh, int rt, int crank, int csize) {
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  if (warp == 8 && lane == 0) tc::gemm_init_barriers<NPW, 1>(sh);   // the rings start from phase 0 in every contraction
+  if (warp == 8 && lane == 0) tc::gemm_init_barriers<NPW, 1>(sh, tc::MAXST);   // the rings start from phase 0 in every contraction
   __syncthreads();
   const int per_rt = g.NT * g.KS;
-  tc::gemm_roles<NPW, EPI, 1, false>(g, sh, crank, csize, rt * per_rt, (rt + 1) * per_rt, 0);
+  tc::gemm_roles<NPW, EPI, 1, false, true>(g, sh, crank, csize, rt * per_rt, (rt + 1) * per_rt, 0);
   phase_sync();
 }
 
@@ -79,7 +79,7 @@ template <int NPW>
 __global__ void __launch_bounds__(NTHREADS, 1) k_step_persist(const Args p) {
   using C = tc::Cfg<NPW>;
   extern __shared__ uint8_t smem_raw[];
-  __shared__ __align__(8) uint64_t full_bar[C::NST], empty_bar[C::NST], acc_full[2], acc_empty[2];
+  __shared__ __align__(8) uint64_t full_bar[tc::MAXST], empty_bar[tc::MAXST], acc_full[2], acc_empty[2];
   __shared__ uint32_t tmem_base_s;
   const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   uint32_t csize_u;

@@ -307,8 +307,8 @@ struct GemmShared {
 };
 // (Re-)initialise the barriers of the ring: one thread; the caller fences and synchronises the block (and cluster).
 template <int NPW, int CS>
-__device__ __forceinline__ void gemm_init_barriers(const GemmShared& sh) {
-  for (int s = 0; s < Cfg<NPW>::NST; ++s) {
+__device__ __forceinline__ void gemm_init_barriers(const GemmShared& sh, int nst = Cfg<NPW>::NST) {
+  for (int s = 0; s < nst; ++s) {
     mbar_init(smem_u32(&sh.full_bar[s]), 1);     // the copy warp's arrive.expect_tx
     mbar_init(smem_u32(&sh.empty_bar[s]), CS);   // one tcgen05.commit per CTA of the cluster
   }
@@ -323,10 +323,17 @@ __device__ __forceinline__ void gemm_init_barriers(const GemmShared& sh) {
 // (row tile, column tile [pair], k-split), k-split fastest).  Called by all NTHREADS threads with freshly initialised
 // barriers; returns when this CTA's copies are issued, its MMAs committed and its epilogues done (the caller
 // synchronises).  Shared by k_tc_gemm (one launch per contraction) and the persistent step kernel (step_persist.cuh).
-template <int NPW, int EPI, int CS, bool SLAB>
+// COMPACT (the persistent step kernel at few streams; all items of a call share one row tile): when the row tile has at
+// most 64 live rows only their 8-row groups of each activation piece are copied (1 KB per group instead of the 16 KB
+// plane; the MMA still reads 128 rows, the rows beyond are whatever follows in shared memory and only reach accumulator
+// rows nobody reads), which makes a stage small enough for a ring of up to MAXST stages: every k-block of a work item is
+// in flight at once instead of NST at a time.  The result rows of live streams are the same bits either way.
+constexpr int MAXST = 16;        // barrier slots a COMPACT caller provides
+template <int NPW, int EPI, int CS, bool SLAB, bool COMPACT = false>
 __device__ __forceinline__ void gemm_roles(const GemmArgs& g, const GemmShared& sh, int item0, int item_step, int tile_begin,
                                            int tile_end, int crank) {
   using C = Cfg<NPW>;
+  static_assert(!COMPACT || CS == 1, "compact stages: no multicast");
   constexpr uint16_t CMASK = (uint16_t)((1u << CS) - 1u);
   uint8_t* smem_raw = sh.raw;
   uint64_t *full_bar = sh.full_bar, *empty_bar = sh.empty_bar, *acc_full = sh.acc_full, *acc_empty = sh.acc_empty;
@@ -337,6 +344,17 @@ __device__ __forceinline__ void gemm_roles(const GemmArgs& g, const GemmShared& 
   item0 += tile_begin;
   const uint32_t sbase = (smem_u32(smem_raw) + 1023u) & ~1023u;
   const uint32_t tmem = sh.tmem;
+  // stage geometry: compile-time constants unless COMPACT
+  uint32_t plane = (uint32_t)A_PLANE, stage = (uint32_t)C::STAGE;
+  int nst = C::NST;
+  if (COMPACT) {
+    const int live = min(g.M - (tile_begin / KS / NTI) * BM, BM), r8 = (live + 7) >> 3;
+    if (r8 <= 8) {
+      plane = (uint32_t)r8 * 1024u;
+      stage = NPA * plane + (uint32_t)C::W_BYTES;
+      nst = min(MAXST, (int)((uint32_t)(C::NST * C::STAGE - A_PLANE) / stage));
+    }
+  }
 
   if (warp == 9) {
     // ===================================================================== copy warp
@@ -347,16 +365,20 @@ __device__ __forceinline__ void gemm_roles(const GemmArgs& g, const GemmShared& 
         const uint8_t* asrc = g.A + img_block((size_t)mt, (size_t)ks * KB, (size_t)g.KB);
         const uint16_t* wsrc = g.W + ((size_t)nt * g.KB + (size_t)ks * KB) * (NPW * BN * 64);
         for (int kb = 0; kb < KB; ++kb, ++kbc) {
-          const int s = kbc % C::NST, round = kbc / C::NST;
+          const int s = kbc % nst, round = kbc / nst;
           if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
-          const uint32_t sA = sbase + (uint32_t)s * C::STAGE, fb = smem_u32(&full_bar[s]);
-          mbar_arrive_expect_tx(fb, (uint32_t)C::STAGE);
-          if (CS > 1)                              // this CTA's part of the block, delivered to every CTA of the cluster
+          const uint32_t sA = sbase + (uint32_t)s * stage, fb = smem_u32(&full_bar[s]);
+          mbar_arrive_expect_tx(fb, stage);
+          if (COMPACT && plane != (uint32_t)A_PLANE) {   // the live 8-row groups of each piece plane
+#pragma unroll
+            for (int q = 0; q < NPA; ++q)
+              bulk_g2s(sA + (uint32_t)q * plane, asrc + (size_t)kb * C::A_BYTES + (size_t)q * A_PLANE, plane, fb);
+          } else if (CS > 1)                              // this CTA's part of the block, delivered to every CTA of the cluster
             bulk_g2s_mc(sA + (uint32_t)crank * (C::A_BYTES / CS), asrc + (size_t)kb * C::A_BYTES + (size_t)crank * (C::A_BYTES / CS),
                         (uint32_t)(C::A_BYTES / CS), fb, CMASK);
           else
             bulk_g2s(sA, asrc + (size_t)kb * C::A_BYTES, (uint32_t)C::A_BYTES, fb);
-          bulk_g2s(sA + C::A_BYTES, wsrc + (size_t)kb * (NPW * BN * 64), (uint32_t)C::W_BYTES, fb);
+          bulk_g2s(sA + NPA * plane, wsrc + (size_t)kb * (NPW * BN * 64), (uint32_t)C::W_BYTES, fb);
         }
       }
     }
@@ -372,16 +394,16 @@ __device__ __forceinline__ void gemm_roles(const GemmArgs& g, const GemmShared& 
         }
         const uint32_t tacc = tmem + (uint32_t)(b * C::ACC_COLS);
         for (int kb = 0; kb < KB; ++kb, ++kbc) {
-          const int s = kbc % C::NST, round = kbc / C::NST;
+          const int s = kbc % nst, round = kbc / nst;
           mbar_wait(smem_u32(&full_bar[s]), (uint32_t)(round & 1));
           tc_fence_after();
-          const uint32_t sA = sbase + (uint32_t)s * C::STAGE;
-          const uint32_t sW = sA + C::A_BYTES;
+          const uint32_t sA = sbase + (uint32_t)s * stage;
+          const uint32_t sW = sA + NPA * plane;
 #pragma unroll
           for (int k4 = 0; k4 < BK / 16; ++k4) {
             const uint32_t first = (kb | k4) ? 1u : 0u;
             const uint32_t ko = (uint32_t)k4 * 32u;
-            auto A_ = [&](int p) { return smem_desc_sw128(sA + p * A_PLANE + ko); };
+            auto A_ = [&](int p) { return smem_desc_sw128(sA + (uint32_t)p * plane + ko); };
             const uint64_t wd = smem_desc_sw128(sW + ko);
             if (NPW == 3) {
               umma(tacc, A_(0), wd, idesc_bf16(192), first);         // a1 x [w1;w2;w3] -> classes 0,1,2
