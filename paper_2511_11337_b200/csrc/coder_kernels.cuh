@@ -132,13 +132,47 @@ struct EncState {            // eq. 8-11; `low` uses bits 0..32 (bit 32 = carry)
   uint8_t started;
 };
 
-__device__ __forceinline__ void enc_shift_low(EncState& s, uint8_t* out) {
+// Where the encoder's bytes go.  ByteSink: one store per byte (test kernels, rows of any alignment).  VecSink: the
+// stream's payload scratch row in 16-byte blocks ("coalesced vectorised stores", north_star): bytes are collected in four
+// registers and leave as one aligned 16-byte store when a block is full; begin() reloads a block left partly filled by
+// an earlier launch, end() stores the current partial block (the bytes beyond wpos in it are not payload: the row is
+// 16-byte aligned and padded, and the compaction copies sizes[i] bytes only).
+struct ByteSink {
+  uint8_t* out;
+  __device__ __forceinline__ void begin(uint8_t* row, uint32_t) { out = row; }
+  __device__ __forceinline__ void put(uint32_t& wpos, uint8_t b) { out[wpos++] = b; }
+  __device__ __forceinline__ void end(uint32_t) {}
+};
+struct VecSink {
+  uint8_t* out;
+  uint32_t w[4];
+  __device__ __forceinline__ void begin(uint8_t* row, uint32_t wpos) {
+    out = row;
+    uint4 v = make_uint4(0u, 0u, 0u, 0u);
+    if (wpos & 15u) v = *reinterpret_cast<const uint4*>(row + (wpos & ~15u));
+    w[0] = v.x; w[1] = v.y; w[2] = v.z; w[3] = v.w;
+  }
+  __device__ __forceinline__ void put(uint32_t& wpos, uint8_t b) {
+    const uint32_t k = wpos & 15u, sh = (k & 3u) * 8u;
+#pragma unroll
+    for (int j = 0; j < 4; ++j)
+      if ((k >> 2) == (uint32_t)j) w[j] = (w[j] & ~(0xFFu << sh)) | ((uint32_t)b << sh);
+    ++wpos;
+    if ((wpos & 15u) == 0u) *reinterpret_cast<uint4*>(out + wpos - 16u) = make_uint4(w[0], w[1], w[2], w[3]);
+  }
+  __device__ __forceinline__ void end(uint32_t wpos) {
+    if (wpos & 15u) *reinterpret_cast<uint4*>(out + (wpos & ~15u)) = make_uint4(w[0], w[1], w[2], w[3]);
+  }
+};
+
+template <class Sink>
+__device__ __forceinline__ void enc_shift_low(EncState& s, Sink& out) {
   const uint32_t lo32 = (uint32_t)s.low;
   const uint32_t carry = (uint32_t)(s.low >> 32);
   if (lo32 < 0xFF000000u || carry == 1u) {
-    if (s.started) out[s.wpos++] = (uint8_t)(s.cache + carry);
+    if (s.started) out.put(s.wpos, (uint8_t)(s.cache + carry));
     const uint8_t fill = (uint8_t)(0xFFu + carry);
-    for (; s.pending; --s.pending) out[s.wpos++] = fill;
+    for (; s.pending; --s.pending) out.put(s.wpos, fill);
     s.started = 1;
     s.cache = (uint8_t)(lo32 >> 24);
   } else {
@@ -147,7 +181,8 @@ __device__ __forceinline__ void enc_shift_low(EncState& s, uint8_t* out) {
   s.low = (uint64_t)(lo32 & 0x00FFFFFFu) << 8;
 }
 
-__device__ __forceinline__ void enc_symbol(EncState& s, uint32_t c_lo, uint32_t c_hi, uint8_t* out) {
+template <class Sink>
+__device__ __forceinline__ void enc_symbol(EncState& s, uint32_t c_lo, uint32_t c_hi, Sink& out) {
   s.low += ((uint64_t)s.range * c_lo) >> kFreqBits;                      // eq. 8
   s.range = (uint32_t)(((uint64_t)s.range * (c_hi - c_lo)) >> kFreqBits); // eq. 9
   while (s.range < kRcTop) {                                              // eq. 10-11 (R#6)
@@ -282,7 +317,10 @@ __device__ __forceinline__ void coder_step_one(int i, int lane, const float* __r
       EncState st;
       st.low = ca.low[i]; st.range = ca.range[i]; st.pending = ca.pending[i]; st.wpos = ca.wpos[i];
       st.cache = ca.cache[i]; st.started = ca.started[i];
-      enc_symbol(st, c_lo, c_hi, ca.scratch + (size_t)i * ca.cap);
+      VecSink sink;
+      sink.begin(ca.scratch + (size_t)i * ca.cap, st.wpos);
+      enc_symbol(st, c_lo, c_hi, sink);
+      sink.end(st.wpos);
       ca.low[i] = st.low; ca.range[i] = st.range; ca.pending[i] = st.pending; ca.wpos[i] = st.wpos;
       ca.cache[i] = st.cache; ca.started[i] = st.started;
       ca.pos[i] = pos + 1u;
@@ -339,7 +377,8 @@ k_coder_slab(const float* __restrict__ logits, const uint8_t* __restrict__ data,
   st.low = ca.low[i]; st.range = ca.range[i]; st.pending = ca.pending[i]; st.wpos = ca.wpos[i];
   st.cache = ca.cache[i]; st.started = ca.started[i];
   const uint8_t* sdata = data + (size_t)i * chunk_bytes;
-  uint8_t* out = ca.scratch + (size_t)i * ca.cap;
+  VecSink out;                                    // (used by lane 0 only) the slab's bytes leave in 16-byte blocks
+  out.begin(ca.scratch + (size_t)i * ca.cap, st.wpos);
   uint32_t done = 0;
   for (int t = 0; t < T && pos + 1u + (uint32_t)t < len; ++t) {
     float l[8];
@@ -355,6 +394,7 @@ k_coder_slab(const float* __restrict__ logits, const uint8_t* __restrict__ data,
     ++done;
   }
   if (lane == 0) {
+    out.end(st.wpos);
     ca.low[i] = st.low; ca.range[i] = st.range; ca.pending[i] = st.pending; ca.wpos[i] = st.wpos;
     ca.cache[i] = st.cache; ca.started[i] = st.started;
     ca.pos[i] = pos + done;
@@ -396,8 +436,10 @@ __global__ void k_coder_finish(CoderArrays ca, int B) {
     EncState st;
     st.low = ca.low[i]; st.range = ca.range[i]; st.pending = ca.pending[i]; st.wpos = ca.wpos[i];
     st.cache = ca.cache[i]; st.started = ca.started[i];
-    uint8_t* out = ca.scratch + (size_t)i * ca.cap;
+    VecSink out;
+    out.begin(ca.scratch + (size_t)i * ca.cap, st.wpos);
     for (int k = 0; k < 5; ++k) enc_shift_low(st, out);
+    out.end(st.wpos);
     ca.wpos[i] = st.wpos;
   } else {
     if (ca.rpos[i] != ca.size[i] || ca.pos[i] + 1u != ca.len[i]) *ca.err = 1;
@@ -502,7 +544,8 @@ __global__ void k_debug_rc_encode(const uint32_t* __restrict__ cdf, const uint8_
   if (i >= B) return;
   EncState st;
   st.low = 0; st.range = 0xFFFFFFFFu; st.pending = 0; st.wpos = 0; st.cache = 0; st.started = 0;
-  uint8_t* o = out + (size_t)i * cap;
+  ByteSink o;
+  o.begin(out + (size_t)i * cap, 0u);
   for (uint32_t t = 0; t < len; ++t) {
     if (st.wpos + st.pending + 8u > cap) { *err = 1; sizes[i] = 0; return; }
     const uint32_t* C = cdf + ((size_t)i * len + t) * 257;

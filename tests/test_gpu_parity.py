@@ -342,6 +342,10 @@ def test_parity_subset_of_the_configured_inputs(boa, name):
     assert err <= PROB_TOL                                                                                  # check 2
     assert abs(comp.numel() - ref_size) <= SIZE_TOL * ref_size                                              # check 3
     assert all(0 < g < 5 for g in gaps)
+    # check 1 on the product path itself (time-slab coder, 16-byte staged stores, device-side compaction): every payload is,
+    # byte for byte, what the ORACLE's range coder writes for the GPU's own tables
+    for i in range(len(ids)):
+        assert payloads[i] == rangecoder.encode_stream(C_gpu[i], chunks[i, 1:].astype(np.int64)), (name, ids[i])
 
 
 # ---------------------------------------------------------------------------------------------- edges
