@@ -64,8 +64,11 @@ typedef struct boa_model boa_model; /* opaque: device weights + workspace */
 int boa_model_load(const void* weights, size_t nbytes, boa_model** out);
 void boa_model_free(boa_model* m);
 
-/* 64-bit fingerprint stored in every container: (arithmetic version << 32) | CRC-32(blob).
- * Tables are only reproducible with the same weights AND the same arithmetic. */
+/* 64-bit fingerprint stored in every container: (arithmetic word << 32) | CRC-32(blob).
+ * Tables are only reproducible with the same weights AND the same arithmetic.  The arithmetic word is the
+ * kernel generation number XOR the CRC-32 of the fp32 logits that this build's step kernels produce, on this device, for
+ * a fixed 120-byte probe input stepped through this model at boa_model_load: a build whose kernels round differently
+ * cannot forget to change it. */
 uint64_t boa_model_fingerprint(const boa_model* m);
 
 /* ---- compress ---------------------------------------------------------------------------

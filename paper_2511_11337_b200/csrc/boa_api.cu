@@ -88,6 +88,7 @@ struct boa_model {
   int ks_x = 1;                // k-splits of x_proj (a function of the model shape only: results must not depend on B)
   int n_sm = 148;              // SM count of the device (persistent grids)
   uint32_t blob_crc = 0;
+  uint32_t arith_crc = 0;      // CRC-32 of the logits this device's kernels produce for a fixed probe input (boa_model_load)
   GrowBuf weights, wimg;
   const float* emb = nullptr;
   const uint16_t* img_head = nullptr;
@@ -972,6 +973,20 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
       w.img_ffn1 = wbase + o.img_ffn1; w.img_ffn2 = wbase + o.img_ffn2;
     }
   }
+  // Arithmetic probe: the tables are reproducible only with the same per-step arithmetic, and nothing
+  // forces a developer to bump kArithVersion when a kernel upstream of the quantiser changes.  So the fingerprint also
+  // carries what the arithmetic DOES: three streams of 40 fixed bytes are stepped through this model with the step
+  // kernels and the CRC-32 of all their fp32 logits is folded into the arithmetic word.  A build (or device) whose
+  // kernels round differently writes and accepts a different fingerprint: BOA_E_MODEL_MISMATCH instead of garbage.
+  {
+    constexpr size_t kChunks = 3, kLen = 40, kSteps = kLen - 1;
+    std::vector<uint8_t> probe(kChunks * kLen);
+    for (size_t i = 0; i < probe.size(); ++i) probe[i] = (uint8_t)((i * 37u + 11u) ^ (i >> 3));
+    std::vector<float> logits(kChunks * kSteps * 256);
+    rc = boa_debug_step_dump(m, probe.data(), probe.size(), kLen, kSteps, logits.data(), nullptr, nullptr, nullptr);
+    if (rc != BOA_OK) { delete m; return rc; }
+    m->arith_crc = crc32_ieee(reinterpret_cast<const uint8_t*>(logits.data()), logits.size() * sizeof(float));
+  }
   *out = m;
   return BOA_OK;
 }
@@ -979,7 +994,7 @@ int boa_model_load(const void* weights, size_t nbytes, boa_model** out) {
 void boa_model_free(boa_model* m) { delete m; }
 
 uint64_t boa_model_fingerprint(const boa_model* m) {
-  return m ? (((uint64_t)kArithVersion << 32) | m->blob_crc) : 0;
+  return m ? (((uint64_t)(kArithVersion ^ m->arith_crc) << 32) | m->blob_crc) : 0;
 }
 
 size_t boa_compress_bound(size_t n, size_t chunk_bytes) {

@@ -364,6 +364,20 @@ def test_edge_cases(boa):
     assert len(comp) == container.index_bytes(5) + 5 * 4
 
 
+def test_fingerprint_is_stable_and_follows_weights_and_arithmetic(boa):
+    """The fingerprint = (generation ^ CRC of the probe logits) << 32 | CRC(blob): the same for two handles of one blob,
+    different in BOTH halves for another blob (other weights give other probe logits), and what containers carry."""
+    cfg = synth.CONFIGS[1]
+    a1, a2, b = boa.Model(cfg.weights()), boa.Model(cfg.weights()), boa.Model(cfg.weights(emb_std=0.25))
+    assert a1.fingerprint == a2.fingerprint
+    assert (a1.fingerprint >> 32) != (b.fingerprint >> 32) and (a1.fingerprint & 0xFFFFFFFF) != (b.fingerprint & 0xFFFFFFFF)
+    import zlib
+    assert (a1.fingerprint & 0xFFFFFFFF) == (zlib.crc32(cfg.weights()) & 0xFFFFFFFF)
+    comp = _np(a1.compress(cfg.data(300), 100)).tobytes()
+    assert int.from_bytes(comp[32:40], "little") == a1.fingerprint
+    assert _np(a2.decompress(torch.frombuffer(bytearray(comp), dtype=torch.uint8).cuda())).tobytes() == cfg.data(300)
+
+
 def test_errors(boa):
     cfg = synth.CONFIGS[1]
     gm = boa.Model(cfg.weights())
