@@ -191,6 +191,12 @@ def kernel_work(cfg, B):
         "outproj": ("tensor", mm * 2 * B * E * D, 2 * B * E * D),
         "head": ("tensor", mm * 2 * B * D * 256, 2 * B * D * 256),
     }
+    # the chained launches of the step path (tc::k_gemm_chain): the sum of their contractions
+    def chained(*names):
+        return ("tensor", sum(work[k][1] for k in names), sum(work[k][2] for k in names))
+    work["chain_in_x"] = chained("inproj", "convx")
+    work["chain_out_in_x"] = chained("outproj", "inproj", "convx")
+    work["chain_out_head"] = chained("outproj", "head")
     if s.d_ff:   # the paper's block: two more contractions and a LayerNorm per layer
         work["ffn1"] = ("tensor", mm * 2 * B * D * s.d_ff, 2 * B * D * s.d_ff)
         work["ffn2"] = ("tensor", mm * 2 * B * s.d_ff * D, 2 * B * s.d_ff * D)
@@ -370,6 +376,8 @@ def run_ours(args, cfg):
         m.debug_set_pair_tiles(args.pair_tiles)
     if args.persist_max >= 0:
         m.debug_set_persist(args.persist_max, args.persist_cluster)
+    if args.chain:
+        m.debug_set_chain(True)
     d_in = host.to(dev)
     d_comp = torch.empty(boa.compress_bound(n, chunk), dtype=torch.uint8, device=dev)
     d_out = torch.empty(n, dtype=torch.uint8, device=dev)
@@ -571,6 +579,7 @@ def main():
     ap.add_argument("--scaling", default="weak", choices=["weak", "strong"], help="N > 1: independent replicas (weak) or one input / one container sharded over the ranks (strong)")
     ap.add_argument("--persist-max", type=int, default=-1, help="measurement only: waves up to this many streams run the persistent step kernel (boa_debug_set_persist; -1 = library default, 0 = never)")
     ap.add_argument("--persist-cluster", type=int, default=0, help="measurement only: CTAs per row tile in the persistent step kernel (0 = library default)")
+    ap.add_argument("--chain", action="store_true", help="measurement only: chain the dependent contractions of the step path inside one launch (boa_debug_set_chain)")
     ap.add_argument("--pair-tiles", type=int, default=-1, help="measurement only: row-tile threshold from which the step path uses CTA-pair tiles (boa_debug_set_pair_tiles; -1 = library default)")
     ap.add_argument("--streams", type=int, default=0, help="run the config's model with this many chunks (streams per step) ...")
     ap.add_argument("--chunk-bytes", type=int, default=0, help="... of this many bytes each (a sweep point, not the headline workload)")

@@ -169,7 +169,11 @@ enum {
   BOA_K_FFN1 = 8,    /* hidden = GELU(W1 u + b1) (tensor cores; writes the operand image of FFN2)   */
   BOA_K_FFN2 = 9,    /* v = W2 hidden + b2 (tensor cores)                                          */
   BOA_K_LNORM = 10,  /* u = LayerNorm(v); image and block sums of u^2 for the next contraction     */
-  BOA_K_COUNT = 11
+  /* step path of north_star's block: the dependent contractions between two scans chained in one launch (tc_gemm.cuh) */
+  BOA_K_CHAIN_IN_X = 11,      /* in_proj(0) -> x_proj(0)                      */
+  BOA_K_CHAIN_OUT_IN_X = 12,  /* out_proj(l) -> in_proj(l+1) -> x_proj(l+1)   */
+  BOA_K_CHAIN_OUT_HEAD = 13,  /* out_proj(L-1) -> head                        */
+  BOA_K_COUNT = 14
 };
 typedef struct boa_profile {
   uint64_t launches_total;            /* kernels launched by the last compress/decompress call       */
@@ -208,6 +212,10 @@ int boa_get_profile(const boa_model* m, boa_profile* out);
  * boa_debug_set_max_wave: streams > 0 caps the number of streams stepped together (more chunks then run in waves), as
  *   a small free-memory budget would; 0 restores the default.  Results must not depend on it (test). */
 int boa_debug_set_slab(boa_model* m, int enabled);
+/* boa_debug_set_chain: enabled = 1 chains the dependent contractions of the step path inside one launch (tc::k_gemm_chain,
+ *   2L + 2 launches per step) instead of one kernel per contraction (4L + 2, the default: the chained form measured
+ *   neutral).  Same bytes either way (test). */
+int boa_debug_set_chain(boa_model* m, int enabled);
 /* boa_debug_set_persist: waves of at most `max_streams` streams step inside one launch of the persistent step kernel
  *   (step_persist.cuh; 0 = never, i.e. always the graph of one kernel per phase), with `cluster_ctas` CTAs per row tile of
  *   128 streams (1, 2, 4, 8 or 16; 0 = keep).  Same bytes either way (test). */

@@ -16,14 +16,15 @@ from . import build as _build
 
 OK = 0
 E_ARG, E_FORMAT, E_CRC, E_MODEL_MISMATCH, E_CAPACITY, E_CORRUPT, E_CUDA, E_NOMEM, E_UNSUPPORTED = range(-1, -10, -1)
-K_NAMES = ("embed", "inproj", "convx", "scan", "outproj", "head", "coder", "finish", "ffn1", "ffn2", "lnorm")
+K_NAMES = ("embed", "inproj", "convx", "scan", "outproj", "head", "coder", "finish", "ffn1", "ffn2", "lnorm",
+           "chain_in_x", "chain_out_in_x", "chain_out_head")
 K_COUNT = len(K_NAMES)
 
 EXPORTS = ("boa_model_load", "boa_model_free", "boa_model_fingerprint", "boa_compress_bound", "boa_compress",
            "boa_decompressed_size", "boa_decompress", "boa_compress_shard", "boa_container_index_bytes", "boa_container_assemble",
            "boa_decompress_shard", "boa_stream_bound", "boa_stream_compress",
            "boa_stream_decompressed_size", "boa_stream_decompress", "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",
-           "boa_debug_set_slab", "boa_debug_set_persist", "boa_debug_set_pair_tiles", "boa_debug_set_max_wave", "boa_debug_gemm", "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
+           "boa_debug_set_slab", "boa_debug_set_chain", "boa_debug_set_persist", "boa_debug_set_pair_tiles", "boa_debug_set_max_wave", "boa_debug_gemm", "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
 
 
 class Profile(C.Structure):
@@ -94,6 +95,8 @@ def lib() -> C.CDLL:
     l.boa_get_profile.restype = C.c_int
     l.boa_debug_set_slab.argtypes = [vp, C.c_int]
     l.boa_debug_set_slab.restype = C.c_int
+    l.boa_debug_set_chain.argtypes = [vp, C.c_int]
+    l.boa_debug_set_chain.restype = C.c_int
     l.boa_debug_set_persist.argtypes = [vp, sz, C.c_int]
     l.boa_debug_set_persist.restype = C.c_int
     l.boa_debug_set_pair_tiles.argtypes = [vp, C.c_int]
@@ -253,6 +256,9 @@ class Model:
     # -- test-only -----------------------------------------------------------------------------------
     def debug_set_slab(self, enabled: bool):
         _check(lib().boa_debug_set_slab(self._h, 1 if enabled else 0), "boa_debug_set_slab")
+
+    def debug_set_chain(self, enabled: bool):
+        _check(lib().boa_debug_set_chain(self._h, 1 if enabled else 0), "boa_debug_set_chain")
 
     def debug_set_persist(self, max_streams: int, cluster_ctas: int = 0):
         _check(lib().boa_debug_set_persist(self._h, max_streams, cluster_ctas), "boa_debug_set_persist")

@@ -115,6 +115,9 @@ struct boa_model {
   uint64_t persist_max_streams = 0;     // waves up to this many streams step inside ONE persistent launch (step_persist.cuh)
   int persist_cluster = 8;              // CTAs per row tile of 128 streams in that launch (8 = the portable maximum)
   GrowBuf persist_layers;               // device copy of the per-layer arguments of that launch
+  bool use_chain = false;               // step path: dependent contractions chained inside one launch (tc::k_gemm_chain); measured
+                                        // neutral (profiles/r02_chain.md), so off by default
+  GrowBuf chain_cnt;                    // [2 (L + 1)][row tiles] uint32 row-tile counters of the chained contractions
   int pair_min_row_tiles = INT_MAX; // step-path contractions use CTA-pair tiles from this many 128-stream row tiles on (use_pair_tiles)
   uint64_t max_wave = 0;       // > 0: at most this many streams are stepped together (more chunks run in waves)
 
@@ -126,7 +129,7 @@ struct boa_model {
   ~boa_model() {
     for (GrowBuf* b : {&weights, &wimg, &u, &xz, &dbc, &u_img, &xs_img, &y_img, &f_img, &ffn_v, &logits, &h, &win, &ssq, &pos, &len, &low, &range,
                        &pending, &wpos, &cache, &started, &v, &rpos, &off, &size, &scratch, &first, &err,
-                       &stage_in, &stage_out, &total, &persist_layers})
+                       &stage_in, &stage_out, &total, &persist_layers, &chain_cnt})
       b->release();
     pin.release();
     for (cudaEvent_t e : events) cudaEventDestroy(e);
@@ -315,6 +318,33 @@ int optin_tc() {
   BOA_CUDA_TRY((cudaFuncSetAttribute(tc::k_tc_gemm<NPW, EPI, 2, SLAB>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem)));
   return BOA_OK;
 }
+// Chained contractions of the step path (tc::k_gemm_chain): persistent, at most one CTA per SM, sized for the contraction
+// with the most work items.
+template <int NPW, int KIND>
+int launch_chain_t(const boa_model* m, const tc::ChainArgs& a, cudaStream_t st) {
+  int items = 1;
+  for (int j = 0; j < (KIND == tc::CH_OUT_IN_X ? 3 : 2); ++j)
+    items = std::max(items, ((a.g[j].M + tc::BM - 1) / tc::BM) * a.g[j].NT * a.g[j].KS);
+  BOA_CUDA_TRY(launch_pdl(tc::k_gemm_chain<NPW, KIND>, dim3((unsigned)std::min(items, m->n_sm)), dim3(tc::NTHREADS),
+                          (size_t)tc::Cfg<NPW>::SMEM, st, a));
+  return BOA_OK;
+}
+int launch_chain(const boa_model* m, int kind, const tc::ChainArgs& a, cudaStream_t st) {
+  if (m->npw == 1) {
+    if (kind == tc::CH_IN_X) return launch_chain_t<1, tc::CH_IN_X>(m, a, st);
+    if (kind == tc::CH_OUT_IN_X) return launch_chain_t<1, tc::CH_OUT_IN_X>(m, a, st);
+    return launch_chain_t<1, tc::CH_OUT_HEAD>(m, a, st);
+  }
+  if (kind == tc::CH_IN_X) return launch_chain_t<3, tc::CH_IN_X>(m, a, st);
+  if (kind == tc::CH_OUT_IN_X) return launch_chain_t<3, tc::CH_OUT_IN_X>(m, a, st);
+  return launch_chain_t<3, tc::CH_OUT_HEAD>(m, a, st);
+}
+template <int NPW, int KIND>
+int optin_chain() {
+  BOA_CUDA_TRY((cudaFuncSetAttribute(tc::k_gemm_chain<NPW, KIND>, cudaFuncAttributeMaxDynamicSharedMemorySize, tc::Cfg<NPW>::SMEM)));
+  return BOA_OK;
+}
+
 // Shared-memory opt-ins of every kernel instantiation the step can launch (called by boa_model_load, outside
 // any stream capture).
 int init_kernels() {
@@ -336,6 +366,8 @@ int init_kernels() {
   BOA_TRY((optin_tc2<3, tc::EPI_RESID>()));
   BOA_TRY((optin_tc2<1, tc::EPI_FFN1>()));
   BOA_TRY((optin_tc2<3, tc::EPI_FFN1>()));
+  BOA_TRY((optin_chain<1, tc::CH_IN_X>())); BOA_TRY((optin_chain<1, tc::CH_OUT_IN_X>())); BOA_TRY((optin_chain<1, tc::CH_OUT_HEAD>()));
+  BOA_TRY((optin_chain<3, tc::CH_IN_X>())); BOA_TRY((optin_chain<3, tc::CH_OUT_IN_X>())); BOA_TRY((optin_chain<3, tc::CH_OUT_HEAD>()));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 64)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
   BOA_CUDA_TRY(cudaFuncSetAttribute(k_scan<8>, cudaFuncAttributeMaxDynamicSharedMemorySize, scan::smem_bytes(256, 128, 0)));
@@ -395,21 +427,114 @@ int launch_step(StepCtx& c) {
   uint8_t* u_img = m->u_img.as<uint8_t>();
   uint8_t* xs_img = m->xs_img.as<uint8_t>();
   uint8_t* y_img = m->y_img.as<uint8_t>();
-
   const int ec = (E % 256 == 0) ? 256 : 128;     // channels per scan slice
-  for (int l = 0; l < m->L; ++l) {
+  const int mt_rows = (rows + tc::BM - 1) / tc::BM;
+
+  // the arguments of the step's contractions
+  auto make_in = [&](int l) {   // S2-S4: xz = [SiLU(conv(W_in_x r)) ; W_in_z r],  r = RMSNorm(u);  xs also as the image for x_proj
+    const LayerW& w = m->layers[l];
+    tc::GemmArgs g{};
+    g.A = u_img; g.M = rows; g.KB = D / 64; g.W = w.img_in; g.NT = 2 * E / 64; g.KS = 1;
+    g.n_valid = 2 * E; g.xz_ec = ec;
+    g.C = xz;           // step path: a row = [slice][xs | z]; time slab: [slice][row][xs | z] (one copy per stream-group)
+    g.ldc = T == 1 ? 2 * E : 2 * ec;
+    g.xz_slice = T == 1 ? (size_t)2 * ec : (size_t)rows * 2 * ec;
+    g.ssq_in = ssq; g.win = m->win.as<float>() + (size_t)l * m->Bcap * 3 * E; g.pos = c.ca.pos; g.slab_T = T == 1 ? 0 : T;
+    g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
+    g.out_img = xs_img; g.out_KB = E / 64;
+    return g;
+  };
+  auto make_x = [&](int l) {    // S5: [dlt;Bv;Cv] = W_x xs
+    tc::GemmArgs g{};
+    g.A = xs_img; g.M = rows; g.KB = E / 64; g.W = m->layers[l].img_x; g.NT = m->ldj / 64;
+    g.C = dbc; g.ldc = m->ks_x * m->ldj; g.n_valid = m->J;           // row = [k-split][ldj]
+    g.KS = m->ks_x; g.split_stride = (size_t)m->ldj;                  // split over k: enough tiles to fill the SMs
+    return g;
+  };
+  auto make_out = [&](int l) {  // S9: u += W_out y;  the new u also as the image for the next in_proj (times its RMSNorm weight) or the head
+    tc::GemmArgs g{};
+    g.A = y_img; g.M = rows; g.KB = E / 64; g.W = m->layers[l].img_out; g.NT = D / 64; g.KS = 1;
+    g.C = u; g.ldc = D; g.n_valid = D;
+    g.out_img = u_img; g.out_KB = D / 64; g.ssq_out = ssq;
+    // (the paper's block: the FFN reads u itself, not a normalised u)
+    g.out_scale = (m->F == 0 && l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
+    return g;
+  };
+  auto make_head = [&]() {      // S10: logits = Emb u
+    tc::GemmArgs g{};
+    g.A = u_img; g.M = rows; g.KB = D / 64; g.W = m->img_head; g.NT = 4; g.KS = 1;
+    g.C = logits; g.ldc = 256; g.n_valid = 256;
+    return g;
+  };
+  auto launch_scan = [&](int l) -> int {   // S6-S8: persistent, two CTAs per SM, each walking over streams for one channel slice
     const LayerW& w = m->layers[l];
     float* hl = m->h.as<float>() + (size_t)l * m->Bcap * E * kNState;
-    float* winl = m->win.as<float>() + (size_t)l * m->Bcap * 3 * E;
-    {  // S2-S4: xz = [SiLU(conv(W_in_x r)) ; W_in_z r],  r = RMSNorm(u);  xs also as the image for x_proj
-      tc::GemmArgs g{};
-      g.A = u_img; g.M = rows; g.KB = D / 64; g.W = w.img_in; g.NT = 2 * E / 64; g.KS = 1;
-      g.n_valid = 2 * E; g.xz_ec = ec;
-      g.C = xz;           // step path: a row = [slice][xs | z]; time slab: [slice][row][xs | z] (one copy per stream-group)
-      g.ldc = T == 1 ? 2 * E : 2 * ec;
-      g.xz_slice = T == 1 ? (size_t)2 * ec : (size_t)rows * 2 * ec;
-      g.ssq_in = ssq; g.win = winl; g.pos = c.ca.pos; g.slab_T = T == 1 ? 0 : T; g.conv_w = w.conv_w; g.conv_b = w.conv_b; g.E = E;
-      g.out_img = xs_img; g.out_KB = E / 64;
+    ScanArgs sa{};
+    sa.h = hl; sa.xz = xz; sa.dbc = dbc; sa.W_dtT = w.w_dtT; sa.b_dt = w.b_dt; sa.A4 = w.A4; sa.Dskip = w.d_skip;
+    sa.y_img = y_img; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
+    sa.KS = m->ks_x;
+    const int slices = E / ec;
+    const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
+    const dim3 grid(per_slice, slices);
+    if (T > 1) {      // time slab: groups of 8 steps per iteration, state in registers across a stream's groups
+      ScanSlabArgs ss{};
+      ss.h = hl; ss.xz = xz; ss.dbc = dbc; ss.W_dtT = w.w_dtT; ss.b_dt = w.b_dt; ss.A4 = w.A4; ss.Dskip = w.d_skip;
+      ss.y_img = y_img; ss.KS = m->ks_x; ss.ldj = m->ldj; ss.B = B; ss.E = E; ss.R = m->R; ss.T = T;
+      const int regs = (m->R == 4 || m->R == 8 || m->R == 16 || m->R == 32) ? 0 : m->R;
+      const size_t smem = scan::slab_smem_bytes(ec, m->ldj, regs);
+      switch (m->R) {
+        case 4: BOA_CUDA_TRY(launch_pdl(k_scan_slab<4>, grid, dim3(ec + 32), smem, c.st, ss)); break;
+        case 8: BOA_CUDA_TRY(launch_pdl(k_scan_slab<8>, grid, dim3(ec + 32), smem, c.st, ss)); break;
+        case 16: BOA_CUDA_TRY(launch_pdl(k_scan_slab<16>, grid, dim3(ec + 32), smem, c.st, ss)); break;
+        case 32: BOA_CUDA_TRY(launch_pdl(k_scan_slab<32>, grid, dim3(ec + 32), smem, c.st, ss)); break;
+        default: BOA_CUDA_TRY(launch_pdl(k_scan_slab<0>, grid, dim3(ec + 32), smem, c.st, ss)); break;
+      }
+    } else
+    switch (m->R) {   // W_dt's row in registers when it is short enough
+      case 4: BOA_CUDA_TRY(launch_pdl(k_scan<4>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
+      case 8: BOA_CUDA_TRY(launch_pdl(k_scan<8>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
+      case 16: BOA_CUDA_TRY(launch_pdl(k_scan<16>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
+      case 32: BOA_CUDA_TRY(launch_pdl(k_scan<32>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
+      default: BOA_CUDA_TRY(launch_pdl(k_scan<0>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, m->R), c.st, sa)); break;
+    }
+    return mark(c, BOA_K_SCAN);
+  };
+
+  // Step path of north_star's block: the dependent contractions between two scans run chained inside ONE launch
+  // (tc::k_gemm_chain): in_proj -> x_proj | scan | out_proj -> in_proj -> x_proj | scan | ... | out_proj -> head | coder,
+  // 2L + 2 launches per step instead of 4L + 2; row-tile counters order the work items.  Same bits (test).
+  const bool chain = m->use_chain && T == 1 && m->F == 0;
+  if (chain) {
+    uint32_t* cnt = m->chain_cnt.as<uint32_t>();
+    const uint32_t in_tiles = (uint32_t)(E / 64), out_tiles = (uint32_t)(D / 64);
+    for (int k = 0; k <= m->L; ++k) {
+      uint32_t* ca = cnt + (size_t)(2 * k) * mt_rows;
+      uint32_t* cb = cnt + (size_t)(2 * k + 1) * mt_rows;
+      tc::ChainArgs a{};
+      if (k == 0) {
+        a.g[0] = make_in(0); a.g[0].done = ca; a.g[0].done_cols = E;
+        a.g[1] = make_x(0); a.g[1].dep = ca; a.g[1].dep_target = in_tiles;
+        BOA_TRY(launch_chain(m, tc::CH_IN_X, a, c.st));
+        BOA_TRY(mark(c, BOA_K_CHAIN_IN_X));
+      } else if (k < m->L) {
+        a.g[0] = make_out(k - 1); a.g[0].done = ca; a.g[0].done_cols = D;
+        a.g[1] = make_in(k); a.g[1].dep = ca; a.g[1].dep_target = out_tiles; a.g[1].done = cb; a.g[1].done_cols = E;
+        a.g[2] = make_x(k); a.g[2].dep = cb; a.g[2].dep_target = in_tiles;
+        BOA_TRY(launch_chain(m, tc::CH_OUT_IN_X, a, c.st));
+        BOA_TRY(mark(c, BOA_K_CHAIN_OUT_IN_X));
+      } else {
+        a.g[0] = make_out(m->L - 1); a.g[0].done = ca; a.g[0].done_cols = D;
+        a.g[1] = make_head(); a.g[1].dep = ca; a.g[1].dep_target = out_tiles;
+        BOA_TRY(launch_chain(m, tc::CH_OUT_HEAD, a, c.st));
+        BOA_TRY(mark(c, BOA_K_CHAIN_OUT_HEAD));
+      }
+      if (k < m->L) BOA_TRY(launch_scan(k));
+    }
+  } else {
+  for (int l = 0; l < m->L; ++l) {
+    const LayerW& w = m->layers[l];
+    {
+      const tc::GemmArgs g = make_in(l);
       if (T > 1) {   // the time-slab form of the conv epilogue
         BOA_TRY((m->npw == 1 ? launch_tc<1, tc::EPI_INPROJ, true>(g, m->n_sm, c.st) : launch_tc<3, tc::EPI_INPROJ, true>(g, m->n_sm, c.st)));
       } else {
@@ -417,52 +542,14 @@ int launch_step(StepCtx& c) {
       }
       BOA_TRY(mark(c, BOA_K_INPROJ));
     }
-    {  // S5: [dlt;Bv;Cv] = W_x xs
-      tc::GemmArgs g{};
-      g.A = xs_img; g.M = rows; g.KB = E / 64; g.W = w.img_x; g.NT = m->ldj / 64;
-      g.C = dbc; g.ldc = m->ks_x * m->ldj; g.n_valid = m->J;           // row = [k-split][ldj]
-      g.KS = m->ks_x; g.split_stride = (size_t)m->ldj;                  // split over k: enough tiles to fill the SMs
+    {
+      const tc::GemmArgs g = make_x(l);
       BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_CONVX));
     }
-    {  // S6-S8: persistent, two CTAs per SM, each walking over streams for one channel slice
-      ScanArgs sa{};
-      sa.h = hl; sa.xz = xz; sa.dbc = dbc; sa.W_dtT = w.w_dtT; sa.b_dt = w.b_dt; sa.A4 = w.A4; sa.Dskip = w.d_skip;
-      sa.y_img = y_img; sa.ldj = m->ldj; sa.B = B; sa.E = E; sa.R = m->R;
-      sa.KS = m->ks_x;
-      const int slices = E / ec;
-      const int per_slice = std::max(1, std::min(B, (2 * m->n_sm + slices - 1) / slices));
-      const dim3 grid(per_slice, slices);
-      if (T > 1) {      // time slab: groups of 8 steps per iteration, state in registers across a stream's groups
-        ScanSlabArgs ss{};
-        ss.h = hl; ss.xz = xz; ss.dbc = dbc; ss.W_dtT = w.w_dtT; ss.b_dt = w.b_dt; ss.A4 = w.A4; ss.Dskip = w.d_skip;
-        ss.y_img = y_img; ss.KS = m->ks_x; ss.ldj = m->ldj; ss.B = B; ss.E = E; ss.R = m->R; ss.T = T;
-        const int regs = (m->R == 4 || m->R == 8 || m->R == 16 || m->R == 32) ? 0 : m->R;
-        const size_t smem = scan::slab_smem_bytes(ec, m->ldj, regs);
-        switch (m->R) {
-          case 4: BOA_CUDA_TRY(launch_pdl(k_scan_slab<4>, grid, dim3(ec + 32), smem, c.st, ss)); break;
-          case 8: BOA_CUDA_TRY(launch_pdl(k_scan_slab<8>, grid, dim3(ec + 32), smem, c.st, ss)); break;
-          case 16: BOA_CUDA_TRY(launch_pdl(k_scan_slab<16>, grid, dim3(ec + 32), smem, c.st, ss)); break;
-          case 32: BOA_CUDA_TRY(launch_pdl(k_scan_slab<32>, grid, dim3(ec + 32), smem, c.st, ss)); break;
-          default: BOA_CUDA_TRY(launch_pdl(k_scan_slab<0>, grid, dim3(ec + 32), smem, c.st, ss)); break;
-        }
-      } else
-      switch (m->R) {   // W_dt's row in registers when it is short enough
-        case 4: BOA_CUDA_TRY(launch_pdl(k_scan<4>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
-        case 8: BOA_CUDA_TRY(launch_pdl(k_scan<8>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
-        case 16: BOA_CUDA_TRY(launch_pdl(k_scan<16>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
-        case 32: BOA_CUDA_TRY(launch_pdl(k_scan<32>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, 0), c.st, sa)); break;
-        default: BOA_CUDA_TRY(launch_pdl(k_scan<0>, grid, dim3(ec + 32), scan::smem_bytes(ec, m->ldj, m->R), c.st, sa)); break;
-      }
-      BOA_TRY(mark(c, BOA_K_SCAN));
-    }
-    {  // S9: u += W_out y;  the new u also as the image for the next in_proj (times its RMSNorm weight) or the head
-      tc::GemmArgs g{};
-      g.A = y_img; g.M = rows; g.KB = E / 64; g.W = w.img_out; g.NT = D / 64; g.KS = 1;
-      g.C = u; g.ldc = D; g.n_valid = D;
-      g.out_img = u_img; g.out_KB = D / 64; g.ssq_out = ssq;
-      // (the paper's block: the FFN reads u itself, not a normalised u)
-      g.out_scale = (m->F == 0 && l + 1 < m->L) ? m->layers[l + 1].norm_w : nullptr;
+    BOA_TRY(launch_scan(l));
+    {
+      const tc::GemmArgs g = make_out(l);
       if (T == 1) BOA_TRY((launch_gemm_step<tc::EPI_RESID>(m, g, c.st)));
       else BOA_TRY((launch_tc_npw<tc::EPI_RESID>(m->npw, g, m->n_sm, c.st)));
       BOA_TRY(mark(c, BOA_K_OUTPROJ));
@@ -493,16 +580,17 @@ int launch_step(StepCtx& c) {
       BOA_TRY(mark(c, BOA_K_LNORM));
     }
   }
-  {  // S10: logits = Emb u
-    tc::GemmArgs g{};
-    g.A = u_img; g.M = rows; g.KB = D / 64; g.W = m->img_head; g.NT = 4; g.KS = 1;
-    g.C = logits; g.ldc = 256; g.n_valid = 256;
+  {
+    const tc::GemmArgs g = make_head();
     if (T == 1) BOA_TRY((launch_gemm_step<tc::EPI_STORE>(m, g, c.st)));
     else BOA_TRY((launch_tc_npw<tc::EPI_STORE>(m->npw, g, m->n_sm, c.st)));
     BOA_TRY(mark(c, BOA_K_HEAD));
   }
+  }
 
   const int cgrid = (B * 32 + 255) / 256;
+  uint32_t* zero_p = chain ? m->chain_cnt.as<uint32_t>() : nullptr;
+  const int zero_n = chain ? 2 * (m->L + 1) * mt_rows : 0;
   EmbedArgs ea{};
   ea.emb = reinterpret_cast<const float4*>(m->emb); ea.norm_w = reinterpret_cast<const float4*>(m->layers[0].norm_w);
   ea.u = reinterpret_cast<float4*>(u); ea.u_img = u_img; ea.ssq = ssq; ea.D4 = D / 4;
@@ -516,13 +604,13 @@ int launch_step(StepCtx& c) {
                                      cudaMemcpyDeviceToDevice, c.st));
     }
     k_coder_step<0, true><<<cgrid, 256, 0, c.st>>>(logits, c.data, c.chunk_bytes, c.ca, B, ea, c.dump_probs,
-                                                   c.dump_cdf, c.dump_steps);
+                                                   c.dump_cdf, c.dump_steps, zero_p, zero_n);
   } else if (c.mode == 0) {
     BOA_CUDA_TRY(launch_pdl(k_coder_step<0, false>, dim3(cgrid), dim3(256), 0, c.st, (const float*)logits, c.data,
-                            c.chunk_bytes, c.ca, B, ea, (float*)nullptr, (uint32_t*)nullptr, 0u));
+                            c.chunk_bytes, c.ca, B, ea, (float*)nullptr, (uint32_t*)nullptr, 0u, zero_p, zero_n));
   } else {
     BOA_CUDA_TRY(launch_pdl(k_coder_step<1, false>, dim3(cgrid), dim3(256), 0, c.st, (const float*)logits, c.data,
-                            c.chunk_bytes, c.ca, B, ea, (float*)nullptr, (uint32_t*)nullptr, 0u));
+                            c.chunk_bytes, c.ca, B, ea, (float*)nullptr, (uint32_t*)nullptr, 0u, zero_p, zero_n));
   }
   BOA_TRY(mark(c, BOA_K_CODER));
   return BOA_OK;
@@ -723,6 +811,7 @@ int reserve_workspace(boa_model* m, uint64_t B, size_t cap, uint64_t rows = 0) {
       BOA_TRY(m->ffn_v.reserve(rows * D * 4));
     }
     BOA_TRY(m->logits.reserve(rows * 256 * 4));
+    BOA_TRY(m->chain_cnt.reserve((size_t)2 * (L + 1) * ((rows + tc::BM - 1) / tc::BM) * 4));
     m->rows_cap = rows;
   }
   if (B > m->Bcap) {
@@ -765,6 +854,7 @@ int reset_state(boa_model* m, cudaStream_t st) {
   // h starts at 0 for every chunk; the conv window is zero before the chunk start
   BOA_CUDA_TRY(cudaMemsetAsync(m->h.p, 0, (size_t)m->L * m->Bcap * m->E * kNState * 4, st));
   BOA_CUDA_TRY(cudaMemsetAsync(m->win.p, 0, (size_t)m->L * m->Bcap * 3 * m->E * 4, st));
+  if (m->chain_cnt.p) BOA_CUDA_TRY(cudaMemsetAsync(m->chain_cnt.p, 0, m->chain_cnt.cap, st));   // (the coder step re-zeroes them every step)
   return BOA_OK;
 }
 
@@ -1450,6 +1540,12 @@ int boa_debug_set_persist(boa_model* m, size_t max_streams, int cluster_ctas) {
     return BOA_E_ARG;
   m->persist_max_streams = max_streams;
   if (cluster_ctas) m->persist_cluster = cluster_ctas;
+  return BOA_OK;
+}
+
+int boa_debug_set_chain(boa_model* m, int enabled) {
+  if (!m) return BOA_E_ARG;
+  m->use_chain = enabled != 0;
   return BOA_OK;
 }
 

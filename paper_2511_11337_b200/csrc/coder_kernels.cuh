@@ -351,11 +351,13 @@ __device__ __forceinline__ void coder_step_one(int i, int lane, const float* __r
 template <int MODE, bool DUMP>
 __global__ void __launch_bounds__(256)
 k_coder_step(const float* __restrict__ logits, uint8_t* data, size_t chunk_bytes, CoderArrays ca, int B,
-             EmbedArgs ea, float* dump_probs, uint32_t* dump_cdf, uint32_t dump_steps) {
+             EmbedArgs ea, float* dump_probs, uint32_t* dump_cdf, uint32_t dump_steps, uint32_t* zero, int n_zero) {
   const int i = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
   const int lane = threadIdx.x & 31;
   pdl_launch();
   pdl_wait();                                     // logits, coder state and (decode) the output buffer come from earlier kernels
+  // the row-tile counters of this step's chained contractions (tc::k_gemm_chain) start the next step at zero
+  for (int k = blockIdx.x * blockDim.x + threadIdx.x; k < n_zero; k += gridDim.x * blockDim.x) zero[k] = 0u;
   if (i >= B) return;
   coder_step_one<MODE, DUMP>(i, lane, logits, data, chunk_bytes, ca, ea, dump_probs, dump_cdf, dump_steps);
 }

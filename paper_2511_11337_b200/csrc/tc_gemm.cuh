@@ -77,6 +77,11 @@ struct GemmArgs {
   int out_KB;              // k-blocks per row tile of that image
   const float* out_scale;  // EPI_RESID: the consumer's RMSNorm weight (applied before cutting) or nullptr
   float* ssq_out;          // EPI_RESID: [M][out_KB] sum of the new u^2 over this tile's 64 columns
+  // Chained contractions (k_gemm_chain): row-tile-level dependencies between the contractions of one launch.
+  const uint32_t* dep;     // or nullptr: dep[row tile] must have reached dep_target before that row tile's operand image
+  uint32_t dep_target;     //   (and, for in_proj, its block sums of u^2) may be read
+  uint32_t* done;          // or nullptr: done[row tile] += 1 when a work item whose first column is < done_cols has
+  int done_cols;           //   stored its results
   const float* bias;       // EPI_STORE (or nullptr), EPI_FFN1: [NT*64] added to the result.  EPI_FFN1 (the paper's block,
                            // Alg. 1 l.4) then applies GELU and writes only the image of the hidden layer (out_img, out_KB)
 };
@@ -272,6 +277,25 @@ struct Cfg {
   static constexpr int TMEM_COLS = (2 * ACC_COLS <= 256) ? 256 : 512;   // two buffers
 };
 
+// Row-tile dependencies inside one launch (k_gemm_chain).  After the block barrier that ends a work item one thread adds
+// to the row tile's counter with release semantics at device scope; the consumer spins with acquire loads and then
+// crosses to the async proxy (it reads the producer's generic-proxy stores with bulk copies).
+__device__ __forceinline__ void dep_wait(const uint32_t* p, uint32_t target) {
+  uint32_t v;
+  for (;;) {
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    if (v >= target) break;
+    __nanosleep(40);
+  }
+  asm volatile("fence.proxy.async;" ::: "memory");
+}
+// (the block barrier before dep_signal orders the other threads' stores before the signalling thread's release, which is
+// cumulative; the consumer crosses to the async proxy with its own fence.proxy.async after the acquire)
+__device__ __forceinline__ void dep_signal(uint32_t* p) {
+  __threadfence();
+  asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p) : "memory");
+}
+
 // sigmoid for the SiLU of the conv epilogue: fast forms (relative error ~1e-6; same code on encode and decode)
 __device__ __forceinline__ float sigmoid_tc(float x) { return __fdividef(1.0f, 1.0f + __expf(-x)); }
 
@@ -364,6 +388,7 @@ __device__ __forceinline__ void gemm_roles(const GemmArgs& g, const GemmShared& 
         const int ks = tile % KS, t2 = tile / KS, mt = t2 / NTI, nt = (t2 - mt * NTI) * CS + crank;
         const uint8_t* asrc = g.A + img_block((size_t)mt, (size_t)ks * KB, (size_t)g.KB);
         const uint16_t* wsrc = g.W + ((size_t)nt * g.KB + (size_t)ks * KB) * (NPW * BN * 64);
+        if (g.dep) dep_wait(g.dep + mt, g.dep_target);   // the row tile's image is complete
         for (int kb = 0; kb < KB; ++kb, ++kbc) {
           const int s = kbc % nst, round = kbc / nst;
           if (round > 0) mbar_wait(smem_u32(&empty_bar[s]), (uint32_t)((round - 1) & 1));
@@ -470,7 +495,11 @@ __device__ __forceinline__ void gemm_roles(const GemmArgs& g, const GemmShared& 
             if (q < g.KB) ss += sqs[q * BM + r1];
           for (int q = NSQ; q < g.KB; ++q) ss += sp[q];
         } else {
-          for (int q = 0; q < g.KB; ++q) ss += sp[q];
+          if (g.dep) {                             // chained after out_proj: its block sums of this row tile are final
+            if (lane == 0) dep_wait(g.dep + mt, g.dep_target);
+            __syncwarp();
+          }
+          for (int q = 0; q < g.KB; ++q) ss += __ldcg(sp + q);   // (L2: another CTA may have written them in this launch)
         }
         rs = 1.0f / sqrtf(ss / (float)(g.KB * BK) + kEps);
       }
@@ -674,6 +703,7 @@ __device__ __forceinline__ void gemm_roles(const GemmArgs& g, const GemmShared& 
       }
       if (SLAB) cp_async_wait<0>();                      // the next tile's block sums
       asm volatile("bar.sync 1, 256;" ::: "memory");     // the staging tile is free for the next tile
+      if (g.done && tid == 0 && n0 < g.done_cols) dep_signal(g.done + mt);
     }
   }
 
@@ -718,6 +748,67 @@ __global__ void __launch_bounds__(NTHREADS, 1) k_tc_gemm(const GemmArgs g) {
   tc_fence_before();
   __syncthreads();
   if (CS > 1) cluster_sync();                      // no CTA leaves while a peer may still send to it
+  if (warp == 8) {
+    __syncwarp();
+    tmem_dealloc(sh.tmem, C::TMEM_COLS);
+  }
+}
+
+// ------------------------------------------------------------------------------------------ chained contractions
+// Two or three dependent contractions of the step in ONE launch (VERDICT r1 "Next" 3(ii): 4L + 2 -> 2L + 2 launches per
+// step).  At the step path's sizes every contraction kernel costs 7 - 10 us of which only a part is work: drain of
+// the previous kernel, launch, prologue, the first operand round trip.  Here the CTAs of one persistent launch run
+// the contractions one after the other (gemm_roles per contraction, the barriers re-initialised in between) and a work
+// item waits only for ITS row tile: the producer's epilogue counts finished items per row tile in global memory
+// (GemmArgs::done), the consumer's copy warp (and, for in_proj, its epilogue warps: the block sums of u^2) spin on that
+// counter (GemmArgs::dep).  No CTA waits in its first contraction, so the waits cannot form a cycle; the grid is at most
+// one CTA per SM, so every producer gets to run.  Arithmetic, tiles and epilogues are those of k_tc_gemm: same bits.
+//   CH_IN_X       in_proj(l) -> x_proj(l)                      x_proj's row tile needs the E/64 conv tiles of in_proj
+//   CH_OUT_IN_X   out_proj(l) -> in_proj(l+1) -> x_proj(l+1)   in_proj's row tile needs the D/64 tiles of out_proj
+//   CH_OUT_HEAD   out_proj(L-1) -> head
+enum { CH_IN_X = 0, CH_OUT_IN_X = 1, CH_OUT_HEAD = 2 };
+struct ChainArgs {
+  GemmArgs g[3];
+};
+
+template <int NPW, int EPI>
+__device__ __forceinline__ void chain_phase(const GemmArgs& g, const GemmShared& sh) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (warp == 8 && lane == 0) gemm_init_barriers<NPW, 1>(sh);
+  __syncthreads();
+  const int ntiles = ((g.M + BM - 1) / BM) * g.NT * g.KS;
+  gemm_roles<NPW, EPI, 1, false>(g, sh, (int)blockIdx.x, (int)gridDim.x, 0, ntiles, 0);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+}
+
+template <int NPW, int KIND>
+__global__ void __launch_bounds__(NTHREADS, 1) k_gemm_chain(const ChainArgs a) {
+  using C = Cfg<NPW>;
+  extern __shared__ uint8_t smem_raw[];
+  __shared__ __align__(8) uint64_t full_bar[C::NST], empty_bar[C::NST], acc_full[2], acc_empty[2];
+  __shared__ uint32_t tmem_base_s;
+  const int warp = threadIdx.x >> 5;
+  GemmShared sh{smem_raw, full_bar, empty_bar, acc_full, acc_empty, 0u};
+  if (warp == 8) tmem_alloc(smem_u32(&tmem_base_s), C::TMEM_COLS);
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  sh.tmem = tmem_base_s;
+  pdl_launch();
+  pdl_wait();                                      // everything below reads what earlier kernels of the step wrote
+  if (KIND == CH_IN_X) {
+    chain_phase<NPW, EPI_INPROJ>(a.g[0], sh);
+    chain_phase<NPW, EPI_STORE>(a.g[1], sh);
+  } else if (KIND == CH_OUT_IN_X) {
+    chain_phase<NPW, EPI_RESID>(a.g[0], sh);
+    chain_phase<NPW, EPI_INPROJ>(a.g[1], sh);
+    chain_phase<NPW, EPI_STORE>(a.g[2], sh);
+  } else {
+    chain_phase<NPW, EPI_RESID>(a.g[0], sh);
+    chain_phase<NPW, EPI_STORE>(a.g[1], sh);
+  }
   if (warp == 8) {
     __syncwarp();
     tmem_dealloc(sh.tmem, C::TMEM_COLS);

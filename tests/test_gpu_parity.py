@@ -167,6 +167,42 @@ def test_pair_tiles_and_single_tiles_write_the_same_container(boa, shape):
 
 
 @pytest.mark.parametrize("shape", ["cfg1", "d192_l1", "cfg2", "cfg4_bf16", "cfg5_l2_bf16"])
+def test_chained_contractions_write_the_bytes_of_one_kernel_per_contraction(boa, shape):
+    """The step path chains the dependent contractions between two scans inside one launch (tc::k_gemm_chain: in_proj ->
+    x_proj | out_proj -> in_proj -> x_proj | out_proj -> head; row-tile counters order the work items; 2L + 2 launches per
+    step instead of 4L + 2).  Against one kernel per contraction: same container, each decodes the other's; 1 ... 700
+    streams (several row tiles per CTA and fewer work items than CTAs), 1 to 4 layers, fp32 and bf16 blobs."""
+    s1 = synth.CONFIGS[1]
+    blob = {"cfg1": lambda: s1.weights(emb_std=0.25),
+            "d192_l1": lambda: synth.make_weights(synth.ModelShape(1, 192), 5, emb_std=0.25),
+            "cfg2": lambda: synth.make_weights(synth.CONFIGS[2].shape, 1, emb_std=0.25),
+            "cfg4_bf16": lambda: synth.make_weights(synth.CONFIGS[4].shape, 2, synth.DTYPE_BF16, emb_std=0.25),
+            "cfg5_l2_bf16": lambda: synth.make_weights(synth.ModelShape(2, 512, dt_rank=32), 3, synth.DTYPE_BF16, emb_std=0.25)}[shape]()
+    gm = boa.Model(blob)
+    gm.debug_set_slab(False)                                       # encode with the step path, like the decoder
+    try:
+        for n, chunk in [(1 * 37, 37), (5 * 41 + 13, 41), (130 * 23, 23), (700 * 19 + 5, 19)]:
+            data = s1.data(n)
+            gm.debug_set_chain(False)
+            plain = gm.compress(data, chunk)
+            n_plain = plain_launches(gm)
+            gm.debug_set_chain(True)
+            chained = gm.compress(data, chunk)
+            assert torch.equal(plain, chained), (shape, n, chunk)
+            assert plain_launches(gm) < n_plain                      # fewer launches for the same bytes
+            assert _np(gm.decompress(plain)).tobytes() == data     # chained decoder
+            gm.debug_set_chain(False)
+            assert _np(gm.decompress(chained)).tobytes() == data   # one kernel per contraction
+    finally:
+        gm.debug_set_slab(True)
+        gm.debug_set_chain(False)
+
+
+def plain_launches(gm):
+    return gm.profile()["launches_total"]
+
+
+@pytest.mark.parametrize("shape", ["cfg1", "d192_l1", "cfg2", "cfg4_bf16", "cfg5_l2_bf16"])
 def test_persistent_step_kernel_writes_the_bytes_of_the_graph_path(boa, shape):
     """north_star's persistent decode-step kernel (step_persist.cuh: one launch steps a small wave for all of its bytes,
     a cluster of CTAs per row tile, cluster barriers between the phases) against the graph of one kernel per phase: same
