@@ -473,7 +473,8 @@ def run_ours(args, cfg):
                 (5, 64, 273, "configs[4] model at B = 64 (per-stream latency)"),
                 (5, 1, 273, "configs[4] model at B = 1 (per-stream latency)"),
                 (1, 16, 4096, "configs[0] as it is: 16 chunks x 4 KiB, 1-layer d=64")]:
-            sweep.append(sweep_point(boa, peaks, config, streams, chunk_b, label))
+            # (few streams: no event-bracketed eager batches - they would be most of a step that is pure latency)
+            sweep.append(sweep_point(boa, peaks, config, streams, chunk_b, label, sample_every=2 if streams > 1024 else 0))
         line["sweep"] = sweep
         if not args.no_largest:
             # the largest single-GPU configuration: configs[3] at 65,536 chunks x 16 KiB = 1 GiB, one pass, no warm-up pass
