@@ -150,6 +150,32 @@ int boa_stream_decompressed_size(const uint8_t* in, size_t in_len, size_t* n, si
 int boa_stream_decompress(boa_model* m, const uint8_t* in, size_t in_len, uint8_t* out, size_t* out_len,
                           void* cuda_stream);
 
+/* ---- FX1: the deterministic fixed-point pipeline (PAPER "Portability") -----------------
+ * The paper proposes INT8 / fixed-point Mamba transformations "with explicitly specified rounding and saturation rules" and
+ * deterministic normalisation and softmax, so that a container written on one device decodes on another.
+ * DESIGN.md section 11 is that specification (Q12.20 values, INT8 rows with power-of-two scales, round-half-even,
+ * saturating stores, table-driven integer exp / sigmoid / softplus, integer RMSNorm, the integer table rule); these entry
+ * points run it on the GPU, every step an integer kernel (csrc/fx_kernels.cuh).  Integer arithmetic has one correct
+ * answer: logits, tables and whole containers are bit-identical to the exact-integer oracle's (tests).
+ *   boa_fx_model_load   parse a BOAW blob of north_star's block with the tied head (flags == 1; else BOA_E_UNSUPPORTED;
+ *                       d_model <= 1024), quantise it as section 11 says (host), copy it to the device
+ *   boa_fx_model_fingerprint   ('FX01' << 32) | CRC-32(blob): the arithmetic word is a constant - FX1 containers are
+ *                       portable by construction, and are never accepted by a floating-point boa_model (nor vice versa)
+ *   boa_fx_compress / boa_fx_decompress   as boa_compress / boa_decompress (same BOA1 container, same pointer and error
+ *                       conventions); both directions step one byte at a time
+ *   boa_fx_debug_step_dump   test-only: logits[r][256] (int32, Q12.20) and cdf[r][257] of row r = stream * n_steps + step
+ *   boa_fx_last_launches     kernels launched by the last compress / decompress call of the handle */
+typedef struct boa_fx_model boa_fx_model;
+int boa_fx_model_load(const void* weights, size_t nbytes, boa_fx_model** out);
+void boa_fx_model_free(boa_fx_model* m);
+uint64_t boa_fx_model_fingerprint(const boa_fx_model* m);
+int boa_fx_compress(boa_fx_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, uint8_t* out, size_t* out_len,
+                    void* cuda_stream);
+int boa_fx_decompress(boa_fx_model* m, const uint8_t* in, size_t in_len, uint8_t* out, size_t* out_len, void* cuda_stream);
+uint64_t boa_fx_last_launches(const boa_fx_model* m);
+int boa_fx_debug_step_dump(boa_fx_model* m, const uint8_t* in, size_t n, size_t chunk_bytes, size_t n_steps, int32_t* logits,
+                           uint32_t* cdf, void* cuda_stream);
+
 const char* boa_strerror(int code);
 /* "file:line: cudaErrorName" of the last CUDA failure seen by the calling thread ("" if none).  Diagnostic only. */
 const char* boa_last_cuda_error(void);

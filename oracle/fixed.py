@@ -265,9 +265,10 @@ def embed(fx: FxWeights, s):
 
 
 def rmsnorm(u, w, sqrt_d: int):
-    """r_i = u_i / sqrt(mean(u^2) + eps) * w_i in Q, integer only.  Per row:  e = bitlen(max|u|);  t = u scaled so that
-    max|t| is in [2^23, 2^24);  S = sum t^2 (< 2^58 for D <= 1024);  eps in t's scale = EPS_Q40 * 2^(2F + 8 - 2e);
-    Y = isqrt(S + D * eps_t);  r = rdiv(t * sqrt(D)_Q20, Y)  (the scale cancels);  out = qmul(r, w)."""
+    """r_i = u_i / sqrt(mean(u^2) + eps) * w_i in Q, integer only.  Per row:  e = bitlen(max|u|);  c = min(24 - e, 12);
+    t = u * 2^c (rne when c < 0), so max|t| < 2^24;  S = sum t^2 (< 2^58 for D <= 1024);  eps in t's scale = EPS_Q40 * 2^(2c)
+    (< 2^48: everything fits 64 bits);  Y = isqrt(S + D * eps_t);  r = rdiv(t * sqrt(D)_Q20, Y)  (the scale cancels);
+    out = qmul(r, w)."""
     u = np.asarray(u, I64)
     D = u.shape[1]
     out = np.zeros_like(u)
@@ -275,10 +276,10 @@ def rmsnorm(u, w, sqrt_d: int):
     for i in range(u.shape[0]):
         if m[i] == 0:
             continue
-        e = int(m[i]).bit_length()
-        t = rne(u[i], e - 24)
+        c = min(24 - int(m[i]).bit_length(), 12)
+        t = rne(u[i], -c)
         S = int(np.sum(t * t))
-        eps_t = rne(EPS_Q40, -(2 * F + 8 - 2 * e))               # eps in t's scale: a left shift while e <= 24
+        eps_t = rne(EPS_Q40, -2 * c)                              # eps in t's scale: a left shift while c >= 0
         Y = isqrt(S + D * int(eps_t))
         r = rdiv(t * I64(sqrt_d), np.full(D, Y, I64))
         out[i] = qmul(r, w)
@@ -419,10 +420,10 @@ def scalar_step(fx: FxWeights, state, s: int):
         if m == 0:
             r = [0] * D
         else:
-            e = m.bit_length()
-            t = [rne(v, e - 24) for v in u]
+            c = min(24 - m.bit_length(), 12)
+            t = [rne(v, -c) for v in u]
             S = sum(v * v for v in t)
-            Y = isqrt(S + D * rne(EPS_Q40, -(2 * F + 8 - 2 * e)))
+            Y = isqrt(S + D * rne(EPS_Q40, -2 * c))
             r = [qmul(rdiv(v * fx.sqrt_d, Y), int(w)) for v, w in zip(t, l.norm_w)]
         xz = gemm(r, *l.w_in)
         x, z = xz[:E], xz[E:]

@@ -23,7 +23,9 @@ K_COUNT = len(K_NAMES)
 EXPORTS = ("boa_model_load", "boa_model_free", "boa_model_fingerprint", "boa_compress_bound", "boa_compress",
            "boa_decompressed_size", "boa_decompress", "boa_compress_shard", "boa_container_index_bytes", "boa_container_assemble",
            "boa_decompress_shard", "boa_stream_bound", "boa_stream_compress",
-           "boa_stream_decompressed_size", "boa_stream_decompress", "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",
+           "boa_stream_decompressed_size", "boa_stream_decompress", "boa_fx_model_load", "boa_fx_model_free",
+           "boa_fx_model_fingerprint", "boa_fx_compress", "boa_fx_decompress", "boa_fx_last_launches", "boa_fx_debug_step_dump",
+           "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",
            "boa_debug_set_slab", "boa_debug_set_chain", "boa_debug_set_persist", "boa_debug_set_pair_tiles", "boa_debug_set_max_wave", "boa_debug_gemm", "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
 
 
@@ -85,6 +87,20 @@ def lib() -> C.CDLL:
     l.boa_stream_decompressed_size.restype = C.c_int
     l.boa_stream_decompress.argtypes = [vp, u8p, sz, u8p, C.POINTER(sz), vp]
     l.boa_stream_decompress.restype = C.c_int
+    l.boa_fx_model_load.argtypes = [vp, sz, C.POINTER(vp)]
+    l.boa_fx_model_load.restype = C.c_int
+    l.boa_fx_model_free.argtypes = [vp]
+    l.boa_fx_model_free.restype = None
+    l.boa_fx_model_fingerprint.argtypes = [vp]
+    l.boa_fx_model_fingerprint.restype = C.c_uint64
+    l.boa_fx_compress.argtypes = [vp, u8p, sz, sz, u8p, C.POINTER(sz), vp]
+    l.boa_fx_compress.restype = C.c_int
+    l.boa_fx_decompress.argtypes = [vp, u8p, sz, u8p, C.POINTER(sz), vp]
+    l.boa_fx_decompress.restype = C.c_int
+    l.boa_fx_last_launches.argtypes = [vp]
+    l.boa_fx_last_launches.restype = C.c_uint64
+    l.boa_fx_debug_step_dump.argtypes = [vp, u8p, sz, sz, sz, vp, vp, vp]
+    l.boa_fx_debug_step_dump.restype = C.c_int
     l.boa_strerror.argtypes = [C.c_int]
     l.boa_strerror.restype = C.c_char_p
     l.boa_last_cuda_error.argtypes = []
@@ -287,6 +303,64 @@ class Model:
 
 def stream_bound(n: int, chunk_bytes: int, group_chunks: int) -> int:
     return lib().boa_stream_bound(n, chunk_bytes, group_chunks)
+
+
+class FxModel:
+    """boa_fx_model handle: FX1, the deterministic fixed-point pipeline.  `weights` is a BOAW blob."""
+
+    def __init__(self, weights: bytes):
+        self._h = C.c_void_p()
+        buf = (C.c_char * len(weights)).from_buffer_copy(weights)
+        _check(lib().boa_fx_model_load(C.cast(buf, C.c_void_p), len(weights), C.byref(self._h)), "boa_fx_model_load")
+
+    def close(self):
+        if self._h:
+            lib().boa_fx_model_free(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    @property
+    def fingerprint(self) -> int:
+        return lib().boa_fx_model_fingerprint(self._h)
+
+    @property
+    def last_launches(self) -> int:
+        return lib().boa_fx_last_launches(self._h)
+
+    def compress_into(self, src: torch.Tensor, chunk_bytes: int, dst: torch.Tensor) -> int:
+        n = C.c_size_t(dst.numel())
+        _check(lib().boa_fx_compress(self._h, _ptr(src), src.numel(), chunk_bytes, _ptr(dst), C.byref(n), _stream()), "boa_fx_compress")
+        return n.value
+
+    def decompress_into(self, src: torch.Tensor, dst: torch.Tensor) -> int:
+        n = C.c_size_t(dst.numel())
+        _check(lib().boa_fx_decompress(self._h, _ptr(src), src.numel(), _ptr(dst) or 0, C.byref(n), _stream()), "boa_fx_decompress")
+        return n.value
+
+    def compress(self, data, chunk_bytes: int, device="cuda") -> torch.Tensor:
+        src = as_u8(data, device)
+        dst = torch.empty(compress_bound(src.numel(), chunk_bytes), dtype=torch.uint8, device=src.device)
+        return dst[: self.compress_into(src, chunk_bytes, dst)]
+
+    def decompress(self, blob, device="cuda") -> torch.Tensor:
+        src = as_u8(blob, device)
+        dst = torch.empty(decompressed_size(src), dtype=torch.uint8, device=src.device)
+        self.decompress_into(src, dst)
+        return dst
+
+    def debug_step_dump(self, data, chunk_bytes: int, n_steps: int, device="cuda"):
+        src = as_u8(data, device)
+        b = src.numel() // chunk_bytes
+        logits = torch.empty((b * n_steps, 256), dtype=torch.int32, device=device)
+        cdf = torch.empty((b * n_steps, 257), dtype=torch.int32, device=device)
+        _check(lib().boa_fx_debug_step_dump(self._h, _ptr(src), src.numel(), chunk_bytes, n_steps, _ptr(logits), _ptr(cdf), _stream()),
+               "boa_fx_debug_step_dump")
+        return {"logits": logits.view(b, n_steps, 256), "cdf": cdf.view(b, n_steps, 257)}
 
 
 def container_assemble(fingerprint: int, n: int, chunk_bytes: int, parts, out: torch.Tensor, payloads=None):

@@ -1211,7 +1211,7 @@ struct Index {
 };
 
 // S16: read and validate header, index CRC, fingerprint and total length of a container (host|device pointer).
-int read_index(const boa_model* m, const uint8_t* in, size_t in_len, bool in_dev, cudaStream_t st, Index& ix) {
+int read_index(uint64_t fingerprint, const uint8_t* in, size_t in_len, bool in_dev, cudaStream_t st, Index& ix) {
   if (in_len < kHeaderBytes + 4) return BOA_E_FORMAT;
   uint8_t hb[kHeaderBytes];
   if (in_dev) {
@@ -1232,7 +1232,7 @@ int read_index(const boa_model* m, const uint8_t* in, size_t in_len, bool in_dev
     memcpy(ix.bytes.data(), in, ix.ib);
   }
   if (get_u32(ix.bytes.data() + ix.ib - 4) != crc32_ieee(ix.bytes.data(), ix.ib - 4)) return BOA_E_CRC;
-  if (ix.h.fingerprint != boa_model_fingerprint(m)) return BOA_E_MODEL_MISMATCH;
+  if (ix.h.fingerprint != fingerprint) return BOA_E_MODEL_MISMATCH;
   const uint8_t* sp = ix.bytes.data() + kHeaderBytes + first_padded(nc);
   ix.sizes.resize((size_t)nc);
   ix.offs.resize((size_t)nc);
@@ -1450,7 +1450,7 @@ int decompress_entry(boa_model* m, const uint8_t* in, size_t in_len, uint64_t c_
   prof_begin(m);
   CallTimer timer(st);
   Index ix;
-  BOA_TRY(read_index(m, in, in_len, in_dev, st, ix));
+  BOA_TRY(read_index(boa_model_fingerprint(m), in, in_len, in_dev, st, ix));
   const uint64_t nc = ix.h.n_chunks;
   if (count == SIZE_MAX) count = nc - std::min(nc, c_lo);
   if (c_lo > nc || count > nc - c_lo) return BOA_E_ARG;
@@ -1709,3 +1709,5 @@ int boa_debug_rc_decode(const uint32_t* cdf, const uint8_t* in, size_t cap, cons
 }
 
 }  // extern "C"
+
+#include "boa_fx.cuh"   // FX1, the deterministic fixed-point pipeline (same translation unit: it reuses the helpers above)
