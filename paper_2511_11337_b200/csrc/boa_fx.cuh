@@ -3,11 +3,13 @@
 // Product path: nothing here touches oracle/; without a usable device every computing entry point returns BOA_E_CUDA.
 #pragma once
 #include "fx_coder.cuh"
+#include "fx_gemm_tc.cuh"
 #include "fx_kernels.cuh"
 
 struct FxLayerDev {
   const int32_t *norm_w, *conv_w, *conv_b, *b_dt, *a_neg, *d_skip;     // Q
-  const int8_t *q_in, *q_x, *q_dt, *q_out;                             // int8 rows
+  const uint8_t *q_in, *q_x, *q_out;                                   // int8 rows as tensor-core operand images
+  const int8_t* q_dt;                                                  // int8 rows [E][R] (read by the scan)
   const int32_t *s_in, *s_x, *s_dt, *s_out;                            // row exponents
 };
 
@@ -16,7 +18,8 @@ struct boa_fx_model {
   uint32_t blob_crc = 0;
   int64_t sqrt_d = 0;
   GrowBuf w32, w8;                      // device copies of all int32 / int8 weight data
-  const int8_t* q_emb = nullptr;
+  const int8_t* q_emb = nullptr;        // [256][D] rows (embedding look-up)
+  const uint8_t* q_head = nullptr;      // the same rows as an operand image (tied head)
   const int32_t* s_emb = nullptr;
   fx::Tables tab{};
   std::vector<FxLayerDev> layers;
@@ -77,7 +80,16 @@ void fx_to_q(const std::vector<double>& x, std::vector<int32_t>& out) {
     out.push_back((int32_t)t);
   }
 }
-size_t fx_pad16(size_t k) { return (k + 15) / 16 * 16; }
+size_t fx_kb(size_t k) { return (k + fx::TBK - 1) / fx::TBK; }
+// int8 rows q [N][K] -> operand image [ceil(N/64)][KB][64 x 128 bytes, swizzled], zero beyond N and K; appended 1024-aligned
+size_t fx_weight_image(const int8_t* q, size_t N, size_t K, std::vector<int8_t>& w8) {
+  while (w8.size() % 1024) w8.push_back(0);
+  const size_t o = w8.size(), KB = fx_kb(K), NT = (N + fx::TBN - 1) / fx::TBN;
+  w8.resize(o + NT * KB * fx::W_BLK, 0);
+  for (size_t n = 0; n < N; ++n)
+    for (size_t k = 0; k < K; ++k) w8[o + fx::w_img_off((int)n, (int)k, (int)KB)] = q[n * K + k];
+  return o;
+}
 
 }  // namespace
 
@@ -129,21 +141,28 @@ int boa_fx_model_load(const void* weights, size_t nbytes, boa_fx_model** out) {
   std::vector<int32_t> sv;
   auto vec_q = [&](const std::vector<float>& f) {
     std::vector<double> d(f.begin(), f.end());
+    while (w32.size() % 4) w32.push_back(0);       // 16-byte alignment: the kernels read taps and |A| rows as int4
     const size_t o = w32.size();
     fx_to_q(d, w32);
     return o;
   };
-  auto mat_q = [&](size_t Nr, size_t Kc, size_t& q_off, size_t& s_off) {
-    while (w8.size() % 16) w8.push_back(0);
-    q_off = w8.size();
+  std::vector<int8_t> rows;
+  auto mat_q = [&](size_t Nr, size_t Kc, size_t& q_off, size_t& s_off) {   // int8 rows -> operand image + exponents
+    rows.clear();
     sv.clear();
-    fx_quantise_rows(t, Nr, Kc, fx_pad16(Kc), w8, sv);
+    fx_quantise_rows(t, Nr, Kc, Kc, rows, sv);
+    q_off = fx_weight_image(rows.data(), Nr, Kc, w8);
     s_off = w32.size();
     w32.insert(w32.end(), sv.begin(), sv.end());
   };
-  size_t q_emb = 0, s_emb = 0;
+  size_t q_emb = 0, q_head = 0, s_emb = 0;
   bool ok = br.take(256 * (size_t)D, true, t);
-  if (ok) mat_q(256, D, q_emb, s_emb);
+  if (ok) {
+    mat_q(256, D, q_head, s_emb);
+    while (w8.size() % 16) w8.push_back(0);
+    q_emb = w8.size();
+    w8.insert(w8.end(), rows.begin(), rows.end());
+  }
   for (uint32_t l = 0; l < L && ok; ++l) {
     Off& o = offs[l];
     ok = ok && br.take(D, false, t); if (ok) o.norm_w = vec_q(t);
@@ -165,6 +184,7 @@ int boa_fx_model_load(const void* weights, size_t nbytes, boa_fx_model** out) {
     if (ok) {                                       // |A| = exp(A_log) in Q
       std::vector<double> d(t.size());
       for (size_t i = 0; i < t.size(); ++i) d[i] = exp((double)t[i]);
+      while (w32.size() % 4) w32.push_back(0);
       o.a_neg = w32.size();
       fx_to_q(d, w32);
     }
@@ -185,18 +205,24 @@ int boa_fx_model_load(const void* weights, size_t nbytes, boa_fx_model** out) {
     (void)cudaGetLastError();
     rc = BOA_E_CUDA;
   }
+  if (rc == BOA_OK && cudaFuncSetAttribute(fx::k_fx_gemm_tc, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                           fx::TC_MAXST * (fx::A_BLK + fx::W_BLK) + 1024) != cudaSuccess) {
+    (void)cudaGetLastError();
+    rc = BOA_E_CUDA;
+  }
   if (rc != BOA_OK) { delete m; return rc; }
   const int32_t* b32 = m->w32.as<int32_t>();
   const int8_t* b8 = m->w8.as<int8_t>();
+  const uint8_t* bi = m->w8.as<uint8_t>();
   m->tab.exp2 = b32 + off_exp2; m->tab.log1p = b32 + off_log1p;
-  m->q_emb = b8 + q_emb; m->s_emb = b32 + s_emb;
+  m->q_emb = b8 + q_emb; m->q_head = bi + q_head; m->s_emb = b32 + s_emb;
   m->layers.resize(L);
   for (uint32_t l = 0; l < L; ++l) {
     const Off& o = offs[l];
     FxLayerDev& w = m->layers[l];
     w.norm_w = b32 + o.norm_w; w.conv_w = b32 + o.conv_w; w.conv_b = b32 + o.conv_b; w.b_dt = b32 + o.b_dt;
     w.a_neg = b32 + o.a_neg; w.d_skip = b32 + o.d_skip;
-    w.q_in = b8 + o.q_in; w.q_x = b8 + o.q_x; w.q_dt = b8 + o.q_dt; w.q_out = b8 + o.q_out;
+    w.q_in = bi + o.q_in; w.q_x = bi + o.q_x; w.q_dt = b8 + o.q_dt; w.q_out = bi + o.q_out;
     w.s_in = b32 + o.s_in; w.s_x = b32 + o.s_x; w.s_dt = b32 + o.s_dt; w.s_out = b32 + o.s_out;
   }
   *out = m;
@@ -212,7 +238,7 @@ int fx_reserve(boa_fx_model* m, uint64_t B, size_t cap) {
   if (B > m->Bcap) {
     BOA_TRY(m->u.reserve(B * D * 4)); BOA_TRY(m->r.reserve(B * std::max(D, E) * 4)); BOA_TRY(m->xz.reserve(B * 2 * E * 4));
     BOA_TRY(m->xs.reserve(B * E * 4)); BOA_TRY(m->dbc.reserve(B * m->ldj * 4)); BOA_TRY(m->y.reserve(B * E * 4));
-    BOA_TRY(m->logits.reserve(B * 256 * 4)); BOA_TRY(m->qa.reserve(B * fx_pad16(E))); BOA_TRY(m->ka.reserve(B * 4));
+    BOA_TRY(m->logits.reserve(B * 256 * 4)); BOA_TRY(m->qa.reserve(fx::a_img_bytes(B, fx_kb(E)))); BOA_TRY(m->ka.reserve(B * 4));
     BOA_TRY(m->h.reserve(L * B * E * kNState * 4)); BOA_TRY(m->win.reserve(L * B * 3 * E * 4));
     BOA_TRY(m->pos.reserve(B * 4)); BOA_TRY(m->len.reserve(B * 4)); BOA_TRY(m->low.reserve(B * 8)); BOA_TRY(m->range.reserve(B * 4));
     BOA_TRY(m->pending.reserve(B * 4)); BOA_TRY(m->wpos.reserve(B * 4)); BOA_TRY(m->cache.reserve(B)); BOA_TRY(m->started.reserve(B));
@@ -248,30 +274,31 @@ struct FxCtx {
   uint32_t dump_steps = 0, dump_t = 0;
 };
 
-// a contraction of the step: rows of Q values `a` [B][K] -> int8 rows -> out [B][N] (+ resid)
-int fx_contract(FxCtx& c, const int32_t* a, int K, const int8_t* qw, const int32_t* sw, int N, int32_t* out, int ldo,
-                const int32_t* resid) {
+// a contraction of the step: the activation image in qa and the row shifts in ka (written by the producing kernel)
+// against a weight image -> out [B][N] (+ resid)
+int fx_contract(FxCtx& c, int K, const uint8_t* qw, const int32_t* sw, int N, int32_t* out, int ldo, const int32_t* resid) {
   boa_fx_model* m = c.m;
-  const int ldq = (int)fx_pad16((size_t)K);
-  fx::k_fx_quant_rows<<<c.B, 128, 0, c.st>>>(a, K, K, m->qa.as<int8_t>(), ldq, m->ka.as<int32_t>());
-  const dim3 grid((unsigned)((N + fx::GT - 1) / fx::GT), (unsigned)((c.B + fx::GT - 1) / fx::GT));
-  fx::k_fx_gemm<<<grid, 256, 0, c.st>>>(m->qa.as<int8_t>(), ldq, m->ka.as<int32_t>(), qw, ldq, sw, out, ldo, resid, c.B, N, K);
-  m->launches += 2;
+  const int KB = (int)fx_kb((size_t)K), nst = std::min(KB, fx::TC_MAXST);
+  const dim3 grid((unsigned)((N + fx::TBN - 1) / fx::TBN), (unsigned)((c.B + fx::TBM - 1) / fx::TBM));
+  fx::k_fx_gemm_tc<<<grid, 160, (size_t)nst * (fx::A_BLK + fx::W_BLK) + 1024, c.st>>>(m->qa.as<uint8_t>(), m->ka.as<int32_t>(), qw, sw, out,
+                                                                                     ldo, resid, c.B, N, KB, nst);
+  ++m->launches;
   BOA_CUDA_TRY(cudaPeekAtLastError());
   return BOA_OK;
 }
 
-// one model step + one coder step for the B streams of the wave, every operation an FX1 kernel
+// one model step + one coder step for the B streams of the wave, every operation an FX1 kernel (6 L + 4 launches)
 int fx_step(FxCtx& c) {
   boa_fx_model* m = c.m;
   const int B = c.B, D = m->D, E = m->E;
   int32_t* u = m->u.as<int32_t>();
-  int32_t* r = m->r.as<int32_t>();
   int32_t* xz = m->xz.as<int32_t>();
   int32_t* xs = m->xs.as<int32_t>();
   int32_t* dbc = m->dbc.as<int32_t>();
-  int32_t* y = m->y.as<int32_t>();
   int32_t* logits = m->logits.as<int32_t>();
+  int8_t* qa = m->qa.as<int8_t>();
+  int32_t* ka = m->ka.as<int32_t>();
+  const int ldd = (int)fx_kb((size_t)D), lde = (int)fx_kb((size_t)E);       // k-blocks of the activation images
   fx::k_fx_embed<<<(unsigned)(((size_t)B * D + 255) / 256), 256, 0, c.st>>>(c.data, c.chunk_bytes, c.ca.pos, c.ca.len, m->q_emb, m->s_emb,
                                                                            u, B, D);
   ++m->launches;
@@ -279,16 +306,17 @@ int fx_step(FxCtx& c) {
     const FxLayerDev& w = m->layers[l];
     int32_t* hl = m->h.as<int32_t>() + (size_t)l * m->Bcap * E * kNState;
     int32_t* winl = m->win.as<int32_t>() + (size_t)l * m->Bcap * 3 * E;
-    fx::k_fx_rmsnorm<<<B, 128, 0, c.st>>>(u, w.norm_w, r, D, m->sqrt_d);
-    BOA_TRY(fx_contract(c, r, D, w.q_in, w.s_in, 2 * E, xz, 2 * E, nullptr));
-    fx::k_fx_conv_silu<<<(unsigned)(((size_t)B * E + 255) / 256), 256, 0, c.st>>>(xz, winl, w.conv_w, w.conv_b, xs, m->tab, B, E);
-    BOA_TRY(fx_contract(c, xs, E, w.q_x, w.s_x, m->J, dbc, m->ldj, nullptr));
-    fx::k_fx_scan<<<(unsigned)(((size_t)B * E + 127) / 128), 128, 0, c.st>>>(dbc, m->ldj, w.q_dt, w.s_dt, w.b_dt, w.a_neg, w.d_skip, xs, xz,
-                                                                             hl, y, m->tab, B, E, m->R);
-    BOA_TRY(fx_contract(c, y, E, w.q_out, w.s_out, D, u, D, u));
+    fx::k_fx_rmsnorm_q<<<B, 256, 0, c.st>>>(u, w.norm_w, D, m->sqrt_d, qa, ldd, ka);
+    BOA_TRY(fx_contract(c, D, w.q_in, w.s_in, 2 * E, xz, 2 * E, nullptr));
+    fx::k_fx_conv_silu_q<<<B, 256, 0, c.st>>>(xz, winl, w.conv_w, w.conv_b, xs, m->tab, E, qa, lde, ka);
+    BOA_TRY(fx_contract(c, E, w.q_x, w.s_x, m->J, dbc, m->ldj, nullptr));
+    fx::k_fx_scan_q<<<B, 256, 0, c.st>>>(dbc, m->ldj, w.q_dt, w.s_dt, w.b_dt, w.a_neg, w.d_skip, xs, xz, hl, m->tab, E, m->R, qa, lde, ka);
+    BOA_TRY(fx_contract(c, E, w.q_out, w.s_out, D, u, D, u));
     m->launches += 3;
   }
-  BOA_TRY(fx_contract(c, u, D, m->q_emb, m->s_emb, 256, logits, 256, nullptr));
+  fx::k_fx_quant_rows<<<B, 128, 0, c.st>>>(u, D, D, qa, ldd, ka);
+  ++m->launches;
+  BOA_TRY(fx_contract(c, D, m->q_head, m->s_emb, 256, logits, 256, nullptr));
   if (c.dump_logits)
     BOA_CUDA_TRY(cudaMemcpy2DAsync(c.dump_logits + (size_t)c.dump_t * 256, (size_t)c.dump_steps * 256 * 4, logits, 256 * 4, 256 * 4, B,
                                    cudaMemcpyDeviceToDevice, c.st));

@@ -8,8 +8,8 @@
 //
 //   Q    int32, 20 fraction bits          U30  exp / sigmoid values in [0, 2^30]
 //   int8 rows: a row of Q values is cut to q in [-127, 127] with one shift k (a ~ q 2^(k-20)); weight rows are stored as
-//   q in [-127, 127] with an exponent s (w ~ q 2^-s); a contraction is an exact int32 dot product (dp4a) followed by
-//   sat(rne(acc, s - k)).
+//   q in [-127, 127] with an exponent s (w ~ q 2^-s); a contraction is an exact int32 dot product (tcgen05.mma kind::i8,
+//   fx_gemm_tc.cuh) followed by sat(rne(acc, s - k)).
 #pragma once
 #include "common.cuh"
 
@@ -25,10 +25,10 @@ constexpr int TB = 8, NTAB = 1 << TB;                   // 256 intervals, 257 en
 constexpr uint32_t TABLE_CRC = 0x6B76FB0Du;             // CRC-32 of both tables as little-endian int64 (part of the specification)
 
 // round-half-even(v / 2^k); k <= 0: exact left shift
+// (the remainder plus half - 1 plus the quotient's low bit carries into bit k exactly when the value rounds up)
 __device__ __forceinline__ int64_t rne(int64_t v, int k) {
   if (k <= 0) return v << (-k);
-  const int64_t q = v >> k, r = v & ((1ll << k) - 1), half = 1ll << (k - 1);
-  return q + ((r > half || (r == half && (q & 1))) ? 1 : 0);
+  return (v + ((1ll << (k - 1)) - 1) + ((v >> k) & 1)) >> k;
 }
 __device__ __forceinline__ int64_t sat(int64_t v) { return v > QMAX ? QMAX : (v < QMIN ? QMIN : v); }
 __device__ __forceinline__ int64_t qmul(int64_t a, int64_t b) { return sat(rne(a * b, F)); }
@@ -45,6 +45,26 @@ __device__ __forceinline__ int64_t isqrt64(int64_t x) {  // floor(sqrt(x)) exact
   return y;
 }
 __device__ __forceinline__ int bitlen64(int64_t m) { return 64 - __clzll((long long)m); }   // m >= 0
+
+// ---- operand images of the tensor-core contractions (fx_gemm_tc.cuh)
+constexpr int TBM = 128, TBN = 64, TBK = 128;         // tile rows, tile columns, int8 k per block
+constexpr int A_BLK = TBM * TBK, W_BLK = TBN * TBK;   // bytes of one k-block of a row tile / of a column tile
+constexpr int TC_MAXST = 8;                           // k-blocks in flight
+
+// Byte offset of element (r, k) inside one k-block of a tile: rows of 128 bytes, the 16-byte chunk index XORed with the
+// row index mod 8 (128-byte swizzle), 8-row groups 1024 bytes apart.
+__host__ __device__ inline uint32_t blk_off8(int r, int k) {
+  return (uint32_t)((r >> 3) * 1024 + (r & 7) * 128 + ((((k >> 4) ^ r) & 7) << 4) + (k & 15));
+}
+// activation image of A[M][K]: [ceil(M/128)][KB][128 x 128 bytes]
+__host__ __device__ inline size_t a_img_off(int m, int k, int KB) {
+  return ((size_t)(m >> 7) * KB + (size_t)(k >> 7)) * A_BLK + blk_off8(m & 127, k & 127);
+}
+__host__ __device__ inline size_t a_img_bytes(size_t M, size_t KB) { return (M + TBM - 1) / TBM * KB * A_BLK; }
+// weight image of W[N][K]: [ceil(N/64)][KB][64 x 128 bytes], rows and columns beyond N, K zero
+__host__ __device__ inline size_t w_img_off(int n, int k, int KB) {
+  return ((size_t)(n >> 6) * KB + (size_t)(k >> 7)) * W_BLK + blk_off8(n & 63, k & 127);
+}
 
 struct Tables {
   const int32_t* exp2;     // [257]  rne(2^30 2^(-i/256))
@@ -108,33 +128,61 @@ __global__ void k_fx_embed(const uint8_t* __restrict__ data, size_t chunk_bytes,
   u[idx] = (int32_t)sat(rne((int64_t)qemb[b * D + d], semb[b] - F));
 }
 
-// ---- S2: r = RMSNorm(u) * w in Q (integer only).  One block per row.
-__global__ void k_fx_rmsnorm(const int32_t* __restrict__ u, const int32_t* __restrict__ w, int32_t* __restrict__ r, int D,
-                             int64_t sqrt_d) {
+// int8 cut of one value with the row's shift k
+__device__ __forceinline__ int8_t cut8(int32_t a, int k) {
+  int64_t v = rne((int64_t)a, k);
+  v = v > 127 ? 127 : (v < -127 ? -127 : v);
+  return (int8_t)v;
+}
+__device__ __forceinline__ int64_t abs64(int64_t a) { return a < 0 ? -a : a; }
+
+// ---- S2: r = RMSNorm(u) * w in Q (integer only), cut to an int8 row for in_proj in the same
+// kernel (the Q values of r have no other reader).  One block of 256 threads per row, D <= 1024 (<= 4 values per thread).
+__global__ void __launch_bounds__(256) k_fx_rmsnorm_q(const int32_t* __restrict__ u, const int32_t* __restrict__ w, int D,
+                                                      int64_t sqrt_d, int8_t* __restrict__ q, int KB, int32_t* __restrict__ kshift) {
   __shared__ int64_t red[32];
   const int row = blockIdx.x;
   const int32_t* ur = u + (size_t)row * D;
+  int32_t uv[4], rv[4];
   int64_t m = 0;
-  for (int d = threadIdx.x; d < D; d += blockDim.x) { const int64_t a = ur[d]; m = max(m, a < 0 ? -a : a); }
+#pragma unroll
+  for (int it = 0; it < 4; ++it) {
+    const int d = threadIdx.x + 256 * it;
+    uv[it] = d < D ? ur[d] : 0;
+    rv[it] = 0;
+    m = max(m, abs64(uv[it]));
+  }
   m = block_max(m, red);
-  if (m == 0) {
-    for (int d = threadIdx.x; d < D; d += blockDim.x) r[(size_t)row * D + d] = 0;
-    return;
+  int64_t rm = 0;
+  if (m != 0) {
+    const int c = min(24 - bitlen64(m), 12);
+    int64_t s = 0;
+#pragma unroll
+    for (int it = 0; it < 4; ++it) { const int64_t t = rne((int64_t)uv[it], -c); s += t * t; }
+    s = block_sum(s, red);
+    const int64_t Y = isqrt64(s + (int64_t)D * rne(EPS_Q40, -2 * c));
+#pragma unroll
+    for (int it = 0; it < 4; ++it) {
+      const int d = threadIdx.x + 256 * it;
+      if (d < D) {
+        rv[it] = (int32_t)qmul(rdiv(rne((int64_t)uv[it], -c) * sqrt_d, Y), w[d]);
+        rm = max(rm, abs64(rv[it]));
+      }
+    }
   }
-  const int c = min(24 - bitlen64(m), 12);
-  int64_t s = 0;
-  for (int d = threadIdx.x; d < D; d += blockDim.x) { const int64_t t = rne((int64_t)ur[d], -c); s += t * t; }
-  s = block_sum(s, red);
-  const int64_t Y = isqrt64(s + (int64_t)D * rne(EPS_Q40, -2 * c));
-  for (int d = threadIdx.x; d < D; d += blockDim.x) {
-    const int64_t t = rne((int64_t)ur[d], -c);
-    r[(size_t)row * D + d] = (int32_t)qmul(rdiv(t * sqrt_d, Y), w[d]);
+  rm = block_max(rm, red);
+  const int k = max(bitlen64(rm) - 7, 0);
+#pragma unroll
+  for (int it = 0; it < 4; ++it) {
+    const int d = threadIdx.x + 256 * it;
+    if (d < D) q[a_img_off(row, d, KB)] = cut8(rv[it], k);
   }
+  if (threadIdx.x == 0) kshift[row] = k;
 }
 
 // ---- a row of Q values -> int8 with one shift per row: k = max(0, bitlen(max|a|) - 7), q = clip(rne(a, k), +-127).
-// One block per row.  K % 4 == 0; the int8 row is padded with zeros to ldq (a multiple of 16).
-__global__ void k_fx_quant_rows(const int32_t* __restrict__ a, int lda, int K, int8_t* __restrict__ q, int ldq,
+// One block per row; the int8 row goes into the activation image (KB k-blocks per row tile).
+__global__ void k_fx_quant_rows(const int32_t* __restrict__ a, int lda, int K, int8_t* __restrict__ q, int KB,
                                 int32_t* __restrict__ kshift) {
   __shared__ int64_t red[32];
   const int row = blockIdx.x;
@@ -143,115 +191,197 @@ __global__ void k_fx_quant_rows(const int32_t* __restrict__ a, int lda, int K, i
   for (int d = threadIdx.x; d < K; d += blockDim.x) { const int64_t v = ar[d]; m = max(m, v < 0 ? -v : v); }
   m = block_max(m, red);
   const int k = max(bitlen64(m) - 7, 0);
-  for (int d = threadIdx.x; d < ldq; d += blockDim.x) {
-    int64_t v = d < K ? rne((int64_t)ar[d], k) : 0;
-    v = v > 127 ? 127 : (v < -127 ? -127 : v);
-    q[(size_t)row * ldq + d] = (int8_t)v;
-  }
+  for (int d = threadIdx.x; d < K; d += blockDim.x) q[a_img_off(row, d, KB)] = cut8(ar[d], k);
   if (threadIdx.x == 0) kshift[row] = k;
 }
 
-// ---- contraction: out[m][n] = sat(rne(sum_k qa[m][k] qw[n][k], s[n] - ka[m])) (+ resid[m][n], saturating).
-// 64 x 64 output tile per block of 256 threads (4 x 4 outputs per thread), 64-byte k-slabs through shared memory, dp4a.
-// Integer sums: the tile shape has no influence on the result.
-constexpr int GT = 64;
-__global__ void __launch_bounds__(256) k_fx_gemm(const int8_t* __restrict__ qa, int lda, const int32_t* __restrict__ ka,
-                                                 const int8_t* __restrict__ qw, int ldw, const int32_t* __restrict__ sw,
-                                                 int32_t* __restrict__ out, int ldo, const int32_t* __restrict__ resid,
-                                                 int M, int N, int K) {
-  __shared__ __align__(16) int32_t As[GT][17], Ws[GT][17];      // 64 rows x 64 bytes (16 words) + pad
-  const int tx = threadIdx.x & 15, ty = threadIdx.x >> 4;
-  const int m0 = blockIdx.y * GT, n0 = blockIdx.x * GT;
-  int acc[4][4] = {};
-  for (int k0 = 0; k0 < K; k0 += 64) {
-    for (int e = threadIdx.x; e < GT * 16; e += 256) {
-      const int r = e >> 4, cw = e & 15;
-      const int kk = k0 + cw * 4;
-      int32_t va = 0, vw = 0;
-      if (m0 + r < M && kk < K) va = *reinterpret_cast<const int32_t*>(qa + (size_t)(m0 + r) * lda + kk);
-      if (n0 + r < N && kk < K) vw = *reinterpret_cast<const int32_t*>(qw + (size_t)(n0 + r) * ldw + kk);
-      As[r][cw] = va; Ws[r][cw] = vw;
-    }
-    __syncthreads();
-#pragma unroll
-    for (int cw = 0; cw < 16; ++cw) {
-      int a[4], w[4];
-#pragma unroll
-      for (int i = 0; i < 4; ++i) { a[i] = As[ty * 4 + i][cw]; w[i] = Ws[tx * 4 + i][cw]; }
-#pragma unroll
-      for (int i = 0; i < 4; ++i)
-#pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = __dp4a(a[i], w[j], acc[i][j]);
-    }
-    __syncthreads();
-  }
-#pragma unroll
-  for (int i = 0; i < 4; ++i) {
-    const int m = m0 + ty * 4 + i;
-    if (m >= M) continue;
-    const int km = ka[m];
-#pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      const int n = n0 + tx * 4 + j;
-      if (n >= N) continue;
-      int64_t v = sat(rne((int64_t)acc[i][j], max(sw[n] - km, -31)));
-      if (resid) v = sat(v + (int64_t)resid[(size_t)m * ldo + n]);
-      out[(size_t)m * ldo + n] = (int32_t)v;
-    }
-  }
-}
-
 // ---- S4: causal depthwise conv over the window (x_{t-3}, x_{t-2}, x_{t-1}) and x_t, SiLU; the window shifts.
-// xz [B][2E] Q (x | z);  win [B][3][E];  xs [B][E].  One thread per (stream, channel).
-__global__ void k_fx_conv_silu(const int32_t* __restrict__ xz, int32_t* __restrict__ win, const int32_t* __restrict__ conv_w,
-                               const int32_t* __restrict__ conv_b, int32_t* __restrict__ xs, Tables t, int B, int E) {
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= B * E) return;
-  const int i = idx / E, e = idx - i * E;
-  const int64_t x = xz[(size_t)i * 2 * E + e];
-  int32_t* w = win + (size_t)i * 3 * E + e;
-  const int64_t w0 = w[0], w1 = w[E], w2 = w[2 * E];
-  const int32_t* cw = conv_w + (size_t)e * 4;
-  const int64_t acc = (int64_t)conv_b[e] + rne((int64_t)cw[3] * x, F) + rne((int64_t)cw[0] * w0, F) + rne((int64_t)cw[1] * w1, F) +
-                      rne((int64_t)cw[2] * w2, F);
-  w[0] = (int32_t)w1; w[E] = (int32_t)w2; w[2 * E] = (int32_t)x;
-  xs[idx] = (int32_t)silu(t, sat(acc));
+// xz [B][2E] Q (x | z);  win [B][3][E];  xs [B][E] Q (read by the scan) and its int8 cut (q, kshift) for x_proj.
+// One block of 256 threads per stream, E <= 2048 (<= 8 channels per thread).
+__global__ void __launch_bounds__(256) k_fx_conv_silu_q(const int32_t* __restrict__ xz, int32_t* __restrict__ win,
+                                                        const int32_t* __restrict__ conv_w, const int32_t* __restrict__ conv_b,
+                                                        int32_t* __restrict__ xs, Tables t, int E, int8_t* __restrict__ q, int KB,
+                                                        int32_t* __restrict__ kshift) {
+  __shared__ int64_t red[32];
+  const int i = blockIdx.x;
+  int32_t v[8];
+  int64_t m = 0;
+#pragma unroll
+  for (int it = 0; it < 8; ++it) {
+    const int e = threadIdx.x + 256 * it;
+    v[it] = 0;
+    if (e < E) {
+      const int64_t x = xz[(size_t)i * 2 * E + e];
+      int32_t* w = win + (size_t)i * 3 * E + e;
+      const int64_t w0 = w[0], w1 = w[E], w2 = w[2 * E];
+      const int4 cw = *reinterpret_cast<const int4*>(conv_w + (size_t)e * 4);
+      const int64_t acc = (int64_t)conv_b[e] + rne((int64_t)cw.w * x, F) + rne((int64_t)cw.x * w0, F) + rne((int64_t)cw.y * w1, F) +
+                          rne((int64_t)cw.z * w2, F);
+      w[0] = (int32_t)w1; w[E] = (int32_t)w2; w[2 * E] = (int32_t)x;
+      v[it] = (int32_t)silu(t, sat(acc));
+      xs[(size_t)i * E + e] = v[it];
+      m = max(m, abs64(v[it]));
+    }
+  }
+  m = block_max(m, red);
+  const int k = max(bitlen64(m) - 7, 0);
+#pragma unroll
+  for (int it = 0; it < 8; ++it) {
+    const int e = threadIdx.x + 256 * it;
+    if (e < E) q[a_img_off(i, e, KB)] = cut8(v[it], k);
+  }
+  if (threadIdx.x == 0) kshift[i] = k;
 }
 
-// ---- S6-S8: dt_proj (int8 rows, K = R) + softplus, the recurrence on the 16 state values, D skip, gate.
-// dbc [B][ldj] Q = delta[R] | B[16] | C[16];  h [B][E][16] Q;  y [B][E] Q.  One thread per (stream, channel).
-__global__ void k_fx_scan(const int32_t* __restrict__ dbc, int ldj, const int8_t* __restrict__ qwdt, const int32_t* __restrict__ swdt,
-                          const int32_t* __restrict__ b_dt, const int32_t* __restrict__ a_neg, const int32_t* __restrict__ d_skip,
-                          const int32_t* __restrict__ xs, const int32_t* __restrict__ xz, int32_t* __restrict__ h,
-                          int32_t* __restrict__ y, Tables t, int B, int E, int R) {
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= B * E) return;
-  const int i = idx / E, e = idx - i * E;
+// ---- S6-S8: dt_proj (int8 rows, K = R) + softplus, the recurrence on the 16 state values, D skip, gate; y is cut to an
+// int8 row for out_proj in the same kernel (its Q values have no other reader).
+// dbc [B][ldj] Q = delta[R] | B[16] | C[16];  h [B][E][16] Q.  One block of 256 threads per stream; a warp takes 32
+// channels at a time.  Per-channel values (dt, x, z, the gate) belong to lane = channel; the 2 KB of state of the 32
+// channels are read as four fully coalesced 512-byte rows, lane l holding states 4 (l % 4) .. + 3 of channel
+// 8 j + l / 4 in row j, so a channel's sum over n is an (order-free, integer) sum over four lanes.
+// The recurrence of one state value, every product 32 x 32 -> 64 bits:
+//   dA = exp_neg(qmul(dt, |A|));  h = sat(rne(dA h, 30) + qmul(qmul(dt, B_n), x));  y += rne(C_n h, 20)
+// The integer ALU pipe is what bounds this kernel, so the roundings are written on 32-bit halves: the rounding constant
+// rides on the multiply (mad.wide), "ties to even" is "add half, shift, clear the low bit if the shifted-out bits are
+// all zero", and a saturation test is a range test of the high word.  Same integers as rne / sat / qmul above.
+__device__ __forceinline__ int64_t madw(int32_t a, int32_t b, int64_t c) {
+  int64_t r;
+  asm("mad.wide.s32 %0, %1, %2, %3;" : "=l"(r) : "r"(a), "r"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ uint32_t lo32(int64_t v) { return (uint32_t)v; }
+__device__ __forceinline__ int32_t hi32(int64_t v) { return (int32_t)(v >> 32); }
+__device__ __forceinline__ int32_t add_sat32(int32_t a, int32_t b) {
+  int32_t r;
+  asm("add.sat.s32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+  return r;
+}
+// low 32 bits of rne(p, K), given p2 = p + 2^(K-1), 1 <= K <= 31
+template <int K>
+__device__ __forceinline__ uint32_t rne_lo32(int64_t p2) {
+  uint32_t q = __funnelshift_r(lo32(p2), (uint32_t)hi32(p2), K);
+  if ((lo32(p2) & ((1u << K) - 1u)) == 0u) q &= ~1u;
+  return q;
+}
+// sat(rne(a b, 20))
+__device__ __forceinline__ int32_t qmul32(int32_t a, int32_t b) {
+  const int64_t p2 = madw(a, b, 1ll << (F - 1));
+  uint32_t q = rne_lo32<F>(p2);
+  const int32_t h = hi32(p2);                       // the quotient fits 32 bits iff -2^19 <= h < 2^19
+  if ((uint32_t)(h + (1 << (F - 1))) >= (1u << F)) q = 0x7FFFFFFFu ^ (uint32_t)(h >> 31);
+  return (int32_t)q;
+}
+// exp_neg for 0 <= x <= QMAX from the table (value, difference to the next entry) in shared memory: the same integers
+// as fx::exp_neg (n >= 31 rounds to 0 through the shift; val <= 2^30 so the last rounding is 32-bit)
+__device__ __forceinline__ int32_t exp_neg_s(const int2* tab, int32_t x) {
+  const uint32_t tq = rne_lo32<30>(madw(x, (int32_t)LOG2E_Q30, 1ll << 29));     // < 2^32
+  const uint32_t n = min(tq >> F, 31u);
+  const int2 e = tab[(tq >> (F - TB)) & (NTAB - 1)];
+  const uint32_t val = (uint32_t)e.x + rne_lo32<F - TB>(madw(e.y, (int32_t)(tq & ((1u << (F - TB)) - 1u)), 1ll << (F - TB - 1)));
+  const uint32_t v2 = val + ((1u << n) >> 1);
+  uint32_t q = v2 >> n;
+  if ((v2 & ((1u << n) - 1u)) == 0u) q &= ~1u;
+  return (int32_t)(n ? q : val);
+}
+__device__ __forceinline__ void scan_state(const int2* tab, int32_t dl, int32_t x, int32_t a, int32_t b, int32_t c, int32_t& h,
+                                           uint32_t& ya_lo, int32_t& ya_hi) {
+  const int32_t dA = exp_neg_s(tab, qmul32(dl, a));
+  h = add_sat32((int32_t)rne_lo32<30>(madw(dA, h, 1ll << 29)), qmul32(qmul32(dl, b), x));
+  // ya += rne(c h, 20): the 64-bit sum kept as two words, the low word's carry through a wide multiply-add
+  const int64_t p2 = madw(c, h, 1ll << (F - 1));
+  const uint32_t ql = rne_lo32<F>(p2);
+  const int32_t qh = hi32(p2) >> F;
+  uint64_t s;
+  asm("mad.wide.u32 %0, %1, 1, %2;" : "=l"(s) : "r"(ql), "l"((uint64_t)ya_lo));
+  ya_lo = (uint32_t)s;
+  ya_hi += qh + (int32_t)(s >> 32);
+}
+
+__global__ void __launch_bounds__(256) k_fx_scan_q(const int32_t* __restrict__ dbc, int ldj, const int8_t* __restrict__ qwdt,
+                                                   const int32_t* __restrict__ swdt, const int32_t* __restrict__ b_dt,
+                                                   const int32_t* __restrict__ a_neg, const int32_t* __restrict__ d_skip,
+                                                   const int32_t* __restrict__ xs, const int32_t* __restrict__ xz, int32_t* __restrict__ h,
+                                                   Tables t, int E, int R, int8_t* __restrict__ q, int KB,
+                                                   int32_t* __restrict__ kshift) {
+  __shared__ int2 s_tab[NTAB];
+  __shared__ __align__(16) int32_t s_bc[2 * kNState];
+  __shared__ __align__(16) int8_t s_q[64];
+  __shared__ int s_k;
+  __shared__ int64_t red[32];
+  __shared__ int32_t s_y[2048];                     // E <= 2048
+  const int i = blockIdx.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int32_t* row = dbc + (size_t)i * ldj;
-  // delta's row cut to int8 (every thread of the stream computes the same k and q)
-  int64_t m = 0;
-  for (int r = 0; r < R; ++r) { const int64_t v = row[r]; m = max(m, v < 0 ? -v : v); }
-  const int k = max(bitlen64(m) - 7, 0);
-  int acc = 0;
-  for (int r = 0; r < R; ++r) {
-    int64_t q = rne((int64_t)row[r], k);
-    q = q > 127 ? 127 : (q < -127 ? -127 : q);
-    acc += (int)q * (int)qwdt[(size_t)e * R + r];
+  {
+    const int32_t a = t.exp2[tid];
+    s_tab[tid] = make_int2(a, t.exp2[tid + 1] - a);
   }
-  const int64_t v = sat(rne((int64_t)acc, max(swdt[e] - k, -31)));
-  const int64_t dl = softplus(t, sat(v + (int64_t)b_dt[e]));
-  const int64_t x = xs[idx], z = xz[(size_t)i * 2 * E + E + e];
-  int32_t* hp = h + (size_t)idx * kNState;
-  int64_t ya = 0;
-#pragma unroll 4
-  for (int n = 0; n < kNState; ++n) {
-    const int64_t dA = exp_neg(t, qmul(dl, a_neg[(size_t)e * kNState + n]));
-    const int64_t hv = sat(rne(dA * (int64_t)hp[n], 30) + qmul(qmul(dl, row[R + n]), x));
-    hp[n] = (int32_t)hv;
-    ya += rne((int64_t)row[R + kNState + n] * hv, F);
+  if (tid < 2 * kNState) s_bc[tid] = row[R + tid];
+  if (warp == 1) {                                  // delta's row cut to int8 (R <= 64)
+    const int32_t v0 = lane < R ? row[lane] : 0, v1 = lane + 32 < R ? row[lane + 32] : 0;
+    int64_t m = max(abs64(v0), abs64(v1));
+    for (int o = 16; o > 0; o >>= 1) { const int64_t w = __shfl_xor_sync(0xffffffffu, m, o); m = w > m ? w : m; }
+    const int k = max(bitlen64(m) - 7, 0);
+    s_q[lane] = cut8(v0, k);
+    s_q[lane + 32] = cut8(v1, k);
+    if (lane == 0) s_k = k;
   }
-  const int64_t yv = sat(ya + rne((int64_t)d_skip[e] * x, F));
-  y[idx] = (int32_t)qmul(yv, silu(t, z));
+  __syncthreads();
+  const int kd = s_k;
+  int64_t ym = 0;
+#pragma unroll 1
+  for (int cg = warp; cg * 32 < E; cg += 8) {       // channel group: warp-uniform
+    {
+      const int e = cg * 32 + lane;
+      int acc = 0;
+      if ((R & 3) == 0) {
+        const int* wq = reinterpret_cast<const int*>(qwdt + (size_t)e * R);
+        const int* sq = reinterpret_cast<const int*>(s_q);
+        for (int r = 0; r < (R >> 2); ++r) acc = __dp4a(sq[r], wq[r], acc);
+      } else {
+        for (int r = 0; r < R; ++r) acc += (int)s_q[r] * (int)qwdt[(size_t)e * R + r];
+      }
+      const int64_t dv = sat(rne((int64_t)acc, max(swdt[e] - kd, -31)));
+      const int32_t dl = (int32_t)softplus(t, sat(dv + (int64_t)b_dt[e]));
+      const int32_t x = xs[(size_t)i * E + e];
+      const int64_t z = xz[(size_t)i * 2 * E + E + e];
+      int4* hp = reinterpret_cast<int4*>(h + ((size_t)i * E + (size_t)cg * 32) * kNState) + lane;
+      const int4* ap = reinterpret_cast<const int4*>(a_neg + (size_t)cg * 32 * kNState) + lane;
+      const int4 b4 = reinterpret_cast<const int4*>(s_bc)[lane & 3], c4 = reinterpret_cast<const int4*>(s_bc)[4 + (lane & 3)];
+      int4 hv[4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) hv[j] = __ldcs(hp + 32 * j);
+      int64_t ya_own = 0;
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        const int src = 8 * j + (lane >> 2);
+        const int32_t dlj = __shfl_sync(0xffffffffu, dl, src), xj = __shfl_sync(0xffffffffu, x, src);
+        const int4 a4 = __ldg(ap + 32 * j);
+        uint32_t ya_lo = 0;
+        int32_t ya_hi = 0;
+        scan_state(s_tab, dlj, xj, a4.x, b4.x, c4.x, hv[j].x, ya_lo, ya_hi);
+        scan_state(s_tab, dlj, xj, a4.y, b4.y, c4.y, hv[j].y, ya_lo, ya_hi);
+        scan_state(s_tab, dlj, xj, a4.z, b4.z, c4.z, hv[j].z, ya_lo, ya_hi);
+        scan_state(s_tab, dlj, xj, a4.w, b4.w, c4.w, hv[j].w, ya_lo, ya_hi);
+        __stcs(hp + 32 * j, hv[j]);
+        int64_t ya = (int64_t)(((uint64_t)(uint32_t)ya_hi << 32) | ya_lo);
+        ya += __shfl_xor_sync(0xffffffffu, ya, 1);
+        ya += __shfl_xor_sync(0xffffffffu, ya, 2);
+        const int64_t got = __shfl_sync(0xffffffffu, ya, 4 * (lane & 7));
+        if ((lane >> 3) == j) ya_own = got;
+      }
+      const int64_t ys = sat(ya_own + rne((int64_t)d_skip[e] * (int64_t)x, F));
+      const int32_t yv = (int32_t)qmul(ys, silu(t, z));
+      s_y[e] = yv;                                  // read back by the same thread below
+      ym = max(ym, abs64(yv));
+    }
+  }
+  ym = block_max(ym, red);
+  const int k = max(bitlen64(ym) - 7, 0);
+  for (int cg = warp; cg * 32 < E; cg += 8) {
+    const int e = cg * 32 + lane;
+    q[a_img_off(i, e, KB)] = cut8(s_y[e], k);
+  }
+  if (tid == 0) kshift[i] = k;
 }
 
 }  // namespace fx
