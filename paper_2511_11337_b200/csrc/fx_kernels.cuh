@@ -32,12 +32,29 @@ __device__ __forceinline__ int64_t rne(int64_t v, int k) {
 }
 __device__ __forceinline__ int64_t sat(int64_t v) { return v > QMAX ? QMAX : (v < QMIN ? QMIN : v); }
 __device__ __forceinline__ int64_t qmul(int64_t a, int64_t b) { return sat(rne(a * b, F)); }
-// round-half-even(n / d), d > 0
-__device__ __forceinline__ int64_t rdiv(int64_t n, int64_t d) {
-  int64_t q = n / d, r = n - q * d;
-  if (r < 0) { r += d; q -= 1; }                        // floor division
-  return q + ((2 * r > d || (2 * r == d && (q & 1))) ? 1 : 0);
+// round-half-even(n / d), d > 0, |n| < 2^62.  The quotient is estimated in double precision and then corrected with
+// the exact remainder until 0 <= r < d, and the rounding is decided on that exact remainder: the result is the integer
+// the definition names whatever the quality of the estimate (which only decides how many correction steps run: none or
+// one with the reciprocal below), without the 64-bit division subroutine.
+// rcp ~ 1 / d, passed in so that a row with one divisor computes it once.
+__device__ __forceinline__ double rcp_est(int64_t d) {        // two Newton steps on the hardware's approximation
+  const double dd = __ll2double_rn(d);
+  double x;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(x) : "d"(dd));
+  x = fma(fma(-dd, x, 1.0), x, x);
+  x = fma(fma(-dd, x, 1.0), x, x);
+  return x;
 }
+__device__ __forceinline__ int64_t rdiv_rcp(int64_t n, int64_t d, double rcp) {
+  const int64_t a = n < 0 ? -n : n;
+  int64_t q = __double2ll_rz(__ll2double_rz(a) * rcp);
+  int64_t r = a - q * d;
+  while (r < 0) { q -= 1; r += d; }
+  while (r >= d) { q += 1; r -= d; }
+  q += (2 * r > d || (2 * r == d && (q & 1))) ? 1 : 0;      // ties to even (symmetric in the sign of n)
+  return n < 0 ? -q : q;
+}
+__device__ __forceinline__ int64_t rdiv(int64_t n, int64_t d) { return rdiv_rcp(n, d, rcp_est(d)); }
 __device__ __forceinline__ int64_t isqrt64(int64_t x) {  // floor(sqrt(x)) exactly, 0 <= x < 2^62
   int64_t y = (int64_t)floor(sqrt((double)x));
   if (y * y > x) --y;
@@ -161,11 +178,12 @@ __global__ void __launch_bounds__(256) k_fx_rmsnorm_q(const int32_t* __restrict_
     for (int it = 0; it < 4; ++it) { const int64_t t = rne((int64_t)uv[it], -c); s += t * t; }
     s = block_sum(s, red);
     const int64_t Y = isqrt64(s + (int64_t)D * rne(EPS_Q40, -2 * c));
+    const double rcp_y = rcp_est(Y);
 #pragma unroll
     for (int it = 0; it < 4; ++it) {
       const int d = threadIdx.x + 256 * it;
       if (d < D) {
-        rv[it] = (int32_t)qmul(rdiv(rne((int64_t)uv[it], -c) * sqrt_d, Y), w[d]);
+        rv[it] = (int32_t)qmul(rdiv_rcp(rne((int64_t)uv[it], -c) * sqrt_d, Y, rcp_y), w[d]);
         rm = max(rm, abs64(rv[it]));
       }
     }
@@ -195,6 +213,85 @@ __global__ void k_fx_quant_rows(const int32_t* __restrict__ a, int lda, int K, i
   if (threadIdx.x == 0) kshift[row] = k;
 }
 
+// ---- 32-bit forms.  The integer ALU pipe is what bounds the scan, so the roundings are written on 32-bit halves: the rounding constant
+// rides on the multiply (mad.wide), "ties to even" is "add half, shift, clear the low bit if the shifted-out bits are
+// all zero", and a saturation test is a range test of the high word.  Same integers as rne / sat / qmul above.
+// (the rounding constants live in constant memory, so that they are the multiply-add's addend operand instead of an
+// immediate the compiler adds with a separate 64-bit addition on the bounding pipe)
+__constant__ int64_t c_half[3] = {1ll << (F - TB - 1), 1ll << (F - 1), 1ll << 29};
+#define FX_HALF12 c_half[0]
+#define FX_HALF20 c_half[1]
+#define FX_HALF30 c_half[2]
+__device__ __forceinline__ int64_t madw(int32_t a, int32_t b, int64_t c) {
+  int64_t r;
+  asm("mad.wide.s32 %0, %1, %2, %3;" : "=l"(r) : "r"(a), "r"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ uint32_t lo32(int64_t v) { return (uint32_t)v; }
+__device__ __forceinline__ int32_t hi32(int64_t v) { return (int32_t)(v >> 32); }
+__device__ __forceinline__ int32_t add_sat32(int32_t a, int32_t b) {
+  int32_t r;
+  asm("add.sat.s32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
+  return r;
+}
+// low 32 bits of rne(p, K), given p2 = p + 2^(K-1), 1 <= K <= 31
+template <int K>
+__device__ __forceinline__ uint32_t rne_lo32(int64_t p2) {
+  uint32_t q = __funnelshift_r(lo32(p2), (uint32_t)hi32(p2), K);
+  if ((lo32(p2) & ((1u << K) - 1u)) == 0u) q &= ~1u;
+  return q;
+}
+// sat(rne(a b, 20));  SAT = false: the caller has shown that the quotient fits 32 bits
+template <bool SAT = true>
+__device__ __forceinline__ int32_t qmul32(int32_t a, int32_t b) {
+  const int64_t p2 = madw(a, b, FX_HALF20);
+  uint32_t q = rne_lo32<F>(p2);
+  if (SAT) {
+    const int32_t h = hi32(p2);                     // the quotient fits 32 bits iff -2^19 <= h < 2^19
+    if ((uint32_t)(h + (1 << (F - 1))) >= (1u << F)) q = 0x7FFFFFFFu ^ (uint32_t)(h >> 31);
+  }
+  return (int32_t)q;
+}
+// qmul(a, b) for a, b >= 0 as the argument of exp_neg: any value >= 2^25 (32.0) stands for "exp_neg = 0"
+// (n >= 46 there), so the saturation is one comparison of the high word (2^13 <-> quotient 2^25)
+__device__ __forceinline__ int32_t qmul32_exparg(int32_t a, int32_t b) {
+  const int64_t p2 = madw(a, b, FX_HALF20);
+  const uint32_t q = rne_lo32<F>(p2);
+  return hi32(p2) >= (1 << 13) ? (1 << 26) : (int32_t)q;
+}
+// exp_neg for 0 <= x <= QMAX from the table (value, difference to the next entry) in shared memory: the same integers
+// as fx::exp_neg (n >= 31 rounds to 0 through the shift; val <= 2^30 so the last rounding is 32-bit)
+__device__ __forceinline__ int32_t exp_neg_s(const int2* tab, int32_t x) {
+  const uint32_t tq = rne_lo32<30>(madw(x, (int32_t)LOG2E_Q30, FX_HALF30));     // < 2^32
+  const uint32_t n = min(tq >> F, 31u);
+  const int2 e = tab[(tq >> (F - TB)) & (NTAB - 1)];
+  const uint32_t val = (uint32_t)e.x + rne_lo32<F - TB>(madw(e.y, (int32_t)(tq & ((1u << (F - TB)) - 1u)), FX_HALF12));
+  const uint32_t v2 = val + ((1u << n) >> 1);
+  uint32_t q = v2 >> n;
+  if ((v2 & ((1u << n) - 1u)) == 0u) q &= ~1u;
+  return (int32_t)(n ? q : val);
+}
+// the table of exp2_neg as (value, difference to the next entry) pairs in shared memory; blockDim.x >= 256
+__device__ __forceinline__ void load_exp_table(int2* s_tab, const Tables& t) {
+  if (threadIdx.x < NTAB) {
+    const int32_t a = t.exp2[threadIdx.x];
+    s_tab[threadIdx.x] = make_int2(a, t.exp2[threadIdx.x + 1] - a);
+  }
+}
+// sigmoid, SiLU, softplus on the shared table: the same integers as fx::sigmoid / silu / softplus (|x| = 2^31 is cut to
+// QMAX: exp_neg is 0 for both)
+__device__ __forceinline__ int64_t sigmoid_s(const int2* tab, int32_t x) {
+  const uint32_t ax = min(x < 0 ? -(uint32_t)x : (uint32_t)x, (uint32_t)QMAX);
+  const int64_t s = rdiv(1ll << 60, U30 + (int64_t)exp_neg_s(tab, (int32_t)ax));
+  return x >= 0 ? s : U30 - s;
+}
+__device__ __forceinline__ int64_t silu_s(const int2* tab, int32_t x) { return sat(rne((int64_t)x * sigmoid_s(tab, x), 30)); }
+__device__ __forceinline__ int64_t softplus_s(const int2* tab, const Tables& t, int32_t v) {
+  const uint32_t av = min(v < 0 ? -(uint32_t)v : (uint32_t)v, (uint32_t)QMAX);
+  const int64_t l30 = interp(t.log1p, (int64_t)exp_neg_s(tab, (int32_t)av), 30);
+  return sat((int64_t)(v > 0 ? v : 0) + rne(l30, 30 - F));
+}
+
 // ---- S4: causal depthwise conv over the window (x_{t-3}, x_{t-2}, x_{t-1}) and x_t, SiLU; the window shifts.
 // xz [B][2E] Q (x | z);  win [B][3][E];  xs [B][E] Q (read by the scan) and its int8 cut (q, kshift) for x_proj.
 // One block of 256 threads per stream, E <= 2048 (<= 8 channels per thread).
@@ -203,6 +300,9 @@ __global__ void __launch_bounds__(256) k_fx_conv_silu_q(const int32_t* __restric
                                                         int32_t* __restrict__ xs, Tables t, int E, int8_t* __restrict__ q, int KB,
                                                         int32_t* __restrict__ kshift) {
   __shared__ int64_t red[32];
+  __shared__ int2 s_tab[NTAB];
+  load_exp_table(s_tab, t);
+  __syncthreads();
   const int i = blockIdx.x;
   int32_t v[8];
   int64_t m = 0;
@@ -218,7 +318,7 @@ __global__ void __launch_bounds__(256) k_fx_conv_silu_q(const int32_t* __restric
       const int64_t acc = (int64_t)conv_b[e] + rne((int64_t)cw.w * x, F) + rne((int64_t)cw.x * w0, F) + rne((int64_t)cw.y * w1, F) +
                           rne((int64_t)cw.z * w2, F);
       w[0] = (int32_t)w1; w[E] = (int32_t)w2; w[2 * E] = (int32_t)x;
-      v[it] = (int32_t)silu(t, sat(acc));
+      v[it] = (int32_t)silu_s(s_tab, (int32_t)sat(acc));
       xs[(size_t)i * E + e] = v[it];
       m = max(m, abs64(v[it]));
     }
@@ -241,54 +341,13 @@ __global__ void __launch_bounds__(256) k_fx_conv_silu_q(const int32_t* __restric
 // 8 j + l / 4 in row j, so a channel's sum over n is an (order-free, integer) sum over four lanes.
 // The recurrence of one state value, every product 32 x 32 -> 64 bits:
 //   dA = exp_neg(qmul(dt, |A|));  h = sat(rne(dA h, 30) + qmul(qmul(dt, B_n), x));  y += rne(C_n h, 20)
-// The integer ALU pipe is what bounds this kernel, so the roundings are written on 32-bit halves: the rounding constant
-// rides on the multiply (mad.wide), "ties to even" is "add half, shift, clear the low bit if the shifted-out bits are
-// all zero", and a saturation test is a range test of the high word.  Same integers as rne / sat / qmul above.
-__device__ __forceinline__ int64_t madw(int32_t a, int32_t b, int64_t c) {
-  int64_t r;
-  asm("mad.wide.s32 %0, %1, %2, %3;" : "=l"(r) : "r"(a), "r"(b), "l"(c));
-  return r;
-}
-__device__ __forceinline__ uint32_t lo32(int64_t v) { return (uint32_t)v; }
-__device__ __forceinline__ int32_t hi32(int64_t v) { return (int32_t)(v >> 32); }
-__device__ __forceinline__ int32_t add_sat32(int32_t a, int32_t b) {
-  int32_t r;
-  asm("add.sat.s32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(b));
-  return r;
-}
-// low 32 bits of rne(p, K), given p2 = p + 2^(K-1), 1 <= K <= 31
-template <int K>
-__device__ __forceinline__ uint32_t rne_lo32(int64_t p2) {
-  uint32_t q = __funnelshift_r(lo32(p2), (uint32_t)hi32(p2), K);
-  if ((lo32(p2) & ((1u << K) - 1u)) == 0u) q &= ~1u;
-  return q;
-}
-// sat(rne(a b, 20))
-__device__ __forceinline__ int32_t qmul32(int32_t a, int32_t b) {
-  const int64_t p2 = madw(a, b, 1ll << (F - 1));
-  uint32_t q = rne_lo32<F>(p2);
-  const int32_t h = hi32(p2);                       // the quotient fits 32 bits iff -2^19 <= h < 2^19
-  if ((uint32_t)(h + (1 << (F - 1))) >= (1u << F)) q = 0x7FFFFFFFu ^ (uint32_t)(h >> 31);
-  return (int32_t)q;
-}
-// exp_neg for 0 <= x <= QMAX from the table (value, difference to the next entry) in shared memory: the same integers
-// as fx::exp_neg (n >= 31 rounds to 0 through the shift; val <= 2^30 so the last rounding is 32-bit)
-__device__ __forceinline__ int32_t exp_neg_s(const int2* tab, int32_t x) {
-  const uint32_t tq = rne_lo32<30>(madw(x, (int32_t)LOG2E_Q30, 1ll << 29));     // < 2^32
-  const uint32_t n = min(tq >> F, 31u);
-  const int2 e = tab[(tq >> (F - TB)) & (NTAB - 1)];
-  const uint32_t val = (uint32_t)e.x + rne_lo32<F - TB>(madw(e.y, (int32_t)(tq & ((1u << (F - TB)) - 1u)), 1ll << (F - TB - 1)));
-  const uint32_t v2 = val + ((1u << n) >> 1);
-  uint32_t q = v2 >> n;
-  if ((v2 & ((1u << n) - 1u)) == 0u) q &= ~1u;
-  return (int32_t)(n ? q : val);
-}
+template <bool SAT>
 __device__ __forceinline__ void scan_state(const int2* tab, int32_t dl, int32_t x, int32_t a, int32_t b, int32_t c, int32_t& h,
                                            uint32_t& ya_lo, int32_t& ya_hi) {
-  const int32_t dA = exp_neg_s(tab, qmul32(dl, a));
-  h = add_sat32((int32_t)rne_lo32<30>(madw(dA, h, 1ll << 29)), qmul32(qmul32(dl, b), x));
+  const int32_t dA = exp_neg_s(tab, qmul32_exparg(dl, a));
+  h = add_sat32((int32_t)rne_lo32<30>(madw(dA, h, FX_HALF30)), qmul32<SAT>(qmul32<SAT>(dl, b), x));
   // ya += rne(c h, 20): the 64-bit sum kept as two words, the low word's carry through a wide multiply-add
-  const int64_t p2 = madw(c, h, 1ll << (F - 1));
+  const int64_t p2 = madw(c, h, FX_HALF20);
   const uint32_t ql = rne_lo32<F>(p2);
   const int32_t qh = hi32(p2) >> F;
   uint64_t s;
@@ -311,10 +370,7 @@ __global__ void __launch_bounds__(256) k_fx_scan_q(const int32_t* __restrict__ d
   __shared__ int32_t s_y[2048];                     // E <= 2048
   const int i = blockIdx.x, tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
   const int32_t* row = dbc + (size_t)i * ldj;
-  {
-    const int32_t a = t.exp2[tid];
-    s_tab[tid] = make_int2(a, t.exp2[tid + 1] - a);
-  }
+  load_exp_table(s_tab, t);
   if (tid < 2 * kNState) s_bc[tid] = row[R + tid];
   if (warp == 1) {                                  // delta's row cut to int8 (R <= 64)
     const int32_t v0 = lane < R ? row[lane] : 0, v1 = lane + 32 < R ? row[lane + 32] : 0;
@@ -327,6 +383,9 @@ __global__ void __launch_bounds__(256) k_fx_scan_q(const int32_t* __restrict__ d
   }
   __syncthreads();
   const int kd = s_k;
+  int bB = 0;                                       // bit length of max_n |B_n|
+#pragma unroll
+  for (int n = 0; n < kNState; ++n) bB = max(bB, bitlen64(abs64(s_bc[n])));
   int64_t ym = 0;
 #pragma unroll 1
   for (int cg = warp; cg * 32 < E; cg += 8) {       // channel group: warp-uniform
@@ -341,9 +400,9 @@ __global__ void __launch_bounds__(256) k_fx_scan_q(const int32_t* __restrict__ d
         for (int r = 0; r < R; ++r) acc += (int)s_q[r] * (int)qwdt[(size_t)e * R + r];
       }
       const int64_t dv = sat(rne((int64_t)acc, max(swdt[e] - kd, -31)));
-      const int32_t dl = (int32_t)softplus(t, sat(dv + (int64_t)b_dt[e]));
+      const int32_t dl = (int32_t)softplus_s(s_tab, t, (int32_t)sat(dv + (int64_t)b_dt[e]));
       const int32_t x = xs[(size_t)i * E + e];
-      const int64_t z = xz[(size_t)i * 2 * E + E + e];
+      const int32_t z = xz[(size_t)i * 2 * E + E + e];
       int4* hp = reinterpret_cast<int4*>(h + ((size_t)i * E + (size_t)cg * 32) * kNState) + lane;
       const int4* ap = reinterpret_cast<const int4*>(a_neg + (size_t)cg * 32 * kNState) + lane;
       const int4 b4 = reinterpret_cast<const int4*>(s_bc)[lane & 3], c4 = reinterpret_cast<const int4*>(s_bc)[4 + (lane & 3)];
@@ -358,10 +417,21 @@ __global__ void __launch_bounds__(256) k_fx_scan_q(const int32_t* __restrict__ d
         const int4 a4 = __ldg(ap + 32 * j);
         uint32_t ya_lo = 0;
         int32_t ya_hi = 0;
-        scan_state(s_tab, dlj, xj, a4.x, b4.x, c4.x, hv[j].x, ya_lo, ya_hi);
-        scan_state(s_tab, dlj, xj, a4.y, b4.y, c4.y, hv[j].y, ya_lo, ya_hi);
-        scan_state(s_tab, dlj, xj, a4.z, b4.z, c4.z, hv[j].z, ya_lo, ya_hi);
-        scan_state(s_tab, dlj, xj, a4.w, b4.w, c4.w, hv[j].w, ya_lo, ya_hi);
+        // |dt B_n| 2^-20 <= 2^(bd + bB - 20) and |(dt B_n) x| 2^-40 <= 2^(bd + bB + bx - 39) with bd, bB, bx the bit
+        // lengths of dt, max_n |B_n|, |x|: when both stay below 2^31 for every lane the two products cannot saturate
+        // and the warp takes the instantiation without the range tests (the same integers either way)
+        const int bd = 32 - __clz(dlj), bx = 32 - __clz(xj < 0 ? -(uint32_t)xj : (uint32_t)xj);
+        if (__all_sync(0xffffffffu, bd + bB <= 50 && bd + bB + bx <= 69)) {
+          scan_state<false>(s_tab, dlj, xj, a4.x, b4.x, c4.x, hv[j].x, ya_lo, ya_hi);
+          scan_state<false>(s_tab, dlj, xj, a4.y, b4.y, c4.y, hv[j].y, ya_lo, ya_hi);
+          scan_state<false>(s_tab, dlj, xj, a4.z, b4.z, c4.z, hv[j].z, ya_lo, ya_hi);
+          scan_state<false>(s_tab, dlj, xj, a4.w, b4.w, c4.w, hv[j].w, ya_lo, ya_hi);
+        } else {
+          scan_state<true>(s_tab, dlj, xj, a4.x, b4.x, c4.x, hv[j].x, ya_lo, ya_hi);
+          scan_state<true>(s_tab, dlj, xj, a4.y, b4.y, c4.y, hv[j].y, ya_lo, ya_hi);
+          scan_state<true>(s_tab, dlj, xj, a4.z, b4.z, c4.z, hv[j].z, ya_lo, ya_hi);
+          scan_state<true>(s_tab, dlj, xj, a4.w, b4.w, c4.w, hv[j].w, ya_lo, ya_hi);
+        }
         __stcs(hp + 32 * j, hv[j]);
         int64_t ya = (int64_t)(((uint64_t)(uint32_t)ya_hi << 32) | ya_lo);
         ya += __shfl_xor_sync(0xffffffffu, ya, 1);
@@ -370,7 +440,7 @@ __global__ void __launch_bounds__(256) k_fx_scan_q(const int32_t* __restrict__ d
         if ((lane >> 3) == j) ya_own = got;
       }
       const int64_t ys = sat(ya_own + rne((int64_t)d_skip[e] * (int64_t)x, F));
-      const int32_t yv = (int32_t)qmul(ys, silu(t, z));
+      const int32_t yv = (int32_t)qmul(ys, silu_s(s_tab, z));
       s_y[e] = yv;                                  // read back by the same thread below
       ym = max(ym, abs64(yv));
     }
