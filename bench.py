@@ -349,6 +349,42 @@ def sweep_point(boa, peaks, config, streams, chunk, label, sample_every=2):
     return ent
 
 
+def fx_point(boa, config, streams, chunk, label):
+    """One pass (after one warm-up pass) of FX1, the deterministic fixed-point pipeline, on a configs[]
+    model shape at `streams` x `chunk` bytes, device buffers, CUDA events around boa_fx_compress / boa_fx_decompress."""
+    import torch
+    from paper_2511_11337_b200 import synth
+    base = synth.CONFIGS[config]
+    n = streams * chunk
+    dev = torch.device("cuda", torch.cuda.current_device())
+    m = boa.FxModel(base.weights())
+    d_in = torch.frombuffer(bytearray(base.data(n)), dtype=torch.uint8).to(dev)
+    d_comp = torch.empty(boa.compress_bound(n, chunk), dtype=torch.uint8, device=dev)
+    d_out = torch.empty(n, dtype=torch.uint8, device=dev)
+    for _ in range(2):
+        ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        ev[0].record()
+        clen = m.compress_into(d_in, chunk, d_comp)
+        launches = m.last_launches
+        ev[1].record()
+        m.decompress_into(d_comp[:clen], d_out)
+        launches += m.last_launches
+        ev[2].record()
+        torch.cuda.synchronize()
+    if not torch.equal(d_out, d_in):
+        raise SystemExit("bench.py: FX1 round trip is not byte-exact")
+    tc, td = ev[0].elapsed_time(ev[1]), ev[1].elapsed_time(ev[2])
+    ent = {"point": label, "model": f"{base.shape.n_layer}-layer d_model={base.shape.d_model}, INT8 rows / Q12.20 values",
+           "streams": streams, "chunk_bytes": chunk, "round_trip": "byte-exact",
+           "compress_MiBps": n / MiB / (tc / 1e3), "decompress_MiBps": n / MiB / (td / 1e3),
+           "us_per_step_compress": 1e3 * tc / (chunk - 1), "us_per_step_decompress": 1e3 * td / (chunk - 1),
+           "bits_per_byte": 8.0 * clen / n, "gpu_launches": int(launches)}
+    m.close()
+    del d_in, d_comp, d_out
+    torch.cuda.empty_cache()
+    return ent
+
+
 def run_ours(args, cfg):
     import torch
     import torch.distributed as dist
@@ -476,6 +512,12 @@ def run_ours(args, cfg):
             # (few streams: no event-bracketed eager batches - they would be most of a step that is pure latency)
             sweep.append(sweep_point(boa, peaks, config, streams, chunk_b, label, sample_every=2 if streams > 1024 else 0))
         line["sweep"] = sweep
+        # FX1: the integer pipeline whose containers do not depend on the device, once per point
+        line["fx1"] = [fx_point(boa, 2, 4096, 273, "configs[1] model shape at B = 4,096 streams"),
+                       fx_point(boa, 4, 65536, 65, "configs[3] model shape at B = 65,536 streams")]
+        line["fx1_note"] = ("every step an integer kernel (tcgen05.mma kind::i8 contractions, integer RMSNorm / exp / sigmoid / "
+                            "softplus by table, Q12.20 recurrence); logits, tables and containers bit-identical to oracle/fixed.py "
+                            "(tests/test_gpu_fixed.py); both directions run the step path")
         if not args.no_largest:
             # the largest single-GPU configuration: configs[3] at 65,536 chunks x 16 KiB = 1 GiB, one pass, no warm-up pass
             # of its own (the sweep point above has run the same model at the same B)
@@ -584,8 +626,16 @@ def main():
     ap.add_argument("--pair-tiles", type=int, default=-1, help="measurement only: row-tile threshold from which the step path uses CTA-pair tiles (boa_debug_set_pair_tiles; -1 = library default)")
     ap.add_argument("--streams", type=int, default=0, help="run the config's model with this many chunks (streams per step) ...")
     ap.add_argument("--chunk-bytes", type=int, default=0, help="... of this many bytes each (a sweep point, not the headline workload)")
+    ap.add_argument("--fx-only", action="store_true", help="measurement only: one FX1 point (--config, --streams, --chunk-bytes) and nothing else; prints that entry")
     args = ap.parse_args()
     from paper_2511_11337_b200 import synth
+    if args.fx_only:
+        import torch
+        from paper_2511_11337_b200 import boa
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py: no CUDA device — the product path has no CPU fallback")
+        print(json.dumps(fx_point(boa, args.config, args.streams or 4096, args.chunk_bytes or 273, "--fx-only")))
+        return
     cfg = synth.CONFIGS[args.config]
     if args.streams or args.chunk_bytes:
         chunk = args.chunk_bytes or cfg.chunk_bytes
