@@ -1,5 +1,5 @@
 """NEXT-3 — the deterministic fixed-point pipeline "FX1" (PAPER "Portability").
-Oracle; test infrastructure.  parity: no kernel exists yet - this file IS the specification's executable form.
+Oracle; test infrastructure.  parity: the GPU kernels (boa_fx_*, csrc/fx_*.cuh) are compared with this file bit for bit (tests/test_gpu_fixed.py); this file IS the specification's executable form.
 
 The paper proposes to "quantise all Mamba state-space and affine transformations to a bit-deterministic INT8
 (or fixed-point) representation with explicitly specified rounding and saturation rules" and to make normalisation and
