@@ -155,10 +155,12 @@ int boa_stream_decompress(boa_model* m, const uint8_t* in, size_t in_len, uint8_
  * deterministic normalisation and softmax, so that a container written on one device decodes on another.
  * DESIGN.md section 11 is that specification (Q12.20 values, INT8 rows with power-of-two scales, round-half-even,
  * saturating stores, table-driven integer exp / sigmoid / softplus, integer RMSNorm, the integer table rule); these entry
- * points run it on the GPU, every step an integer kernel (csrc/fx_kernels.cuh).  Integer arithmetic has one correct
+ * points run it on the GPU, every step an integer kernel (csrc/fx_kernels.cuh; the contractions on tcgen05.mma kind::i8,
+ * csrc/fx_gemm_tc.cuh).  Integer arithmetic has one correct
  * answer: logits, tables and whole containers are bit-identical to the exact-integer oracle's (tests).
  *   boa_fx_model_load   parse a BOAW blob of north_star's block with the tied head (flags == 1; else BOA_E_UNSUPPORTED;
- *                       d_model <= 1024), quantise it as section 11 says (host), copy it to the device
+ *                       d_model a multiple of 64 and <= 1024, dt_rank <= 64, at most 64 layers), quantise it as section 11
+ *                       says (host), lay the INT8 rows out as tensor-core operand images, copy them to the device
  *   boa_fx_model_fingerprint   ('FX01' << 32) | CRC-32(blob): the arithmetic word is a constant - FX1 containers are
  *                       portable by construction, and are never accepted by a floating-point boa_model (nor vice versa)
  *   boa_fx_compress / boa_fx_decompress   as boa_compress / boa_decompress (same BOA1 container, same pointer and error

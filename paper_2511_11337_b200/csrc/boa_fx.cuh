@@ -25,7 +25,7 @@ struct boa_fx_model {
   std::vector<FxLayerDev> layers;
   // workspace of a wave
   uint64_t Bcap = 0;
-  GrowBuf u, r, xz, xs, dbc, y, logits, qa, ka, h, win;
+  GrowBuf u, xz, xs, dbc, logits, qa, ka, h, win;
   GrowBuf pos, len, low, range, pending, wpos, cache, started, v, rpos, off, size, scratch, first, err, total;
   GrowBuf stage_in, stage_out;
   PinBuf pin;
@@ -33,7 +33,7 @@ struct boa_fx_model {
   cudaEvent_t user_ev = nullptr;
   uint64_t launches = 0;
   ~boa_fx_model() {
-    for (GrowBuf* b : {&w32, &w8, &u, &r, &xz, &xs, &dbc, &y, &logits, &qa, &ka, &h, &win, &pos, &len, &low, &range, &pending,
+    for (GrowBuf* b : {&w32, &w8, &u, &xz, &xs, &dbc, &logits, &qa, &ka, &h, &win, &pos, &len, &low, &range, &pending,
                        &wpos, &cache, &started, &v, &rpos, &off, &size, &scratch, &first, &err, &total, &stage_in, &stage_out})
       b->release();
     pin.release();
@@ -236,8 +236,8 @@ namespace {
 int fx_reserve(boa_fx_model* m, uint64_t B, size_t cap) {
   const size_t D = m->D, E = m->E, L = m->L;
   if (B > m->Bcap) {
-    BOA_TRY(m->u.reserve(B * D * 4)); BOA_TRY(m->r.reserve(B * std::max(D, E) * 4)); BOA_TRY(m->xz.reserve(B * 2 * E * 4));
-    BOA_TRY(m->xs.reserve(B * E * 4)); BOA_TRY(m->dbc.reserve(B * m->ldj * 4)); BOA_TRY(m->y.reserve(B * E * 4));
+    BOA_TRY(m->u.reserve(B * D * 4)); BOA_TRY(m->xz.reserve(B * 2 * E * 4));
+    BOA_TRY(m->xs.reserve(B * E * 4)); BOA_TRY(m->dbc.reserve(B * m->ldj * 4));
     BOA_TRY(m->logits.reserve(B * 256 * 4)); BOA_TRY(m->qa.reserve(fx::a_img_bytes(B, fx_kb(E)))); BOA_TRY(m->ka.reserve(B * 4));
     BOA_TRY(m->h.reserve(L * B * E * kNState * 4)); BOA_TRY(m->win.reserve(L * B * 3 * E * 4));
     BOA_TRY(m->pos.reserve(B * 4)); BOA_TRY(m->len.reserve(B * 4)); BOA_TRY(m->low.reserve(B * 8)); BOA_TRY(m->range.reserve(B * 4));
@@ -366,7 +366,7 @@ int fx_reset(boa_fx_model* m, cudaStream_t st) {
 }
 
 uint64_t fx_wave_streams(const boa_fx_model* m, uint64_t nc, size_t cap) {
-  const size_t per = (size_t)m->L * m->E * (kNState + 3) * 4 + (size_t)(2 * m->D + 5 * m->E + m->ldj + 256) * 4 + 128 + cap;
+  const size_t per = (size_t)m->L * m->E * (kNState + 3) * 4 + (size_t)(m->D + 3 * m->E + m->ldj + 256) * 4 + m->E + 128 + cap;
   size_t free_b = 0, total_b = 0;
   uint64_t w = std::min<uint64_t>(nc, kMaxWaveStreams);
   if (cudaMemGetInfo(&free_b, &total_b) == cudaSuccess) w = std::min<uint64_t>(w, std::max<uint64_t>(1, (uint64_t)(free_b * 0.8) / per + m->Bcap));

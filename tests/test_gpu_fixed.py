@@ -26,6 +26,8 @@ def _cases():
         "cfg2_shape_sharp": synth.make_weights(synth.CONFIGS[2].shape, 1, emb_std=0.25),
         "cfg5_shape_l2_sharp": synth.make_weights(synth.ModelShape(2, 512, dt_rank=32), 3, synth.DTYPE_BF16, emb_std=0.25),
         "wide_scales": synth.make_weights(synth.ModelShape(1, 64, dt_rank=4), 31, std=0.5, emb_std=2.0),   # saturation is reached
+        # the widest model FX1 accepts: K = 2048 = 16 k-blocks (the contraction's 8-stage ring is refilled), dt_rank 64
+        "d1024_r64_bf16_sharp": synth.make_weights(synth.ModelShape(1, 1024, dt_rank=64), 11, synth.DTYPE_BF16, emb_std=0.25),
     }
 
 
@@ -70,9 +72,9 @@ def test_fx_edges_errors_and_batch_independence(boa):
     for n, chunk in [(1, 64), (5, 1), (300, 2), (1000, 7)]:
         data = cfg.data(n)
         assert _np(gm.decompress(gm.compress(data, chunk))).tobytes() == data, (n, chunk)
-    data = cfg.data(140 * 30)                                      # 140 streams: more than one 64-row tile of the contraction
+    data = cfg.data(140 * 30)                                      # 140 streams: more than one 128-row tile of the contraction
     _, _, _, _, pa = container.unpack(_np(gm.compress(data, 30)).tobytes())
-    for i in (0, 63, 64, 139):
+    for i in (0, 63, 64, 127, 128, 139):
         _, _, _, _, ps = container.unpack(_np(gm.compress(data[i * 30:(i + 1) * 30], 30)).tobytes())
         assert ps[0] == pa[i], i
     # an FX1 container and a floating-point model reject each other
