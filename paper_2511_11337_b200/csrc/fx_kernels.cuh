@@ -356,7 +356,7 @@ __device__ __forceinline__ void scan_state(const int2* tab, int32_t dl, int32_t 
   ya_hi += qh + (int32_t)(s >> 32);
 }
 
-__global__ void __launch_bounds__(256) k_fx_scan_q(const int32_t* __restrict__ dbc, int ldj, const int8_t* __restrict__ qwdt,
+__global__ void __launch_bounds__(256, 4) k_fx_scan_q(const int32_t* __restrict__ dbc, int ldj, const int8_t* __restrict__ qwdt,
                                                    const int32_t* __restrict__ swdt, const int32_t* __restrict__ b_dt,
                                                    const int32_t* __restrict__ a_neg, const int32_t* __restrict__ d_skip,
                                                    const int32_t* __restrict__ xs, const int32_t* __restrict__ xz, int32_t* __restrict__ h,
