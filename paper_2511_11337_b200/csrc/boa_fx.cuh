@@ -287,7 +287,7 @@ int fx_contract(FxCtx& c, int K, const uint8_t* qw, const int32_t* sw, int N, in
   return BOA_OK;
 }
 
-// one model step + one coder step for the B streams of the wave, every operation an FX1 kernel (6 L + 4 launches)
+// one model step + one coder step for the B streams of the wave, every operation an FX1 kernel (6 L + 3 launches)
 int fx_step(FxCtx& c) {
   boa_fx_model* m = c.m;
   const int B = c.B, D = m->D, E = m->E;
@@ -299,14 +299,14 @@ int fx_step(FxCtx& c) {
   int8_t* qa = m->qa.as<int8_t>();
   int32_t* ka = m->ka.as<int32_t>();
   const int ldd = (int)fx_kb((size_t)D), lde = (int)fx_kb((size_t)E);       // k-blocks of the activation images
-  fx::k_fx_embed<<<(unsigned)(((size_t)B * D + 255) / 256), 256, 0, c.st>>>(c.data, c.chunk_bytes, c.ca.pos, c.ca.len, m->q_emb, m->s_emb,
-                                                                           u, B, D);
-  ++m->launches;
+  const int rgrid = (B + fx::RMS_ROWS - 1) / fx::RMS_ROWS;
+  const fx::EmbedSrc es{c.data, c.chunk_bytes, c.ca.pos, c.ca.len, m->q_emb, m->s_emb};
   for (int l = 0; l < m->L; ++l) {
     const FxLayerDev& w = m->layers[l];
     int32_t* hl = m->h.as<int32_t>() + (size_t)l * m->Bcap * E * kNState;
     int32_t* winl = m->win.as<int32_t>() + (size_t)l * m->Bcap * 3 * E;
-    fx::k_fx_rmsnorm_q<<<B, 256, 0, c.st>>>(u, w.norm_w, D, m->sqrt_d, qa, ldd, ka);
+    if (l == 0) fx::k_fx_rmsnorm_q<true><<<rgrid, 32 * fx::RMS_ROWS, 0, c.st>>>(u, w.norm_w, D, m->sqrt_d, qa, ldd, ka, B, es);   // S1 + S2
+    else fx::k_fx_rmsnorm_q<false><<<rgrid, 32 * fx::RMS_ROWS, 0, c.st>>>(u, w.norm_w, D, m->sqrt_d, qa, ldd, ka, B, es);
     BOA_TRY(fx_contract(c, D, w.q_in, w.s_in, 2 * E, xz, 2 * E, nullptr));
     fx::k_fx_conv_silu_q<<<B, 256, 0, c.st>>>(xz, winl, w.conv_w, w.conv_b, xs, m->tab, E, qa, lde, ka);
     BOA_TRY(fx_contract(c, E, w.q_x, w.s_x, m->J, dbc, m->ldj, nullptr));
@@ -314,7 +314,7 @@ int fx_step(FxCtx& c) {
     BOA_TRY(fx_contract(c, E, w.q_out, w.s_out, D, u, D, u));
     m->launches += 3;
   }
-  fx::k_fx_quant_rows<<<B, 128, 0, c.st>>>(u, D, D, qa, ldd, ka);
+  fx::k_fx_quant_rows<<<rgrid, 32 * fx::RMS_ROWS, 0, c.st>>>(u, D, D, qa, ldd, ka, B);
   ++m->launches;
   BOA_TRY(fx_contract(c, D, m->q_head, m->s_emb, 256, logits, 256, nullptr));
   if (c.dump_logits)

@@ -133,18 +133,6 @@ __device__ __forceinline__ int64_t block_sum(int64_t v, int64_t* red) {   // int
   return s;
 }
 
-// ---- S1: u = Emb[previous byte], Q.  One thread per (stream, column).
-__global__ void k_fx_embed(const uint8_t* __restrict__ data, size_t chunk_bytes, const uint32_t* __restrict__ pos,
-                           const uint32_t* __restrict__ len, const int8_t* __restrict__ qemb, const int32_t* __restrict__ semb,
-                           int32_t* __restrict__ u, int B, int D) {
-  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
-  if (idx >= B * D) return;
-  const int i = idx / D, d = idx - i * D;
-  const uint32_t p = min(pos[i], len[i] - 1u);
-  const int b = data[(size_t)i * chunk_bytes + p];
-  u[idx] = (int32_t)sat(rne((int64_t)qemb[b * D + d], semb[b] - F));
-}
-
 // int8 cut of one value with the row's shift k
 __device__ __forceinline__ int8_t cut8(int32_t a, int k) {
   int64_t v = rne((int64_t)a, k);
@@ -153,64 +141,78 @@ __device__ __forceinline__ int8_t cut8(int32_t a, int k) {
 }
 __device__ __forceinline__ int64_t abs64(int64_t a) { return a < 0 ? -a : a; }
 
+__device__ __forceinline__ int64_t warp_max64(int64_t v) {
+  for (int o = 16; o > 0; o >>= 1) { const int64_t w = __shfl_xor_sync(0xffffffffu, v, o); v = w > v ? w : v; }
+  return v;
+}
+__device__ __forceinline__ int64_t warp_sum64(int64_t v) {                 // integers: order-free
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+
 // ---- S2: r = RMSNorm(u) * w in Q (integer only), cut to an int8 row for in_proj in the same
-// kernel (the Q values of r have no other reader).  One block of 256 threads per row, D <= 1024 (<= 4 values per thread).
-__global__ void __launch_bounds__(256) k_fx_rmsnorm_q(const int32_t* __restrict__ u, const int32_t* __restrict__ w, int D,
-                                                      int64_t sqrt_d, int8_t* __restrict__ q, int KB, int32_t* __restrict__ kshift) {
-  __shared__ int64_t red[32];
-  const int row = blockIdx.x;
-  const int32_t* ur = u + (size_t)row * D;
-  int32_t uv[4], rv[4];
-  int64_t m = 0;
-#pragma unroll
-  for (int it = 0; it < 4; ++it) {
-    const int d = threadIdx.x + 256 * it;
-    uv[it] = d < D ? ur[d] : 0;
-    rv[it] = 0;
-    m = max(m, abs64(uv[it]));
+// kernel (the Q values of r have no other reader).  One warp per row (shuffle reductions, no block barrier), eight rows
+// per block; r waits in shared memory for the row's shift.  D <= 1024.
+// EMBED (the first layer of a step): the row is first written as u = Emb[previous byte] (S1) by the same warp.
+struct EmbedSrc {
+  const uint8_t* data; size_t chunk_bytes; const uint32_t *pos, *len; const int8_t* qemb; const int32_t* semb;
+};
+constexpr int RMS_ROWS = 8;
+template <bool EMBED>
+__global__ void __launch_bounds__(32 * RMS_ROWS) k_fx_rmsnorm_q(int32_t* __restrict__ u, const int32_t* __restrict__ w, int D,
+                                                                int64_t sqrt_d, int8_t* __restrict__ q, int KB,
+                                                                int32_t* __restrict__ kshift, int B, EmbedSrc es) {
+  __shared__ int32_t s_r[RMS_ROWS][1024];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int row = blockIdx.x * RMS_ROWS + warp;
+  if (row >= B) return;
+  int32_t* ur = u + (size_t)row * D;
+  if (EMBED) {
+    const uint32_t p = min(es.pos[row], es.len[row] - 1u);
+    const int b = es.data[(size_t)row * es.chunk_bytes + p];
+    const int sh = es.semb[b] - F;
+    for (int d = lane; d < D; d += 32) ur[d] = (int32_t)sat(rne((int64_t)es.qemb[b * D + d], sh));
+    __syncwarp();                                   // (each lane re-reads only what it wrote; the barrier is for clarity)
   }
-  m = block_max(m, red);
+  int32_t* rr = s_r[warp];
+  int64_t m = 0;
+  for (int d = lane; d < D; d += 32) m = max(m, abs64(ur[d]));
+  m = warp_max64(m);
   int64_t rm = 0;
   if (m != 0) {
     const int c = min(24 - bitlen64(m), 12);
     int64_t s = 0;
-#pragma unroll
-    for (int it = 0; it < 4; ++it) { const int64_t t = rne((int64_t)uv[it], -c); s += t * t; }
-    s = block_sum(s, red);
+    for (int d = lane; d < D; d += 32) { const int64_t t = rne((int64_t)ur[d], -c); s += t * t; }
+    s = warp_sum64(s);
     const int64_t Y = isqrt64(s + (int64_t)D * rne(EPS_Q40, -2 * c));
     const double rcp_y = rcp_est(Y);
-#pragma unroll
-    for (int it = 0; it < 4; ++it) {
-      const int d = threadIdx.x + 256 * it;
-      if (d < D) {
-        rv[it] = (int32_t)qmul(rdiv_rcp(rne((int64_t)uv[it], -c) * sqrt_d, Y, rcp_y), w[d]);
-        rm = max(rm, abs64(rv[it]));
-      }
+#pragma unroll 2
+    for (int d = lane; d < D; d += 32) {
+      const int32_t r = (int32_t)qmul(rdiv_rcp(rne((int64_t)ur[d], -c) * sqrt_d, Y, rcp_y), w[d]);
+      rr[d] = r;
+      rm = max(rm, abs64(r));
     }
+    rm = warp_max64(rm);
   }
-  rm = block_max(rm, red);
   const int k = max(bitlen64(rm) - 7, 0);
-#pragma unroll
-  for (int it = 0; it < 4; ++it) {
-    const int d = threadIdx.x + 256 * it;
-    if (d < D) q[a_img_off(row, d, KB)] = cut8(rv[it], k);
-  }
-  if (threadIdx.x == 0) kshift[row] = k;
+  for (int d = lane; d < D; d += 32) q[a_img_off(row, d, KB)] = m != 0 ? cut8(rr[d], k) : (int8_t)0;
+  if (lane == 0) kshift[row] = k;
 }
 
 // ---- a row of Q values -> int8 with one shift per row: k = max(0, bitlen(max|a|) - 7), q = clip(rne(a, k), +-127).
-// One block per row; the int8 row goes into the activation image (KB k-blocks per row tile).
-__global__ void k_fx_quant_rows(const int32_t* __restrict__ a, int lda, int K, int8_t* __restrict__ q, int KB,
-                                int32_t* __restrict__ kshift) {
-  __shared__ int64_t red[32];
-  const int row = blockIdx.x;
+// One warp per row; the int8 row goes into the activation image (KB k-blocks per row tile).
+__global__ void __launch_bounds__(32 * RMS_ROWS) k_fx_quant_rows(const int32_t* __restrict__ a, int lda, int K, int8_t* __restrict__ q,
+                                                                 int KB, int32_t* __restrict__ kshift, int B) {
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int row = blockIdx.x * RMS_ROWS + warp;
+  if (row >= B) return;
   const int32_t* ar = a + (size_t)row * lda;
   int64_t m = 0;
-  for (int d = threadIdx.x; d < K; d += blockDim.x) { const int64_t v = ar[d]; m = max(m, v < 0 ? -v : v); }
-  m = block_max(m, red);
+  for (int d = lane; d < K; d += 32) m = max(m, abs64(ar[d]));
+  m = warp_max64(m);
   const int k = max(bitlen64(m) - 7, 0);
-  for (int d = threadIdx.x; d < K; d += blockDim.x) q[a_img_off(row, d, KB)] = cut8(ar[d], k);
-  if (threadIdx.x == 0) kshift[row] = k;
+  for (int d = lane; d < K; d += 32) q[a_img_off(row, d, KB)] = cut8(ar[d], k);
+  if (lane == 0) kshift[row] = k;
 }
 
 // ---- 32-bit forms.  The integer ALU pipe is what bounds the scan, so the roundings are written on 32-bit halves: the rounding constant
