@@ -263,6 +263,31 @@ int boa_debug_rc_encode(const uint32_t* cdf, const uint8_t* syms, size_t n_strea
 int boa_debug_rc_decode(const uint32_t* cdf, const uint8_t* in, size_t cap, const uint32_t* sizes,
                         size_t n_streams, size_t len, uint8_t* syms, void* cuda_stream);
 
+/* ---- an entry point that allocates nothing ----------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it).  boa_rc_encode_packed_noalloc runs S13e-S15 (eq. 8-11) on given tables: one GPU thread per stream
+ * codes symbols syms[i][0..len) under cdf[i][t][257] (as boa_debug_rc_encode) into a scratch row, the sizes are scanned
+ * on the device, and the payloads are packed back to back into `payload` (stream 0 first):
+ *   sizes[i]   bytes of stream i;   payload[sum_{j<i} sizes[j] ...]   its bytes;
+ *   status[0]  total payload bytes; status[1]  flags: bit 0 = payload_cap too small (streams that would end beyond
+ *              it are not written), bit 1 = a stream overflowed its scratch row (its size reads 0; cannot happen for
+ *              valid tables, whose cost is below 2.0007 bytes per symbol).
+ * The scratch rows, offsets and running totals - what the other entry points keep in a model's cudaMalloc'ed
+ * workspace - live in ONE static device array of boa_noalloc_scratch_bytes() = 4 MiB that every GPU loading the
+ * library holds until exit.  The call makes no cudaMalloc / cudaFree / allocating library call and does not
+ * synchronise: it enqueues five kernels on `cuda_stream` (used as it is, unlike the calls above) and returns; read
+ * sizes / status / payload after synchronising that stream.
+ * ALL pointers are DEVICE pointers (staging a host buffer would need an allocation): a host pointer -> BOA_E_ARG.
+ * Limit: 256 + 8 n_streams (rounded up to 256) + n_streams * round_up(2 len + 8, 16) <= 4 MiB and n_streams <= 65,536,
+ * i.e. n_streams <= boa_noalloc_max_streams(len) (e.g. 255 streams of 8,192 symbols, 7,824 of 256); beyond it
+ * BOA_E_CAPACITY, with the numbers in boa_last_cuda_error().  len >= 2^30: the limit is 0.
+ * Every call shares the array, which keeps the last call's contents: the call clears the words that must start at
+ * zero itself, but calls that OVERLAP on the GPU (different streams, different host threads) race - serialise them. */
+size_t boa_noalloc_scratch_bytes(void);
+size_t boa_noalloc_max_streams(size_t len);
+int boa_rc_encode_packed_noalloc(const uint32_t* cdf, const uint8_t* syms, size_t n_streams, size_t len, uint8_t* payload,
+                                 size_t payload_cap, uint32_t* sizes, uint64_t* status, void* cuda_stream);
+
 #ifdef __cplusplus
 }
 #endif

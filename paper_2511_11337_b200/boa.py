@@ -26,7 +26,8 @@ EXPORTS = ("boa_model_load", "boa_model_free", "boa_model_fingerprint", "boa_com
            "boa_stream_decompressed_size", "boa_stream_decompress", "boa_fx_model_load", "boa_fx_model_free",
            "boa_fx_model_fingerprint", "boa_fx_compress", "boa_fx_decompress", "boa_fx_last_launches", "boa_fx_debug_step_dump",
            "boa_strerror", "boa_last_cuda_error", "boa_set_profiling", "boa_get_profile",
-           "boa_debug_set_slab", "boa_debug_set_chain", "boa_debug_set_persist", "boa_debug_set_pair_tiles", "boa_debug_set_max_wave", "boa_debug_gemm", "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode")
+           "boa_debug_set_slab", "boa_debug_set_chain", "boa_debug_set_persist", "boa_debug_set_pair_tiles", "boa_debug_set_max_wave", "boa_debug_gemm", "boa_debug_step_dump", "boa_debug_quantise", "boa_debug_rc_encode", "boa_debug_rc_decode",
+           "boa_noalloc_scratch_bytes", "boa_noalloc_max_streams", "boa_rc_encode_packed_noalloc")
 
 
 class Profile(C.Structure):
@@ -129,6 +130,12 @@ def lib() -> C.CDLL:
     l.boa_debug_rc_encode.restype = C.c_int
     l.boa_debug_rc_decode.argtypes = [vp, u8p, sz, vp, sz, sz, u8p, vp]
     l.boa_debug_rc_decode.restype = C.c_int
+    l.boa_noalloc_scratch_bytes.argtypes = []
+    l.boa_noalloc_scratch_bytes.restype = sz
+    l.boa_noalloc_max_streams.argtypes = [sz]
+    l.boa_noalloc_max_streams.restype = sz
+    l.boa_rc_encode_packed_noalloc.argtypes = [vp, u8p, sz, sz, u8p, sz, vp, vp, vp]
+    l.boa_rc_encode_packed_noalloc.restype = C.c_int
     _lib = l
     return l
 
@@ -434,3 +441,23 @@ def debug_rc_decode(cdf: torch.Tensor, payload: torch.Tensor, sizes: torch.Tenso
     _check(lib().boa_debug_rc_decode(_ptr(cdf.contiguous()), _ptr(payload.contiguous()), cap, _ptr(sizes.contiguous()),
                                      s, length, _ptr(syms), _stream()), "boa_debug_rc_decode")
     return syms
+
+
+def noalloc_scratch_bytes() -> int:
+    return lib().boa_noalloc_scratch_bytes()
+
+
+def noalloc_max_streams(length: int) -> int:
+    return lib().boa_noalloc_max_streams(length)
+
+
+def rc_encode_packed_noalloc(cdf: torch.Tensor, syms: torch.Tensor, payload: torch.Tensor, sizes: torch.Tensor,
+                             status: torch.Tensor) -> None:
+    """The allocation-free entry point (include/boa.h): cdf [S,len,257] int32, syms [S,len] uint8 -> payload (packed),
+    sizes [S] int32, status [2] int64, all CUDA tensors the CALLER provides.  Asynchronous on torch's current stream."""
+    s, ln = syms.shape
+    code = lib().boa_rc_encode_packed_noalloc(_ptr(cdf), _ptr(syms), s, ln, _ptr(payload), payload.numel(), _ptr(sizes),
+                                              _ptr(status), _stream())
+    if code == E_CAPACITY:
+        raise BoaError(code, "boa_rc_encode_packed_noalloc: " + lib().boa_last_cuda_error().decode())
+    _check(code, "boa_rc_encode_packed_noalloc")

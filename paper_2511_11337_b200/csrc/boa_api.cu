@@ -1710,4 +1710,119 @@ int boa_debug_rc_decode(const uint32_t* cdf, const uint8_t* in, size_t cap, cons
 
 }  // extern "C"
 
+// ===================================================================================== allocation-free entry point
+// boa_rc_encode_packed_noalloc (include/boa.h): S13e-S15 on given tables - one thread per stream codes into a scratch
+// row, a device-side exclusive scan of the sizes, a compaction pass - for callers that must not allocate (CUDA graph
+// capture, serving loops).  Everything the existing path keeps in a model's cudaMalloc'ed workspace (per-stream scratch
+// rows, offsets, running total and flags) lives in ONE file-scope device array of fixed size; every GPU that loads the
+// library holds it until exit.  Its name is a host-side stand-in in host code: the kernels get the device address
+// that cudaGetSymbolAddress returns for the current device (looked up once per device, below).
+// Every call shares the array: calls that overlap on the GPU (two streams, two threads) race.
+#include <mutex>
+
+constexpr size_t kNoAllocScratchBytes = 4u << 20;                      // 4 MiB
+constexpr size_t kNoAllocCtrlBytes = 256;                              // [0] u64 payload total, [8] int flags payload / row
+static __device__ __align__(256) uint8_t g_noalloc_scratch[kNoAllocScratchBytes];
+
+namespace {
+
+constexpr int kNoAllocMaxDevices = 64;
+std::mutex g_noalloc_mu;
+uint8_t* g_noalloc_dev[kNoAllocMaxDevices] = {};
+
+// device address of the array on the CURRENT device (set-up: first call on that device)
+int noalloc_scratch(uint8_t** out) {
+  int dev = 0;
+  BOA_CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kNoAllocMaxDevices) return BOA_E_UNSUPPORTED;
+  std::lock_guard<std::mutex> lock(g_noalloc_mu);
+  if (!g_noalloc_dev[dev]) {
+    void* p = nullptr;
+    BOA_CUDA_TRY(cudaGetSymbolAddress(&p, g_noalloc_scratch));
+    if (!p) return BOA_E_CUDA;
+    g_noalloc_dev[dev] = static_cast<uint8_t*>(p);
+  }
+  *out = g_noalloc_dev[dev];
+  return BOA_OK;
+}
+
+size_t noalloc_need(size_t n_streams, size_t cap) { return kNoAllocCtrlBytes + round_up(8 * n_streams, 256) + n_streams * cap; }
+
+// the control words of the shared array start every call at zero (they keep the last call's values otherwise)
+__global__ void k_noalloc_clear(uint64_t* ctrl) {
+  if (threadIdx.x < kNoAllocCtrlBytes / 8) ctrl[threadIdx.x] = 0;
+}
+// k_debug_rc_encode with the rows in the scratch array: stream i -> rows + i * cap, its size -> sizes[i] (caller's)
+__global__ void k_noalloc_rc_encode(const uint32_t* __restrict__ cdf, const uint8_t* __restrict__ syms, int B, uint32_t len,
+                                    uint8_t* rows, uint32_t cap, uint32_t* __restrict__ sizes, int* row_overflow) {
+  const int i = blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= B) return;
+  EncState st;
+  st.low = 0; st.range = 0xFFFFFFFFu; st.pending = 0; st.wpos = 0; st.cache = 0; st.started = 0;
+  ByteSink o;
+  o.begin(rows + (size_t)i * cap, 0u);
+  for (uint32_t t = 0; t < len; ++t) {
+    if (st.wpos + st.pending + 8u > cap) { *row_overflow = 1; sizes[i] = 0; return; }
+    const uint32_t* C = cdf + ((size_t)i * len + t) * 257;
+    const uint32_t s = syms[(size_t)i * len + t];
+    enc_symbol(st, C[s], C[s + 1], o);
+  }
+  if (st.wpos + st.pending + 8u > cap) { *row_overflow = 1; sizes[i] = 0; return; }
+  for (int k = 0; k < 5; ++k) enc_shift_low(st, o);
+  sizes[i] = st.wpos;
+}
+// status[0] = payload bytes, status[1] = flags (bit 0: payload_cap too small, bit 1: a scratch row overflowed)
+__global__ void k_noalloc_status(const uint8_t* ctrl, uint64_t* status) {
+  status[0] = *reinterpret_cast<const uint64_t*>(ctrl);
+  const int* f = reinterpret_cast<const int*>(ctrl + 8);
+  status[1] = (f[0] ? 1u : 0u) | (f[1] ? 2u : 0u);
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t boa_noalloc_scratch_bytes(void) { return kNoAllocScratchBytes; }
+
+size_t boa_noalloc_max_streams(size_t len) {
+  if (len == 0 || len >= (1ull << 30)) return 0;
+  const size_t cap = stream_cap(len);
+  size_t n = (kNoAllocScratchBytes - kNoAllocCtrlBytes) / (cap + 8);
+  while (n > 0 && noalloc_need(n, cap) > kNoAllocScratchBytes) --n;
+  return std::min<size_t>(n, kMaxWaveStreams);
+}
+
+// No cudaMalloc / cudaFree / allocating routine below: pointer queries, one symbol look-up per device, five launches.
+int boa_rc_encode_packed_noalloc(const uint32_t* cdf, const uint8_t* syms, size_t n_streams, size_t len, uint8_t* payload,
+                                 size_t payload_cap, uint32_t* sizes, uint64_t* status, void* cuda_stream) {
+  if (!cdf || !syms || !payload || !sizes || !status || n_streams == 0 || len == 0) return BOA_E_ARG;
+  if (n_streams > boa_noalloc_max_streams(len)) {
+    snprintf(last_cuda_error_buf(), 256, "boa_rc_encode_packed_noalloc: %zu streams x %zu symbols need more than the %zu-byte static scratch (at most %zu streams of this length)",
+             n_streams, len, kNoAllocScratchBytes, boa_noalloc_max_streams(len));
+    return BOA_E_CAPACITY;
+  }
+  BOA_TRY(check_device());
+  // staging a host buffer would need an allocation: every pointer is a device pointer
+  if (!is_device_ptr(cdf) || !is_device_ptr(syms) || !is_device_ptr(payload) || !is_device_ptr(sizes) || !is_device_ptr(status))
+    return BOA_E_ARG;
+  uint8_t* scratch = nullptr;
+  BOA_TRY(noalloc_scratch(&scratch));
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  const uint32_t cap = stream_cap(len);
+  const int B = (int)n_streams;
+  uint64_t* total = reinterpret_cast<uint64_t*>(scratch);
+  int* flags = reinterpret_cast<int*>(scratch + 8);                 // [0] payload_cap too small, [1] a row overflowed
+  uint64_t* off = reinterpret_cast<uint64_t*>(scratch + kNoAllocCtrlBytes);
+  uint8_t* rows = scratch + kNoAllocCtrlBytes + round_up(8 * n_streams, 256);
+  k_noalloc_clear<<<1, 32, 0, st>>>(total);
+  k_noalloc_rc_encode<<<(unsigned)((n_streams + 63) / 64), 64, 0, st>>>(cdf, syms, B, (uint32_t)len, rows, cap, sizes, flags + 1);
+  k_wave_offsets<<<1, 1024, 0, st>>>(sizes, off, B, total);
+  k_compact<<<(unsigned)((n_streams * 32 + 255) / 256), 256, 0, st>>>(rows, cap, sizes, off, payload, (uint64_t)payload_cap, flags, B);
+  k_noalloc_status<<<1, 1, 0, st>>>(scratch, status);
+  BOA_CUDA_TRY(cudaPeekAtLastError());
+  return BOA_OK;
+}
+
+}  // extern "C"
+
 #include "boa_fx.cuh"   // FX1, the deterministic fixed-point pipeline (same translation unit: it reuses the helpers above)
