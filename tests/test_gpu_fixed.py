@@ -110,3 +110,20 @@ def test_fx_round_trip_at_scale(boa):
         _, _, _, _, g1 = container.unpack(_np(gm.compress(data[i * T:(i + 1) * T][:60], 60)).tobytes())
         assert g1[0] == p1[0], i
     assert len(pays) == B
+
+
+def test_fx_more_chunks_than_one_wave(boa):
+    """70,001 chunks of 3 bytes: more than the 65,536 streams a wave steps together, so the second wave starts at a stream
+    offset inside the input, the size index and the payload.  Byte-exact round trip, and chunks on both sides of the wave
+    boundary code to the bytes they get when compressed alone (a stream does not depend on its neighbours)."""
+    cfg = synth.CONFIGS[1]
+    gm = boa.FxModel(cfg.weights(emb_std=0.25))
+    chunk, nc = 3, 70001
+    data = cfg.data(nc * chunk - 1)                                # ragged last chunk (2 bytes)
+    comp = gm.compress(data, chunk)
+    assert _np(gm.decompress(comp)).tobytes() == data
+    _, _, _, _, pa = container.unpack(_np(comp).tobytes())
+    assert len(pa) == nc
+    for i in (0, 65535, 65536, 70000):
+        _, _, _, _, ps = container.unpack(_np(gm.compress(data[i * chunk:(i + 1) * chunk], chunk)).tobytes())
+        assert ps[0] == pa[i], i
