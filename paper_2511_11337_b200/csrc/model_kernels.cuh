@@ -492,12 +492,22 @@ __global__ void __launch_bounds__(288, 2) k_scan_slab(const ScanSlabArgs a) {
       const int s = kk & (NSL - 1);
       bar_wait(s_u32(&bars[s]), (uint32_t)((kk / NSL) & 1));
       float* d = reinterpret_cast<float*>(stages + s * SB + D_OFF);
-      const int rl = a.KS * a.ldj;
-      for (int c = lane; c < G * a.ldj; c += 32) {
-        const int t = c / a.ldj, col = c - t * a.ldj;
-        float v = d[t * rl + col];
-        for (int p = 1; p < a.KS; ++p) v += d[t * rl + p * a.ldj + col];
-        d[t * rl + col] = v;
+      // (this warp is the only producer of `ready`: no divisions, every load of an element in flight before the adds)
+      const int KS = a.KS, ldj = a.ldj, rl = KS * ldj;
+      int t = 0, col = lane;
+      while (col >= ldj) { col -= ldj; ++t; }
+      for (int c = lane; c < G * ldj; c += 32) {
+        float* p0 = d + t * rl + col;
+        float x[KSMAX];
+#pragma unroll
+        for (int p = 0; p < KSMAX; ++p) x[p] = p < KS ? p0[p * ldj] : 0.0f;
+        float v = x[0];
+#pragma unroll
+        for (int p = 1; p < KSMAX; ++p)
+          if (p < KS) v += x[p];
+        p0[0] = v;
+        col += 32;
+        while (col >= ldj) { col -= ldj; ++t; }
       }
       __syncwarp();
       if (lane == 0) asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(s_u32(&bars[2 * NSL + s])) : "memory");
