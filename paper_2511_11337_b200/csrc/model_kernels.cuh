@@ -307,9 +307,15 @@ __device__ __forceinline__ void scan_roles(const ScanArgs& a, uint8_t* scan_smem
       const int s = kk & (NSTG - 1);
       bar_wait(s_u32(&bars[s]), (uint32_t)((kk / NSTG) & 1));
       float* row = reinterpret_cast<float*>(stages + s * SB + 2 * EC * 4 + EC * 6);
-      for (int c = lane; c < a.ldj; c += 32) {
-        float v = row[c];
-        for (int p = 1; p < a.KS; ++p) v += row[p * a.ldj + c];
+      const int KS = a.KS, ldj = a.ldj;
+      for (int c = lane; c < ldj; c += 32) {       // every partial of an element in flight before the adds (ascending order)
+        float x[KSMAX];
+#pragma unroll
+        for (int p = 0; p < KSMAX; ++p) x[p] = p < KS ? row[p * ldj + c] : 0.0f;
+        float v = x[0];
+#pragma unroll
+        for (int p = 1; p < KSMAX; ++p)
+          if (p < KS) v += x[p];
         row[c] = v;
       }
       __syncwarp();
