@@ -349,8 +349,8 @@ def sweep_point(boa, peaks, config, streams, chunk, label, sample_every=2):
     return ent
 
 
-def fx_point(boa, config, streams, chunk, label):
-    """One pass (after one warm-up pass) of FX1, the deterministic fixed-point pipeline, on a configs[]
+def fx_point(boa, config, streams, chunk, label, passes=2):
+    """One timed pass (the last of `passes`: by default after one warm-up pass) of FX1, the deterministic fixed-point pipeline, on a configs[]
     model shape at `streams` x `chunk` bytes, device buffers, CUDA events around boa_fx_compress / boa_fx_decompress."""
     import torch
     from paper_2511_11337_b200 import synth
@@ -361,7 +361,7 @@ def fx_point(boa, config, streams, chunk, label):
     d_in = torch.frombuffer(bytearray(base.data(n)), dtype=torch.uint8).to(dev)
     d_comp = torch.empty(boa.compress_bound(n, chunk), dtype=torch.uint8, device=dev)
     d_out = torch.empty(n, dtype=torch.uint8, device=dev)
-    for _ in range(2):
+    for _ in range(passes):
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
         ev[0].record()
         clen = m.compress_into(d_in, chunk, d_comp)
@@ -513,8 +513,10 @@ def run_ours(args, cfg):
             sweep.append(sweep_point(boa, peaks, config, streams, chunk_b, label, sample_every=2 if streams > 1024 else 0))
         line["sweep"] = sweep
         # FX1: the integer pipeline whose containers do not depend on the device, once per point
-        line["fx1"] = [fx_point(boa, 2, 4096, 273, "configs[1] model shape at B = 4,096 streams"),
-                       fx_point(boa, 4, 65536, 65, "configs[3] model shape at B = 65,536 streams")]
+        line["fx1"] = [fx_point(boa, 2, 4096, 273, "configs[1] model shape at B = 4,096 streams", passes=3),
+                       fx_point(boa, 4, 65536, 65, "configs[3] model shape at B = 65,536 streams", passes=3),
+                       # the metric's own workload once, no warm-up pass (a pass is 16,383 steps: first-call overheads are noise)
+                       fx_point(boa, 2, 4096, 16384, "configs[1] as it is: 64 MiB, 4,096 chunks x 16 KiB (one pass)", passes=1)]
         line["fx1_note"] = ("every step an integer kernel (tcgen05.mma kind::i8 contractions, integer RMSNorm / exp / sigmoid / "
                             "softplus by table, Q12.20 recurrence); logits, tables and containers bit-identical to oracle/fixed.py "
                             "(tests/test_gpu_fixed.py); both directions run the step path")
