@@ -267,8 +267,10 @@ int launch_tc(const tc::GemmArgs& g, int n_sm, cudaStream_t st) {
   at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
   at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at; cfg.numAttrs = 1;
-  if (g.NT % 2 == 0) {
-    // clusters of two CTAs share the activation k-blocks of a row tile (multicast): persistent, one cluster per SM pair
+  if (g.NT % 2 == 0 && mt > 1) {
+    // clusters of two CTAs share the activation k-blocks of a row tile (multicast): persistent, one cluster per SM pair.
+    // (Not for a wave of one row tile: there a launch is a chain of latencies and the two cluster barriers are 3 - 6 %
+    // of the step - cfg5 at 64 streams 296 -> 283 us per byte; same arithmetic, same bits.)
     const int items = mt * (g.NT / 2) * g.KS;
     cfg.gridDim = dim3(2 * std::min(items, std::max(1, n_sm / 2)));
     at[1].id = cudaLaunchAttributeClusterDimension;
